@@ -1,0 +1,139 @@
+"""CPU oracle (TEST INFRASTRUCTURE — see the header of hk_oracle.c).
+
+Thin ctypes wrapper around `oracle/hk_oracle.c`.  Only tests/, `__graft_entry__.smoke()` and
+bench.py's cpu_baseline / `--impl reference` leg may import this module; the CUDA path under
+`paper_1503_03806_b200/` never does, and this module never imports that package.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "hk_oracle.c")
+_LIB = os.path.join(_HERE, "libhk_oracle.so")
+_lib = None
+
+_dp = C.POINTER(C.c_double)
+_i64 = C.c_int64
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (-O2, OpenMP).  No fast-math: the arithmetic is as written."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-std=gnu11", "-fopenmp", "-fPIC", "-shared", "-ffp-contract=off",
+               "-o", _LIB, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        L = C.CDLL(_LIB)
+        L.orc_faddeeva_re.restype = C.c_double
+        L.orc_faddeeva_re.argtypes = [C.c_double, C.c_double]
+        L.orc_voigt_K.restype = None
+        L.orc_voigt_K.argtypes = [_dp, _dp, _i64, _dp]
+        L.orc_voigt_V.restype = C.c_double
+        L.orc_voigt_V.argtypes = [C.c_double] * 3
+        L.orc_line_strength.restype = C.c_double
+        L.orc_line_strength.argtypes = [C.c_double] * 5
+        L.orc_gauss_legendre.restype = C.c_int
+        L.orc_gauss_legendre.argtypes = [C.c_int, _dp, _dp]
+        L.orc_count_evals.restype = _i64
+        L.orc_count_evals.argtypes = [_dp, _i64, C.c_double, _i64, C.c_double, C.c_double]
+        L.orc_opacity.restype = C.c_int
+        L.orc_opacity.argtypes = [_dp, _dp, _dp, _dp, _dp, _i64, C.c_double, C.c_double, C.c_double, _i64,
+                                  C.c_double, C.c_double, C.c_double, C.c_double, _i64, _i64, _dp]
+        L.orc_kdist.restype = C.c_int
+        L.orc_kdist.argtypes = [_dp, _i64, _i64, C.c_int, _dp]
+        _lib = L
+    return _lib
+
+
+def _arr(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(_dp)
+
+
+def set_threads(n: int) -> None:
+    """Number of OpenMP threads the oracle uses (default: all cores)."""
+    os.environ["OMP_NUM_THREADS"] = str(n)
+    try:
+        C.CDLL("libgomp.so.1").omp_set_num_threads(int(n))
+    except OSError:
+        pass
+
+
+def faddeeva_re(x, y):
+    """K(x,y) = Re w(x+iy), elementwise (H_V is the real part of the Faddeeva function)."""
+    x, y = np.broadcast_arrays(_arr(x), _arr(y))
+    x, y = _arr(x), _arr(y)
+    out = np.empty(x.shape, dtype=np.float64)
+    lib().orc_voigt_K(_p(x), _p(y), x.size, _p(out))
+    return out
+
+
+def voigt_V(dv: float, alpha: float, gamma: float) -> float:
+    """V(dv; alpha, gamma) = K(dv/alpha, gamma/alpha)/(alpha sqrt(pi))  (eq. 19)."""
+    return lib().orc_voigt_V(float(dv), float(alpha), float(gamma))
+
+
+def line_strength(S, nu0, E_low, T, q_ratio) -> float:
+    """S(T) from S(296 K), eq. 18 in the DESIGN.md G1 reading."""
+    return lib().orc_line_strength(float(S), float(nu0), float(E_low), float(T), float(q_ratio))
+
+
+def gauss_legendre(n_g: int):
+    g = np.empty(n_g)
+    w = np.empty(n_g)
+    rc = lib().orc_gauss_legendre(int(n_g), _p(g), _p(w))
+    if rc != 0:
+        raise ValueError(f"orc_gauss_legendre: {rc}")
+    return g, w
+
+
+def grid_size(nu_min: float, nu_max: float, dnu: float) -> int:
+    return int(round((nu_max - nu_min) / dnu))
+
+
+def count_evals(nu0, nu_min, N, dnu, cutoff) -> int:
+    nu0 = _arr(nu0)
+    return int(lib().orc_count_evals(_p(nu0), nu0.size, nu_min, int(N), dnu, cutoff))
+
+
+def opacity(nu0, S, gamma0, T, P_atm, nu_min, nu_max, dnu, cutoff, mass_amu=18.0, n_T=None, E_low=None,
+            q_ratio=1.0, j_begin=0, j_end=None):
+    """kappa(nu_j), j in [j_begin, j_end), on nu_j = nu_min + j*dnu  (eq. 16 + 19)."""
+    nu0, S, gamma0 = _arr(nu0), _arr(S), _arr(gamma0)
+    n_T = None if n_T is None else _arr(n_T)
+    E_low = None if E_low is None else _arr(E_low)
+    N = grid_size(nu_min, nu_max, dnu)
+    if j_end is None:
+        j_end = N
+    out = np.empty(max(j_end - j_begin, 0), dtype=np.float64)
+    rc = lib().orc_opacity(_p(nu0), _p(S), _p(gamma0), _p(n_T), _p(E_low), nu0.size, T, P_atm, nu_min, N, dnu, cutoff,
+                           mass_amu, q_ratio, j_begin, j_end, _p(out))
+    if rc != 0:
+        raise ValueError(f"orc_opacity: error {rc}")
+    return out
+
+
+def kdist(kappa, ppb: int, n_g: int):
+    """k_out[n_bins, n_g]: per-bin sorted kappa resampled at the Gauss-Legendre nodes (eqs. 14-15)."""
+    kappa = _arr(kappa)
+    if kappa.size % ppb:
+        raise ValueError("n_points is not a multiple of ppb")
+    out = np.empty((kappa.size // ppb, n_g), dtype=np.float64)
+    rc = lib().orc_kdist(_p(kappa), kappa.size, int(ppb), int(n_g), _p(out))
+    if rc != 0:
+        raise ValueError(f"orc_kdist: error {rc}")
+    return out
