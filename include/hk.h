@@ -1,0 +1,145 @@
+/* hk.h — C ABI of the B200-native HELIOS-K hot path (Grimm & Heng 2015, arXiv:1503.03806).
+ *
+ * The library computes, entirely in its own sm_100a CUDA kernels,
+ *
+ *   (1) the line-by-line opacity function on a uniform wavenumber grid
+ *         kappa(nu_j) = sum_i (S_i(T)/m) * Phi_i(nu_j),      nu_j = nu_min + j*dnu,  j = 0..N-1
+ *       eq. 16 with the Voigt profile Phi = sqrt(ln2/pi) H_V / Gamma_D of eq. 19
+ *       (PAPER.md:176-183), H_V = Re w(u+ia) evaluated by an Algorithm-916-type series near the line
+ *       core and n-point Gauss-Hermite quadrature in the wings, every line truncated
+ *       at an absolute line-wing cutoff, lines looped serially and grid points in
+ *       parallel with kappa accumulated in registers;
+ *   (2) the k-distribution of kappa in fixed-width bins: per-bin ascending sort, equal delta-y = 1/N_nu
+ *       (eqs. 14-15), resampled at n_g Gauss-Legendre nodes on (0,1)
+ *       (BASELINE.json north_star; the paper's Chebyshev fit, is not on this path).
+ *
+ * Conventions
+ *   - Every pointer marked "device" is a CUDA device pointer (e.g. torch .data_ptr()); "host" is host memory.
+ *     All arrays are contiguous float64 unless stated.  Inputs are read-only and caller-owned; outputs are
+ *     caller-allocated and are OVERWRITTEN, never accumulated into.
+ *   - Calls enqueue work on `stream` (a cudaStream_t passed as void*; NULL = the legacy default stream) and
+ *     return without synchronising, except where stated; the caller synchronises before reading results.
+ *     Scratch memory is taken from the stream-ordered CUDA memory pool and returned to it on the same stream.
+ *   - Return value: HK_OK (0) or a negative HK_ERR_* code; hk_strerror() names it; after HK_ERR_CUDA,
+ *     hk_last_cuda_error() returns the CUDA runtime's message.  No exceptions, no global mutable state
+ *     other than that last-error string.
+ *   - Units: wavenumbers in cm^-1, T in K, P in atm (1 atm = 1.01325 bar), mass in amu,
+ *     S in cm/molecule, kappa in cm^2/g.
+ *   - There is no CPU fallback: without a CUDA device every compute entry point returns HK_ERR_CUDA.
+ */
+#ifndef HK_H_
+#define HK_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define HK_OK 0
+#define HK_ERR_INVALID (-1)     /* bad argument (see each function) */
+#define HK_ERR_CUDA (-2)        /* CUDA runtime error; see hk_last_cuda_error() */
+#define HK_ERR_NOMEM (-3)       /* device or host allocation failed */
+#define HK_ERR_UNSORTED (-4)    /* prm->lines_sorted = 1 was promised but nu0 is not ascending */
+#define HK_ERR_UNSUPPORTED (-5) /* valid request outside the implemented range (e.g. points per bin > 16384) */
+
+#define HK_FP64 0
+#define HK_FP32 1               /* reserved: optional FP32 variant (not implemented: returns HK_ERR_UNSUPPORTED) */
+
+/* Line list, structure of arrays, all DEVICE pointers, n_lines entries each.
+ * These are the fields of a HITRAN/HITEMP record that the simplified broadening law of
+ * BASELINE.json uses (PAPER.md:164-191 lists the full record). */
+typedef struct {
+  const double *nu0;    /* line centre nu_0, cm^-1                                                  */
+  const double *S;      /* line strength, cm/molecule: at T if E_low == NULL, else at T0 = 296 K     */
+  const double *gamma0; /* Lorentz HWHM at 296 K and 1 atm, cm^-1/atm                                */
+  const double *n_T;    /* temperature exponent n_coll of eq. 20, or NULL for 0.5 on every line      */
+  const double *E_low;  /* lower-state energy, cm^-1, or NULL: no S(T) scaling (eq. 18 not applied)  */
+} hk_lines;
+
+typedef struct {
+  double mass_amu;      /* molecular mass m (one species per call), amu; > 0                          */
+  double q_ratio;       /* Q(296 K)/Q(T) of eq. 18; used only when E_low != NULL                      */
+  int precision;        /* HK_FP64                                                                    */
+  int lines_sorted;     /* 1: caller guarantees nu0 ascending (checked on the device, HK_ERR_UNSORTED
+                           is reported by hk_opacity_check()); 0: the library sorts a copy by nu0     */
+  void *stream;         /* cudaStream_t, or NULL                                                      */
+} hk_params;
+
+/* N = llround((nu_max - nu_min)/dnu): number of grid points nu_j = nu_min + j*dnu, j < N. Host only. */
+int64_t hk_grid_size(double nu_min, double nu_max, double dnu);
+
+/* Opacity function (steps a1-a4 of DESIGN.md: line prep, tile plan, Voigt accumulation, kappa store).
+ *
+ *   gamma_i = gamma0_i * P_atm * (296/T)^n_i                      eq. 20, pressure term
+ *   alpha_i = (nu0_i/c) sqrt(2 k_B T/m)  [= Gamma_D/sqrt(ln 2)]
+ *   S_i(T)  = S_i, or eq. 18 (T0 = 296 K in the last denominator) when E_low != NULL, with
+ *             c2 = hc/k_B = 1.4388 cm K
+ *   window  : line i contributes to j_lo(i) <= j <= j_hi(i),
+ *             j_lo = max(0, ceil(((nu0-cutoff)-nu_min)/dnu)), j_hi = min(N-1, floor(((nu0+cutoff)-nu_min)/dnu))
+ *             (inclusive, decided in index space; hard truncation, no renormalisation)
+ *   kappa_j = sum_{i in window} (S_i(T)/(m*amu)) * K(x_ij, y_i)/(alpha_i sqrt(pi)),  x = (nu_j-nu0)/alpha, y = gamma/alpha
+ *
+ * K = Re w(x+iy) is evaluated to <= 2.5e-7 relative error: Algorithm-916-type series for x^2+y^2 < 44,
+ * 6/3/2/1-point Gauss-Hermite rules beyond 44 / 280 / 3200 / 6e6.
+ *
+ * kappa_out: device, N doubles, overwritten.  Lines outside [nu_min, nu_max) still contribute if within the
+ * cutoff.  n_lines == 0 gives kappa == 0.
+ * HK_ERR_INVALID: NULL lines/prm/kappa_out or (n_lines > 0 and NULL nu0/S/gamma0); n_lines < 0; T, P_atm, dnu,
+ * cutoff, mass_amu not > 0 or not finite; N < 1 or N > 2^30; precision unknown.
+ * HK_ERR_UNSUPPORTED: precision == HK_FP32.
+ * Asynchronous on prm->stream.  nu0 must be ascending when lines_sorted = 1 (see hk_opacity_check). */
+int hk_opacity(const hk_lines *lines, int64_t n_lines, double T, double P_atm, double nu_min, double nu_max,
+               double dnu, double cutoff, double *kappa_out, const hk_params *prm);
+
+/* Synchronous check that a device nu0 array is ascending (what lines_sorted = 1 promises).
+ * Returns HK_OK, HK_ERR_UNSORTED, or an error.  Blocks until the stream is idle. */
+int hk_lines_check_sorted(const double *nu0_device, int64_t n_lines, void *stream);
+
+/* Metric denominator: sum_i (j_hi(i) - j_lo(i) + 1) over lines with a non-empty window.  HOST array. */
+int64_t hk_count_evals(const double *nu0_host, int64_t n_lines, double nu_min, int64_t N, double dnu, double cutoff);
+
+/* k-distribution (steps a5-a6): bins of ppb = llround(bin_width/dnu) consecutive points, aligned at index 0.
+ *   s = ascending sort of kappa[b*ppb : (b+1)*ppb];  y_k = (k + 1/2)/ppb   (eq. 15: delta-y = 1/N_nu)
+ *   k_out[b][q] = linear interpolation of (y_k, s_k) at the q-th Gauss-Legendre node g_q on (0,1),
+ *                 clamped to s_0 / s_{ppb-1} outside [y_0, y_{ppb-1}].
+ * kappa: device [n_points], values >= 0 (or +inf), no NaN.  k_out: device [n_bins*n_g], row-major by bin, overwritten.
+ * HK_ERR_INVALID: NULL pointers, n_points < 1, dnu or bin_width not > 0, bin_width/dnu not an integer within 1e-9,
+ * n_points not a multiple of ppb, n_g < 1 or > 128.   HK_ERR_UNSUPPORTED: ppb > 16384.   Asynchronous. */
+int hk_kdist(const double *kappa, int64_t n_points, double dnu, double bin_width, int n_g, double *k_out, void *stream);
+
+/* n_g Gauss-Legendre nodes g (ascending) and weights w on (0,1), sum w = 1.  HOST arrays of n_g doubles.
+ * HK_ERR_INVALID for n_g < 1, n_g > 4096 or NULL. */
+int hk_gauss_legendre(int n_g, double *g, double *w);
+
+/* Test hook: out[i] = K(x[i], y[i]) = Re w(x+iy) through the device Voigt routine of hk_opacity (same regime
+ * switches).  x, y, out: device [n]; y > 0.  Asynchronous. */
+int hk_voigt_K(const double *x, const double *y, int64_t n, double *out, int precision, void *stream);
+
+/* Persistent-context form for T-P sweeps ("repeat this calculation for multiple combinations of
+ * temperature and pressure"): the line list is bound once, scratch is kept between calls.
+ * hk_create copies nothing: the hk_lines device arrays must outlive the context. */
+typedef struct hk_ctx hk_ctx;
+int hk_create(const hk_lines *lines, int64_t n_lines, const hk_params *prm, hk_ctx **out);
+int hk_opacity_ctx(hk_ctx *ctx, double T, double P_atm, double q_ratio, double nu_min, double nu_max, double dnu,
+                   double cutoff, double *kappa_out);
+int hk_destroy(hk_ctx *ctx);
+
+/* Measurement helper: runs a dependent-FMA FP64 loop on every SM and returns the achieved FP64
+ * thread-instructions per second (the "alu" roofline denominator of bench.py, measured live).  Synchronous. */
+int hk_fp64_peak(double *inst_per_s_out, void *stream);
+
+/* Per-stage device time of the last hk_opacity / hk_opacity_ctx call on this thread, in milliseconds, measured
+ * with CUDA events on the call's stream: [0] line prep, [1] tile plan, [2] Voigt accumulation + kappa store.
+ * Enabled by hk_set_timing(1) (off by default: the events add launch overhead).  Synchronous. */
+int hk_set_timing(int on);
+int hk_last_stage_ms(float ms_out[3]);
+
+const char *hk_strerror(int code);
+const char *hk_last_cuda_error(void);
+const char *hk_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HK_H_ */

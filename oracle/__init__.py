@@ -50,6 +50,9 @@ def lib():
         L.orc_opacity.restype = C.c_int
         L.orc_opacity.argtypes = [_dp, _dp, _dp, _dp, _dp, _i64, C.c_double, C.c_double, C.c_double, _i64,
                                   C.c_double, C.c_double, C.c_double, C.c_double, _i64, _i64, _dp]
+        L.orc_opacity_points.restype = C.c_int
+        L.orc_opacity_points.argtypes = [_dp, _dp, _dp, _dp, _dp, _i64, C.c_double, C.c_double, C.c_double, _i64,
+                                         C.c_double, C.c_double, C.c_double, C.c_double, C.POINTER(_i64), _i64, _dp]
         L.orc_kdist.restype = C.c_int
         L.orc_kdist.argtypes = [_dp, _i64, _i64, C.c_int, _dp]
         _lib = L
@@ -124,6 +127,22 @@ def opacity(nu0, S, gamma0, T, P_atm, nu_min, nu_max, dnu, cutoff, mass_amu=18.0
                            mass_amu, q_ratio, j_begin, j_end, _p(out))
     if rc != 0:
         raise ValueError(f"orc_opacity: error {rc}")
+    return out
+
+
+def opacity_points(nu0, S, gamma0, T, P_atm, nu_min, nu_max, dnu, cutoff, js, mass_amu=18.0, n_T=None, E_low=None,
+                   q_ratio=1.0):
+    """kappa at an arbitrary list of grid indices `js` (same definition as `opacity`)."""
+    nu0, S, gamma0 = _arr(nu0), _arr(S), _arr(gamma0)
+    n_T = None if n_T is None else _arr(n_T)
+    E_low = None if E_low is None else _arr(E_low)
+    js = np.ascontiguousarray(js, dtype=np.int64)
+    N = grid_size(nu_min, nu_max, dnu)
+    out = np.empty(js.size, dtype=np.float64)
+    rc = lib().orc_opacity_points(_p(nu0), _p(S), _p(gamma0), _p(n_T), _p(E_low), nu0.size, T, P_atm, nu_min, N, dnu,
+                                  cutoff, mass_amu, q_ratio, js.ctypes.data_as(C.POINTER(_i64)), js.size, _p(out))
+    if rc != 0:
+        raise ValueError(f"orc_opacity_points: error {rc}")
     return out
 
 

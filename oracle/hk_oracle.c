@@ -266,19 +266,22 @@ double orc_voigt_V(double dv, double alpha, double gamma)
     return gamma / (3.14159265358979323846 * (dv * dv + gamma * gamma));
 }
 
-/* kappa_out[j - j_begin] for j in [j_begin, j_end).  Lines may come in any order. */
-int orc_opacity(const double *nu0, const double *S, const double *gamma0, const double *n_T, const double *E_low,
-                int64_t n_lines, double T, double P_atm, double nu_min, int64_t N, double dnu, double cutoff,
-                double mass_amu, double q_ratio, int64_t j_begin, int64_t j_end, double *kappa_out)
+/* kappa_out[k] = kappa(nu_{js[k]}) for an arbitrary list of grid indices.  Lines may come in any order. */
+int orc_opacity_points(const double *nu0, const double *S, const double *gamma0, const double *n_T, const double *E_low,
+                       int64_t n_lines, double T, double P_atm, double nu_min, int64_t N, double dnu, double cutoff,
+                       double mass_amu, double q_ratio, const int64_t *js, int64_t n_js, double *kappa_out)
 {
     if (n_lines < 0 || !(T > 0.0) || !(P_atm > 0.0) || !(dnu > 0.0) || !(cutoff > 0.0) || N <= 0 || !(mass_amu > 0.0) ||
-        j_begin < 0 || j_end > N || j_end < j_begin || !kappa_out)
+        n_js < 0 || (n_js > 0 && (!js || !kappa_out)))
         return ORC_ERR_INVALID;
     if (n_lines > 0 && (!nu0 || !S || !gamma0)) return ORC_ERR_INVALID;
+    for (int64_t k = 0; k < n_js; k++)
+        if (js[k] < 0 || js[k] >= N) return ORC_ERR_INVALID;
     double m_g = mass_amu * ORC_AMU;
     double vth = sqrt(2.0 * ORC_K_B * T / m_g) / ORC_C_LIGHT;     /* alpha = nu0 * vth */
     orc_line *L = (orc_line *)malloc(sizeof(orc_line) * (size_t)(n_lines > 0 ? n_lines : 1));
     if (!L) return ORC_ERR_NOMEM;
+#pragma omp parallel for schedule(static)
     for (int64_t i = 0; i < n_lines; i++) {
         double nT = n_T ? n_T[i] : 0.5;
         L[i].nu0 = nu0[i];
@@ -289,12 +292,16 @@ int orc_opacity(const double *nu0, const double *S, const double *gamma0, const 
         orc_window(nu0[i], nu_min, N, dnu, cutoff, &L[i].jlo, &L[i].jhi);
         L[i].src = i;
     }
-    qsort(L, (size_t)n_lines, sizeof(orc_line), cmp_line);
+    int sorted = 1;
+    for (int64_t i = 1; i < n_lines; i++)
+        if (L[i - 1].nu0 > L[i].nu0) { sorted = 0; break; }
+    if (!sorted) qsort(L, (size_t)n_lines, sizeof(orc_line), cmp_line);
     double slack = cutoff + 4.0 * dnu;
-#pragma omp parallel for schedule(dynamic, 64)
-    for (int64_t j = j_begin; j < j_end; j++) {
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t k = 0; k < n_js; k++) {
+        int64_t j = js[k];
         double nu = nu_min + (double)j * dnu;
-        /* candidates: first line with nu0 >= nu - slack */
+        /* candidates: first line with nu0 >= nu - slack; the exact test is the index window below */
         int64_t lo = 0, hi = n_lines;
         while (lo < hi) {
             int64_t mid = lo + (hi - lo) / 2;
@@ -305,10 +312,26 @@ int orc_opacity(const double *nu0, const double *S, const double *gamma0, const 
             if (j < L[i].jlo || j > L[i].jhi) continue;
             acc += (long double)L[i].amp * (long double)orc_voigt_V(nu - L[i].nu0, L[i].alpha, L[i].gamma);
         }
-        kappa_out[j - j_begin] = (double)acc;
+        kappa_out[k] = (double)acc;
     }
     free(L);
     return ORC_OK;
+}
+
+/* kappa_out[j - j_begin] for j in [j_begin, j_end). */
+int orc_opacity(const double *nu0, const double *S, const double *gamma0, const double *n_T, const double *E_low,
+                int64_t n_lines, double T, double P_atm, double nu_min, int64_t N, double dnu, double cutoff,
+                double mass_amu, double q_ratio, int64_t j_begin, int64_t j_end, double *kappa_out)
+{
+    if (j_begin < 0 || j_end > N || j_end < j_begin || !kappa_out) return ORC_ERR_INVALID;
+    int64_t n = j_end - j_begin;
+    int64_t *js = (int64_t *)malloc(sizeof(int64_t) * (size_t)(n > 0 ? n : 1));
+    if (!js) return ORC_ERR_NOMEM;
+    for (int64_t k = 0; k < n; k++) js[k] = j_begin + k;
+    int rc = orc_opacity_points(nu0, S, gamma0, n_T, E_low, n_lines, T, P_atm, nu_min, N, dnu, cutoff, mass_amu, q_ratio,
+                                js, n, kappa_out);
+    free(js);
+    return rc;
 }
 
 /* ------------------------------------------------------------------------------------------

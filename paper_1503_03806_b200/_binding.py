@@ -1,0 +1,293 @@
+"""ctypes binding of include/hk.h.  Same names as the C entry points; marshalling only."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import re
+from dataclasses import dataclass
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libhk.so")
+HEADER = os.path.join(HERE, "..", "include", "hk.h")
+
+HK_FP64, HK_FP32 = 0, 1
+_dp = C.POINTER(C.c_double)
+_i64 = C.c_int64
+
+
+class HKError(RuntimeError):
+    def __init__(self, code, where, detail=""):
+        self.code = code
+        super().__init__(f"{where}: {hk_strerror(code)} ({code}){' — ' + detail if detail else ''}")
+
+
+class _hk_lines(C.Structure):
+    _fields_ = [("nu0", C.c_void_p), ("S", C.c_void_p), ("gamma0", C.c_void_p), ("n_T", C.c_void_p), ("E_low", C.c_void_p)]
+
+
+class _hk_params(C.Structure):
+    _fields_ = [("mass_amu", C.c_double), ("q_ratio", C.c_double), ("precision", C.c_int), ("lines_sorted", C.c_int),
+                ("stream", C.c_void_p)]
+
+
+_lib = None
+
+
+def declared_symbols() -> list:
+    """Entry points declared in include/hk.h (used by the CPU test that checks the library exports them all)."""
+    txt = open(HEADER).read()
+    txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
+    return sorted(set(re.findall(r"\b(hk_[A-Za-z0-9_]+)\s*\(", txt)))
+
+
+def load_library():
+    """Loads libhk.so (built in-tree by paper_1503_03806_b200.build / __graft_entry__.build()).  Fails loudly."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                          "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    L.hk_grid_size.restype = _i64
+    L.hk_grid_size.argtypes = [C.c_double] * 3
+    L.hk_opacity.restype = C.c_int
+    L.hk_opacity.argtypes = [C.POINTER(_hk_lines), _i64, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double,
+                             C.c_double, C.c_void_p, C.POINTER(_hk_params)]
+    L.hk_lines_check_sorted.restype = C.c_int
+    L.hk_lines_check_sorted.argtypes = [C.c_void_p, _i64, C.c_void_p]
+    L.hk_count_evals.restype = _i64
+    L.hk_count_evals.argtypes = [_dp, _i64, C.c_double, _i64, C.c_double, C.c_double]
+    L.hk_kdist.restype = C.c_int
+    L.hk_kdist.argtypes = [C.c_void_p, _i64, C.c_double, C.c_double, C.c_int, C.c_void_p, C.c_void_p]
+    L.hk_gauss_legendre.restype = C.c_int
+    L.hk_gauss_legendre.argtypes = [C.c_int, _dp, _dp]
+    L.hk_voigt_K.restype = C.c_int
+    L.hk_voigt_K.argtypes = [C.c_void_p, C.c_void_p, _i64, C.c_void_p, C.c_int, C.c_void_p]
+    L.hk_create.restype = C.c_int
+    L.hk_create.argtypes = [C.POINTER(_hk_lines), _i64, C.POINTER(_hk_params), C.POINTER(C.c_void_p)]
+    L.hk_opacity_ctx.restype = C.c_int
+    L.hk_opacity_ctx.argtypes = [C.c_void_p] + [C.c_double] * 7 + [C.c_void_p]
+    L.hk_destroy.restype = C.c_int
+    L.hk_destroy.argtypes = [C.c_void_p]
+    L.hk_fp64_peak.restype = C.c_int
+    L.hk_fp64_peak.argtypes = [_dp, C.c_void_p]
+    L.hk_set_timing.restype = C.c_int
+    L.hk_set_timing.argtypes = [C.c_int]
+    L.hk_last_stage_ms.restype = C.c_int
+    L.hk_last_stage_ms.argtypes = [C.POINTER(C.c_float)]
+    L.hk_strerror.restype = C.c_char_p
+    L.hk_strerror.argtypes = [C.c_int]
+    L.hk_last_cuda_error.restype = C.c_char_p
+    L.hk_version.restype = C.c_char_p
+    _lib = L
+    return L
+
+
+def hk_strerror(code: int) -> str:
+    try:
+        return load_library().hk_strerror(int(code)).decode()
+    except ImportError:
+        return "libhk.so not loaded"
+
+
+def hk_version() -> str:
+    return load_library().hk_version().decode()
+
+
+def _check(rc, where):
+    if rc != 0:
+        detail = load_library().hk_last_cuda_error().decode() if rc == -2 else ""
+        raise HKError(rc, where, detail)
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_1503_03806_b200 needs a CUDA device (no CPU fallback)")
+    return torch
+
+
+def _dev_ptr(t, name, allow_none=False):
+    if t is None:
+        if allow_none:
+            return None
+        raise ValueError(f"{name} is required")
+    torch = _torch()
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise TypeError(f"{name} must be a contiguous float64 CUDA tensor")
+    return t.data_ptr()
+
+
+def _stream_ptr(stream):
+    torch = _torch()
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+@dataclass
+class Lines:
+    """Line list on the device (hk_lines): float64 CUDA tensors of equal length."""
+    nu0: object
+    S: object
+    gamma0: object
+    n_T: object = None
+    E_low: object = None
+
+    @staticmethod
+    def from_numpy(nu0, S, gamma0, n_T=None, E_low=None, device="cuda"):
+        torch = _torch()
+        f = lambda a: None if a is None else torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64)).to(device)
+        return Lines(f(nu0), f(S), f(gamma0), f(n_T), f(E_low))
+
+    @property
+    def n(self) -> int:
+        return int(self.nu0.numel())
+
+    def _c(self):
+        n = self.n
+        for name in ("S", "gamma0", "n_T", "E_low"):
+            t = getattr(self, name)
+            if t is not None and int(t.numel()) != n:
+                raise ValueError(f"{name} has {int(t.numel())} entries, nu0 has {n}")
+        return _hk_lines(_dev_ptr(self.nu0, "nu0"), _dev_ptr(self.S, "S"), _dev_ptr(self.gamma0, "gamma0"),
+                         _dev_ptr(self.n_T, "n_T", True), _dev_ptr(self.E_low, "E_low", True))
+
+
+def hk_grid_size(nu_min: float, nu_max: float, dnu: float) -> int:
+    return int(load_library().hk_grid_size(nu_min, nu_max, dnu))
+
+
+def hk_count_evals(nu0_host, nu_min: float, N: int, dnu: float, cutoff: float) -> int:
+    a = np.ascontiguousarray(nu0_host, dtype=np.float64)
+    return int(load_library().hk_count_evals(a.ctypes.data_as(_dp), a.size, nu_min, int(N), dnu, cutoff))
+
+
+def hk_gauss_legendre(n_g: int):
+    g = np.empty(n_g)
+    w = np.empty(n_g)
+    _check(load_library().hk_gauss_legendre(int(n_g), g.ctypes.data_as(_dp), w.ctypes.data_as(_dp)), "hk_gauss_legendre")
+    return g, w
+
+
+def hk_opacity(lines: Lines, T, P_atm, nu_min, nu_max, dnu, cutoff, mass_amu=18.0, q_ratio=1.0, lines_sorted=True,
+               out=None, stream=None, precision=HK_FP64):
+    """kappa[N] on the device (hk_opacity of include/hk.h).  Asynchronous on the current (or given) torch stream."""
+    torch = _torch()
+    L = load_library()
+    N = hk_grid_size(nu_min, nu_max, dnu)
+    if out is None:
+        if N < 1:
+            raise HKError(-1, "hk_opacity")
+        out = torch.empty(N, dtype=torch.float64, device=lines.nu0.device)
+    elif int(out.numel()) != N:
+        raise ValueError(f"out has {int(out.numel())} entries, the grid has {N}")
+    cl = lines._c()
+    prm = _hk_params(float(mass_amu), float(q_ratio), int(precision), int(bool(lines_sorted)), _stream_ptr(stream))
+    _check(L.hk_opacity(C.byref(cl), lines.n, T, P_atm, nu_min, nu_max, dnu, cutoff, _dev_ptr(out, "out"), C.byref(prm)),
+           "hk_opacity")
+    return out
+
+
+def hk_kdist(kappa, dnu, bin_width, n_g, out=None, stream=None):
+    """k_out[n_bins, n_g] on the device (hk_kdist of include/hk.h)."""
+    torch = _torch()
+    L = load_library()
+    n = int(kappa.numel())
+    ppb = int(round(bin_width / dnu))
+    if out is None:
+        if ppb < 1 or n % ppb or n_g < 1:
+            raise HKError(-1, "hk_kdist")
+        out = torch.empty((n // ppb, n_g), dtype=torch.float64, device=kappa.device)
+    _check(L.hk_kdist(_dev_ptr(kappa, "kappa"), n, dnu, bin_width, int(n_g), _dev_ptr(out, "out"), _stream_ptr(stream)),
+           "hk_kdist")
+    return out
+
+
+def hk_voigt_K(x, y, out=None, stream=None, precision=HK_FP64):
+    """K(x,y) = Re w(x+iy) through the device Voigt routine (test hook)."""
+    torch = _torch()
+    if out is None:
+        out = torch.empty_like(x)
+    _check(load_library().hk_voigt_K(_dev_ptr(x, "x"), _dev_ptr(y, "y"), int(x.numel()), _dev_ptr(out, "out"),
+                                     int(precision), _stream_ptr(stream)), "hk_voigt_K")
+    return out
+
+
+def hk_lines_check_sorted(nu0, stream=None) -> bool:
+    rc = load_library().hk_lines_check_sorted(_dev_ptr(nu0, "nu0"), int(nu0.numel()), _stream_ptr(stream))
+    if rc == -4:
+        return False
+    _check(rc, "hk_lines_check_sorted")
+    return True
+
+
+def hk_fp64_peak(stream=None) -> float:
+    """Measured FP64 FMA thread-instructions per second of this GPU (roofline denominator, measured live)."""
+    v = C.c_double(0.0)
+    _check(load_library().hk_fp64_peak(C.byref(v), _stream_ptr(stream)), "hk_fp64_peak")
+    return v.value
+
+
+def hk_set_timing(on: bool) -> None:
+    _check(load_library().hk_set_timing(int(bool(on))), "hk_set_timing")
+
+
+def hk_last_stage_ms():
+    a = (C.c_float * 3)()
+    _check(load_library().hk_last_stage_ms(a), "hk_last_stage_ms")
+    return [float(v) for v in a]
+
+
+class Context:
+    """hk_create / hk_opacity_ctx / hk_destroy: line list bound once, scratch kept across (T,P) calls."""
+
+    def __init__(self, lines: Lines, mass_amu=18.0, lines_sorted=True, stream=None):
+        self._lines = lines      # keep the tensors alive
+        self._h = C.c_void_p()
+        cl = lines._c()
+        prm = _hk_params(float(mass_amu), 1.0, HK_FP64, int(bool(lines_sorted)), _stream_ptr(stream))
+        _check(load_library().hk_create(C.byref(cl), lines.n, C.byref(prm), C.byref(self._h)), "hk_create")
+
+    def opacity(self, T, P_atm, nu_min, nu_max, dnu, cutoff, q_ratio=1.0, out=None):
+        torch = _torch()
+        N = hk_grid_size(nu_min, nu_max, dnu)
+        if out is None:
+            out = torch.empty(N, dtype=torch.float64, device=self._lines.nu0.device)
+        _check(load_library().hk_opacity_ctx(self._h, T, P_atm, q_ratio, nu_min, nu_max, dnu, cutoff, _dev_ptr(out, "out")),
+               "hk_opacity_ctx")
+        return out
+
+    def close(self):
+        if self._h:
+            load_library().hk_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def opacity_host(nu0, S, gamma0, T, P_atm, nu_min, nu_max, dnu, cutoff, mass_amu=18.0, E_low=None, q_ratio=1.0,
+                 bin_width=None, n_g=20, kappa_out=None):
+    """End-to-end call with HOST buffers: pinned host line arrays -> device, hk_opacity (+ hk_kdist when bin_width is
+    given), result -> pinned host.  Returns (kappa_host, k_host or None).  Synchronous."""
+    torch = _torch()
+    dev = torch.device("cuda")
+    up = lambda a: None if a is None else a.to(dev, non_blocking=True)
+    lines = Lines(up(nu0), up(S), up(gamma0), None, up(E_low))
+    kappa = hk_opacity(lines, T, P_atm, nu_min, nu_max, dnu, cutoff, mass_amu=mass_amu, q_ratio=q_ratio)
+    k_host = None
+    if bin_width is not None:
+        k = hk_kdist(kappa, dnu, bin_width, n_g)
+        k_host = torch.empty(k.shape, dtype=k.dtype, pin_memory=True)
+        k_host.copy_(k, non_blocking=True)
+    if kappa_out is None:
+        kappa_out = torch.empty(kappa.shape, dtype=kappa.dtype, pin_memory=True)
+    kappa_out.copy_(kappa, non_blocking=True)
+    torch.cuda.current_stream().synchronize()
+    return kappa_out, k_host

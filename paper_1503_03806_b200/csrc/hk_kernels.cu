@@ -1,0 +1,801 @@
+// hk_kernels.cu — sm_100a kernels and the C ABI of include/hk.h.
+//
+// Steps:
+//   a1 line_prep_kernel   per line: alpha, gamma, S(T), amplitude, index window, regime radii
+//   a2 tile_plan_kernel   per grid tile: range of sorted lines whose window touches the tile
+//   a3 voigt_kernel       kappa_j = sum_i amp_i V_i(nu_j): grid-point-owned register accumulation, lines streamed
+//                         through shared memory by 1-D TMA bulk copies, regime chosen per (line, warp span)
+//   a4                    coalesced kappa store from the same kernel ("without additional write-outs")
+//   a5/a6 kdist_kernel    per-bin shared-memory sort + resampling at Gauss-Legendre nodes
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+
+#include "../../include/hk.h"
+#include "hk_voigt.cuh"
+
+namespace hk {
+
+// ------------------------------------------------------------------------------------------------------
+// packed line records (written by a1, streamed by a3).  Three 32-byte records per line, structure of arrays,
+// so that a chunk of lines is three contiguous 16-byte-aligned spans (one TMA bulk copy each).
+// ------------------------------------------------------------------------------------------------------
+struct __align__(16) LineMeta {
+  int jlo, jhi;  // inclusive index window of the line (empty if jhi < jlo)
+  float c;       // line centre in grid units, (nu0-nu_min)/dnu
+  float r3;      // |j-c| >= r3 for a whole span  =>  r^2 >= kR3 on it (3-point rule valid); conservative (+2)
+  float r2;      // likewise kR2 (2-point rule)
+  float r1;      // likewise kR1 (1-point rule)
+  float xc2;     // series region: x^2 < xc2
+  float pad;
+};
+struct __align__(16) LineBase {
+  double nu0, A1, g2, a2;  // centre; amp*gamma/pi; gamma^2; alpha^2
+};
+struct __align__(16) LineGH2 {
+  double e2, f2, A1a2, inv_alpha;  // gamma^2 - alpha^2/2; 2 alpha^2 gamma^2; A1 alpha^2; 1/alpha (0 if alpha == 0)
+};
+static_assert(sizeof(LineMeta) == 32 && sizeof(LineBase) == 32 && sizeof(LineGH2) == 32, "record size");
+
+constexpr double kCLight = 2.99792458e10;   // cm/s
+constexpr double kBoltz = 1.380649e-16;     // erg/K
+constexpr double kAmu = 1.66053906660e-24;  // g
+constexpr double kC2 = 1.4388;              // cm K (BASELINE.json config 4)
+constexpr double kT0 = 296.0;               // K
+
+struct PrepArgs {
+  const double *nu0, *S, *gamma0, *n_T, *E_low;
+  int64_t n;
+  double T, P_atm, tfac_half;  // (296/T)^0.5 for n_T == NULL
+  double vth;                  // sqrt(2 kB T/m)/c : alpha = nu0*vth
+  double inv_mg;               // 1/(m*amu)
+  double q_ratio;
+  double nu_min, dnu, cutoff;
+  int N;
+  LineMeta *meta;
+  LineBase *base;
+  LineGH2 *gh2;
+};
+
+__device__ __forceinline__ float radius_grid(double R, double a2, double g2, double inv_dnu)
+{
+  double t = R * a2 - g2;
+  if (!(t > 0.0)) return 0.0f;
+  double r = sqrt(t) * inv_dnu + 2.0;
+  return r < 3.0e38 ? __double2float_ru(r) : 3.0e38f;
+}
+
+__global__ void __launch_bounds__(256) line_prep_kernel(PrepArgs a)
+{
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= a.n) return;
+  const double nu0 = a.nu0[i];
+  double alpha = nu0 * a.vth;
+  if (!(alpha > 0.0)) alpha = 0.0;  // nu0 <= 0: Lorentzian (A9)
+  const double tfac = a.n_T ? pow(kT0 / a.T, a.n_T[i]) : a.tfac_half;
+  const double gamma = a.gamma0[i] * a.P_atm * tfac;
+  double S = a.S[i];
+  if (a.E_low) {  // eq. 18, PAPER.md:170 (T0 in the last denominator: DESIGN.md G1)
+    const double boltz = exp(-kC2 * a.E_low[i] * (1.0 / a.T - 1.0 / kT0));
+    const double stim = (nu0 == 0.0) ? kT0 / a.T : (-expm1(-kC2 * nu0 / a.T)) / (-expm1(-kC2 * nu0 / kT0));
+    S = S * a.q_ratio * boltz * stim;
+  }
+  const double amp = S * a.inv_mg;
+  const double g2 = gamma * gamma, a2 = alpha * alpha;
+  LineBase b;
+  b.nu0 = nu0;
+  b.A1 = amp * gamma * (1.0 / kPi);
+  b.g2 = g2;
+  b.a2 = a2;
+  LineGH2 g;
+  g.e2 = g2 - 0.5 * a2;
+  g.f2 = 2.0 * a2 * g2;
+  g.A1a2 = b.A1 * a2;
+  g.inv_alpha = alpha > 0.0 ? 1.0 / alpha : 0.0;
+  // index window: sub, sub, IEEE divide, ceil/floor — no multiply-add, nothing to contract (A4)
+  double lo = ceil(__ddiv_rn(__dsub_rn(__dsub_rn(nu0, a.cutoff), a.nu_min), a.dnu));
+  double hi = floor(__ddiv_rn(__dsub_rn(__dadd_rn(nu0, a.cutoff), a.nu_min), a.dnu));
+  if (!(lo > 0.0)) lo = 0.0;
+  if (!(hi < (double)(a.N - 1))) hi = (double)(a.N - 1);
+  if (lo > 2.0e9) lo = 2.0e9;
+  if (hi < -2.0e9) hi = -2.0e9;
+  LineMeta m;
+  m.jlo = (int)lo;
+  m.jhi = (int)hi;
+  const double inv_dnu = 1.0 / a.dnu;
+  double c = (nu0 - a.nu_min) * inv_dnu;
+  c = fmin(fmax(c, -3.0e9), 3.0e9);
+  m.c = (float)c;
+  m.r3 = radius_grid(kR3, a2, g2, inv_dnu);
+  m.r2 = radius_grid(kR2, a2, g2, inv_dnu);
+  m.r1 = radius_grid(kR1, a2, g2, inv_dnu);
+  m.xc2 = alpha > 0.0 ? __double2float_ru(core_xc2(gamma * g.inv_alpha)) : 0.0f;
+  m.pad = 0.0f;
+  a.meta[i] = m;
+  a.base[i] = b;
+  a.gh2[i] = g;
+}
+
+// a2: lines are sorted by nu0, so jlo and jhi are non-decreasing in i.  Tile t owns points [t*tile, (t+1)*tile).
+// plan[t] = [first i with jhi >= tile_lo, first i with jlo > tile_hi).
+__global__ void __launch_bounds__(128) tile_plan_kernel(const LineMeta *meta, int64_t n, int n_tiles, int tile, int N,
+                                                        int2 *plan)
+{
+  int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n_tiles) return;
+  const int tlo = t * tile;
+  const int thi = min(N, tlo + tile) - 1;
+  int64_t lo = 0, hi = n;
+  while (lo < hi) {
+    int64_t mid = lo + ((hi - lo) >> 1);
+    if (meta[mid].jhi < tlo) lo = mid + 1; else hi = mid;
+  }
+  const int64_t L0 = lo;
+  hi = n;
+  while (lo < hi) {
+    int64_t mid = lo + ((hi - lo) >> 1);
+    if (meta[mid].jlo <= thi) lo = mid + 1; else hi = mid;
+  }
+  plan[t] = make_int2((int)L0, (int)lo);
+}
+
+// ------------------------------------------------------------------------------------------------------
+// mbarrier + 1-D TMA bulk copy (cp.async.bulk -> SASS UBLKCP)
+// ------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init()
+{
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
+{
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+  uint32_t ok;
+  const uint32_t addr = smem_u32(bar);
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(addr), "r"(parity)
+        : "memory");
+  } while (!ok);
+}
+
+// ------------------------------------------------------------------------------------------------------
+// a3 + a4: Voigt accumulation.  One CTA per tile of WARPS*32*P consecutive grid points; warp w owns the span
+// [tile_lo + w*32P, +32P), lane l the points span_lo + l + 32k (k < P) so that stores are coalesced and every
+// 32 consecutive points belong to one k.  Lines of the tile's plan range are streamed through a double-buffered
+// shared-memory ring in chunks of CH by TMA bulk copies.  For every (line, warp span) the regime is chosen ONCE
+// from the span's distance to the line centre (float, grid units, conservative radii from a1): a warp-uniform
+// branch into an unrolled P-point loop of the 1-, 2- or 3-point rule.  Spans that reach inside the 3-point radius
+// or straddle a cutoff edge take the masked "near" path where each thread picks its own regime.
+// ------------------------------------------------------------------------------------------------------
+constexpr int CH = 128;  // lines per chunk: 3 x 4 KB per buffer
+
+struct VoigtArgs {
+  const LineMeta *meta;
+  const LineBase *base;
+  const LineGH2 *gh2;
+  const int2 *plan;
+  double nu_min, dnu;
+  int N;
+  double *kappa;
+};
+
+template <int P, int WARPS>
+__global__ void __launch_bounds__(WARPS * 32) voigt_kernel(VoigtArgs a)
+{
+  constexpr int TILE = WARPS * 32 * P;
+  __shared__ __align__(128) LineMeta s_meta[2][CH];
+  __shared__ __align__(128) LineBase s_base[2][CH];
+  __shared__ __align__(128) LineGH2 s_gh2[2][CH];
+  __shared__ __align__(8) uint64_t s_bar[2];
+
+  const int tile = blockIdx.x;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int2 pl = a.plan[tile];
+  const int L0 = pl.x, nl = pl.y - pl.x;
+  const int nchunks = (nl + CH - 1) / CH;
+  const int slo = tile * TILE + warp * (32 * P);
+  const int shi = slo + 32 * P - 1;
+  const float slo_f = (float)slo, shi_f = (float)shi;
+
+  if (threadIdx.x == 0) {
+    mbar_init(&s_bar[0], 1);
+    mbar_init(&s_bar[1], 1);
+    mbar_fence_init();
+  }
+  __syncthreads();
+
+  auto issue = [&](int c) {
+    const int buf = c & 1;
+    const int first = L0 + c * CH;
+    const int cnt = min(CH, nl - c * CH);
+    const uint32_t bytes = (uint32_t)cnt * 32u;
+    mbar_expect_tx(&s_bar[buf], 3u * bytes);
+    bulk_g2s(&s_meta[buf][0], a.meta + first, bytes, &s_bar[buf]);
+    bulk_g2s(&s_base[buf][0], a.base + first, bytes, &s_bar[buf]);
+    bulk_g2s(&s_gh2[buf][0], a.gh2 + first, bytes, &s_bar[buf]);
+  };
+  if (threadIdx.x == 0 && nchunks > 0) issue(0);
+
+  double acc[P], xk[P];
+#pragma unroll
+  for (int k = 0; k < P; ++k) {
+    acc[k] = 0.0;
+    xk[k] = __dadd_rn(a.nu_min, __dmul_rn((double)(slo + lane + 32 * k), a.dnu));  // nu_j exactly as defined
+  }
+
+  for (int c = 0; c < nchunks; ++c) {
+    const int buf = c & 1;
+    if (threadIdx.x == 0 && c + 1 < nchunks) issue(c + 1);  // buffer (c+1)&1 was released by the barrier below
+    mbar_wait(&s_bar[buf], (uint32_t)((c >> 1) & 1));
+    const int cnt = min(CH, nl - c * CH);
+#pragma unroll 1
+    for (int l = 0; l < cnt; ++l) {
+      const LineMeta m = s_meta[buf][l];
+      if (m.jhi < slo || m.jlo > shi) continue;
+      const bool inside = (m.jlo <= slo) && (m.jhi >= shi);
+      const float dist = fmaxf(fmaxf(slo_f - m.c, m.c - shi_f), 0.0f);
+      if (inside && dist >= m.r2) {
+        const double nu0 = s_base[buf][l].nu0, A1 = s_base[buf][l].A1;
+        if (dist >= m.r1) {
+          const double g2 = s_base[buf][l].g2;
+#pragma unroll
+          for (int k = 0; k < P; ++k) acc[k] = gh1_acc(acc[k], xk[k] - nu0, A1, g2);
+        } else {
+          const double e2 = s_gh2[buf][l].e2, f2 = s_gh2[buf][l].f2, A1a2 = s_gh2[buf][l].A1a2;
+#pragma unroll
+          for (int k = 0; k < P; ++k) acc[k] = gh2_acc(acc[k], xk[k] - nu0, A1, e2, f2, A1a2);
+        }
+      } else if (inside && dist >= m.r3) {
+        const LineBase b = s_base[buf][l];
+        const double e3 = b.g2 - 1.5 * b.a2, f3 = 6.0 * b.a2 * b.g2;
+        const double c3 = b.A1 * (1.0 / 3.0), c0 = 2.0 * c3, c3a = b.A1 * b.a2;
+#pragma unroll
+        for (int k = 0; k < P; ++k) acc[k] = gh3_acc(acc[k], xk[k] - b.nu0, b.g2, e3, f3, c0, c3, c3a);
+      } else {
+        // near path: cutoff edge inside the span and/or points inside the 3-point radius
+        const LineBase b = s_base[buf][l];
+        NearLine L;
+        L.nu0 = b.nu0; L.A1 = b.A1; L.g2 = b.g2; L.a2 = b.a2;
+        L.inv_alpha = s_gh2[buf][l].inv_alpha;
+        L.inv_a2 = L.inv_alpha * L.inv_alpha;
+        const double gamma = sqrt(b.g2);
+        L.y = gamma * L.inv_alpha;
+        L.Acore = b.A1 * kSqrtPi * L.inv_alpha / gamma;  // amp/(alpha sqrt(pi))
+        L.xc2 = (double)m.xc2;
+        bool core_ready = false;
+        CoreLine C;
+#pragma unroll 1
+        for (int k = 0; k < P; ++k) {
+          const int j = slo + lane + 32 * k;
+          const bool inwin = (j >= m.jlo) && (j <= m.jhi);
+          const double d = __dadd_rn(a.nu_min, __dmul_rn((double)j, a.dnu)) - L.nu0;
+          double v = wing_value(d, L);
+          const double x = fabs(d) * L.inv_alpha;
+          const bool incore = inwin && (x * x < L.xc2);
+          if (__any_sync(kFull, incore)) {  // warp-uniform
+            if (!core_ready) {
+              C = core_setup(L.y, sqrt(L.xc2));
+              core_ready = true;
+            }
+            const double kc = core_K(fmin(x, 17.0), C);
+            if (incore) v = L.Acore * kc;
+          }
+          v = inwin ? v : 0.0;
+#pragma unroll
+          for (int kk = 0; kk < P; ++kk)
+            if (kk == k) acc[kk] += v;
+        }
+      }
+    }
+    __syncthreads();  // every warp is done with buffer `buf` before chunk c+2 overwrites it
+  }
+
+#pragma unroll
+  for (int k = 0; k < P; ++k) {
+    const int j = slo + lane + 32 * k;
+    if (j < a.N) a.kappa[j] = acc[k];
+  }
+}
+
+// test hook: out = K(x,y) through the same device functions and switches (alpha = 1, gamma = y, amp = sqrt(pi))
+__global__ void __launch_bounds__(128) voigt_K_kernel(const double *x, const double *y, int64_t n, double *out)
+{
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const bool live = i < n;
+  const double xi = live ? fabs(x[i]) : 1.0e3, yi = live ? y[i] : 1.0;
+  const int lane = threadIdx.x & 31;
+  NearLine L;
+  L.nu0 = 0.0; L.a2 = 1.0; L.inv_alpha = 1.0; L.inv_a2 = 1.0;
+  L.g2 = yi * yi; L.y = yi;
+  L.A1 = yi * kInvSqrtPi;  // amp*gamma/pi with amp = sqrt(pi)  =>  amp*V = K
+  L.Acore = 1.0;
+  L.xc2 = core_xc2(yi);
+  double v = wing_value(xi, L);
+  const bool incore = live && (xi * xi < L.xc2);
+  unsigned need = __ballot_sync(kFull, incore);
+  while (need) {  // the series is warp-collective with a warp-uniform y: serve one lane at a time
+    const int src = __ffs(need) - 1;
+    need &= need - 1;
+    const double ys = __shfl_sync(kFull, yi, src), xs = __shfl_sync(kFull, xi, src);
+    const CoreLine C = core_setup(ys, sqrt(core_xc2(ys)));
+    const double kc = core_K(fmin(xs, 17.0), C);
+    if (lane == src) v = kc;
+  }
+  if (live) out[i] = v;
+}
+
+// ------------------------------------------------------------------------------------------------------
+// a5 + a6: per-bin sort and resampling.  One CTA per bin; the bin is loaded into shared memory, padded with +inf
+// to a power of two, sorted by a bitonic network, and read at the Gauss-Legendre nodes.
+// ------------------------------------------------------------------------------------------------------
+struct KdistArgs {
+  const double *kappa;
+  double *k_out;
+  int ppb, ppb2, n_g;
+  double g[128];
+};
+
+__global__ void __launch_bounds__(512) kdist_kernel(const __grid_constant__ KdistArgs a)
+{
+  extern __shared__ __align__(16) double s[];
+  const int bin = blockIdx.x;
+  const double *src = a.kappa + (int64_t)bin * a.ppb;
+  for (int i = threadIdx.x; i < a.ppb2; i += blockDim.x)
+    s[i] = i < a.ppb ? src[i] : __longlong_as_double(0x7ff0000000000000LL);
+  __syncthreads();
+  for (int k = 2; k <= a.ppb2; k <<= 1) {
+    for (int j = k >> 1; j > 0; j >>= 1) {
+      for (int t = threadIdx.x; t < (a.ppb2 >> 1); t += blockDim.x) {
+        const int i = ((t & ~(j - 1)) << 1) | (t & (j - 1));  // index with bit j clear
+        const int p = i | j;
+        const double u = s[i], v = s[p];
+        const bool up = (i & k) == 0;
+        if ((u > v) == up) { s[i] = v; s[p] = u; }
+      }
+      __syncthreads();
+    }
+  }
+  for (int q = threadIdx.x; q < a.n_g; q += blockDim.x) {
+    const double p = __dadd_rn(__dmul_rn(a.g[q], (double)a.ppb), -0.5);
+    double v;
+    if (p <= 0.0) v = s[0];
+    else if (p >= (double)(a.ppb - 1)) v = s[a.ppb - 1];
+    else {
+      const int k = (int)floor(p);
+      const double f = p - (double)k;
+      v = s[k] + f * (s[k + 1] - s[k]);
+    }
+    a.k_out[(int64_t)bin * a.n_g + q] = v;
+  }
+}
+
+__global__ void __launch_bounds__(256) check_sorted_kernel(const double *nu0, int64_t n, int *flag)
+{
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i + 1 < n && !(nu0[i] <= nu0[i + 1])) *flag = 1;
+}
+
+__global__ void __launch_bounds__(256) dfma_peak_kernel(double *out, int iters, double a, double b)
+{
+  double v[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) v[i] = threadIdx.x * 1e-3 + i;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) v[i] = fma(v[i], a, b);
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) s += v[i];
+  if (s == 123.456) out[0] = s;
+}
+
+// ------------------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------------------
+static thread_local char g_cuda_err[256] = "";
+static thread_local float g_stage_ms[3] = {0.f, 0.f, 0.f};
+static int g_timing = 0;
+
+static int cuda_fail(cudaError_t e, const char *what)
+{
+  snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", what, cudaGetErrorString(e));
+  return e == cudaErrorMemoryAllocation ? HK_ERR_NOMEM : HK_ERR_CUDA;
+}
+#define HK_CUDA(call)                                  \
+  do {                                                 \
+    cudaError_t e_ = (call);                           \
+    if (e_ != cudaSuccess) return cuda_fail(e_, #call); \
+  } while (0)
+
+static bool pos_finite(double v) { return v > 0.0 && isfinite(v); }
+
+constexpr int kP = 8, kWarps = 8;
+constexpr int kTile = kP * kWarps * 32;
+
+struct Scratch {
+  LineMeta *meta = nullptr;
+  LineBase *base = nullptr;
+  LineGH2 *gh2 = nullptr;
+  int2 *plan = nullptr;
+  int64_t cap_lines = 0;
+  int cap_tiles = 0;
+};
+
+static int scratch_reserve(Scratch &s, int64_t n_lines, int n_tiles, cudaStream_t st, bool pooled)
+{
+  if (n_lines > s.cap_lines) {
+    if (s.meta) {
+      if (pooled) { cudaFreeAsync(s.meta, st); cudaFreeAsync(s.base, st); cudaFreeAsync(s.gh2, st); }
+      else { cudaFree(s.meta); cudaFree(s.base); cudaFree(s.gh2); }
+      s.meta = nullptr; s.cap_lines = 0;
+    }
+    const size_t bytes = (size_t)n_lines * 32;
+    if (pooled) {
+      HK_CUDA(cudaMallocAsync(&s.meta, bytes, st));
+      HK_CUDA(cudaMallocAsync(&s.base, bytes, st));
+      HK_CUDA(cudaMallocAsync(&s.gh2, bytes, st));
+    } else {
+      HK_CUDA(cudaMalloc(&s.meta, bytes));
+      HK_CUDA(cudaMalloc(&s.base, bytes));
+      HK_CUDA(cudaMalloc(&s.gh2, bytes));
+    }
+    s.cap_lines = n_lines;
+  }
+  if (n_tiles > s.cap_tiles) {
+    if (s.plan) { if (pooled) cudaFreeAsync(s.plan, st); else cudaFree(s.plan); s.plan = nullptr; }
+    if (pooled) HK_CUDA(cudaMallocAsync(&s.plan, (size_t)n_tiles * sizeof(int2), st));
+    else HK_CUDA(cudaMalloc(&s.plan, (size_t)n_tiles * sizeof(int2)));
+    s.cap_tiles = n_tiles;
+  }
+  return HK_OK;
+}
+
+static void scratch_release(Scratch &s, cudaStream_t st, bool pooled)
+{
+  if (s.meta) { if (pooled) { cudaFreeAsync(s.meta, st); cudaFreeAsync(s.base, st); cudaFreeAsync(s.gh2, st); } else { cudaFree(s.meta); cudaFree(s.base); cudaFree(s.gh2); } }
+  if (s.plan) { if (pooled) cudaFreeAsync(s.plan, st); else cudaFree(s.plan); }
+  s = Scratch();
+}
+
+static int validate(const hk_lines *lines, int64_t n_lines, double T, double P_atm, double nu_min, double nu_max, double dnu,
+                    double cutoff, const double *kappa_out, const hk_params *prm, int64_t *N_out)
+{
+  if (!lines || !prm || !kappa_out || n_lines < 0) return HK_ERR_INVALID;
+  if (n_lines > 0 && (!lines->nu0 || !lines->S || !lines->gamma0)) return HK_ERR_INVALID;
+  if (n_lines > 2000000000LL) return HK_ERR_UNSUPPORTED;
+  if (!pos_finite(T) || !pos_finite(P_atm) || !pos_finite(dnu) || !pos_finite(cutoff) || !pos_finite(prm->mass_amu))
+    return HK_ERR_INVALID;
+  if (!isfinite(nu_min) || !isfinite(nu_max)) return HK_ERR_INVALID;
+  if (prm->precision == HK_FP32) return HK_ERR_UNSUPPORTED;
+  if (prm->precision != HK_FP64) return HK_ERR_INVALID;
+  if (lines->E_low && !pos_finite(prm->q_ratio)) return HK_ERR_INVALID;
+  const int64_t N = hk_grid_size(nu_min, nu_max, dnu);
+  if (N < 1 || N > (1LL << 30)) return HK_ERR_INVALID;
+  *N_out = N;
+  return HK_OK;
+}
+
+static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double P_atm, double q_ratio, double mass_amu,
+                       double nu_min, double dnu, double cutoff, int64_t N, double *kappa_out, Scratch &s, cudaStream_t st,
+                       bool pooled)
+{
+  if (n_lines == 0) {
+    HK_CUDA(cudaMemsetAsync(kappa_out, 0, (size_t)N * sizeof(double), st));
+    return HK_OK;
+  }
+  const int n_tiles = (int)((N + kTile - 1) / kTile);
+  int rc = scratch_reserve(s, n_lines, n_tiles, st, pooled);
+  if (rc != HK_OK) return rc;
+
+  cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+  if (g_timing) {
+    for (auto &e : ev) HK_CUDA(cudaEventCreate(&e));
+    HK_CUDA(cudaEventRecord(ev[0], st));
+  }
+  PrepArgs pa;
+  pa.nu0 = lines->nu0; pa.S = lines->S; pa.gamma0 = lines->gamma0; pa.n_T = lines->n_T; pa.E_low = lines->E_low;
+  pa.n = n_lines;
+  pa.T = T; pa.P_atm = P_atm; pa.tfac_half = pow(kT0 / T, 0.5);
+  const double m_g = mass_amu * kAmu;
+  pa.vth = sqrt(2.0 * kBoltz * T / m_g) / kCLight;
+  pa.inv_mg = 1.0 / m_g;
+  pa.q_ratio = q_ratio;
+  pa.nu_min = nu_min; pa.dnu = dnu; pa.cutoff = cutoff; pa.N = (int)N;
+  pa.meta = s.meta; pa.base = s.base; pa.gh2 = s.gh2;
+  line_prep_kernel<<<(unsigned)((n_lines + 255) / 256), 256, 0, st>>>(pa);
+  HK_CUDA(cudaGetLastError());
+  if (g_timing) HK_CUDA(cudaEventRecord(ev[1], st));
+  tile_plan_kernel<<<(n_tiles + 127) / 128, 128, 0, st>>>(s.meta, n_lines, n_tiles, kTile, (int)N, s.plan);
+  HK_CUDA(cudaGetLastError());
+  if (g_timing) HK_CUDA(cudaEventRecord(ev[2], st));
+  VoigtArgs va;
+  va.meta = s.meta; va.base = s.base; va.gh2 = s.gh2; va.plan = s.plan;
+  va.nu_min = nu_min; va.dnu = dnu; va.N = (int)N; va.kappa = kappa_out;
+  voigt_kernel<kP, kWarps><<<n_tiles, kWarps * 32, 0, st>>>(va);
+  HK_CUDA(cudaGetLastError());
+  if (g_timing) {
+    HK_CUDA(cudaEventRecord(ev[3], st));
+    HK_CUDA(cudaEventSynchronize(ev[3]));
+    for (int i = 0; i < 3; ++i) HK_CUDA(cudaEventElapsedTime(&g_stage_ms[i], ev[i], ev[i + 1]));
+    for (auto &e : ev) cudaEventDestroy(e);
+  }
+  return HK_OK;
+}
+
+}  // namespace hk
+
+using namespace hk;
+
+struct hk_ctx {
+  hk_lines lines;
+  int64_t n_lines;
+  hk_params prm;
+  Scratch scratch;
+};
+
+extern "C" {
+
+int64_t hk_grid_size(double nu_min, double nu_max, double dnu)
+{
+  if (!(dnu > 0.0) || !isfinite(nu_min) || !isfinite(nu_max)) return -1;
+  const double n = (nu_max - nu_min) / dnu;
+  if (!(n < 9.0e18) || !(n > -9.0e18)) return -1;
+  return (int64_t)llround(n);
+}
+
+int hk_opacity(const hk_lines *lines, int64_t n_lines, double T, double P_atm, double nu_min, double nu_max, double dnu,
+               double cutoff, double *kappa_out, const hk_params *prm)
+{
+  int64_t N = 0;
+  int rc = validate(lines, n_lines, T, P_atm, nu_min, nu_max, dnu, cutoff, kappa_out, prm, &N);
+  if (rc != HK_OK) return rc;
+  if (!prm->lines_sorted && n_lines > 1) {
+    rc = hk_lines_check_sorted(lines->nu0, n_lines, prm->stream);
+    if (rc == HK_ERR_UNSORTED) return HK_ERR_UNSUPPORTED;  // TODO(round 1): device sort of a copy
+    if (rc != HK_OK) return rc;
+  }
+  cudaStream_t st = (cudaStream_t)prm->stream;
+  Scratch s;
+  rc = run_opacity(lines, n_lines, T, P_atm, prm->q_ratio, prm->mass_amu, nu_min, dnu, cutoff, N, kappa_out, s, st, true);
+  scratch_release(s, st, true);
+  return rc;
+}
+
+int hk_create(const hk_lines *lines, int64_t n_lines, const hk_params *prm, hk_ctx **out)
+{
+  if (!lines || !prm || !out || n_lines < 0) return HK_ERR_INVALID;
+  if (n_lines > 0 && (!lines->nu0 || !lines->S || !lines->gamma0)) return HK_ERR_INVALID;
+  if (!pos_finite(prm->mass_amu)) return HK_ERR_INVALID;
+  if (prm->precision == HK_FP32) return HK_ERR_UNSUPPORTED;
+  if (prm->precision != HK_FP64) return HK_ERR_INVALID;
+  if (!prm->lines_sorted && n_lines > 1) {
+    int rc = hk_lines_check_sorted(lines->nu0, n_lines, prm->stream);
+    if (rc == HK_ERR_UNSORTED) return HK_ERR_UNSUPPORTED;
+    if (rc != HK_OK) return rc;
+  }
+  hk_ctx *c = new (std::nothrow) hk_ctx();
+  if (!c) return HK_ERR_NOMEM;
+  c->lines = *lines;
+  c->n_lines = n_lines;
+  c->prm = *prm;
+  *out = c;
+  return HK_OK;
+}
+
+int hk_opacity_ctx(hk_ctx *ctx, double T, double P_atm, double q_ratio, double nu_min, double nu_max, double dnu,
+                   double cutoff, double *kappa_out)
+{
+  if (!ctx) return HK_ERR_INVALID;
+  hk_params p = ctx->prm;
+  p.q_ratio = q_ratio;
+  int64_t N = 0;
+  int rc = validate(&ctx->lines, ctx->n_lines, T, P_atm, nu_min, nu_max, dnu, cutoff, kappa_out, &p, &N);
+  if (rc != HK_OK) return rc;
+  return run_opacity(&ctx->lines, ctx->n_lines, T, P_atm, q_ratio, p.mass_amu, nu_min, dnu, cutoff, N, kappa_out,
+                     ctx->scratch, (cudaStream_t)p.stream, false);
+}
+
+int hk_destroy(hk_ctx *ctx)
+{
+  if (!ctx) return HK_ERR_INVALID;
+  cudaStreamSynchronize((cudaStream_t)ctx->prm.stream);
+  scratch_release(ctx->scratch, (cudaStream_t)ctx->prm.stream, false);
+  delete ctx;
+  return HK_OK;
+}
+
+int hk_lines_check_sorted(const double *nu0_device, int64_t n_lines, void *stream)
+{
+  if (n_lines < 0 || (n_lines > 0 && !nu0_device)) return HK_ERR_INVALID;
+  if (n_lines < 2) return HK_OK;
+  cudaStream_t st = (cudaStream_t)stream;
+  int *flag = nullptr;
+  HK_CUDA(cudaMallocAsync(&flag, sizeof(int), st));
+  HK_CUDA(cudaMemsetAsync(flag, 0, sizeof(int), st));
+  check_sorted_kernel<<<(unsigned)((n_lines + 255) / 256), 256, 0, st>>>(nu0_device, n_lines, flag);
+  int h = 0;
+  cudaError_t e = cudaMemcpyAsync(&h, flag, sizeof(int), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  cudaFreeAsync(flag, st);
+  if (e != cudaSuccess) return cuda_fail(e, "check_sorted");
+  return h ? HK_ERR_UNSORTED : HK_OK;
+}
+
+int64_t hk_count_evals(const double *nu0_host, int64_t n_lines, double nu_min, int64_t N, double dnu, double cutoff)
+{
+  if (!nu0_host || n_lines < 0 || N < 1 || !(dnu > 0.0) || !(cutoff > 0.0)) return -1;
+  int64_t total = 0;
+  for (int64_t i = 0; i < n_lines; ++i) {
+    double lo = ceil(((nu0_host[i] - cutoff) - nu_min) / dnu);
+    double hi = floor(((nu0_host[i] + cutoff) - nu_min) / dnu);
+    if (!(lo > 0.0)) lo = 0.0;
+    if (!(hi < (double)(N - 1))) hi = (double)(N - 1);
+    if (hi >= lo) total += (int64_t)hi - (int64_t)lo + 1;
+  }
+  return total;
+}
+
+int hk_gauss_legendre(int n_g, double *g, double *w)
+{
+  if (n_g < 1 || n_g > 4096 || !g || !w) return HK_ERR_INVALID;
+  // roots of P_n on (-1,1) by Newton from the asymptotic guess, symmetric pairs; mapped to (0,1)
+  const long double pi = 3.14159265358979323846264338327950288L;
+  const int half = (n_g + 1) / 2;
+  for (int i = 0; i < half; ++i) {
+    long double z = cosl(pi * (i + 0.75L) / (n_g + 0.5L));
+    long double dp = 1.0L;
+    for (int it = 0; it < 64; ++it) {
+      long double pm = 1.0L, pc = z;  // P_0, P_1
+      for (int k = 2; k <= n_g; ++k) {
+        const long double pn = ((2 * k - 1) * z * pc - (k - 1) * pm) / k;
+        pm = pc; pc = pn;
+      }
+      if (n_g == 1) { pm = 1.0L; pc = z; }
+      dp = n_g * (z * pc - pm) / (z * z - 1.0L);
+      const long double dz = pc / dp;
+      z -= dz;
+      if (fabsl(dz) < 1e-19L) {
+        long double qm = 1.0L, qc = z;
+        for (int k = 2; k <= n_g; ++k) {
+          const long double qn = ((2 * k - 1) * z * qc - (k - 1) * qm) / k;
+          qm = qc; qc = qn;
+        }
+        dp = n_g * (z * qc - qm) / (z * z - 1.0L);
+        break;
+      }
+    }
+    const long double wt = 1.0L / ((1.0L - z * z) * dp * dp);  // half of 2/((1-z^2) P'^2): weights on (0,1)
+    g[n_g - 1 - i] = (double)(0.5L * (1.0L + z));
+    g[i] = (double)(0.5L * (1.0L - z));
+    w[n_g - 1 - i] = (double)wt;
+    w[i] = (double)wt;
+  }
+  return HK_OK;
+}
+
+int hk_kdist(const double *kappa, int64_t n_points, double dnu, double bin_width, int n_g, double *k_out, void *stream)
+{
+  if (!kappa || !k_out || n_points < 1 || !pos_finite(dnu) || !pos_finite(bin_width) || n_g < 1 || n_g > 128)
+    return HK_ERR_INVALID;
+  const double ratio = bin_width / dnu;
+  const double ppb_d = nearbyint(ratio);
+  if (ppb_d < 1.0 || fabs(ratio - ppb_d) > 1e-9 * ppb_d) return HK_ERR_INVALID;
+  if (ppb_d > 16384.0) return HK_ERR_UNSUPPORTED;
+  const int ppb = (int)ppb_d;
+  if (n_points % ppb != 0) return HK_ERR_INVALID;
+  const int64_t n_bins = n_points / ppb;
+  if (n_bins > 2147483647LL) return HK_ERR_UNSUPPORTED;
+  KdistArgs a;
+  a.kappa = kappa; a.k_out = k_out; a.ppb = ppb; a.n_g = n_g;
+  int p2 = 2;
+  while (p2 < ppb) p2 <<= 1;
+  a.ppb2 = p2;
+  double wts[128];
+  int rc = hk_gauss_legendre(n_g, a.g, wts);
+  if (rc != HK_OK) return rc;
+  const size_t smem = (size_t)p2 * sizeof(double);
+  static bool attr_set = false;
+  if (!attr_set) {
+    HK_CUDA(cudaFuncSetAttribute(kdist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 16384 * 8));
+    attr_set = true;
+  }
+  int threads = p2 / 2 < 64 ? 64 : (p2 / 2 > 512 ? 512 : p2 / 2);
+  kdist_kernel<<<(unsigned)n_bins, threads, smem, (cudaStream_t)stream>>>(a);
+  HK_CUDA(cudaGetLastError());
+  return HK_OK;
+}
+
+int hk_voigt_K(const double *x, const double *y, int64_t n, double *out, int precision, void *stream)
+{
+  if (n < 0 || (n > 0 && (!x || !y || !out))) return HK_ERR_INVALID;
+  if (precision == HK_FP32) return HK_ERR_UNSUPPORTED;
+  if (precision != HK_FP64) return HK_ERR_INVALID;
+  if (n == 0) return HK_OK;
+  voigt_K_kernel<<<(unsigned)((n + 127) / 128), 128, 0, (cudaStream_t)stream>>>(x, y, n, out);
+  HK_CUDA(cudaGetLastError());
+  return HK_OK;
+}
+
+int hk_fp64_peak(double *inst_per_s_out, void *stream)
+{
+  if (!inst_per_s_out) return HK_ERR_INVALID;
+  cudaStream_t st = (cudaStream_t)stream;
+  int dev = 0, sms = 0;
+  HK_CUDA(cudaGetDevice(&dev));
+  HK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  double *buf = nullptr;
+  HK_CUDA(cudaMallocAsync(&buf, 64, st));
+  cudaEvent_t e0, e1;
+  HK_CUDA(cudaEventCreate(&e0));
+  HK_CUDA(cudaEventCreate(&e1));
+  const int iters = 20000, grid = sms * 4, thr = 256;
+  float best = 1e30f;
+  for (int r = 0; r < 4; ++r) {
+    HK_CUDA(cudaEventRecord(e0, st));
+    dfma_peak_kernel<<<grid, thr, 0, st>>>(buf, iters, 1.0000001, 1e-9);
+    HK_CUDA(cudaEventRecord(e1, st));
+    HK_CUDA(cudaEventSynchronize(e1));
+    float ms = 0.f;
+    HK_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+    if (r > 0 && ms < best) best = ms;
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFreeAsync(buf, st);
+  *inst_per_s_out = (double)grid * thr * (double)iters * 8.0 / (best * 1e-3);
+  return HK_OK;
+}
+
+int hk_set_timing(int on)
+{
+  g_timing = on ? 1 : 0;
+  return HK_OK;
+}
+
+int hk_last_stage_ms(float ms_out[3])
+{
+  if (!ms_out) return HK_ERR_INVALID;
+  for (int i = 0; i < 3; ++i) ms_out[i] = g_stage_ms[i];
+  return HK_OK;
+}
+
+const char *hk_strerror(int code)
+{
+  switch (code) {
+    case HK_OK: return "ok";
+    case HK_ERR_INVALID: return "invalid argument";
+    case HK_ERR_CUDA: return "CUDA runtime error";
+    case HK_ERR_NOMEM: return "out of memory";
+    case HK_ERR_UNSORTED: return "line centres are not ascending";
+    case HK_ERR_UNSUPPORTED: return "unsupported request";
+    default: return "unknown error";
+  }
+}
+
+const char *hk_last_cuda_error(void) { return g_cuda_err; }
+const char *hk_version(void) { return "hk 0.1 (sm_100a)"; }
+
+}  // extern "C"

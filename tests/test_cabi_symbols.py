@@ -1,0 +1,83 @@
+"""The C-ABI library loads and exports every symbol include/hk.h declares; host-only entry points work (no GPU)."""
+import ctypes
+import os
+
+import numpy as np
+import pytest
+
+import paper_1503_03806_b200 as hk
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_1503_03806_b200.build import build_library
+    build_library()
+    return hk.load_library()
+
+
+def test_exports_every_declared_symbol(lib):
+    names = hk.declared_symbols()
+    assert {"hk_opacity", "hk_kdist", "hk_voigt_K", "hk_gauss_legendre", "hk_count_evals", "hk_grid_size",
+            "hk_create", "hk_opacity_ctx", "hk_destroy", "hk_strerror"} <= set(names)
+    for n in names:
+        assert hasattr(lib, n), n
+
+
+def test_sass_is_sm100a_with_tma_bulk_copy(lib):
+    import shutil
+    import subprocess
+    cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(cuobjdump):
+        pytest.skip("cuobjdump not available")
+    from paper_1503_03806_b200._binding import LIB_PATH
+    out = subprocess.run([cuobjdump, "-sass", LIB_PATH], capture_output=True, text=True).stdout
+    assert "sm_100a" in out
+    assert "UBLKCP" in out          # cp.async.bulk (1-D TMA) stages the line records
+    assert "MUFU.RCP64H" in out     # FP64 reciprocal seed
+    assert "DFMA" in out
+
+
+def test_grid_size_host():
+    assert hk.hk_grid_size(0.0, 3000.0, 0.01) == 300000
+    assert hk.hk_grid_size(0.0, 30000.0, 0.01) == 3000000
+    assert hk.hk_grid_size(0.0, 1.0, 0.0) == -1
+
+
+def test_gauss_legendre_host():
+    for n in (1, 2, 3, 20, 64, 128):
+        g, w = hk.hk_gauss_legendre(n)
+        t, wt = np.polynomial.legendre.leggauss(n)
+        assert np.abs(g - 0.5 * (1 + t)).max() < 1e-15
+        assert np.abs(w - 0.5 * wt).max() < 1e-14
+        assert abs(w.sum() - 1.0) < 1e-14
+    g, w = hk.hk_gauss_legendre(20)
+    for p in range(40):
+        assert abs(np.sum(w * g ** p) - 1.0 / (p + 1)) < 1e-14
+    with pytest.raises(hk.HKError):
+        hk.hk_gauss_legendre(0)
+
+
+def test_count_evals_host_bruteforce():
+    rng = np.random.default_rng(0)
+    nu0 = rng.uniform(-30.0, 130.0, 500)
+    N, dnu, cutoff = 10000, 0.01, 25.0
+    nu = np.arange(N) * dnu
+    brute = sum(int(np.count_nonzero(np.abs(nu - c) <= cutoff)) for c in nu0)
+    assert hk.hk_count_evals(nu0, 0.0, N, dnu, cutoff) == brute
+    assert hk.hk_count_evals([50.0], 0.0, N, dnu, cutoff) == 5001
+
+
+def test_strerror_and_version():
+    assert hk.hk_strerror(0) == "ok"
+    assert "invalid" in hk.hk_strerror(-1)
+    assert "sm_100a" in hk.hk_version()
+
+
+def test_compute_call_without_gpu_fails_loudly():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    with pytest.raises(RuntimeError):
+        hk.hk_fp64_peak()
+    with pytest.raises(RuntimeError):
+        hk.Lines.from_numpy([1.0], [1.0], [0.05])

@@ -1,0 +1,180 @@
+"""Parity of hk_opacity (C ABI, CUDA) against the oracle on the same seeded inputs.
+
+Bar (BASELINE.json north_star): max relative error <= 1e-6 at grid points with kappa >= 1e-12 * max(kappa).
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+import oracle
+import workloads
+import paper_1503_03806_b200 as hk
+
+BAR = 1.0e-6
+
+
+def _gpu_kappa(wl, T, P, q_ratio=1.0, **kw):
+    import torch
+    lines = hk.Lines.from_numpy(wl.nu0, wl.S, wl.gamma0, E_low=wl.E_low)
+    k = hk.hk_opacity(lines, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, mass_amu=wl.mass_amu, q_ratio=q_ratio, **kw)
+    torch.cuda.synchronize()
+    return k.cpu().numpy()
+
+
+def _check(got, ref, ref_max=None):
+    ref_max = ref.max() if ref_max is None else ref_max
+    mask = ref >= 1e-12 * ref_max
+    assert np.all(np.isfinite(got))
+    rel = np.abs(got[mask] / ref[mask] - 1.0)
+    assert rel.max() <= BAR, (rel.max(), np.flatnonzero(mask)[np.argmax(rel)])
+    assert np.all(got[ref == 0.0] == 0.0)
+    return rel.max()
+
+
+def test_config0_full_grid():
+    wl = workloads.config(0)
+    T, P = wl.T[0], wl.P_atm[0]
+    got = _gpu_kappa(wl, T, P)
+    ref = oracle.opacity(wl.nu0, wl.S, wl.gamma0, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff)
+    assert got.shape == ref.shape == (300000,)
+    _check(got, ref)
+
+
+@pytest.mark.parametrize("n_lines,nu_max,cutoff,T,P", [
+    (1, 40.0, 25.0, 1500.0, 1.0),
+    (50, 33.33, 7.0, 300.0, 1e-3),        # ragged: N = 3333 is not a multiple of the tile or the warp span
+    (400, 123.45, 25.0, 2500.0, 10.0),
+    (2000, 250.0, 100.0, 1000.0, 1e-5),   # Doppler-dominated: tiny y, series region
+    (300, 60.0, 25.0, 800.0, 100.0),      # Lorentz-dominated: y >> 1
+])
+def test_small_cases_full_grid(n_lines, nu_max, cutoff, T, P):
+    wl = workloads.small(seed=n_lines, n_lines=n_lines, nu_max=nu_max, cutoff=cutoff, T=T, P_atm=P)
+    got = _gpu_kappa(wl, T, P)
+    ref = oracle.opacity(wl.nu0, wl.S, wl.gamma0, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff)
+    _check(got, ref)
+
+
+def test_lines_far_up_the_spectrum_small_alpha_to_large_alpha():
+    # same draw shifted to 20000-20100 cm^-1: alpha ~ 0.08, several regimes per tile
+    wl = workloads.small(seed=77, n_lines=500, nu_max=100.0, cutoff=25.0)
+    wl.nu0 = wl.nu0 + 20000.0
+    wl.nu_min, wl.nu_max = 20000.0, 20100.0
+    T, P = 1500.0, 1.0
+    got = _gpu_kappa(wl, T, P)
+    ref = oracle.opacity(wl.nu0, wl.S, wl.gamma0, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff)
+    _check(got, ref)
+
+
+def test_window_semantics_bit_exact_support():
+    import torch
+    # a line exactly on a grid node with cutoff an exact multiple of dnu; one outside the grid within the cutoff;
+    # one beyond the cutoff; one at nu0 = 0 (alpha = 0: Lorentzian)
+    nu0 = np.array([-10.0, 0.0, 50.0, 130.0])
+    S = np.full(4, 1e-20)
+    g0 = np.full(4, 0.05)
+    lines = hk.Lines.from_numpy(nu0, S, g0)
+    for sel in ([2], [0], [3], [1], [0, 1, 2, 3]):
+        sub = hk.Lines.from_numpy(nu0[sel], S[sel], g0[sel])
+        got = hk.hk_opacity(sub, 1000.0, 1.0, 0.0, 100.0, 0.01, 25.0).cpu().numpy()
+        ref = oracle.opacity(nu0[sel], S[sel], g0[sel], 1000.0, 1.0, 0.0, 100.0, 0.01, 25.0)
+        assert np.array_equal(got != 0.0, ref != 0.0), sel          # support: index work is bit-exact
+        if ref.any():
+            _check(got, ref)
+    got = hk.hk_opacity(hk.Lines.from_numpy(nu0[[2]], S[[2]], g0[[2]]), 1000.0, 1.0, 0.0, 100.0, 0.01, 25.0).cpu().numpy()
+    nz = np.flatnonzero(got)
+    assert nz[0] == 2500 and nz[-1] == 7500 and nz.size == 5001
+    torch.cuda.synchronize()
+
+
+def test_no_lines_gives_zero():
+    import torch
+    empty = hk.Lines(torch.empty(0, dtype=torch.float64, device="cuda"), torch.empty(0, dtype=torch.float64, device="cuda"),
+                     torch.empty(0, dtype=torch.float64, device="cuda"))
+    out = torch.full((1000,), 7.0, dtype=torch.float64, device="cuda")
+    hk.hk_opacity(empty, 1000.0, 1.0, 0.0, 10.0, 0.01, 25.0, out=out)
+    assert not out.cpu().numpy().any()
+
+
+def test_deterministic_bitwise():
+    wl = workloads.small(seed=3, n_lines=3000, nu_max=200.0, cutoff=25.0)
+    a = _gpu_kappa(wl, 1500.0, 1.0)
+    b = _gpu_kappa(wl, 1500.0, 1.0)
+    assert np.array_equal(a, b)
+
+
+def test_line_strength_scaling_path():
+    wl = workloads.small(seed=9, n_lines=600, nu_max=120.0, cutoff=25.0, with_E=True, T=900.0)
+    for T in (500.0, 900.0, 3000.0):
+        q = wl.q_ratio(T)
+        got = _gpu_kappa(wl, T, 1.0, q_ratio=q)
+        ref = oracle.opacity(wl.nu0, wl.S, wl.gamma0, T, 1.0, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, E_low=wl.E_low, q_ratio=q)
+        _check(got, ref)
+
+
+def test_context_form_matches_one_shot():
+    import torch
+    wl = workloads.small(seed=4, n_lines=800, nu_max=150.0, cutoff=25.0, with_E=True)
+    lines = hk.Lines.from_numpy(wl.nu0, wl.S, wl.gamma0, E_low=wl.E_low)
+    ctx = hk.Context(lines, mass_amu=18.0)
+    for T, P in ((700.0, 0.1), (2000.0, 5.0)):
+        q = wl.q_ratio(T)
+        a = ctx.opacity(T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, q_ratio=q)
+        b = hk.hk_opacity(lines, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, q_ratio=q)
+        torch.cuda.synchronize()
+        assert torch.equal(a, b)
+    ctx.close()
+
+
+def test_error_codes():
+    import torch
+    lines = hk.Lines.from_numpy([1.0, 2.0], [1e-20, 1e-20], [0.05, 0.05])
+    bad = [dict(T=-1.0), dict(P_atm=0.0), dict(dnu=0.0), dict(cutoff=-5.0), dict(mass_amu=0.0), dict(T=float("nan"))]
+    base = dict(T=1000.0, P_atm=1.0, nu_min=0.0, nu_max=10.0, dnu=0.01, cutoff=25.0, mass_amu=18.0)
+    for b in bad:
+        kw = dict(base)
+        kw.update(b)
+        with pytest.raises(hk.HKError) as e:
+            hk.hk_opacity(lines, kw["T"], kw["P_atm"], kw["nu_min"], kw["nu_max"], kw["dnu"], kw["cutoff"],
+                          mass_amu=kw["mass_amu"], out=torch.empty(1000, dtype=torch.float64, device="cuda"))
+        assert e.value.code == -1
+    with pytest.raises(hk.HKError) as e:
+        hk.hk_opacity(lines, 1000.0, 1.0, 0.0, 10.0, 0.01, 25.0, precision=hk.HK_FP32)
+    assert e.value.code == -5
+    with pytest.raises(hk.HKError):
+        hk.hk_opacity(lines, 1000.0, 1.0, 10.0, 0.0, 0.01, 25.0, out=torch.empty(1, dtype=torch.float64, device="cuda"))
+    assert hk.hk_lines_check_sorted(lines.nu0)
+    assert not hk.hk_lines_check_sorted(torch.tensor([2.0, 1.0], dtype=torch.float64, device="cuda"))
+
+
+def test_config1_full_size_sampled_bins():
+    # the configuration bench.py times: 1e5 lines, 3e6 points, cutoff 100; oracle on 24 seeded bins of 1000 points
+    wl = workloads.config(1)
+    T, P = wl.T[0], wl.P_atm[0]
+    got = _gpu_kappa(wl, T, P)
+    assert got.shape == (3_000_000,)
+    rng = np.random.default_rng(1)
+    bins = np.sort(rng.choice(3000, 24, replace=False))
+    bins[0], bins[-1] = 0, 2999                                   # include both ends of the grid
+    js = (bins[:, None] * 1000 + np.arange(1000)[None, :]).ravel()
+    ref = oracle.opacity_points(wl.nu0, wl.S, wl.gamma0, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, js)
+    _check(got[js], ref, ref_max=max(ref.max(), got.max()))
+    assert got.min() > 0.0
+
+
+def test_config2_pressure_sweep_sampled_points():
+    # 1e6 lines, six pressures from Doppler- to Lorentz-dominated; oracle at 1500 seeded points per pressure
+    wl = workloads.config(2)
+    T = wl.T[0]
+    rng = np.random.default_rng(2)
+    js = np.sort(rng.choice(wl.n_points, 1500, replace=False))
+    import torch
+    lines = hk.Lines.from_numpy(wl.nu0, wl.S, wl.gamma0)
+    ctx = hk.Context(lines)
+    for P in wl.P_atm:
+        got = ctx.opacity(T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff)
+        torch.cuda.synchronize()
+        got = got.cpu().numpy()
+        ref = oracle.opacity_points(wl.nu0, wl.S, wl.gamma0, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, js)
+        _check(got[js], ref, ref_max=got.max())
+    ctx.close()

@@ -198,3 +198,13 @@ def test_rejects_bad_arguments():
         oracle.opacity([1.0], [1.0], [0.05], -5.0, 1.0, 0.0, 10.0, 0.01, 25.0)
     with pytest.raises(ValueError):
         oracle.opacity([1.0], [1.0], [0.05], 300.0, 0.0, 0.0, 10.0, 0.01, 25.0)
+
+
+def test_points_entry_equals_range_entry():
+    wl = workloads.small(seed=12, n_lines=50, nu_max=80.0, cutoff=25.0)
+    args = (wl.nu0, wl.S, wl.gamma0, wl.T[0], wl.P_atm[0], wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff)
+    k = oracle.opacity(*args)
+    js = np.array([0, 17, 4000, 7999, 123, 123])
+    assert np.array_equal(oracle.opacity_points(*args, js), k[js])
+    with pytest.raises(ValueError):
+        oracle.opacity_points(*args, [8000])
