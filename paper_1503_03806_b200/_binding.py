@@ -182,7 +182,7 @@ def hk_opacity(lines: Lines, T, P_atm, nu_min, nu_max, dnu, cutoff, mass_amu=18.
         if N < 1:
             raise HKError(-1, "hk_opacity")
         out = torch.empty(N, dtype=torch.float64, device=lines.nu0.device)
-    elif int(out.numel()) != N:
+    elif N >= 1 and int(out.numel()) != N:       # (N < 1: let the library report HK_ERR_INVALID)
         raise ValueError(f"out has {int(out.numel())} entries, the grid has {N}")
     cl = lines._c()
     prm = _hk_params(float(mass_amu), float(q_ratio), int(precision), int(bool(lines_sorted)), _stream_ptr(stream))
