@@ -1,0 +1,308 @@
+#!/usr/bin/env python
+"""bench.py — the hot path of HELIOS-K on BASELINE.json config 1.
+
+One "step" = one whole opacity function plus its k-distribution through the C ABI:
+    hk_opacity (a1 line prep, a2 tile plan, a3 Voigt accumulation, a4 kappa store)  +  hk_kdist (a5 per-bin sort, a6 resample)
+on the seeded synthetic 1e5-line workload (workloads.config(1): 3e6 grid points, cutoff 100 cm^-1, 3000 bins x 1000 points,
+20 Gauss-Legendre g-points), FP64.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W]                  our arm (CUDA, sm_100a)
+    python bench.py --impl reference [...]                                the oracle, as it stands, on the host cores
+
+N > 1 (torchrun, one rank per GPU): the path shards with NO collective — rank r computes the opacity function of the r-th
+(T, P) pair of a small T-P table over the same line list ("repeat this calculation for multiple combinations of
+temperature and pressure"); rank 0 keeps config 1's (1500 K, 1 atm).  Per-GPU work is fixed: weak scaling.  NCCL is used only
+for the barrier and the max-over-ranks of the device time.
+
+Prints ONE JSON line (rank 0).  `value` = line-point Voigt evaluations per second, whole job, inputs resident in HBM, device time
+by CUDA events around each step (L2 flushed between steps, outside the events).  `e2e` = the same metric through
+hk.opacity_host(): pinned host line arrays -> device, both calls, kappa and the k-table -> pinned host, wall clock.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads  # noqa: E402
+
+METRIC = "voigt_line_point_evals_per_s"
+UNIT = "line-point evals/s"
+WORKLOAD = "BASELINE.json configs[1]: 1e5 lines, 3e6 grid points, cutoff 100 cm^-1, T=1500 K, P=1 atm, 3000 bins x 1000 pts, 20 g-points"
+
+# FP64-pipe thread-instructions the method needs per line-point evaluation, by regime (counted from
+# the formulas of hk_voigt.cuh with the Newton reciprocal; these are the algorithmic figures, not the executed SASS).
+FP64_INST_PER_EVAL = {"gh1": 5.0, "gh2": 7.0, "gh3": 11.0, "gh6": 22.0, "series": 150.0}
+
+
+def tp_table(wl, world):
+    """(T, P_atm) of each rank: rank 0 is config 1's own pair; further ranks walk a small seeded-free T-P ladder."""
+    pairs = [(wl.T[0], wl.P_atm[0])]
+    for r in range(1, world):
+        pairs.append((wl.T[0] * (1.0 + 0.1 * ((r + 1) // 2) * (1 if r % 2 else -1) / 2.0), wl.P_atm[0] * (2.0 ** ((r % 4) - 1))))
+    return pairs
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs (B200_PROFILING.md)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200",
+                                          "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._read, daemon=True)
+        self.thread.start()
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        self.thread.join(timeout=5)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) < 9:
+                continue
+            try:
+                sm.append(float(r[1]))
+                mx.append(float(r[2]))
+            except ValueError:
+                continue
+            for k, nm in enumerate(names):
+                if r[5 + k].lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_sample(wl, T, P, target_s, seed=1):
+    """Times the oracle, as it stands, on whole seeded bins of the workload (kappa of every point of the bin + the bin's
+    k-distribution).  A 4-bin pilot sizes the sample for about `target_s` seconds.  Returns (evals/s, description, cores)."""
+    import oracle
+    ppb = int(round(wl.bin_width / wl.dnu))
+    n_bins = wl.n_points // ppb
+    rng = np.random.default_rng(seed)
+    order = rng.permutation(n_bins)
+
+    def run(bins):
+        js = (np.sort(bins)[:, None] * ppb + np.arange(ppb)[None, :]).ravel()
+        t0 = time.perf_counter()
+        kap = oracle.opacity_points(wl.nu0, wl.S, wl.gamma0, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, js,
+                                    mass_amu=wl.mass_amu)
+        oracle.kdist(kap, ppb, wl.n_g)
+        dt = time.perf_counter() - t0
+        nu = wl.nu_min + js * wl.dnu
+        ne = int(np.sum(np.searchsorted(wl.nu0, nu + wl.cutoff, "right") - np.searchsorted(wl.nu0, nu - wl.cutoff, "left")))
+        return dt, ne
+
+    dt, ne = run(order[:4])
+    nb = int(min(n_bins, max(4, round(4 * target_s / max(dt, 1e-3)))))
+    dt, ne = run(order[:nb])
+    cores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+    return ne / dt, dt, ne, f"{nb} seeded whole bins ({nb * ppb} grid points, {ne} line-point evals, {dt:.1f} s) of the {n_bins}-bin workload", cores
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores (this tier's reference arm).  Rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    wl = workloads.config(1)
+    T, P = wl.T[0], wl.P_atm[0]
+    import oracle
+    oracle.build()
+    per_step_s = max(2.0, min(20.0, 90.0 / max(1, args.steps + args.warmup)))
+    for _ in range(args.warmup):
+        oracle_sample(wl, T, P, per_step_s)
+    tot_e, tot_t, desc, cores = 0, 0.0, "", 1
+    for _ in range(args.steps):
+        _, dt, ne, desc, cores = oracle_sample(wl, T, P, per_step_s)
+        tot_e += ne
+        tot_t += dt
+    v = tot_e / tot_t
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / max(1, args.steps), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD, "sample": "each step: " + desc},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": "each step: " + desc},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_1503_03806_b200 as hk
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device — the hot path has no CPU fallback (use --impl reference for the oracle)")
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus and world > 1:
+        raise SystemExit(f"--gpus {args.gpus} but WORLD_SIZE={world}")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    hk.load_library()
+    wl = workloads.config(1)
+    T, P = tp_table(wl, world)[rank]
+    N = wl.n_points
+    ppb = int(round(wl.bin_width / wl.dnu))
+    n_evals = hk.hk_count_evals(wl.nu0, wl.nu_min, N, wl.dnu, wl.cutoff)
+    lines = hk.Lines.from_numpy(wl.nu0, wl.S, wl.gamma0)
+    kappa = torch.empty(N, dtype=torch.float64, device="cuda")
+    ktab = torch.empty((N // ppb, wl.n_g), dtype=torch.float64, device="cuda")
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def step():
+        hk.hk_opacity(lines, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, mass_amu=wl.mass_amu, out=kappa)
+        hk.hk_kdist(kappa, wl.dnu, wl.bin_width, wl.n_g, out=ktab)
+
+    fp64_peak = hk.hk_fp64_peak()                                        # DFMA thread-instructions/s, measured live
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+
+    # ---- timed region: K steps, device time by CUDA events around each step, L2 flushed between steps ----------------
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    hk.hk_set_timing(True)                                               # per-stage events inside hk_opacity (same stream)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+          for _ in range(args.steps)]
+    stage = np.zeros(3)
+    barrier()
+    t_wall0 = time.perf_counter()
+    for i in range(args.steps):
+        flush.zero_()
+        ev[i][0].record(stream)
+        hk.hk_opacity(lines, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, mass_amu=wl.mass_amu, out=kappa)
+        ev[i][1].record(stream)
+        hk.hk_kdist(kappa, wl.dnu, wl.bin_width, wl.n_g, out=ktab)
+        ev[i][2].record(stream)
+        stage += np.array(hk.hk_last_stage_ms())
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    hk.hk_set_timing(False)
+    ms_opacity = sum(e[0].elapsed_time(e[1]) for e in ev)
+    ms_kdist = sum(e[1].elapsed_time(e[2]) for e in ev)
+    ms_total = ms_opacity + ms_kdist
+    stage /= args.steps
+    clocks = sampler.stop() if rank == 0 else None
+
+    # ---- e2e: host buffers in, host buffers out, through the public API -----------------------------------------------
+    pin = lambda a: torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64)).pin_memory()
+    h_nu0, h_S, h_g0 = pin(wl.nu0), pin(wl.S), pin(wl.gamma0)
+    h_kappa = torch.empty(N, dtype=torch.float64, pin_memory=True)
+    for _ in range(2):
+        hk.opacity_host(h_nu0, h_S, h_g0, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, mass_amu=wl.mass_amu,
+                        bin_width=wl.bin_width, n_g=wl.n_g, kappa_out=h_kappa)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        _, h_k = hk.opacity_host(h_nu0, h_S, h_g0, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, mass_amu=wl.mass_amu,
+                                 bin_width=wl.bin_width, n_g=wl.n_g, kappa_out=h_kappa)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    h2d = 3 * 8 * wl.n_lines
+    d2h = 8 * N + 8 * (N // ppb) * wl.n_g
+
+    # ---- max over ranks ------------------------------------------------------------------------------------------------
+    red = torch.tensor([ms_total, ms_opacity, ms_kdist, e2e_s * 1e3, stage[2]], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(red, op=dist.ReduceOp.MAX)
+    ms_total, ms_opacity, ms_kdist, e2e_ms, ms_voigt = [float(v) for v in red.cpu()]
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    K = args.steps
+    value = world * n_evals * K / (ms_total * 1e-3)
+    # roofline of the dominant kernel (voigt_kernel, a3+a4): ALU-bound on the FP64 pipe
+    census = hk.hk_regime_census(wl.nu0, wl.gamma0, T, P, wl.mass_amu, wl.nu_min, N, wl.dnu, wl.cutoff)
+    alg_inst = sum(FP64_INST_PER_EVAL[k] * census[k] for k in FP64_INST_PER_EVAL)
+    achieved = 2.0 * alg_inst / (ms_voigt * 1e-3) / 1e12                # FMA-equivalent TFLOP/s (1 FP64 instruction = 2 flop)
+    peak = 2.0 * fp64_peak / 1e12
+    cpu_v, cpu_dt, cpu_ne, cpu_desc, cores = oracle_sample(wl, T, P, 15.0) if world == 1 else (None, 0, 0, "", 0)
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "n_lines": wl.n_lines, "n_points": N, "line_point_evals": n_evals,
+                   "parallelism": f"tp-pairs x{world} (no collective)", "api": "hk_opacity + hk_kdist (C ABI, one-shot form)",
+                   "l2": "flushed between steps by a 512 MiB memset outside the per-step CUDA events",
+                   "T_K": T, "P_atm": P},
+        "s_per_opacity_function": ms_opacity / K * 1e-3, "s_per_kdist": ms_kdist / K * 1e-3,
+        "stage_ms": {"line_prep": stage[0], "tile_plan": stage[1], "voigt_accumulate_store": ms_voigt, "kdist": ms_kdist / K},
+        "wall_s_timed_region": t_wall,
+        "e2e": {"value": world * n_evals * K / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "ms_per_step": e2e_ms / K},
+        "gpu_launches": 4 * K,
+        "roofline": {"kernel": "voigt_kernel (a3+a4)", "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                     "frac": achieved / peak, "traffic": None,
+                     "note": "FP64-pipe thread-instructions x2; algorithmic instructions = regime census x per-eval figure "
+                             "(DESIGN.md); peak = hk_fp64_peak DFMA microbenchmark measured live in this run",
+                     "regime_census": census, "ms": ms_voigt},
+        "clocks": clocks,
+    }
+    if cpu_v is not None:
+        line["cpu_baseline"] = {"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": cpu_desc}
+    line["paper_context"] = "~1 s per opacity function of ~1e5 lines on a Tesla K20 (PAPER.md:9, 267); other hardware, not a target"
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -129,9 +129,18 @@ int hk_destroy(hk_ctx *ctx);
  * thread-instructions per second (the "alu" roofline denominator of bench.py, measured live).  Synchronous. */
 int hk_fp64_peak(double *inst_per_s_out, void *stream);
 
+/* Measurement helper (roofline numerator of bench.py): how many line-point evaluations of the workload fall in each
+ * regime of the device Voigt routine, decided per POINT on r^2 = x^2 + y^2 exactly as hk_voigt_K does:
+ * counts_out[0..4] = 1-point, 2-point, 3-point, 6-point Gauss-Hermite, series.  Their sum equals hk_count_evals().
+ * gamma = gamma0 * P_atm * (296/T)^0.5 (n_T = 0.5), alpha = (nu0/c) sqrt(2 k_B T/m).  HOST arrays, host arithmetic,
+ * O(n_lines).  HK_ERR_INVALID on NULL or non-positive T, P_atm, mass_amu, dnu, cutoff, N. */
+int hk_regime_census(const double *nu0_host, const double *gamma0_host, int64_t n_lines, double T, double P_atm,
+                     double mass_amu, double nu_min, int64_t N, double dnu, double cutoff, int64_t counts_out[5]);
+
 /* Per-stage device time of the last hk_opacity / hk_opacity_ctx call on this thread, in milliseconds, measured
  * with CUDA events on the call's stream: [0] line prep, [1] tile plan, [2] Voigt accumulation + kappa store.
- * Enabled by hk_set_timing(1) (off by default: the events add launch overhead).  Synchronous. */
+ * Enabled by hk_set_timing(1) (off by default).  The timed call stays asynchronous: it only records the events;
+ * hk_last_stage_ms() waits for the last one (synchronous) and must be called before the next timed call. */
 int hk_set_timing(int on);
 int hk_last_stage_ms(float ms_out[3]);
 

@@ -62,6 +62,9 @@ def load_library():
     L.hk_count_evals.argtypes = [_dp, _i64, C.c_double, _i64, C.c_double, C.c_double]
     L.hk_kdist.restype = C.c_int
     L.hk_kdist.argtypes = [C.c_void_p, _i64, C.c_double, C.c_double, C.c_int, C.c_void_p, C.c_void_p]
+    L.hk_regime_census.restype = C.c_int
+    L.hk_regime_census.argtypes = [_dp, _dp, _i64, C.c_double, C.c_double, C.c_double, C.c_double, _i64, C.c_double,
+                                   C.c_double, C.POINTER(_i64)]
     L.hk_gauss_legendre.restype = C.c_int
     L.hk_gauss_legendre.argtypes = [C.c_int, _dp, _dp]
     L.hk_voigt_K.restype = C.c_int
@@ -163,6 +166,18 @@ def hk_grid_size(nu_min: float, nu_max: float, dnu: float) -> int:
 def hk_count_evals(nu0_host, nu_min: float, N: int, dnu: float, cutoff: float) -> int:
     a = np.ascontiguousarray(nu0_host, dtype=np.float64)
     return int(load_library().hk_count_evals(a.ctypes.data_as(_dp), a.size, nu_min, int(N), dnu, cutoff))
+
+
+def hk_regime_census(nu0_host, gamma0_host, T, P_atm, mass_amu, nu_min, N, dnu, cutoff) -> dict:
+    """Line-point evaluations per regime of the device Voigt routine (bench.py's roofline numerator).  Host arrays."""
+    a = np.ascontiguousarray(nu0_host, dtype=np.float64)
+    g = np.ascontiguousarray(gamma0_host, dtype=np.float64)
+    if a.size != g.size:
+        raise ValueError("nu0 and gamma0 differ in length")
+    c = (_i64 * 5)()
+    _check(load_library().hk_regime_census(a.ctypes.data_as(_dp), g.ctypes.data_as(_dp), a.size, T, P_atm, mass_amu, nu_min,
+                                           int(N), dnu, cutoff, c), "hk_regime_census")
+    return dict(zip(("gh1", "gh2", "gh3", "gh6", "series"), (int(v) for v in c)))
 
 
 def hk_gauss_legendre(n_g: int):

@@ -417,6 +417,8 @@ __global__ void __launch_bounds__(256) dfma_peak_kernel(double *out, int iters, 
 // ------------------------------------------------------------------------------------------------------
 static thread_local char g_cuda_err[256] = "";
 static thread_local float g_stage_ms[3] = {0.f, 0.f, 0.f};
+static thread_local cudaEvent_t g_ev[4] = {nullptr, nullptr, nullptr, nullptr};  // stage boundaries of the last timed call
+static thread_local bool g_ev_pending = false;
 static int g_timing = 0;
 
 static int cuda_fail(cudaError_t e, const char *what)
@@ -510,9 +512,10 @@ static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double 
   int rc = scratch_reserve(s, n_lines, n_tiles, st, pooled);
   if (rc != HK_OK) return rc;
 
-  cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+  cudaEvent_t *ev = g_ev;
   if (g_timing) {
-    for (auto &e : ev) HK_CUDA(cudaEventCreate(&e));
+    for (int i = 0; i < 4; ++i)
+      if (!ev[i]) HK_CUDA(cudaEventCreate(&ev[i]));
     HK_CUDA(cudaEventRecord(ev[0], st));
   }
   PrepArgs pa;
@@ -538,9 +541,7 @@ static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double 
   HK_CUDA(cudaGetLastError());
   if (g_timing) {
     HK_CUDA(cudaEventRecord(ev[3], st));
-    HK_CUDA(cudaEventSynchronize(ev[3]));
-    for (int i = 0; i < 3; ++i) HK_CUDA(cudaEventElapsedTime(&g_stage_ms[i], ev[i], ev[i + 1]));
-    for (auto &e : ev) cudaEventDestroy(e);
+    g_ev_pending = true;  // resolved by hk_last_stage_ms(): the call itself stays asynchronous
   }
   return HK_OK;
 }
@@ -656,6 +657,47 @@ int64_t hk_count_evals(const double *nu0_host, int64_t n_lines, double nu_min, i
     if (hi >= lo) total += (int64_t)hi - (int64_t)lo + 1;
   }
   return total;
+}
+
+int hk_regime_census(const double *nu0_host, const double *gamma0_host, int64_t n_lines, double T, double P_atm,
+                     double mass_amu, double nu_min, int64_t N, double dnu, double cutoff, int64_t counts_out[5])
+{
+  if (!nu0_host || !gamma0_host || !counts_out || n_lines < 0 || N < 1 || !pos_finite(T) || !pos_finite(P_atm) ||
+      !pos_finite(mass_amu) || !pos_finite(dnu) || !pos_finite(cutoff))
+    return HK_ERR_INVALID;
+  const double vth = sqrt(2.0 * kBoltz * T / (mass_amu * kAmu)) / kCLight;
+  const double tfac = pow(kT0 / T, 0.5);
+  // points of the window [lo, hi] with |nu_j - nu0| < rho  (rho in cm^-1)
+  auto within = [&](double nu0, double rho, int64_t lo, int64_t hi) -> int64_t {
+    if (!(rho > 0.0)) return 0;
+    double a = ceil(((nu0 - rho) - nu_min) / dnu), b = floor(((nu0 + rho) - nu_min) / dnu);
+    if (a * dnu + nu_min <= nu0 - rho) a += 1.0;  // strict inequality at the edges
+    if (b * dnu + nu_min >= nu0 + rho) b -= 1.0;
+    const int64_t ia = a < (double)lo ? lo : (int64_t)a, ib = b > (double)hi ? hi : (int64_t)b;
+    return ib >= ia ? ib - ia + 1 : 0;
+  };
+  int64_t c[5] = {0, 0, 0, 0, 0};
+  for (int64_t i = 0; i < n_lines; ++i) {
+    const double nu0 = nu0_host[i];
+    double lo = ceil(((nu0 - cutoff) - nu_min) / dnu), hi = floor(((nu0 + cutoff) - nu_min) / dnu);
+    if (!(lo > 0.0)) lo = 0.0;
+    if (!(hi < (double)(N - 1))) hi = (double)(N - 1);
+    if (hi < lo) continue;
+    const int64_t jl = (int64_t)lo, jh = (int64_t)hi, tot = jh - jl + 1;
+    double alpha = nu0 * vth;
+    if (!(alpha > 0.0)) { c[0] += tot; continue; }
+    const double gamma = gamma0_host[i] * P_atm * tfac, a2 = alpha * alpha, g2 = gamma * gamma, y = gamma / alpha;
+    auto rho = [&](double R) { const double t = R * a2 - g2; return t > 0.0 ? sqrt(t) : 0.0; };
+    double xc2 = kRc - y * y;
+    if (y < 1e-8) xc2 = fmax(xc2, -log(1e-10 * fmax(y, 1e-300)));
+    xc2 = fmin(xc2, kXcapSq);
+    const int64_t n1 = within(nu0, rho(kR1), jl, jh), n2 = within(nu0, rho(kR2), jl, jh), n3 = within(nu0, rho(kR3), jl, jh);
+    const int64_t nc = xc2 > 0.0 ? within(nu0, sqrt(xc2) * alpha, jl, jh) : 0;
+    const int64_t ncore = nc < n3 ? nc : n3;
+    c[0] += tot - n1; c[1] += n1 - n2; c[2] += n2 - n3; c[3] += n3 - ncore; c[4] += ncore;
+  }
+  for (int k = 0; k < 5; ++k) counts_out[k] = c[k];
+  return HK_OK;
 }
 
 int hk_gauss_legendre(int n_g, double *g, double *w)
@@ -778,6 +820,11 @@ int hk_set_timing(int on)
 int hk_last_stage_ms(float ms_out[3])
 {
   if (!ms_out) return HK_ERR_INVALID;
+  if (g_ev_pending) {
+    HK_CUDA(cudaEventSynchronize(g_ev[3]));
+    for (int i = 0; i < 3; ++i) HK_CUDA(cudaEventElapsedTime(&g_stage_ms[i], g_ev[i], g_ev[i + 1]));
+    g_ev_pending = false;
+  }
   for (int i = 0; i < 3; ++i) ms_out[i] = g_stage_ms[i];
   return HK_OK;
 }
