@@ -3,8 +3,9 @@
 // Steps:
 //   a1 line_prep_kernel   per line: alpha, gamma, S(T), amplitude, index window, regime radii
 //   a2 tile_plan_kernel   per grid tile: range of sorted lines whose window touches the tile
-//   a3 voigt_kernel       kappa_j = sum_i amp_i V_i(nu_j): grid-point-owned register accumulation, lines streamed
-//                         through shared memory by 1-D TMA bulk copies, regime chosen per (line, warp span)
+//   a3 voigt_kernel       kappa_j = sum_i amp_i V_i(nu_j): grid-point-owned register accumulation, persistent CTAs, lines
+//                         streamed through a shared-memory ring by 1-D TMA bulk copies (producer warp, full/empty
+//                         mbarriers), regime chosen per (line, warp span) or per (line, 32-point group)
 //   a4                    coalesced kappa store from the same kernel ("without additional write-outs")
 //   a5/a6 kdist_kernel    per-bin shared-memory sort + resampling at Gauss-Legendre nodes
 #include <cuda_runtime.h>
@@ -21,17 +22,17 @@
 namespace hk {
 
 // ------------------------------------------------------------------------------------------------------
-// packed line records (written by a1, streamed by a3).  Three 32-byte records per line, structure of arrays,
-// so that a chunk of lines is three contiguous 16-byte-aligned spans (one TMA bulk copy each).
+// packed line records (written by a1, streamed by a3).  Four 32-byte records per line, structure of arrays,
+// so that a chunk of lines is four contiguous 16-byte-aligned spans (one TMA bulk copy each).
 // ------------------------------------------------------------------------------------------------------
 struct __align__(16) LineMeta {
   int jlo, jhi;  // inclusive index window of the line (empty if jhi < jlo)
   float c;       // line centre in grid units, (nu0-nu_min)/dnu
-  float r3;      // |j-c| >= r3 for a whole span  =>  r^2 >= kR3 on it (3-point rule valid); conservative (+2)
+  float r1;      // |j-c| >= r1 on a whole group of points  =>  r^2 >= kR1 there (1-point rule valid); conservative (+2)
   float r2;      // likewise kR2 (2-point rule)
-  float r1;      // likewise kR1 (1-point rule)
-  float xc2;     // series region: x^2 < xc2
-  float pad;
+  float r3;      // likewise kR3 (3-point rule)
+  float r6;      // likewise kRc (6-point rule); inside it the series region may begin
+  float rg;      // the 6-point rule adds the Gaussian term on groups closer than this (0 unless y < 1e-8)
 };
 struct __align__(16) LineBase {
   double nu0, A1, g2, a2;  // centre; amp*gamma/pi; gamma^2; alpha^2
@@ -39,7 +40,11 @@ struct __align__(16) LineBase {
 struct __align__(16) LineGH2 {
   double e2, f2, A1a2, inv_alpha;  // gamma^2 - alpha^2/2; 2 alpha^2 gamma^2; A1 alpha^2; 1/alpha (0 if alpha == 0)
 };
-static_assert(sizeof(LineMeta) == 32 && sizeof(LineBase) == 32 && sizeof(LineGH2) == 32, "record size");
+struct __align__(16) LineCore {
+  double y, erfcx_y, Acore, xc2;  // gamma/alpha; erfcx(y); amp/(alpha sqrt(pi)); series where x^2 < xc2
+};
+static_assert(sizeof(LineMeta) == 32 && sizeof(LineBase) == 32 && sizeof(LineGH2) == 32 && sizeof(LineCore) == 32,
+              "record size");
 
 constexpr double kCLight = 2.99792458e10;   // cm/s
 constexpr double kBoltz = 1.380649e-16;     // erg/K
@@ -59,8 +64,10 @@ struct PrepArgs {
   LineMeta *meta;
   LineBase *base;
   LineGH2 *gh2;
+  LineCore *core;
 };
 
+// grid-unit radius outside which x^2 + y^2 >= R holds: sqrt(R alpha^2 - gamma^2)/dnu, rounded outward
 __device__ __forceinline__ float radius_grid(double R, double a2, double g2, double inv_dnu)
 {
   double t = R * a2 - g2;
@@ -96,6 +103,11 @@ __global__ void __launch_bounds__(256) line_prep_kernel(PrepArgs a)
   g.f2 = 2.0 * a2 * g2;
   g.A1a2 = b.A1 * a2;
   g.inv_alpha = alpha > 0.0 ? 1.0 / alpha : 0.0;
+  LineCore k;
+  k.y = gamma * g.inv_alpha;
+  k.xc2 = alpha > 0.0 ? core_xc2(k.y) : 0.0;
+  k.erfcx_y = k.xc2 > 0.0 ? erfcx(k.y) : 0.0;
+  k.Acore = amp * g.inv_alpha * kInvSqrtPi;
   // index window: sub, sub, IEEE divide, ceil/floor — no multiply-add, nothing to contract (A4)
   double lo = ceil(__ddiv_rn(__dsub_rn(__dsub_rn(nu0, a.cutoff), a.nu_min), a.dnu));
   double hi = floor(__ddiv_rn(__dsub_rn(__dadd_rn(nu0, a.cutoff), a.nu_min), a.dnu));
@@ -110,22 +122,25 @@ __global__ void __launch_bounds__(256) line_prep_kernel(PrepArgs a)
   double c = (nu0 - a.nu_min) * inv_dnu;
   c = fmin(fmax(c, -3.0e9), 3.0e9);
   m.c = (float)c;
-  m.r3 = radius_grid(kR3, a2, g2, inv_dnu);
-  m.r2 = radius_grid(kR2, a2, g2, inv_dnu);
   m.r1 = radius_grid(kR1, a2, g2, inv_dnu);
-  m.xc2 = alpha > 0.0 ? __double2float_ru(core_xc2(gamma * g.inv_alpha)) : 0.0f;
-  m.pad = 0.0f;
+  m.r2 = radius_grid(kR2, a2, g2, inv_dnu);
+  m.r3 = radius_grid(kR3, a2, g2, inv_dnu);
+  m.r6 = radius_grid(kRc, a2, g2, inv_dnu);
+  const double xg2 = alpha > 0.0 ? gauss_xg2(k.y) : 0.0;
+  m.rg = xg2 > 0.0 ? __double2float_ru(sqrt(xg2) * alpha * inv_dnu + 2.0) : 0.0f;
   a.meta[i] = m;
   a.base[i] = b;
   a.gh2[i] = g;
+  a.core[i] = k;
 }
 
 // a2: lines are sorted by nu0, so jlo and jhi are non-decreasing in i.  Tile t owns points [t*tile, (t+1)*tile).
-// plan[t] = [first i with jhi >= tile_lo, first i with jlo > tile_hi).
+// plan[t] = [first i with jhi >= tile_lo, first i with jlo > tile_hi).  Thread 0 also resets the tile queue of a3.
 __global__ void __launch_bounds__(128) tile_plan_kernel(const LineMeta *meta, int64_t n, int n_tiles, int tile, int N,
-                                                        int2 *plan)
+                                                        int2 *plan, int *queue)
 {
   int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t == 0) *queue = 0;
   if (t >= n_tiles) return;
   const int tlo = t * tile;
   const int thi = min(N, tlo + tile) - 1;
@@ -160,6 +175,10 @@ __device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
 {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
 __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
 {
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
@@ -181,141 +200,238 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
 }
 
 // ------------------------------------------------------------------------------------------------------
-// a3 + a4: Voigt accumulation.  One CTA per tile of WARPS*32*P consecutive grid points; warp w owns the span
-// [tile_lo + w*32P, +32P), lane l the points span_lo + l + 32k (k < P) so that stores are coalesced and every
-// 32 consecutive points belong to one k.  Lines of the tile's plan range are streamed through a double-buffered
-// shared-memory ring in chunks of CH by TMA bulk copies.  For every (line, warp span) the regime is chosen ONCE
-// from the span's distance to the line centre (float, grid units, conservative radii from a1): a warp-uniform
-// branch into an unrolled P-point loop of the 1-, 2- or 3-point rule.  Spans that reach inside the 3-point radius
-// or straddle a cutoff edge take the masked "near" path where each thread picks its own regime.
+// a3 + a4: Voigt accumulation.  Persistent CTAs of WARPS consumer warps + 1 producer warp.
+//
+// Work unit = tile of WARPS*32*P consecutive grid points, pulled from an atomic queue (ascending wavenumber).  Consumer
+// warp w owns the span [tile_lo + w*32P, +32P), lane l the points span_lo + l + 32k (k < P): stores are coalesced, every 32
+// consecutive points ("group") belong to one k, and a thread carries P independent dependency chains.
+//
+// The producer warp streams the lines of the tile's plan range through a STAGES-deep shared-memory ring in chunks of CH
+// lines: four 1-D TMA bulk copies per chunk (meta/base/gh2/core spans) completing on the stage's `full` mbarrier; each
+// consumer warp releases the stage on its `empty` mbarrier.  No CTA-wide barrier exists after start-up: warps drift apart by
+// up to STAGES-1 chunks, and the ring keeps flowing across tile boundaries (each stage carries a header naming its tile).
+//
+// For every (line, warp span) the regime is chosen ONCE from the span's distance to the line centre (float, grid units,
+// conservative radii from a1): a warp-uniform branch into an unrolled P-point loop of the 1-, 2- or 3-point rule, accumulated
+// in registers.  Spans that reach inside the 3-point radius or straddle a cutoff edge take the near path: the same choice per
+// 32-point group (still warp-uniform), the series only on groups that hold core points, accumulated in a per-warp
+// shared-memory strip (dynamic k without spilling the register accumulators).  Summation order is fixed: bitwise deterministic.
 // ------------------------------------------------------------------------------------------------------
-constexpr int CH = 128;  // lines per chunk: 3 x 4 KB per buffer
+constexpr int CH = 128;     // lines per ring stage: 4 x 4 KB
+constexpr int STAGES = 4;
+
+struct __align__(16) StageHdr {
+  int tile_lo;  // first grid point of the tile this chunk belongs to; < 0: no more work
+  int cnt;      // lines in the chunk (0 for a tile no line touches)
+  int flags;    // 1: first chunk of its tile, 2: last chunk of its tile
+  int pad;
+};
+
+template <int P, int WARPS>
+struct __align__(128) VoigtSmem {
+  LineMeta meta[STAGES][CH];
+  LineBase base[STAGES][CH];
+  LineGH2 gh2[STAGES][CH];
+  LineCore core[STAGES][CH];
+  double sk[WARPS][32 * P];
+  StageHdr hdr[STAGES];
+  uint64_t full[STAGES], empty[STAGES];
+};
 
 struct VoigtArgs {
   const LineMeta *meta;
   const LineBase *base;
   const LineGH2 *gh2;
+  const LineCore *core;
   const int2 *plan;
+  int *queue;
+  int n_tiles;
   double nu_min, dnu;
   int N;
   double *kappa;
 };
 
-template <int P, int WARPS>
-__global__ void __launch_bounds__(WARPS * 32) voigt_kernel(VoigtArgs a)
+// near path of a3 for one (line, warp span): rule per 32-point group (warp-uniform), accumulated in the warp's shared-memory
+// strip sk[32k + lane].  Kept out of line so that its constants (6-point pairs, series state) do not compete for registers
+// with the P accumulators of the far loops.  Warp-collective (SHFL in the series).
+template <int P>
+__device__ __noinline__ void near_span(const LineMeta m, const LineBase *pb, const LineGH2 *pg, const LineCore *pk, int slo,
+                                       int lane, float dist, double x0, double dnu, double En, double *sk)
+{
+  const LineBase b = *pb;
+  const LineGH2 g = *pg;
+  const double d0 = x0 - b.nu0;
+  Gh6 G6;
+  LineCore kc;
+  CoreLine C;
+  if (dist < m.r3) {  // some group may need the 6-point rule or the series
+    G6 = gh6_consts(b.A1, b.g2, b.a2);
+    kc = *pk;
+    if (dist < m.r6) C = core_setup(kc.y, kc.erfcx_y, En);
+  }
+#pragma unroll 1
+  for (int k = 0; k < P; ++k) {
+    const int glo = slo + 32 * k, ghi = glo + 31;
+    if (ghi < m.jlo || glo > m.jhi) continue;
+    const int j = glo + lane;
+    const bool inwin = (j >= m.jlo) && (j <= m.jhi);
+    const double d = fma((double)(32 * k), dnu, d0);
+    const float dg = fmaxf(fmaxf((float)glo - m.c, m.c - (float)ghi), 0.0f);
+    double v;
+    if (dg >= m.r2) {
+      v = dg >= m.r1 ? gh1_acc(0.0, d, b.A1, b.g2) : gh2_acc(0.0, d, b.A1, g.e2, g.f2, g.A1a2);
+    } else if (dg >= m.r3) {
+      const double c3 = b.A1 * (1.0 / 3.0);
+      v = gh3_acc(0.0, d, b.g2, fma(-1.5, b.a2, b.g2), 6.0 * b.a2 * b.g2, 2.0 * c3, c3, b.A1 * b.a2);
+    } else {
+      v = gh6_val(d * d, G6);
+      if (dg < m.r6) {  // the series region reaches into this group
+        const double x = fabs(d) * g.inv_alpha;
+        const double ks = core_K(fmin(x, 6.7), C);
+        if (x * x < kc.xc2) v = kc.Acore * ks;
+        else if (m.rg > 0.0f) v = fma(kc.Acore, exp(-x * x), v);
+      } else if (dg < m.rg) {
+        const double x = d * g.inv_alpha;
+        v = fma(kc.Acore, exp(-x * x), v);
+      }
+    }
+    sk[32 * k + lane] += inwin ? v : 0.0;
+  }
+}
+
+template <int P, int WARPS, int MINB>
+__global__ void __launch_bounds__((WARPS + 1) * 32, MINB) voigt_kernel(const __grid_constant__ VoigtArgs a)
 {
   constexpr int TILE = WARPS * 32 * P;
-  __shared__ __align__(128) LineMeta s_meta[2][CH];
-  __shared__ __align__(128) LineBase s_base[2][CH];
-  __shared__ __align__(128) LineGH2 s_gh2[2][CH];
-  __shared__ __align__(8) uint64_t s_bar[2];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  VoigtSmem<P, WARPS> &S = *reinterpret_cast<VoigtSmem<P, WARPS> *>(smem_raw);
 
-  const int tile = blockIdx.x;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int2 pl = a.plan[tile];
-  const int L0 = pl.x, nl = pl.y - pl.x;
-  const int nchunks = (nl + CH - 1) / CH;
-  const int slo = tile * TILE + warp * (32 * P);
-  const int shi = slo + 32 * P - 1;
-  const float slo_f = (float)slo, shi_f = (float)shi;
-
   if (threadIdx.x == 0) {
-    mbar_init(&s_bar[0], 1);
-    mbar_init(&s_bar[1], 1);
+    for (int s = 0; s < STAGES; ++s) {
+      mbar_init(&S.full[s], 1);
+      mbar_init(&S.empty[s], WARPS);
+    }
     mbar_fence_init();
   }
-  __syncthreads();
-
-  auto issue = [&](int c) {
-    const int buf = c & 1;
-    const int first = L0 + c * CH;
-    const int cnt = min(CH, nl - c * CH);
-    const uint32_t bytes = (uint32_t)cnt * 32u;
-    mbar_expect_tx(&s_bar[buf], 3u * bytes);
-    bulk_g2s(&s_meta[buf][0], a.meta + first, bytes, &s_bar[buf]);
-    bulk_g2s(&s_base[buf][0], a.base + first, bytes, &s_bar[buf]);
-    bulk_g2s(&s_gh2[buf][0], a.gh2 + first, bytes, &s_bar[buf]);
-  };
-  if (threadIdx.x == 0 && nchunks > 0) issue(0);
-
-  double acc[P], xk[P];
+  if (warp < WARPS) {
 #pragma unroll
-  for (int k = 0; k < P; ++k) {
-    acc[k] = 0.0;
-    xk[k] = __dadd_rn(a.nu_min, __dmul_rn((double)(slo + lane + 32 * k), a.dnu));  // nu_j exactly as defined
+    for (int k = 0; k < P; ++k) S.sk[warp][32 * k + lane] = 0.0;
+  }
+  __syncthreads();  // the only CTA-wide barrier
+
+  if (warp == WARPS) {
+    // ---------------- producer: one thread feeds the ring ----------------
+    if (lane != 0) return;
+    int stage = 0;
+    uint32_t phase = 0;
+    for (;;) {
+      const int tile = atomicAdd(a.queue, 1);
+      const bool stop = tile >= a.n_tiles;
+      int L0 = 0, nl = 0;
+      if (!stop) {
+        const int2 pl = a.plan[tile];
+        L0 = pl.x;
+        nl = pl.y - pl.x;
+      }
+      const int nchunks = nl > 0 ? (nl + CH - 1) / CH : 1;
+      for (int c = 0; c < nchunks; ++c) {
+        mbar_wait(&S.empty[stage], phase ^ 1u);
+        const int cnt = min(CH, nl - c * CH);
+        StageHdr h;
+        h.tile_lo = stop ? -1 : tile * TILE;
+        h.cnt = cnt > 0 ? cnt : 0;
+        h.flags = (c == 0 ? 1 : 0) | (c == nchunks - 1 ? 2 : 0);
+        h.pad = 0;
+        S.hdr[stage] = h;
+        const uint32_t bytes = (uint32_t)h.cnt * 32u;
+        mbar_expect_tx(&S.full[stage], 4u * bytes);  // release: the header store above is visible to the waiters
+        if (bytes) {
+          const int first = L0 + c * CH;
+          bulk_g2s(&S.meta[stage][0], a.meta + first, bytes, &S.full[stage]);
+          bulk_g2s(&S.base[stage][0], a.base + first, bytes, &S.full[stage]);
+          bulk_g2s(&S.gh2[stage][0], a.gh2 + first, bytes, &S.full[stage]);
+          bulk_g2s(&S.core[stage][0], a.core + first, bytes, &S.full[stage]);
+        }
+        if (++stage == STAGES) {
+          stage = 0;
+          phase ^= 1u;
+        }
+      }
+      if (stop) return;
+    }
   }
 
-  for (int c = 0; c < nchunks; ++c) {
-    const int buf = c & 1;
-    if (threadIdx.x == 0 && c + 1 < nchunks) issue(c + 1);  // buffer (c+1)&1 was released by the barrier below
-    mbar_wait(&s_bar[buf], (uint32_t)((c >> 1) & 1));
-    const int cnt = min(CH, nl - c * CH);
+  // ---------------- consumers ----------------
+  double *sk = S.sk[warp];
+  const double En = core_lane_const();
+  double acc[P];
+#pragma unroll
+  for (int k = 0; k < P; ++k) acc[k] = 0.0;
+  int slo = 0, shi = 0;
+  float slo_f = 0.f, shi_f = 0.f;
+  double x0 = 0.0;  // nu of this thread's k = 0 point
+  int stage = 0;
+  uint32_t phase = 0;
+
+  for (;;) {
+    mbar_wait(&S.full[stage], phase);
+    const StageHdr h = S.hdr[stage];
+    if (h.tile_lo < 0) break;
+    if (h.flags & 1) {
+      slo = h.tile_lo + warp * (32 * P);
+      shi = slo + 32 * P - 1;
+      slo_f = (float)slo;
+      shi_f = (float)shi;
+      x0 = __dadd_rn(a.nu_min, __dmul_rn((double)(slo + lane), a.dnu));  // nu_j exactly as defined (A6)
+    }
 #pragma unroll 1
-    for (int l = 0; l < cnt; ++l) {
-      const LineMeta m = s_meta[buf][l];
+    for (int l = 0; l < h.cnt; ++l) {
+      const LineMeta m = S.meta[stage][l];
       if (m.jhi < slo || m.jlo > shi) continue;
       const bool inside = (m.jlo <= slo) && (m.jhi >= shi);
       const float dist = fmaxf(fmaxf(slo_f - m.c, m.c - shi_f), 0.0f);
-      if (inside && dist >= m.r2) {
-        const double nu0 = s_base[buf][l].nu0, A1 = s_base[buf][l].A1;
-        if (dist >= m.r1) {
-          const double g2 = s_base[buf][l].g2;
+      if (inside && dist >= m.r3) {
+        // ---- far: one rule for the whole span, register accumulators ----
+        const double nu0 = S.base[stage][l].nu0, A1 = S.base[stage][l].A1;
+        const double d0 = x0 - nu0;
+        if (dist >= m.r2) {
+          if (dist >= m.r1) {
+            const double g2 = S.base[stage][l].g2;
 #pragma unroll
-          for (int k = 0; k < P; ++k) acc[k] = gh1_acc(acc[k], xk[k] - nu0, A1, g2);
-        } else {
-          const double e2 = s_gh2[buf][l].e2, f2 = s_gh2[buf][l].f2, A1a2 = s_gh2[buf][l].A1a2;
+            for (int k = 0; k < P; ++k) acc[k] = gh1_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), A1, g2);
+          } else {
+            const double e2 = S.gh2[stage][l].e2, f2 = S.gh2[stage][l].f2, A1a2 = S.gh2[stage][l].A1a2;
 #pragma unroll
-          for (int k = 0; k < P; ++k) acc[k] = gh2_acc(acc[k], xk[k] - nu0, A1, e2, f2, A1a2);
-        }
-      } else if (inside && dist >= m.r3) {
-        const LineBase b = s_base[buf][l];
-        const double e3 = b.g2 - 1.5 * b.a2, f3 = 6.0 * b.a2 * b.g2;
-        const double c3 = b.A1 * (1.0 / 3.0), c0 = 2.0 * c3, c3a = b.A1 * b.a2;
-#pragma unroll
-        for (int k = 0; k < P; ++k) acc[k] = gh3_acc(acc[k], xk[k] - b.nu0, b.g2, e3, f3, c0, c3, c3a);
-      } else {
-        // near path: cutoff edge inside the span and/or points inside the 3-point radius
-        const LineBase b = s_base[buf][l];
-        NearLine L;
-        L.nu0 = b.nu0; L.A1 = b.A1; L.g2 = b.g2; L.a2 = b.a2;
-        L.inv_alpha = s_gh2[buf][l].inv_alpha;
-        L.inv_a2 = L.inv_alpha * L.inv_alpha;
-        const double gamma = sqrt(b.g2);
-        L.y = gamma * L.inv_alpha;
-        L.Acore = b.A1 * kSqrtPi * L.inv_alpha / gamma;  // amp/(alpha sqrt(pi))
-        L.xc2 = (double)m.xc2;
-        bool core_ready = false;
-        CoreLine C;
-#pragma unroll 1
-        for (int k = 0; k < P; ++k) {
-          const int j = slo + lane + 32 * k;
-          const bool inwin = (j >= m.jlo) && (j <= m.jhi);
-          const double d = __dadd_rn(a.nu_min, __dmul_rn((double)j, a.dnu)) - L.nu0;
-          double v = wing_value(d, L);
-          const double x = fabs(d) * L.inv_alpha;
-          const bool incore = inwin && (x * x < L.xc2);
-          if (__any_sync(kFull, incore)) {  // warp-uniform
-            if (!core_ready) {
-              C = core_setup(L.y, sqrt(L.xc2));
-              core_ready = true;
-            }
-            const double kc = core_K(fmin(x, 17.0), C);
-            if (incore) v = L.Acore * kc;
+            for (int k = 0; k < P; ++k) acc[k] = gh2_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), A1, e2, f2, A1a2);
           }
-          v = inwin ? v : 0.0;
+        } else {
+          const double g2 = S.base[stage][l].g2, a2 = S.base[stage][l].a2;
+          const double e3 = fma(-1.5, a2, g2), f3 = 6.0 * a2 * g2;
+          const double c3 = A1 * (1.0 / 3.0), c0 = 2.0 * c3, c3a = A1 * a2;
 #pragma unroll
-          for (int kk = 0; kk < P; ++kk)
-            if (kk == k) acc[kk] += v;
+          for (int k = 0; k < P; ++k) acc[k] = gh3_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), g2, e3, f3, c0, c3, c3a);
         }
+      } else {
+        near_span<P>(m, &S.base[stage][l], &S.gh2[stage][l], &S.core[stage][l], slo, lane, dist, x0, a.dnu, En, sk);
       }
     }
-    __syncthreads();  // every warp is done with buffer `buf` before chunk c+2 overwrites it
-  }
-
+    if (h.flags & 2) {
 #pragma unroll
-  for (int k = 0; k < P; ++k) {
-    const int j = slo + lane + 32 * k;
-    if (j < a.N) a.kappa[j] = acc[k];
+      for (int k = 0; k < P; ++k) {
+        const int j = slo + lane + 32 * k;
+        const double v = acc[k] + sk[32 * k + lane];
+        sk[32 * k + lane] = 0.0;
+        acc[k] = 0.0;
+        if (j < a.N) a.kappa[j] = v;
+      }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&S.empty[stage]);
+    if (++stage == STAGES) {
+      stage = 0;
+      phase ^= 1u;
+    }
   }
 }
 
@@ -326,21 +442,30 @@ __global__ void __launch_bounds__(128) voigt_K_kernel(const double *x, const dou
   const bool live = i < n;
   const double xi = live ? fabs(x[i]) : 1.0e3, yi = live ? y[i] : 1.0;
   const int lane = threadIdx.x & 31;
-  NearLine L;
-  L.nu0 = 0.0; L.a2 = 1.0; L.inv_alpha = 1.0; L.inv_a2 = 1.0;
-  L.g2 = yi * yi; L.y = yi;
-  L.A1 = yi * kInvSqrtPi;  // amp*gamma/pi with amp = sqrt(pi)  =>  amp*V = K
-  L.Acore = 1.0;
-  L.xc2 = core_xc2(yi);
-  double v = wing_value(xi, L);
-  const bool incore = live && (xi * xi < L.xc2);
+  const double A1 = yi * kInvSqrtPi;  // amp*gamma/pi with amp = sqrt(pi)  =>  amp*V = K
+  const double g2 = yi * yi, a2 = 1.0, q = xi * xi;
+  const double r2 = q + g2;
+  double v;
+  if (r2 >= kR1) {
+    v = gh1_acc(0.0, xi, A1, g2);
+  } else if (r2 >= kR2) {
+    v = gh2_acc(0.0, xi, A1, g2 - 0.5 * a2, 2.0 * a2 * g2, A1 * a2);
+  } else if (r2 >= kR3) {
+    const double c3 = A1 * (1.0 / 3.0);
+    v = gh3_acc(0.0, xi, g2, g2 - 1.5 * a2, 6.0 * a2 * g2, 2.0 * c3, c3, A1 * a2);
+  } else {
+    v = gh6_val(q, gh6_consts(A1, g2, a2));
+    if (q < gauss_xg2(yi)) v += exp(-q);
+  }
+  const bool incore = live && (q < core_xc2(yi));
+  const double En = core_lane_const();
   unsigned need = __ballot_sync(kFull, incore);
   while (need) {  // the series is warp-collective with a warp-uniform y: serve one lane at a time
     const int src = __ffs(need) - 1;
     need &= need - 1;
     const double ys = __shfl_sync(kFull, yi, src), xs = __shfl_sync(kFull, xi, src);
-    const CoreLine C = core_setup(ys, sqrt(core_xc2(ys)));
-    const double kc = core_K(fmin(xs, 17.0), C);
+    const CoreLine C = core_setup(ys, erfcx(ys), En);
+    const double kc = core_K(fmin(xs, 6.7), C);
     if (lane == src) v = kc;
   }
   if (live) out[i] = v;
@@ -434,42 +559,49 @@ static int cuda_fail(cudaError_t e, const char *what)
 
 static bool pos_finite(double v) { return v > 0.0 && isfinite(v); }
 
-constexpr int kP = 8, kWarps = 8;
+constexpr int kP = 8, kWarps = 7, kMinB = 2;  // 7 consumer warps + 1 producer = 256 threads: 128 registers at 2 CTAs/SM
 constexpr int kTile = kP * kWarps * 32;
+using VoigtSmemT = VoigtSmem<kP, kWarps>;
 
 struct Scratch {
-  LineMeta *meta = nullptr;
+  LineMeta *meta = nullptr;  // one allocation: meta | base | gh2 | core, n_lines records each
   LineBase *base = nullptr;
   LineGH2 *gh2 = nullptr;
-  int2 *plan = nullptr;
+  LineCore *core = nullptr;
+  int2 *plan = nullptr;      // one allocation: plan[n_tiles] | queue
+  int *queue = nullptr;
   int64_t cap_lines = 0;
   int cap_tiles = 0;
 };
 
+static void dev_free(void *p, cudaStream_t st, bool pooled)
+{
+  if (!p) return;
+  if (pooled) cudaFreeAsync(p, st); else cudaFree(p);
+}
+
 static int scratch_reserve(Scratch &s, int64_t n_lines, int n_tiles, cudaStream_t st, bool pooled)
 {
   if (n_lines > s.cap_lines) {
-    if (s.meta) {
-      if (pooled) { cudaFreeAsync(s.meta, st); cudaFreeAsync(s.base, st); cudaFreeAsync(s.gh2, st); }
-      else { cudaFree(s.meta); cudaFree(s.base); cudaFree(s.gh2); }
-      s.meta = nullptr; s.cap_lines = 0;
-    }
+    dev_free(s.meta, st, pooled);
+    s.meta = nullptr; s.cap_lines = 0;
     const size_t bytes = (size_t)n_lines * 32;
-    if (pooled) {
-      HK_CUDA(cudaMallocAsync(&s.meta, bytes, st));
-      HK_CUDA(cudaMallocAsync(&s.base, bytes, st));
-      HK_CUDA(cudaMallocAsync(&s.gh2, bytes, st));
-    } else {
-      HK_CUDA(cudaMalloc(&s.meta, bytes));
-      HK_CUDA(cudaMalloc(&s.base, bytes));
-      HK_CUDA(cudaMalloc(&s.gh2, bytes));
-    }
+    void *p = nullptr;
+    if (pooled) HK_CUDA(cudaMallocAsync(&p, 4 * bytes, st)); else HK_CUDA(cudaMalloc(&p, 4 * bytes));
+    s.meta = (LineMeta *)p;
+    s.base = (LineBase *)((char *)p + bytes);
+    s.gh2 = (LineGH2 *)((char *)p + 2 * bytes);
+    s.core = (LineCore *)((char *)p + 3 * bytes);
     s.cap_lines = n_lines;
   }
   if (n_tiles > s.cap_tiles) {
-    if (s.plan) { if (pooled) cudaFreeAsync(s.plan, st); else cudaFree(s.plan); s.plan = nullptr; }
-    if (pooled) HK_CUDA(cudaMallocAsync(&s.plan, (size_t)n_tiles * sizeof(int2), st));
-    else HK_CUDA(cudaMalloc(&s.plan, (size_t)n_tiles * sizeof(int2)));
+    dev_free(s.plan, st, pooled);
+    s.plan = nullptr; s.cap_tiles = 0;
+    void *p = nullptr;
+    const size_t bytes = (size_t)n_tiles * sizeof(int2) + 16;
+    if (pooled) HK_CUDA(cudaMallocAsync(&p, bytes, st)); else HK_CUDA(cudaMalloc(&p, bytes));
+    s.plan = (int2 *)p;
+    s.queue = (int *)((char *)p + (size_t)n_tiles * sizeof(int2));
     s.cap_tiles = n_tiles;
   }
   return HK_OK;
@@ -477,9 +609,30 @@ static int scratch_reserve(Scratch &s, int64_t n_lines, int n_tiles, cudaStream_
 
 static void scratch_release(Scratch &s, cudaStream_t st, bool pooled)
 {
-  if (s.meta) { if (pooled) { cudaFreeAsync(s.meta, st); cudaFreeAsync(s.base, st); cudaFreeAsync(s.gh2, st); } else { cudaFree(s.meta); cudaFree(s.base); cudaFree(s.gh2); } }
-  if (s.plan) { if (pooled) cudaFreeAsync(s.plan, st); else cudaFree(s.plan); }
+  dev_free(s.meta, st, pooled);
+  dev_free(s.plan, st, pooled);
   s = Scratch();
+}
+
+// persistent grid of a3: CTAs resident per SM x SMs of the current device (queried once per device)
+static int voigt_grid(int *grid_out)
+{
+  static int cached_dev = -1, cached_grid = 0;
+  int dev = 0;
+  HK_CUDA(cudaGetDevice(&dev));
+  if (dev != cached_dev) {
+    int sms = 0, per_sm = 0;
+    HK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    HK_CUDA(cudaFuncSetAttribute(voigt_kernel<kP, kWarps, kMinB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)sizeof(VoigtSmemT)));
+    HK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, voigt_kernel<kP, kWarps, kMinB>, (kWarps + 1) * 32,
+                                                          sizeof(VoigtSmemT)));
+    if (per_sm < 1) per_sm = 1;
+    cached_grid = sms * per_sm;
+    cached_dev = dev;
+  }
+  *grid_out = cached_grid;
+  return HK_OK;
 }
 
 static int validate(const hk_lines *lines, int64_t n_lines, double T, double P_atm, double nu_min, double nu_max, double dnu,
@@ -527,17 +680,22 @@ static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double 
   pa.inv_mg = 1.0 / m_g;
   pa.q_ratio = q_ratio;
   pa.nu_min = nu_min; pa.dnu = dnu; pa.cutoff = cutoff; pa.N = (int)N;
-  pa.meta = s.meta; pa.base = s.base; pa.gh2 = s.gh2;
+  pa.meta = s.meta; pa.base = s.base; pa.gh2 = s.gh2; pa.core = s.core;
   line_prep_kernel<<<(unsigned)((n_lines + 255) / 256), 256, 0, st>>>(pa);
   HK_CUDA(cudaGetLastError());
   if (g_timing) HK_CUDA(cudaEventRecord(ev[1], st));
-  tile_plan_kernel<<<(n_tiles + 127) / 128, 128, 0, st>>>(s.meta, n_lines, n_tiles, kTile, (int)N, s.plan);
+  tile_plan_kernel<<<(n_tiles + 127) / 128, 128, 0, st>>>(s.meta, n_lines, n_tiles, kTile, (int)N, s.plan, s.queue);
   HK_CUDA(cudaGetLastError());
   if (g_timing) HK_CUDA(cudaEventRecord(ev[2], st));
   VoigtArgs va;
-  va.meta = s.meta; va.base = s.base; va.gh2 = s.gh2; va.plan = s.plan;
+  va.meta = s.meta; va.base = s.base; va.gh2 = s.gh2; va.core = s.core; va.plan = s.plan; va.queue = s.queue;
+  va.n_tiles = n_tiles;
   va.nu_min = nu_min; va.dnu = dnu; va.N = (int)N; va.kappa = kappa_out;
-  voigt_kernel<kP, kWarps><<<n_tiles, kWarps * 32, 0, st>>>(va);
+  int grid = 0;
+  rc = voigt_grid(&grid);
+  if (rc != HK_OK) return rc;
+  if (grid > n_tiles) grid = n_tiles;
+  voigt_kernel<kP, kWarps, kMinB><<<grid, (kWarps + 1) * 32, sizeof(VoigtSmemT), st>>>(va);
   HK_CUDA(cudaGetLastError());
   if (g_timing) {
     HK_CUDA(cudaEventRecord(ev[3], st));
@@ -688,9 +846,7 @@ int hk_regime_census(const double *nu0_host, const double *gamma0_host, int64_t 
     if (!(alpha > 0.0)) { c[0] += tot; continue; }
     const double gamma = gamma0_host[i] * P_atm * tfac, a2 = alpha * alpha, g2 = gamma * gamma, y = gamma / alpha;
     auto rho = [&](double R) { const double t = R * a2 - g2; return t > 0.0 ? sqrt(t) : 0.0; };
-    double xc2 = kRc - y * y;
-    if (y < 1e-8) xc2 = fmax(xc2, -log(1e-10 * fmax(y, 1e-300)));
-    xc2 = fmin(xc2, kXcapSq);
+    const double xc2 = core_xc2(y);
     const int64_t n1 = within(nu0, rho(kR1), jl, jh), n2 = within(nu0, rho(kR2), jl, jh), n3 = within(nu0, rho(kR3), jl, jh);
     const int64_t nc = xc2 > 0.0 ? within(nu0, sqrt(xc2) * alpha, jl, jh) : 0;
     const int64_t ncore = nc < n3 ? nc : n3;

@@ -3,13 +3,13 @@
 // The profile value of one line at one grid point (eq. 19),
 //     V(d) = K(d/alpha, gamma/alpha) / (alpha sqrt(pi)),     K(x,y) = H_V = Re w(x+iy)
 // is evaluated in one of five regimes chosen on r^2 = x^2 + y^2 (PAPER.md:197 gives the three-regime
-// structure and calls its switch points "trial-and-error"; DESIGN.md "Regimes" derives these):
+// structure and calls its switch points "trial-and-error"; DESIGN.md §4 derives these):
 //
 //   r^2 >= 6.0e6 : 1-point Gauss-Hermite  (a Lorentzian)                      5 FP64 + 1 MUFU per point
 //   r^2 >= 3200  : 2-point Gauss-Hermite                                       7 FP64 + 1 MUFU
 //   r^2 >= 280   : 3-point Gauss-Hermite ("third-order", Letchworth & Benner) 11 FP64 + 1 MUFU
-//   r^2 >= 44    : 6-point Gauss-Hermite                                      19 FP64 + 3 MUFU
-//   else         : Algorithm-916-type series (Zaghloul & Ali 2012), step a = 0.7, ~16 terms
+//   r^2 >= 44    : 6-point Gauss-Hermite                                      22 FP64 + 3 MUFU
+//   else         : Algorithm-916-type series (Zaghloul & Ali 2012), step a = 0.7, 16 terms
 //
 // n-point Gauss-Hermite in dimensional form (no 1/alpha, safe as alpha -> 0), with nodes +-t_k, normalised
 // weights wn_k (sum 1) and q = d^2:
@@ -27,16 +27,17 @@ constexpr double kR1 = 6.0e6;   // 1-point rule from here   (max rel. error 2.5e
 constexpr double kR2 = 3200.0;  // 2-point rule             (2.4e-7)
 constexpr double kR3 = 280.0;   // 3-point rule             (2.4e-7)
 constexpr double kRc = 44.0;    // 6-point rule from here (3.7e-8); series below
-constexpr double kXcapSq = 289.0;  // series usable up to x = 17 (32 lane-held terms at a = 0.7)
+constexpr double kXgCapSq = 270.0;  // the Gaussian term is never added beyond the 6-point region (exp(-270) = 5e-118)
+constexpr double kTinyY = 1.0e-8;   // below this damping the wing rules miss a visible exp(-x^2) beyond r^2 = 44
 
 constexpr double kPi = 3.14159265358979323846;
+constexpr double kInvPi = 0.31830988618379067153776753;
 constexpr double kSqrtPi = 1.772453850905516027298167;
 constexpr double kInvSqrtPi = 0.5641895835477562869480795;
 
 // Algorithm-916-type series constants, step a = 0.7 (truncation error 1.1e-8 relative, uniform in y)
 constexpr double kA = 0.7;
-constexpr double kExpA2 = 0.61262639418441606898858;      // exp(-a^2)
-constexpr double kExp2A2 = 0.3753110988513995387142672;   // exp(-2 a^2)
+constexpr int kTerms = 16;                                // a n <= x + 4.4 for x <= sqrt(44)
 constexpr double k2AoverPi = 0.4456338406573069401528745; // 2a/pi
 constexpr double kAoverPi = 0.2228169203286534700764373;  // a/pi
 
@@ -59,6 +60,13 @@ __device__ __forceinline__ double rcp_nr(double x)
   double r0 = rcp_seed(x);
   double e = fma(-x, r0, 1.0);
   return fma(r0, e, r0);
+}
+// 1/x to ~2^-80 (two Newton steps): for the few per-line reciprocals that feed the series
+__device__ __forceinline__ double rcp_nr2(double x)
+{
+  double r = rcp_nr(x);
+  double e = fma(-x, r, 1.0);
+  return fma(r, e, r);
 }
 
 // ---- wing rules: contribution amp * V(d) added to acc --------------------------------------------------
@@ -88,103 +96,114 @@ __device__ __forceinline__ double gh3_acc(double acc, double d, double g2, doubl
   double num = fma(c0, D, B * R);
   return fma(num, rcp_nr(R * D), acc);
 }
-// one +-t pair of an n-point rule: 2 wn (E + 2 t^2 a2)/(E^2 + f)
-__device__ __forceinline__ double gh_pair(double q, double g2, double a2, double tsq, double wn)
+// per-line constants of one +-t pair of the 6-point rule: E = q + e, value = (cE * E + c0) / (E^2 + f)
+struct GhPair {
+  double e, f, cE, c0;
+};
+__device__ __forceinline__ GhPair gh_pair_consts(double A1, double g2, double a2, double tsq, double wn)
 {
-  double E = q + (g2 - tsq * a2);
-  double D = fma(E, E, 4.0 * tsq * a2 * g2);
-  return 2.0 * wn * (E + 2.0 * tsq * a2) * rcp_nr(D);
+  GhPair p;
+  p.e = g2 - tsq * a2;
+  p.f = 4.0 * tsq * a2 * g2;
+  p.cE = 2.0 * wn * A1;
+  p.c0 = p.cE * (2.0 * tsq * a2);
+  return p;
 }
-// 6-point: V/(gamma/pi)
-__device__ __forceinline__ double gh6_shape(double q, double g2, double a2)
+__device__ __forceinline__ double gh_pair_val(double q, const GhPair &p)
 {
-  return gh_pair(q, g2, a2, kT6sq0, kW6_0) + gh_pair(q, g2, a2, kT6sq1, kW6_1) + gh_pair(q, g2, a2, kT6sq2, kW6_2);
+  double E = q + p.e;
+  double D = fma(E, E, p.f);
+  return fma(p.cE, E, p.c0) * rcp_nr(D);
+}
+struct Gh6 {
+  GhPair p0, p1, p2;
+};
+__device__ __forceinline__ Gh6 gh6_consts(double A1, double g2, double a2)
+{
+  Gh6 g;
+  g.p0 = gh_pair_consts(A1, g2, a2, kT6sq0, kW6_0);
+  g.p1 = gh_pair_consts(A1, g2, a2, kT6sq1, kW6_1);
+  g.p2 = gh_pair_consts(A1, g2, a2, kT6sq2, kW6_2);
+  return g;
+}
+// 6-point: amp * V(d), 3 x (DADD + 4 DFMA/DMUL + Newton reciprocal) + 2 DADD = 22 FP64 + 3 MUFU
+__device__ __forceinline__ double gh6_val(double q, const Gh6 &g)
+{
+  return gh_pair_val(q, g.p0) + gh_pair_val(q, g.p1) + gh_pair_val(q, g.p2);
 }
 
-// ---- core: Algorithm-916-type series (restated in DESIGN.md "Core series") ----------------
-//   K(x,y) = exp(-x^2) [ erfcx(y) cos(2xy) + (2a/pi) sin^2(xy)/y - (2a/pi) y cos(2xy) S1(y) ]
-//          + (a/pi) y sum_{n>=1} [exp(-(an-x)^2) + exp(-(an+x)^2)] / (a^2 n^2 + y^2),
-//   S1(y) = sum_{n>=1} exp(-a^2 n^2)/(a^2 n^2 + y^2).
-// y is a per-line constant, so the warp holds 1/(a^2 n^2 + y^2) for n = lane+1 in a register and the series
-// loop broadcasts it with SHFL; exp(-(an -+ x)^2) advance by the recurrence
-//   T(n) = T(n-1) * exp(-a^2 (2n-1)) * exp(+-2 a x),  T(0) = exp(-x^2)   (each T <= 1: no overflow).
+// ---- core: Algorithm-916-type series (restated in DESIGN.md §4) ---------------------------
+//   K(x,y) = exp(-x^2) [ erfcx(y) cos(2xy) + (2a/pi) sin^2(xy)/y - (2a/pi) y cos(2xy) S1(y)
+//                        + (a/pi) y sum_{n=1..16} W_n (p^n + p^-n) ],
+//   W_n = exp(-a^2 n^2)/(a^2 n^2 + y^2),  S1 = sum_n W_n,  p = exp(2 a x)
+// (exp(-(an-x)^2) + exp(-(an+x)^2) = exp(-x^2) exp(-a^2 n^2) (p^n + p^-n)).  y is a per-line constant: lane n-1 of the
+// warp holds W_n and the series loop broadcasts it with SHFL; C_n = p^n + p^-n advances by the three-term recurrence
+// C_{n+1} = (p + 1/p) C_n - C_{n-1} (forward-stable: the growing solution dominates), so a term is 2 DFMA + 1 SHFL.
+// p^16 <= exp(1.4 * 6.64 * 16) = 4e64: no overflow for x <= sqrt(44).
 struct CoreLine {
-  double y, erfcx_y, S1, wn;  // wn is lane-dependent: 1/(a^2 (lane+1)^2 + y^2)
-  int nterms;
+  double y, inv_y, erfcx_y, S1, W;  // W is lane-dependent: W_{lane+1} (0 for lane >= 16)
 };
 
-// All 32 lanes must call (warp-collective).
-__device__ __forceinline__ CoreLine core_setup(double y, double xmax)
+// exp(-a^2 n^2) for n = lane + 1 (0 beyond the 16 terms): a per-lane constant, computed once per kernel
+__device__ __forceinline__ double core_lane_const()
+{
+  const int lane = threadIdx.x & 31;
+  const double n = (double)(lane + 1);
+  return lane < kTerms ? exp(-kA * kA * n * n) : 0.0;
+}
+
+// All 32 lanes must call (warp-collective).  En = core_lane_const().
+__device__ __forceinline__ CoreLine core_setup(double y, double erfcx_y, double En)
 {
   CoreLine c;
   const int lane = threadIdx.x & 31;
   const double n = (double)(lane + 1);
-  const double an2 = kA * kA * n * n;
   c.y = y;
-  c.wn = 1.0 / (an2 + y * y);
-  double term = exp(-an2) * c.wn;
+  c.inv_y = 1.0 / y;
+  c.erfcx_y = erfcx_y;
+  c.W = En * rcp_nr2(fma(kA * kA * n, n, y * y));
+  double t = c.W;
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) term += __shfl_xor_sync(kFull, term, o);
-  c.S1 = term;
-  c.erfcx_y = erfcx(y);
-  int nt = (int)ceil((xmax + 4.4) / kA);
-  c.nterms = nt > 32 ? 32 : nt;
+  for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(kFull, t, o);
+  c.S1 = t;
   return c;
 }
 
-// All 32 lanes must call with the same CoreLine (warp-collective: SHFL inside).  x >= 0, x <= 17.
+// All 32 lanes must call with the same CoreLine (warp-collective: SHFL inside).  0 <= x <= 6.7.
 __device__ __forceinline__ double core_K(double x, const CoreLine &c)
 {
   const double ex2 = exp(-x * x);
   const double p = exp(2.0 * kA * x);
-  const double qq = 1.0 / p;
-  const double s = sin(x * c.y);
+  const double s2c = p + rcp_nr2(p);  // 2 cosh(2 a x)
+  double Cm = 2.0, C = s2c, sum = 0.0;
+#pragma unroll
+  for (int n = 0; n < kTerms; ++n) {
+    const double w = __shfl_sync(kFull, c.W, n);
+    sum = fma(w, C, sum);
+    const double Cn = fma(s2c, C, -Cm);
+    Cm = C;
+    C = Cn;
+  }
+  const double s = sinpi(x * c.y * kInvPi);  // x y <= 44; sinpi has no slow range-reduction path
   const double s2 = s * s;
   const double c2 = fma(-2.0, s2, 1.0);
-  double Tm = ex2, Tp = ex2, ck = kExpA2, sum = 0.0;
-  for (int k = 0; k < c.nterms; ++k) {
-    Tm *= ck * p;
-    Tp *= ck * qq;
-    const double w = __shfl_sync(kFull, c.wn, k);
-    sum = fma(w, Tm + Tp, sum);
-    ck *= kExp2A2;
-  }
-  const double head = c.erfcx_y * c2 + k2AoverPi * (s * (s / c.y)) - k2AoverPi * c.y * c2 * c.S1;
-  return fma(ex2, head, kAoverPi * c.y * sum);
+  const double head = fma(c.erfcx_y, c2, k2AoverPi * (s2 * c.inv_y)) - k2AoverPi * c.y * c2 * c.S1;
+  return ex2 * fma(kAoverPi * c.y, sum, head);
 }
 
-// Per-line quantities the near path derives once per (line, warp).
-struct NearLine {
-  double nu0, A1, g2, a2, inv_alpha, inv_a2, y, Acore, xc2;
-};
-
-// Wing value amp*V(d) for one point with the regime chosen per thread (divergent; near path and test hook only).
-// Valid for r^2 >= xc2-region complement, i.e. the caller handles the core separately.
-__device__ __forceinline__ double wing_value(double d, const NearLine &L)
+// series region of a line of damping y: x^2 < xc2 = 44 - y^2 (none for y >= sqrt(44))
+__device__ __host__ __forceinline__ double core_xc2(double y)
 {
-  const double q = d * d;
-  const double r2 = (L.a2 > 0.0) ? (q + L.g2) * L.inv_a2 : __longlong_as_double(0x7ff0000000000000LL);
-  if (r2 >= kR1) {
-    return gh1_acc(0.0, d, L.A1, L.g2);
-  } else if (r2 >= kR2) {
-    return gh2_acc(0.0, d, L.A1, L.g2 - 0.5 * L.a2, 2.0 * L.a2 * L.g2, L.A1 * L.a2);
-  } else if (r2 >= kR3) {
-    const double c3 = L.A1 * (1.0 / 3.0);
-    return gh3_acc(0.0, d, L.g2, L.g2 - 1.5 * L.a2, 6.0 * L.a2 * L.g2, 2.0 * c3, c3, L.A1 * L.a2);
-  } else {
-    return L.A1 * gh6_shape(q, L.g2, L.a2);
-  }
-}
-
-// core switch in x^2 for a line of damping y: series where x^2 < xc2.  Beyond the ring r^2 = 44 the 6-point rule is
-// good to 3.7e-8 except that no wing rule carries the Gaussian term exp(-x^2); for y < 1e-8 that term is still
-// > 1e-10 of K at r^2 = 44, so the series region is widened to x^2 < -ln(1e-10 y) (capped by the 32-term table).
-__device__ __forceinline__ double core_xc2(double y)
-{
-  double xc2 = kRc - y * y;
-  if (y < 1e-8) xc2 = fmax(xc2, -log(1e-10 * fmax(y, 1e-300)));
-  xc2 = fmin(xc2, kXcapSq);
+  const double xc2 = kRc - y * y;
   return xc2 > 0.0 ? xc2 : 0.0;
+}
+// No wing rule carries the Gaussian term exp(-x^2).  For y < 1e-8 it is still > 1e-10 of K beyond the series region, so
+// the 6-point rule adds it out to x^2 = xg2 = -ln(1e-10 y)  (K = exp(-x^2) + wing + O(y^2)); 0 = never.
+__device__ __host__ __forceinline__ double gauss_xg2(double y)
+{
+  if (!(y < kTinyY)) return 0.0;
+  const double v = -log(1e-10 * (y > 1e-300 ? y : 1e-300));
+  return v < kXgCapSq ? v : kXgCapSq;
 }
 
 }  // namespace hk
