@@ -22,15 +22,18 @@
 namespace hk {
 
 // ------------------------------------------------------------------------------------------------------
-// packed line records (written by a1, streamed by a3).  Four 32-byte records per line, structure of arrays,
-// so that a chunk of lines is four contiguous 16-byte-aligned spans (one TMA bulk copy each).
+// packed line records (written by a1, streamed by a3): two 16-byte and three 32-byte records per line, structure of
+// arrays, so that a chunk of lines is five contiguous 16-byte-aligned spans (one TMA bulk copy each) and a warp that
+// classifies 32 lines at once (lane = line) reads the 16-byte meta records without shared-memory bank conflicts.
 // ------------------------------------------------------------------------------------------------------
-struct __align__(16) LineMeta {
+struct __align__(16) MetaA {
   int jlo, jhi;  // inclusive index window of the line (empty if jhi < jlo)
   float c;       // line centre in grid units, (nu0-nu_min)/dnu
-  float r1;      // |j-c| >= r1 on a whole group of points  =>  r^2 >= kR1 there (1-point rule valid); conservative (+2)
+  float r3;      // |j-c| >= r3 on a whole group of points  =>  r^2 >= kR3 there (3-point rule valid); conservative
+};
+struct __align__(16) MetaB {
+  float r1;      // likewise kR1 (1-point rule)
   float r2;      // likewise kR2 (2-point rule)
-  float r3;      // likewise kR3 (3-point rule)
   float r6;      // likewise kRc (6-point rule); inside it the series region may begin
   float rg;      // the 6-point rule adds the Gaussian term on groups closer than this (0 unless y < 1e-8)
 };
@@ -43,8 +46,10 @@ struct __align__(16) LineGH2 {
 struct __align__(16) LineCore {
   double y, erfcx_y, Acore, xc2;  // gamma/alpha; erfcx(y); amp/(alpha sqrt(pi)); series where x^2 < xc2
 };
-static_assert(sizeof(LineMeta) == 32 && sizeof(LineBase) == 32 && sizeof(LineGH2) == 32 && sizeof(LineCore) == 32,
+static_assert(sizeof(MetaA) == 16 && sizeof(MetaB) == 16 && sizeof(LineBase) == 32 && sizeof(LineGH2) == 32 &&
+                  sizeof(LineCore) == 32,
               "record size");
+constexpr size_t kBytesPerLine = sizeof(MetaA) + sizeof(MetaB) + sizeof(LineBase) + sizeof(LineGH2) + sizeof(LineCore);
 
 constexpr double kCLight = 2.99792458e10;   // cm/s
 constexpr double kBoltz = 1.380649e-16;     // erg/K
@@ -61,18 +66,20 @@ struct PrepArgs {
   double q_ratio;
   double nu_min, dnu, cutoff;
   int N;
-  LineMeta *meta;
+  double margin;  // grid units added to every regime radius: covers the float rounding of c and of the span ends
+  MetaA *ma;
+  MetaB *mb;
   LineBase *base;
   LineGH2 *gh2;
   LineCore *core;
 };
 
 // grid-unit radius outside which x^2 + y^2 >= R holds: sqrt(R alpha^2 - gamma^2)/dnu, rounded outward
-__device__ __forceinline__ float radius_grid(double R, double a2, double g2, double inv_dnu)
+__device__ __forceinline__ float radius_grid(double R, double a2, double g2, double inv_dnu, double margin)
 {
   double t = R * a2 - g2;
   if (!(t > 0.0)) return 0.0f;
-  double r = sqrt(t) * inv_dnu + 2.0;
+  double r = sqrt(t) * inv_dnu + margin;
   return r < 3.0e38 ? __double2float_ru(r) : 3.0e38f;
 }
 
@@ -115,20 +122,22 @@ __global__ void __launch_bounds__(256) line_prep_kernel(PrepArgs a)
   if (!(hi < (double)(a.N - 1))) hi = (double)(a.N - 1);
   if (lo > 2.0e9) lo = 2.0e9;
   if (hi < -2.0e9) hi = -2.0e9;
-  LineMeta m;
-  m.jlo = (int)lo;
-  m.jhi = (int)hi;
+  MetaA ma;
+  MetaB mb;
+  ma.jlo = (int)lo;
+  ma.jhi = (int)hi;
   const double inv_dnu = 1.0 / a.dnu;
   double c = (nu0 - a.nu_min) * inv_dnu;
   c = fmin(fmax(c, -3.0e9), 3.0e9);
-  m.c = (float)c;
-  m.r1 = radius_grid(kR1, a2, g2, inv_dnu);
-  m.r2 = radius_grid(kR2, a2, g2, inv_dnu);
-  m.r3 = radius_grid(kR3, a2, g2, inv_dnu);
-  m.r6 = radius_grid(kRc, a2, g2, inv_dnu);
+  ma.c = (float)c;
+  mb.r1 = radius_grid(kR1, a2, g2, inv_dnu, a.margin);
+  mb.r2 = radius_grid(kR2, a2, g2, inv_dnu, a.margin);
+  ma.r3 = radius_grid(kR3, a2, g2, inv_dnu, a.margin);
+  mb.r6 = radius_grid(kRc, a2, g2, inv_dnu, a.margin);
   const double xg2 = alpha > 0.0 ? gauss_xg2(k.y) : 0.0;
-  m.rg = xg2 > 0.0 ? __double2float_ru(sqrt(xg2) * alpha * inv_dnu + 2.0) : 0.0f;
-  a.meta[i] = m;
+  mb.rg = xg2 > 0.0 ? __double2float_ru(sqrt(xg2) * alpha * inv_dnu + a.margin) : 0.0f;
+  a.ma[i] = ma;
+  a.mb[i] = mb;
   a.base[i] = b;
   a.gh2[i] = g;
   a.core[i] = k;
@@ -136,7 +145,7 @@ __global__ void __launch_bounds__(256) line_prep_kernel(PrepArgs a)
 
 // a2: lines are sorted by nu0, so jlo and jhi are non-decreasing in i.  Tile t owns points [t*tile, (t+1)*tile).
 // plan[t] = [first i with jhi >= tile_lo, first i with jlo > tile_hi).  Thread 0 also resets the tile queue of a3.
-__global__ void __launch_bounds__(128) tile_plan_kernel(const LineMeta *meta, int64_t n, int n_tiles, int tile, int N,
+__global__ void __launch_bounds__(128) tile_plan_kernel(const MetaA *meta, int64_t n, int n_tiles, int tile, int N,
                                                         int2 *plan, int *queue)
 {
   int t = blockIdx.x * blockDim.x + threadIdx.x;
@@ -202,22 +211,25 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
 // ------------------------------------------------------------------------------------------------------
 // a3 + a4: Voigt accumulation.  Persistent CTAs of WARPS consumer warps + 1 producer warp.
 //
-// Work unit = tile of WARPS*32*P consecutive grid points, pulled from an atomic queue (ascending wavenumber).  Consumer
-// warp w owns the span [tile_lo + w*32P, +32P), lane l the points span_lo + l + 32k (k < P): stores are coalesced, every 32
-// consecutive points ("group") belong to one k, and a thread carries P independent dependency chains.
+// Work unit = tile of WARPS*32*P consecutive grid points, pulled from an atomic queue.  Consumer warp w owns the span
+// [tile_lo + w*32P, +32P), lane l the points span_lo + l + 32k (k < P): stores are coalesced, every 32 consecutive points
+// ("group") belong to one k, and a thread carries P independent dependency chains.
 //
 // The producer warp streams the lines of the tile's plan range through a STAGES-deep shared-memory ring in chunks of CH
-// lines: four 1-D TMA bulk copies per chunk (meta/base/gh2/core spans) completing on the stage's `full` mbarrier; each
+// lines: five 1-D TMA bulk copies per chunk (the five record spans) completing on the stage's `full` mbarrier; each
 // consumer warp releases the stage on its `empty` mbarrier.  No CTA-wide barrier exists after start-up: warps drift apart by
 // up to STAGES-1 chunks, and the ring keeps flowing across tile boundaries (each stage carries a header naming its tile).
 //
-// For every (line, warp span) the regime is chosen ONCE from the span's distance to the line centre (float, grid units,
-// conservative radii from a1): a warp-uniform branch into an unrolled P-point loop of the 1-, 2- or 3-point rule, accumulated
-// in registers.  Spans that reach inside the 3-point radius or straddle a cutoff edge take the near path: the same choice per
-// 32-point group (still warp-uniform), the series only on groups that hold core points, accumulated in a per-warp
-// shared-memory strip (dynamic k without spilling the register accumulators).  Summation order is fixed: bitwise deterministic.
+// A consumer warp handles a chunk 32 lines at a time.  First it CLASSIFIES them, lane = line: from the span's distance to
+// the line centre (float, grid units, conservative radii from a1) each lane picks the rule valid on the whole span, and four
+// ballots turn that into bit masks (1-, 2-, 3-point rule, near).  Then it walks each mask: a branch-free loop over the lines
+// of one rule, parameters broadcast from shared memory, an unrolled P-point body accumulating in registers.  The regime
+// decision thus costs ~1 instruction per (line, span) instead of a branch ladder, and the per-rule loops have no divergence.
+// Spans that reach inside the 3-point radius or straddle a cutoff edge take the near path: the rule is chosen per 32-point
+// group (still warp-uniform), the series only on groups that hold core points, accumulated in a per-warp shared-memory
+// strip (dynamic k without spilling the register accumulators).  Summation order is fixed: bitwise deterministic.
 // ------------------------------------------------------------------------------------------------------
-constexpr int CH = 128;     // lines per ring stage: 4 x 4 KB
+constexpr int CH = 128;     // lines per ring stage: 128 lines x 128 B
 constexpr int STAGES = 4;
 
 struct __align__(16) StageHdr {
@@ -229,21 +241,25 @@ struct __align__(16) StageHdr {
 
 template <int P, int WARPS>
 struct __align__(128) VoigtSmem {
-  LineMeta meta[STAGES][CH];
+  MetaA ma[STAGES][CH];
+  MetaB mb[STAGES][CH];
   LineBase base[STAGES][CH];
   LineGH2 gh2[STAGES][CH];
   LineCore core[STAGES][CH];
   double sk[WARPS][32 * P];
+  double En[kTerms];  // exp(-a^2 n^2), n = 1..16: lane constants of the series
   StageHdr hdr[STAGES];
   uint64_t full[STAGES], empty[STAGES];
 };
 
 struct VoigtArgs {
-  const LineMeta *meta;
+  const MetaA *ma;
+  const MetaB *mb;
   const LineBase *base;
   const LineGH2 *gh2;
   const LineCore *core;
   const int2 *plan;
+  const int *order;  // tiles in the order they are handed out (descending cost), or NULL: ascending index
   int *queue;
   int n_tiles;
   double nu_min, dnu;
@@ -252,50 +268,93 @@ struct VoigtArgs {
 };
 
 // near path of a3 for one (line, warp span): rule per 32-point group (warp-uniform), accumulated in the warp's shared-memory
-// strip sk[32k + lane].  Kept out of line so that its constants (6-point pairs, series state) do not compete for registers
-// with the P accumulators of the far loops.  Warp-collective (SHFL in the series).
+// strip sk[32k + lane].  Warp-collective (SHFL in the series).
 template <int P>
-__device__ __noinline__ void near_span(const LineMeta m, const LineBase *pb, const LineGH2 *pg, const LineCore *pk, int slo,
-                                       int lane, float dist, double x0, double dnu, double En, double *sk)
+__device__ __forceinline__ void near_span(const MetaA *pa, const MetaB *pm, const LineBase *pb, const LineGH2 *pg,
+                                       const LineCore *pk, int slo, int lane, double x0, double dnu, double En, double *sk)
 {
+  const MetaA ma = *pa;
+  const MetaB mb = *pm;
   const LineBase b = *pb;
   const LineGH2 g = *pg;
+  const float dist = fmaxf(fmaxf((float)slo - ma.c, ma.c - (float)(slo + 32 * P - 1)), 0.0f);
   const double d0 = x0 - b.nu0;
   Gh6 G6;
   LineCore kc;
   CoreLine C;
-  if (dist < m.r3) {  // some group may need the 6-point rule or the series
+  if (dist < ma.r3) {  // some group may need the 6-point rule or the series
     G6 = gh6_consts(b.A1, b.g2, b.a2);
     kc = *pk;
-    if (dist < m.r6) C = core_setup(kc.y, kc.erfcx_y, En);
+    if (dist < mb.r6) C = core_setup(kc.y, kc.erfcx_y, En);
   }
 #pragma unroll 1
   for (int k = 0; k < P; ++k) {
     const int glo = slo + 32 * k, ghi = glo + 31;
-    if (ghi < m.jlo || glo > m.jhi) continue;
+    if (ghi < ma.jlo || glo > ma.jhi) continue;
     const int j = glo + lane;
-    const bool inwin = (j >= m.jlo) && (j <= m.jhi);
+    const bool inwin = (j >= ma.jlo) && (j <= ma.jhi);
     const double d = fma((double)(32 * k), dnu, d0);
-    const float dg = fmaxf(fmaxf((float)glo - m.c, m.c - (float)ghi), 0.0f);
+    const float dg = fmaxf(fmaxf((float)glo - ma.c, ma.c - (float)ghi), 0.0f);
     double v;
-    if (dg >= m.r2) {
-      v = dg >= m.r1 ? gh1_acc(0.0, d, b.A1, b.g2) : gh2_acc(0.0, d, b.A1, g.e2, g.f2, g.A1a2);
-    } else if (dg >= m.r3) {
+    if (dg >= mb.r2) {
+      v = dg >= mb.r1 ? gh1_acc(0.0, d, b.A1, b.g2) : gh2_acc(0.0, d, b.A1, g.e2, g.f2, g.A1a2);
+    } else if (dg >= ma.r3) {
       const double c3 = b.A1 * (1.0 / 3.0);
       v = gh3_acc(0.0, d, b.g2, fma(-1.5, b.a2, b.g2), 6.0 * b.a2 * b.g2, 2.0 * c3, c3, b.A1 * b.a2);
     } else {
       v = gh6_val(d * d, G6);
-      if (dg < m.r6) {  // the series region reaches into this group
+      if (dg < mb.r6) {  // the series region reaches into this group
         const double x = fabs(d) * g.inv_alpha;
         const double ks = core_K(fmin(x, 6.7), C);
         if (x * x < kc.xc2) v = kc.Acore * ks;
-        else if (m.rg > 0.0f) v = fma(kc.Acore, exp(-x * x), v);
-      } else if (dg < m.rg) {
+        else if (mb.rg > 0.0f) v = fma(kc.Acore, exp(-x * x), v);
+      } else if (dg < mb.rg) {
         const double x = d * g.inv_alpha;
         v = fma(kc.Acore, exp(-x * x), v);
       }
     }
     sk[32 * k + lane] += inwin ? v : 0.0;
+  }
+}
+
+// lane = line classification of 32 lines of a chunk against the warp span [slo, slo + 32P): bit masks of the lines that
+// take the 1-, 2-, 3-point rule on the whole span, and of the near lines (span inside the 3-point radius or on a cutoff edge)
+template <int P>
+__device__ __forceinline__ void classify32(const MetaA *ma, const MetaB *mb, int l, int cnt, int slo, unsigned &m1,
+                                           unsigned &m2, unsigned &m3, unsigned &mn)
+{
+  const int shi = slo + 32 * P - 1;
+  const MetaA A = ma[l];
+  const MetaB B = mb[l];
+  const bool act = (l < cnt) && (A.jhi >= slo) && (A.jlo <= shi);
+  const bool inside = (A.jlo <= slo) && (A.jhi >= shi);
+  const float dist = fmaxf(fmaxf((float)slo - A.c, A.c - (float)shi), 0.0f);
+  const bool far = act && inside && (dist >= A.r3);
+  m1 = __ballot_sync(kFull, far && dist >= B.r1);
+  m2 = __ballot_sync(kFull, far && dist < B.r1 && dist >= B.r2);
+  m3 = __ballot_sync(kFull, far && dist < B.r2);
+  mn = __ballot_sync(kFull, act && !far);
+}
+
+// near pass over one chunk: kept out of line (one call per chunk) so that the 6-point and series state never competes for
+// registers with the far loops; the accumulators live in the shared-memory strip across the call.
+template <int P>
+__device__ __noinline__ void near_pass(const MetaA *ma, const MetaB *mb, const LineBase *base, const LineGH2 *gh2,
+                                       const LineCore *core, int cnt, int slo, double nu_min, double dnu, const double *En_tab,
+                                       double *sk)
+{
+  const int lane = threadIdx.x & 31;
+  const double En = lane < kTerms ? En_tab[lane] : 0.0;
+  const double x0 = __dadd_rn(nu_min, __dmul_rn((double)(slo + lane), dnu));
+#pragma unroll 1
+  for (int b0 = 0; b0 < cnt; b0 += 32) {
+    unsigned m1, m2, m3, mn;
+    classify32<P>(ma, mb, b0 + lane, cnt, slo, m1, m2, m3, mn);
+#pragma unroll 1
+    for (unsigned m = mn; m; m &= m - 1) {
+      const int i = b0 + (__ffs(m) - 1);
+      near_span<P>(ma + i, mb + i, base + i, gh2 + i, core + i, slo, lane, x0, dnu, En, sk);
+    }
   }
 }
 
@@ -317,6 +376,8 @@ __global__ void __launch_bounds__((WARPS + 1) * 32, MINB) voigt_kernel(const __g
   if (warp < WARPS) {
 #pragma unroll
     for (int k = 0; k < P; ++k) S.sk[warp][32 * k + lane] = 0.0;
+  } else if (lane < kTerms) {
+    S.En[lane] = core_lane_const();
   }
   __syncthreads();  // the only CTA-wide barrier
 
@@ -326,10 +387,11 @@ __global__ void __launch_bounds__((WARPS + 1) * 32, MINB) voigt_kernel(const __g
     int stage = 0;
     uint32_t phase = 0;
     for (;;) {
-      const int tile = atomicAdd(a.queue, 1);
-      const bool stop = tile >= a.n_tiles;
-      int L0 = 0, nl = 0;
+      const int ticket = atomicAdd(a.queue, 1);
+      const bool stop = ticket >= a.n_tiles;
+      int tile = 0, L0 = 0, nl = 0;
       if (!stop) {
+        tile = a.order ? a.order[ticket] : ticket;
         const int2 pl = a.plan[tile];
         L0 = pl.x;
         nl = pl.y - pl.x;
@@ -344,14 +406,15 @@ __global__ void __launch_bounds__((WARPS + 1) * 32, MINB) voigt_kernel(const __g
         h.flags = (c == 0 ? 1 : 0) | (c == nchunks - 1 ? 2 : 0);
         h.pad = 0;
         S.hdr[stage] = h;
-        const uint32_t bytes = (uint32_t)h.cnt * 32u;
-        mbar_expect_tx(&S.full[stage], 4u * bytes);  // release: the header store above is visible to the waiters
-        if (bytes) {
+        const uint32_t n = (uint32_t)h.cnt;
+        mbar_expect_tx(&S.full[stage], n * (uint32_t)kBytesPerLine);  // release: the header store above is visible to the waiters
+        if (n) {
           const int first = L0 + c * CH;
-          bulk_g2s(&S.meta[stage][0], a.meta + first, bytes, &S.full[stage]);
-          bulk_g2s(&S.base[stage][0], a.base + first, bytes, &S.full[stage]);
-          bulk_g2s(&S.gh2[stage][0], a.gh2 + first, bytes, &S.full[stage]);
-          bulk_g2s(&S.core[stage][0], a.core + first, bytes, &S.full[stage]);
+          bulk_g2s(&S.ma[stage][0], a.ma + first, n * 16u, &S.full[stage]);
+          bulk_g2s(&S.mb[stage][0], a.mb + first, n * 16u, &S.full[stage]);
+          bulk_g2s(&S.base[stage][0], a.base + first, n * 32u, &S.full[stage]);
+          bulk_g2s(&S.gh2[stage][0], a.gh2 + first, n * 32u, &S.full[stage]);
+          bulk_g2s(&S.core[stage][0], a.core + first, n * 32u, &S.full[stage]);
         }
         if (++stage == STAGES) {
           stage = 0;
@@ -363,14 +426,8 @@ __global__ void __launch_bounds__((WARPS + 1) * 32, MINB) voigt_kernel(const __g
   }
 
   // ---------------- consumers ----------------
-  double *sk = S.sk[warp];
-  const double En = core_lane_const();
-  double acc[P];
-#pragma unroll
-  for (int k = 0; k < P; ++k) acc[k] = 0.0;
-  int slo = 0, shi = 0;
-  float slo_f = 0.f, shi_f = 0.f;
-  double x0 = 0.0;  // nu of this thread's k = 0 point
+  double *sk = S.sk[warp];  // this warp's accumulators between chunks (zero at the start of a tile)
+  int slo = 0;
   int stage = 0;
   uint32_t phase = 0;
 
@@ -378,51 +435,63 @@ __global__ void __launch_bounds__((WARPS + 1) * 32, MINB) voigt_kernel(const __g
     mbar_wait(&S.full[stage], phase);
     const StageHdr h = S.hdr[stage];
     if (h.tile_lo < 0) break;
-    if (h.flags & 1) {
-      slo = h.tile_lo + warp * (32 * P);
-      shi = slo + 32 * P - 1;
-      slo_f = (float)slo;
-      shi_f = (float)shi;
-      x0 = __dadd_rn(a.nu_min, __dmul_rn((double)(slo + lane), a.dnu));  // nu_j exactly as defined (A6)
-    }
+    if (h.flags & 1) slo = h.tile_lo + warp * (32 * P);
+    const LineBase *sbase = S.base[stage];
+    const LineGH2 *sgh2 = S.gh2[stage];
+    unsigned any_near = 0;
+    {
+      // ---- far pass: register accumulators ----
+      const double x0 = __dadd_rn(a.nu_min, __dmul_rn((double)(slo + lane), a.dnu));  // nu_j exactly as defined (A6)
+      double acc[P];
+#pragma unroll
+      for (int k = 0; k < P; ++k) acc[k] = sk[32 * k + lane];
 #pragma unroll 1
-    for (int l = 0; l < h.cnt; ++l) {
-      const LineMeta m = S.meta[stage][l];
-      if (m.jhi < slo || m.jlo > shi) continue;
-      const bool inside = (m.jlo <= slo) && (m.jhi >= shi);
-      const float dist = fmaxf(fmaxf(slo_f - m.c, m.c - shi_f), 0.0f);
-      if (inside && dist >= m.r3) {
-        // ---- far: one rule for the whole span, register accumulators ----
-        const double nu0 = S.base[stage][l].nu0, A1 = S.base[stage][l].A1;
-        const double d0 = x0 - nu0;
-        if (dist >= m.r2) {
-          if (dist >= m.r1) {
-            const double g2 = S.base[stage][l].g2;
+      for (int b0 = 0; b0 < h.cnt; b0 += 32) {
+        unsigned m1, m2, m3, mn;
+        classify32<P>(S.ma[stage], S.mb[stage], b0 + lane, h.cnt, slo, m1, m2, m3, mn);
+        any_near |= mn;
+        // ---- 1-point rule ----
+#pragma unroll 1
+        for (unsigned m = m1; m; m &= m - 1) {
+          const LineBase *pb = sbase + b0 + (__ffs(m) - 1);
+          const double nu0 = pb->nu0, A1 = pb->A1, g2 = pb->g2;
+          const double d0 = x0 - nu0;
 #pragma unroll
-            for (int k = 0; k < P; ++k) acc[k] = gh1_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), A1, g2);
-          } else {
-            const double e2 = S.gh2[stage][l].e2, f2 = S.gh2[stage][l].f2, A1a2 = S.gh2[stage][l].A1a2;
+          for (int k = 0; k < P; ++k) acc[k] = gh1_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), A1, g2);
+        }
+        // ---- 2-point rule ----
+#pragma unroll 1
+        for (unsigned m = m2; m; m &= m - 1) {
+          const int i = b0 + (__ffs(m) - 1);
+          const double nu0 = sbase[i].nu0, A1 = sbase[i].A1;
+          const double e2 = sgh2[i].e2, f2 = sgh2[i].f2, A1a2 = sgh2[i].A1a2;
+          const double d0 = x0 - nu0;
 #pragma unroll
-            for (int k = 0; k < P; ++k) acc[k] = gh2_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), A1, e2, f2, A1a2);
-          }
-        } else {
-          const double g2 = S.base[stage][l].g2, a2 = S.base[stage][l].a2;
+          for (int k = 0; k < P; ++k) acc[k] = gh2_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), A1, e2, f2, A1a2);
+        }
+        // ---- 3-point rule ----
+#pragma unroll 1
+        for (unsigned m = m3; m; m &= m - 1) {
+          const LineBase *pb = sbase + b0 + (__ffs(m) - 1);
+          const double nu0 = pb->nu0, A1 = pb->A1, g2 = pb->g2, a2 = pb->a2;
+          const double d0 = x0 - nu0;
           const double e3 = fma(-1.5, a2, g2), f3 = 6.0 * a2 * g2;
           const double c3 = A1 * (1.0 / 3.0), c0 = 2.0 * c3, c3a = A1 * a2;
 #pragma unroll
           for (int k = 0; k < P; ++k) acc[k] = gh3_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), g2, e3, f3, c0, c3, c3a);
         }
-      } else {
-        near_span<P>(m, &S.base[stage][l], &S.gh2[stage][l], &S.core[stage][l], slo, lane, dist, x0, a.dnu, En, sk);
       }
+#pragma unroll
+      for (int k = 0; k < P; ++k) sk[32 * k + lane] = acc[k];
     }
+    // ---- near pass: rule per 32-point group, accumulating in sk ----
+    if (any_near) near_pass<P>(S.ma[stage], S.mb[stage], sbase, sgh2, S.core[stage], h.cnt, slo, a.nu_min, a.dnu, S.En, sk);
     if (h.flags & 2) {
 #pragma unroll
       for (int k = 0; k < P; ++k) {
         const int j = slo + lane + 32 * k;
-        const double v = acc[k] + sk[32 * k + lane];
+        const double v = sk[32 * k + lane];
         sk[32 * k + lane] = 0.0;
-        acc[k] = 0.0;
         if (j < a.N) a.kappa[j] = v;
       }
     }
@@ -559,12 +628,22 @@ static int cuda_fail(cudaError_t e, const char *what)
 
 static bool pos_finite(double v) { return v > 0.0 && isfinite(v); }
 
-constexpr int kP = 8, kWarps = 7, kMinB = 2;  // 7 consumer warps + 1 producer = 256 threads: 128 registers at 2 CTAs/SM
+#ifndef HK_P
+#define HK_P 8
+#endif
+#ifndef HK_WARPS
+#define HK_WARPS 7
+#endif
+#ifndef HK_MINB
+#define HK_MINB 2
+#endif
+constexpr int kP = HK_P, kWarps = HK_WARPS, kMinB = HK_MINB;  // 7 consumer warps + 1 producer = 256 threads: 128 registers at 2 CTAs/SM
 constexpr int kTile = kP * kWarps * 32;
 using VoigtSmemT = VoigtSmem<kP, kWarps>;
 
 struct Scratch {
-  LineMeta *meta = nullptr;  // one allocation: meta | base | gh2 | core, n_lines records each
+  MetaA *ma = nullptr;  // one allocation: ma | mb | base | gh2 | core, n_lines records each
+  MetaB *mb = nullptr;
   LineBase *base = nullptr;
   LineGH2 *gh2 = nullptr;
   LineCore *core = nullptr;
@@ -583,15 +662,16 @@ static void dev_free(void *p, cudaStream_t st, bool pooled)
 static int scratch_reserve(Scratch &s, int64_t n_lines, int n_tiles, cudaStream_t st, bool pooled)
 {
   if (n_lines > s.cap_lines) {
-    dev_free(s.meta, st, pooled);
-    s.meta = nullptr; s.cap_lines = 0;
-    const size_t bytes = (size_t)n_lines * 32;
+    dev_free(s.ma, st, pooled);
+    s.ma = nullptr; s.cap_lines = 0;
+    const size_t n = (size_t)n_lines;
     void *p = nullptr;
-    if (pooled) HK_CUDA(cudaMallocAsync(&p, 4 * bytes, st)); else HK_CUDA(cudaMalloc(&p, 4 * bytes));
-    s.meta = (LineMeta *)p;
-    s.base = (LineBase *)((char *)p + bytes);
-    s.gh2 = (LineGH2 *)((char *)p + 2 * bytes);
-    s.core = (LineCore *)((char *)p + 3 * bytes);
+    if (pooled) HK_CUDA(cudaMallocAsync(&p, n * kBytesPerLine, st)); else HK_CUDA(cudaMalloc(&p, n * kBytesPerLine));
+    s.ma = (MetaA *)p;
+    s.mb = (MetaB *)((char *)p + n * 16);
+    s.base = (LineBase *)((char *)p + n * 32);
+    s.gh2 = (LineGH2 *)((char *)p + n * 64);
+    s.core = (LineCore *)((char *)p + n * 96);
     s.cap_lines = n_lines;
   }
   if (n_tiles > s.cap_tiles) {
@@ -609,7 +689,7 @@ static int scratch_reserve(Scratch &s, int64_t n_lines, int n_tiles, cudaStream_
 
 static void scratch_release(Scratch &s, cudaStream_t st, bool pooled)
 {
-  dev_free(s.meta, st, pooled);
+  dev_free(s.ma, st, pooled);
   dev_free(s.plan, st, pooled);
   s = Scratch();
 }
@@ -680,15 +760,17 @@ static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double 
   pa.inv_mg = 1.0 / m_g;
   pa.q_ratio = q_ratio;
   pa.nu_min = nu_min; pa.dnu = dnu; pa.cutoff = cutoff; pa.N = (int)N;
-  pa.meta = s.meta; pa.base = s.base; pa.gh2 = s.gh2; pa.core = s.core;
+  pa.margin = 2.0 + 2.4e-7 * (double)N;
+  pa.ma = s.ma; pa.mb = s.mb; pa.base = s.base; pa.gh2 = s.gh2; pa.core = s.core;
   line_prep_kernel<<<(unsigned)((n_lines + 255) / 256), 256, 0, st>>>(pa);
   HK_CUDA(cudaGetLastError());
   if (g_timing) HK_CUDA(cudaEventRecord(ev[1], st));
-  tile_plan_kernel<<<(n_tiles + 127) / 128, 128, 0, st>>>(s.meta, n_lines, n_tiles, kTile, (int)N, s.plan, s.queue);
+  tile_plan_kernel<<<(n_tiles + 127) / 128, 128, 0, st>>>(s.ma, n_lines, n_tiles, kTile, (int)N, s.plan, s.queue);
   HK_CUDA(cudaGetLastError());
   if (g_timing) HK_CUDA(cudaEventRecord(ev[2], st));
   VoigtArgs va;
-  va.meta = s.meta; va.base = s.base; va.gh2 = s.gh2; va.core = s.core; va.plan = s.plan; va.queue = s.queue;
+  va.ma = s.ma; va.mb = s.mb; va.base = s.base; va.gh2 = s.gh2; va.core = s.core; va.plan = s.plan; va.queue = s.queue;
+  va.order = nullptr;
   va.n_tiles = n_tiles;
   va.nu_min = nu_min; va.dnu = dnu; va.N = (int)N; va.kappa = kappa_out;
   int grid = 0;
