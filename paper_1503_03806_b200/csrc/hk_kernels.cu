@@ -317,11 +317,16 @@ __device__ __forceinline__ void near_span(const MetaA *pa, const MetaB *pm, cons
   }
 }
 
-// lane = line classification of 32 lines of a chunk against the warp span [slo, slo + 32P): bit masks of the lines that
-// take the 1-, 2-, 3-point rule on the whole span, and of the near lines (span inside the 3-point radius or on a cutoff edge)
+// lane = line classification of 32 lines of a chunk against the warp span [slo, slo + 32P).  Bit masks of the lines that
+//   m1, m2, m3 : take the 1-, 2-, 3-point rule on the whole span, span inside the line's window ("far")
+//   e1, e2     : take the 1- or 2-point rule on the whole span, but a cutoff edge of the line falls inside the span ("edge")
+//   mn         : everything else that touches the span ("near": span reaches inside the 3-point radius, or an edge span
+//                closer than the 2-point radius)
+struct SpanMasks {
+  unsigned m1, m2, m3, e1, e2, mn;
+};
 template <int P>
-__device__ __forceinline__ void classify32(const MetaA *ma, const MetaB *mb, int l, int cnt, int slo, unsigned &m1,
-                                           unsigned &m2, unsigned &m3, unsigned &mn)
+__device__ __forceinline__ SpanMasks classify32(const MetaA *ma, const MetaB *mb, int l, int cnt, int slo)
 {
   const int shi = slo + 32 * P - 1;
   const MetaA A = ma[l];
@@ -329,15 +334,24 @@ __device__ __forceinline__ void classify32(const MetaA *ma, const MetaB *mb, int
   const bool act = (l < cnt) && (A.jhi >= slo) && (A.jlo <= shi);
   const bool inside = (A.jlo <= slo) && (A.jhi >= shi);
   const float dist = fmaxf(fmaxf((float)slo - A.c, A.c - (float)shi), 0.0f);
-  const bool far = act && inside && (dist >= A.r3);
-  m1 = __ballot_sync(kFull, far && dist >= B.r1);
-  m2 = __ballot_sync(kFull, far && dist < B.r1 && dist >= B.r2);
-  m3 = __ballot_sync(kFull, far && dist < B.r2);
-  mn = __ballot_sync(kFull, act && !far);
+  const bool w1 = dist >= B.r1, w2 = dist >= B.r2, w3 = dist >= A.r3;
+  SpanMasks M;
+  M.m1 = __ballot_sync(kFull, act && inside && w1);
+  M.m2 = __ballot_sync(kFull, act && inside && !w1 && w2);
+  M.m3 = __ballot_sync(kFull, act && inside && !w2 && w3);
+  M.e1 = __ballot_sync(kFull, act && !inside && w1);
+  M.e2 = __ballot_sync(kFull, act && !inside && !w1 && w2);
+  M.mn = __ballot_sync(kFull, act && (!w3 || (!inside && !w2)));
+  return M;
 }
 
 // near pass over one chunk: kept out of line (one call per chunk) so that the 6-point and series state never competes for
-// registers with the far loops; the accumulators live in the shared-memory strip across the call.
+// registers with the far loops; the span's accumulators live in the shared-memory strip sk across the call.
+//
+// Fast path (span reaches inside the 3-point radius, y >= 1e-8): the 6-point rule, valid wherever r^2 >= 44, on all P
+// groups at once (unrolled, P independent chains), masked to the window and to the points outside the series region
+// d^2 >= qc = xc2 alpha^2; then the series on the groups that hold series points, adding amp*K at exactly the points the
+// first pass masked (same predicate on the same d^2).  Everything else goes through near_span (rule per group).
 template <int P>
 __device__ __noinline__ void near_pass(const MetaA *ma, const MetaB *mb, const LineBase *base, const LineGH2 *gh2,
                                        const LineCore *core, int cnt, int slo, double nu_min, double dnu, const double *En_tab,
@@ -346,16 +360,58 @@ __device__ __noinline__ void near_pass(const MetaA *ma, const MetaB *mb, const L
   const int lane = threadIdx.x & 31;
   const double En = lane < kTerms ? En_tab[lane] : 0.0;
   const double x0 = __dadd_rn(nu_min, __dmul_rn((double)(slo + lane), dnu));
+  const int shi = slo + 32 * P - 1;
+  double accn[P];
+#pragma unroll
+  for (int k = 0; k < P; ++k) accn[k] = 0.0;
 #pragma unroll 1
   for (int b0 = 0; b0 < cnt; b0 += 32) {
-    unsigned m1, m2, m3, mn;
-    classify32<P>(ma, mb, b0 + lane, cnt, slo, m1, m2, m3, mn);
+    const SpanMasks M = classify32<P>(ma, mb, b0 + lane, cnt, slo);
 #pragma unroll 1
-    for (unsigned m = mn; m; m &= m - 1) {
+    for (unsigned m = M.mn; m; m &= m - 1) {
       const int i = b0 + (__ffs(m) - 1);
-      near_span<P>(ma + i, mb + i, base + i, gh2 + i, core + i, slo, lane, x0, dnu, En, sk);
+      const MetaA A = ma[i];
+      const MetaB B = mb[i];
+      const float dist = fmaxf(fmaxf((float)slo - A.c, A.c - (float)shi), 0.0f);
+      if (!(dist < A.r3) || B.rg > 0.0f) {
+        near_span<P>(ma + i, mb + i, base + i, gh2 + i, core + i, slo, lane, x0, dnu, En, sk);
+        continue;
+      }
+      const LineBase b = base[i];
+      const LineCore kc = core[i];
+      const Gh6 G6 = gh6_consts(b.A1, b.g2, b.a2);
+      const double qc = kc.xc2 * b.a2;
+      const double d0 = x0 - b.nu0;
+      const unsigned wlen = (unsigned)(A.jhi - A.jlo);
+      const int jrel = slo + lane - A.jlo;
+#pragma unroll
+      for (int k = 0; k < P; ++k) {
+        const double d = fma((double)(32 * k), dnu, d0);
+        const double q = d * d;
+        const double v = gh6_val(q, G6);
+        const bool keep = ((unsigned)(jrel + 32 * k) <= wlen) && !(q < qc);
+        accn[k] += keep ? v : 0.0;
+      }
+      if (dist < B.r6) {
+        const double inv_alpha = gh2[i].inv_alpha;
+        const CoreLine C = core_setup(kc.y, kc.erfcx_y, En);
+#pragma unroll 1
+        for (int k = 0; k < P; ++k) {
+          const int glo = slo + 32 * k, ghi = glo + 31;
+          const float dg = fmaxf(fmaxf((float)glo - A.c, A.c - (float)ghi), 0.0f);
+          if (!(dg < B.r6) || ghi < A.jlo || glo > A.jhi) continue;
+          const double d = fma((double)(32 * k), dnu, d0);
+          const double q = d * d;
+          const double x = fabs(d) * inv_alpha;
+          const double ks = core_K(fmin(x, 6.7), C);
+          const bool take = ((unsigned)(jrel + 32 * k) <= wlen) && (q < qc);
+          sk[32 * k + lane] += take ? kc.Acore * ks : 0.0;
+        }
+      }
     }
   }
+#pragma unroll
+  for (int k = 0; k < P; ++k) sk[32 * k + lane] += accn[k];
 }
 
 template <int P, int WARPS, int MINB>
@@ -447,12 +503,11 @@ __global__ void __launch_bounds__((WARPS + 1) * 32, MINB) voigt_kernel(const __g
       for (int k = 0; k < P; ++k) acc[k] = sk[32 * k + lane];
 #pragma unroll 1
       for (int b0 = 0; b0 < h.cnt; b0 += 32) {
-        unsigned m1, m2, m3, mn;
-        classify32<P>(S.ma[stage], S.mb[stage], b0 + lane, h.cnt, slo, m1, m2, m3, mn);
-        any_near |= mn;
+        const SpanMasks M = classify32<P>(S.ma[stage], S.mb[stage], b0 + lane, h.cnt, slo);
+        any_near |= M.mn;
         // ---- 1-point rule ----
 #pragma unroll 1
-        for (unsigned m = m1; m; m &= m - 1) {
+        for (unsigned m = M.m1; m; m &= m - 1) {
           const LineBase *pb = sbase + b0 + (__ffs(m) - 1);
           const double nu0 = pb->nu0, A1 = pb->A1, g2 = pb->g2;
           const double d0 = x0 - nu0;
@@ -461,7 +516,7 @@ __global__ void __launch_bounds__((WARPS + 1) * 32, MINB) voigt_kernel(const __g
         }
         // ---- 2-point rule ----
 #pragma unroll 1
-        for (unsigned m = m2; m; m &= m - 1) {
+        for (unsigned m = M.m2; m; m &= m - 1) {
           const int i = b0 + (__ffs(m) - 1);
           const double nu0 = sbase[i].nu0, A1 = sbase[i].A1;
           const double e2 = sgh2[i].e2, f2 = sgh2[i].f2, A1a2 = sgh2[i].A1a2;
@@ -469,9 +524,39 @@ __global__ void __launch_bounds__((WARPS + 1) * 32, MINB) voigt_kernel(const __g
 #pragma unroll
           for (int k = 0; k < P; ++k) acc[k] = gh2_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), A1, e2, f2, A1a2);
         }
+        // ---- 1- and 2-point rule on spans that hold a cutoff edge: same rules, masked to the line's window ----
+#pragma unroll 1
+        for (unsigned m = M.e1; m; m &= m - 1) {
+          const int i = b0 + (__ffs(m) - 1);
+          const int jlo = S.ma[stage][i].jlo, jhi = S.ma[stage][i].jhi;
+          const double nu0 = sbase[i].nu0, A1 = sbase[i].A1, g2 = sbase[i].g2;
+          const double d0 = x0 - nu0;
+          const unsigned wlen = (unsigned)(jhi - jlo);
+          const int jrel = slo + lane - jlo;
+#pragma unroll
+          for (int k = 0; k < P; ++k) {
+            const double t = gh1_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), A1, g2);
+            acc[k] = ((unsigned)(jrel + 32 * k) <= wlen) ? t : acc[k];
+          }
+        }
+#pragma unroll 1
+        for (unsigned m = M.e2; m; m &= m - 1) {
+          const int i = b0 + (__ffs(m) - 1);
+          const int jlo = S.ma[stage][i].jlo, jhi = S.ma[stage][i].jhi;
+          const double nu0 = sbase[i].nu0, A1 = sbase[i].A1;
+          const double e2 = sgh2[i].e2, f2 = sgh2[i].f2, A1a2 = sgh2[i].A1a2;
+          const double d0 = x0 - nu0;
+          const unsigned wlen = (unsigned)(jhi - jlo);
+          const int jrel = slo + lane - jlo;
+#pragma unroll
+          for (int k = 0; k < P; ++k) {
+            const double t = gh2_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), A1, e2, f2, A1a2);
+            acc[k] = ((unsigned)(jrel + 32 * k) <= wlen) ? t : acc[k];
+          }
+        }
         // ---- 3-point rule ----
 #pragma unroll 1
-        for (unsigned m = m3; m; m &= m - 1) {
+        for (unsigned m = M.m3; m; m &= m - 1) {
           const LineBase *pb = sbase + b0 + (__ffs(m) - 1);
           const double nu0 = pb->nu0, A1 = pb->A1, g2 = pb->g2, a2 = pb->a2;
           const double d0 = x0 - nu0;
