@@ -199,17 +199,23 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
 {
   uint32_t ok;
   const uint32_t addr = smem_u32(bar);
+#ifdef HK_WATCHDOG
+  const long long t0 = clock64();
+#endif
   do {
     asm volatile(
         "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
         : "=r"(ok)
         : "r"(addr), "r"(parity)
         : "memory");
+#ifdef HK_WATCHDOG
+    if (!ok && clock64() - t0 > 4000000000LL) __trap();  // ~2 s: a protocol bug must not hang the GPU
+#endif
   } while (!ok);
 }
 
 // ------------------------------------------------------------------------------------------------------
-// a3 + a4: Voigt accumulation.  Persistent CTAs of WARPS consumer warps + 1 producer warp.
+// a3 + a4: Voigt accumulation.  Persistent CTAs of WARPS warps, all of them consumers.
 //
 // Work unit = tile of WARPS*32*P consecutive grid points, pulled from an atomic queue.  Consumer warp w owns the span
 // [tile_lo + w*32P, +32P), lane l the points span_lo + l + 32k (k < P): stores are coalesced, every 32 consecutive points
@@ -249,7 +255,11 @@ struct __align__(128) VoigtSmem {
   double sk[WARPS][32 * P];
   double En[kTerms];  // exp(-a^2 n^2), n = 1..16: lane constants of the series
   StageHdr hdr[STAGES];
-  uint64_t full[STAGES], empty[STAGES];
+  uint64_t full[STAGES];
+  int done[STAGES];  // warps that have finished with the stage's current chunk
+  int issued;        // chunks handed to the TMA engine so far (ticket that orders the refills)
+  // refill cursor: owned by whoever holds ticket `issued`
+  int cur_tile, cur_L0, cur_nl, cur_c, cur_nchunks, cur_stop;
 };
 
 struct VoigtArgs {
@@ -414,80 +424,85 @@ __device__ __noinline__ void near_pass(const MetaA *ma, const MetaB *mb, const L
   for (int k = 0; k < P; ++k) sk[32 * k + lane] += accn[k];
 }
 
-template <int P, int WARPS, int MINB>
-__global__ void __launch_bounds__((WARPS + 1) * 32, MINB) voigt_kernel(const __grid_constant__ VoigtArgs a)
+// Hands the next chunk of lines (ring sequence number n) to the TMA engine: stage n % STAGES gets a header and, if the chunk
+// holds lines, five bulk copies completing on the stage's `full` mbarrier.  Pulls a new tile from the queue when the current
+// one is exhausted; after the last tile one stop header is posted and nothing more.  Called by one thread at a time, in
+// order of n (ticket S.issued).
+template <int P, int WARPS>
+__device__ __forceinline__ void issue_chunk(VoigtSmem<P, WARPS> &S, const VoigtArgs &a, int n)
 {
   constexpr int TILE = WARPS * 32 * P;
+  if (S.cur_stop) return;
+  const int stage = n % STAGES;
+  if (S.cur_c == S.cur_nchunks) {
+    const int ticket = atomicAdd(a.queue, 1);
+    if (ticket >= a.n_tiles) {
+      S.cur_stop = 1;
+      StageHdr h;
+      h.tile_lo = -1; h.cnt = 0; h.flags = 0; h.pad = 0;
+      S.hdr[stage] = h;
+      mbar_expect_tx(&S.full[stage], 0u);
+      return;
+    }
+    const int tile = a.order ? a.order[ticket] : ticket;
+    const int2 pl = a.plan[tile];
+    const int nl = pl.y - pl.x;
+    S.cur_tile = tile;
+    S.cur_L0 = pl.x;
+    S.cur_nl = nl;
+    S.cur_c = 0;
+    S.cur_nchunks = nl > 0 ? (nl + CH - 1) / CH : 1;
+  }
+  const int c = S.cur_c;
+  const int cnt = min(CH, S.cur_nl - c * CH);
+  StageHdr h;
+  h.tile_lo = S.cur_tile * TILE;
+  h.cnt = cnt > 0 ? cnt : 0;
+  h.flags = (c == 0 ? 1 : 0) | (c == S.cur_nchunks - 1 ? 2 : 0);
+  h.pad = 0;
+  S.hdr[stage] = h;
+  S.cur_c = c + 1;
+  const uint32_t nb = (uint32_t)h.cnt;
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // the stage's previous readers (generic proxy) come first
+  mbar_expect_tx(&S.full[stage], nb * (uint32_t)kBytesPerLine);  // release: the header store above is visible to the waiters
+  if (nb) {
+    const int first = S.cur_L0 + c * CH;
+    bulk_g2s(&S.ma[stage][0], a.ma + first, nb * 16u, &S.full[stage]);
+    bulk_g2s(&S.mb[stage][0], a.mb + first, nb * 16u, &S.full[stage]);
+    bulk_g2s(&S.base[stage][0], a.base + first, nb * 32u, &S.full[stage]);
+    bulk_g2s(&S.gh2[stage][0], a.gh2 + first, nb * 32u, &S.full[stage]);
+    bulk_g2s(&S.core[stage][0], a.core + first, nb * 32u, &S.full[stage]);
+  }
+}
+
+template <int P, int WARPS, int MINB>
+__global__ void __launch_bounds__(WARPS * 32, MINB) voigt_kernel(const __grid_constant__ VoigtArgs a)
+{
   extern __shared__ __align__(128) unsigned char smem_raw[];
   VoigtSmem<P, WARPS> &S = *reinterpret_cast<VoigtSmem<P, WARPS> *>(smem_raw);
 
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int k = 0; k < P; ++k) S.sk[warp][32 * k + lane] = 0.0;
+  if (warp == 1 && lane < kTerms) S.En[lane] = core_lane_const();
   if (threadIdx.x == 0) {
     for (int s = 0; s < STAGES; ++s) {
       mbar_init(&S.full[s], 1);
-      mbar_init(&S.empty[s], WARPS);
+      S.done[s] = 0;
     }
+    S.cur_tile = 0; S.cur_L0 = 0; S.cur_nl = 0; S.cur_c = 0; S.cur_nchunks = 0; S.cur_stop = 0;
     mbar_fence_init();
-  }
-  if (warp < WARPS) {
-#pragma unroll
-    for (int k = 0; k < P; ++k) S.sk[warp][32 * k + lane] = 0.0;
-  } else if (lane < kTerms) {
-    S.En[lane] = core_lane_const();
+    for (int n = 0; n < STAGES; ++n) issue_chunk<P, WARPS>(S, a, n);  // fill the ring
+    S.issued = STAGES;
   }
   __syncthreads();  // the only CTA-wide barrier
 
-  if (warp == WARPS) {
-    // ---------------- producer: one thread feeds the ring ----------------
-    if (lane != 0) return;
-    int stage = 0;
-    uint32_t phase = 0;
-    for (;;) {
-      const int ticket = atomicAdd(a.queue, 1);
-      const bool stop = ticket >= a.n_tiles;
-      int tile = 0, L0 = 0, nl = 0;
-      if (!stop) {
-        tile = a.order ? a.order[ticket] : ticket;
-        const int2 pl = a.plan[tile];
-        L0 = pl.x;
-        nl = pl.y - pl.x;
-      }
-      const int nchunks = nl > 0 ? (nl + CH - 1) / CH : 1;
-      for (int c = 0; c < nchunks; ++c) {
-        mbar_wait(&S.empty[stage], phase ^ 1u);
-        const int cnt = min(CH, nl - c * CH);
-        StageHdr h;
-        h.tile_lo = stop ? -1 : tile * TILE;
-        h.cnt = cnt > 0 ? cnt : 0;
-        h.flags = (c == 0 ? 1 : 0) | (c == nchunks - 1 ? 2 : 0);
-        h.pad = 0;
-        S.hdr[stage] = h;
-        const uint32_t n = (uint32_t)h.cnt;
-        mbar_expect_tx(&S.full[stage], n * (uint32_t)kBytesPerLine);  // release: the header store above is visible to the waiters
-        if (n) {
-          const int first = L0 + c * CH;
-          bulk_g2s(&S.ma[stage][0], a.ma + first, n * 16u, &S.full[stage]);
-          bulk_g2s(&S.mb[stage][0], a.mb + first, n * 16u, &S.full[stage]);
-          bulk_g2s(&S.base[stage][0], a.base + first, n * 32u, &S.full[stage]);
-          bulk_g2s(&S.gh2[stage][0], a.gh2 + first, n * 32u, &S.full[stage]);
-          bulk_g2s(&S.core[stage][0], a.core + first, n * 32u, &S.full[stage]);
-        }
-        if (++stage == STAGES) {
-          stage = 0;
-          phase ^= 1u;
-        }
-      }
-      if (stop) return;
-    }
-  }
-
-  // ---------------- consumers ----------------
   double *sk = S.sk[warp];  // this warp's accumulators between chunks (zero at the start of a tile)
   int slo = 0;
   int stage = 0;
   uint32_t phase = 0;
 
-  for (;;) {
+  for (int n = 0;; ++n) {
     mbar_wait(&S.full[stage], phase);
     const StageHdr h = S.hdr[stage];
     if (h.tile_lo < 0) break;
@@ -524,6 +539,17 @@ __global__ void __launch_bounds__((WARPS + 1) * 32, MINB) voigt_kernel(const __g
 #pragma unroll
           for (int k = 0; k < P; ++k) acc[k] = gh2_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), A1, e2, f2, A1a2);
         }
+        // ---- 3-point rule ----
+#pragma unroll 1
+        for (unsigned m = M.m3; m; m &= m - 1) {
+          const LineBase *pb = sbase + b0 + (__ffs(m) - 1);
+          const double nu0 = pb->nu0, A1 = pb->A1, g2 = pb->g2, a2 = pb->a2;
+          const double d0 = x0 - nu0;
+          const double e3 = fma(-1.5, a2, g2), f3 = 6.0 * a2 * g2;
+          const double c3 = A1 * (1.0 / 3.0), c0 = 2.0 * c3, c3a = A1 * a2;
+#pragma unroll
+          for (int k = 0; k < P; ++k) acc[k] = gh3_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), g2, e3, f3, c0, c3, c3a);
+        }
         // ---- 1- and 2-point rule on spans that hold a cutoff edge: same rules, masked to the line's window ----
 #pragma unroll 1
         for (unsigned m = M.e1; m; m &= m - 1) {
@@ -554,22 +580,11 @@ __global__ void __launch_bounds__((WARPS + 1) * 32, MINB) voigt_kernel(const __g
             acc[k] = ((unsigned)(jrel + 32 * k) <= wlen) ? t : acc[k];
           }
         }
-        // ---- 3-point rule ----
-#pragma unroll 1
-        for (unsigned m = M.m3; m; m &= m - 1) {
-          const LineBase *pb = sbase + b0 + (__ffs(m) - 1);
-          const double nu0 = pb->nu0, A1 = pb->A1, g2 = pb->g2, a2 = pb->a2;
-          const double d0 = x0 - nu0;
-          const double e3 = fma(-1.5, a2, g2), f3 = 6.0 * a2 * g2;
-          const double c3 = A1 * (1.0 / 3.0), c0 = 2.0 * c3, c3a = A1 * a2;
-#pragma unroll
-          for (int k = 0; k < P; ++k) acc[k] = gh3_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), g2, e3, f3, c0, c3, c3a);
-        }
       }
 #pragma unroll
       for (int k = 0; k < P; ++k) sk[32 * k + lane] = acc[k];
     }
-    // ---- near pass: rule per 32-point group, accumulating in sk ----
+    // ---- near pass: 6-point rule and series, accumulating in sk ----
     if (any_near) near_pass<P>(S.ma[stage], S.mb[stage], sbase, sgh2, S.core[stage], h.cnt, slo, a.nu_min, a.dnu, S.En, sk);
     if (h.flags & 2) {
 #pragma unroll
@@ -580,8 +595,28 @@ __global__ void __launch_bounds__((WARPS + 1) * 32, MINB) voigt_kernel(const __g
         if (j < a.N) a.kappa[j] = v;
       }
     }
+    // ---- release the stage; the last warp out refills it (ring sequence number n + STAGES), in ticket order ----
     __syncwarp();
-    if (lane == 0) mbar_arrive(&S.empty[stage]);
+    if (lane == 0) {
+      __threadfence_block();
+      const int old = atomicAdd(&S.done[stage], 1);
+      if (old == WARPS - 1) {
+        volatile int *issued = &S.issued;
+        S.done[stage] = 0;
+#ifdef HK_WATCHDOG
+        const long long t0 = clock64();
+#endif
+        while (*issued != n + STAGES) {
+#ifdef HK_WATCHDOG
+          if (clock64() - t0 > 4000000000LL) __trap();
+#endif
+        }
+        __threadfence_block();
+        issue_chunk<P, WARPS>(S, a, n + STAGES);
+        __threadfence_block();
+        *issued = n + STAGES + 1;
+      }
+    }
     if (++stage == STAGES) {
       stage = 0;
       phase ^= 1u;
@@ -717,12 +752,12 @@ static bool pos_finite(double v) { return v > 0.0 && isfinite(v); }
 #define HK_P 8
 #endif
 #ifndef HK_WARPS
-#define HK_WARPS 7
+#define HK_WARPS 8
 #endif
 #ifndef HK_MINB
 #define HK_MINB 2
 #endif
-constexpr int kP = HK_P, kWarps = HK_WARPS, kMinB = HK_MINB;  // 7 consumer warps + 1 producer = 256 threads: 128 registers at 2 CTAs/SM
+constexpr int kP = HK_P, kWarps = HK_WARPS, kMinB = HK_MINB;  // 8 warps = 256 threads: 128 registers at 2 CTAs/SM
 constexpr int kTile = kP * kWarps * 32;
 using VoigtSmemT = VoigtSmem<kP, kWarps>;
 
@@ -790,7 +825,7 @@ static int voigt_grid(int *grid_out)
     HK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     HK_CUDA(cudaFuncSetAttribute(voigt_kernel<kP, kWarps, kMinB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  (int)sizeof(VoigtSmemT)));
-    HK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, voigt_kernel<kP, kWarps, kMinB>, (kWarps + 1) * 32,
+    HK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, voigt_kernel<kP, kWarps, kMinB>, kWarps * 32,
                                                           sizeof(VoigtSmemT)));
     if (per_sm < 1) per_sm = 1;
     cached_grid = sms * per_sm;
@@ -862,7 +897,7 @@ static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double 
   rc = voigt_grid(&grid);
   if (rc != HK_OK) return rc;
   if (grid > n_tiles) grid = n_tiles;
-  voigt_kernel<kP, kWarps, kMinB><<<grid, (kWarps + 1) * 32, sizeof(VoigtSmemT), st>>>(va);
+  voigt_kernel<kP, kWarps, kMinB><<<grid, kWarps * 32, sizeof(VoigtSmemT), st>>>(va);
   HK_CUDA(cudaGetLastError());
   if (g_timing) {
     HK_CUDA(cudaEventRecord(ev[3], st));
