@@ -16,7 +16,7 @@ for the barrier and the max-over-ranks of the device time.
 
 Prints ONE JSON line (rank 0).  `value` = line-point Voigt evaluations per second, whole job, inputs resident in HBM, device time
 by CUDA events around each step (L2 flushed between steps, outside the events).  `e2e` = the same metric through
-hk.opacity_host(): pinned host line arrays -> device, both calls, kappa and the k-table -> pinned host, wall clock.
+hk.hk_opacity_host(): pinned host line arrays -> device, both calls, kappa and the k-table -> pinned host, wall clock.
 """
 from __future__ import annotations
 
@@ -230,14 +230,15 @@ def run_ours(args):
     pin = lambda a: torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64)).pin_memory()
     h_nu0, h_S, h_g0 = pin(wl.nu0), pin(wl.S), pin(wl.gamma0)
     h_kappa = torch.empty(N, dtype=torch.float64, pin_memory=True)
+    h_ktab = torch.empty((N // ppb, wl.n_g), dtype=torch.float64, pin_memory=True)
     for _ in range(2):
-        hk.opacity_host(h_nu0, h_S, h_g0, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, mass_amu=wl.mass_amu,
-                        bin_width=wl.bin_width, n_g=wl.n_g, kappa_out=h_kappa)
+        hk.hk_opacity_host(h_nu0, h_S, h_g0, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, mass_amu=wl.mass_amu,
+                        bin_width=wl.bin_width, n_g=wl.n_g, kappa_out=h_kappa, k_out=h_ktab)
     barrier()
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        _, h_k = hk.opacity_host(h_nu0, h_S, h_g0, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, mass_amu=wl.mass_amu,
-                                 bin_width=wl.bin_width, n_g=wl.n_g, kappa_out=h_kappa)
+        hk.hk_opacity_host(h_nu0, h_S, h_g0, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, mass_amu=wl.mass_amu,
+                           bin_width=wl.bin_width, n_g=wl.n_g, kappa_out=h_kappa, k_out=h_ktab)
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
     h2d = 3 * 8 * wl.n_lines

@@ -19,7 +19,8 @@
  *     caller-allocated and are OVERWRITTEN, never accumulated into.
  *   - Calls enqueue work on `stream` (a cudaStream_t passed as void*; NULL = the legacy default stream) and
  *     return without synchronising, except where stated; the caller synchronises before reading results.
- *     Scratch memory is taken from the stream-ordered CUDA memory pool and returned to it on the same stream.
+ *     Scratch memory is taken from the library's own stream-ordered CUDA memory pool (one per device, kept for reuse)
+ *     and returned to it on the same stream.
  *   - Return value: HK_OK (0) or a negative HK_ERR_* code; hk_strerror() names it; after HK_ERR_CUDA,
  *     hk_last_cuda_error() returns the CUDA runtime's message.  No exceptions, no global mutable state
  *     other than that last-error string.
@@ -40,7 +41,7 @@ extern "C" {
 #define HK_ERR_INVALID (-1)     /* bad argument (see each function) */
 #define HK_ERR_CUDA (-2)        /* CUDA runtime error; see hk_last_cuda_error() */
 #define HK_ERR_NOMEM (-3)       /* device or host allocation failed */
-#define HK_ERR_UNSORTED (-4)    /* prm->lines_sorted = 1 was promised but nu0 is not ascending */
+#define HK_ERR_UNSORTED (-4)    /* hk_lines_check_sorted(): nu0 is not ascending */
 #define HK_ERR_UNSUPPORTED (-5) /* valid request outside the implemented range (e.g. points per bin > 16384) */
 
 #define HK_FP64 0
@@ -61,8 +62,9 @@ typedef struct {
   double mass_amu;      /* molecular mass m (one species per call), amu; > 0                          */
   double q_ratio;       /* Q(296 K)/Q(T) of eq. 18; used only when E_low != NULL                      */
   int precision;        /* HK_FP64                                                                    */
-  int lines_sorted;     /* 1: caller guarantees nu0 ascending (checked on the device, HK_ERR_UNSORTED
-                           is reported by hk_opacity_check()); 0: the library sorts a copy by nu0     */
+  int lines_sorted;     /* 1: caller guarantees nu0 ascending, as HITRAN/HITEMP files are (not re-checked; see
+                           hk_lines_check_sorted()).  0: the library checks on the device (synchronises the
+                           stream) and, if needed, works on a copy ordered by nu0; inputs are never modified */
   void *stream;         /* cudaStream_t, or NULL                                                      */
 } hk_params;
 
@@ -88,9 +90,20 @@ int64_t hk_grid_size(double nu_min, double nu_max, double dnu);
  * HK_ERR_INVALID: NULL lines/prm/kappa_out or (n_lines > 0 and NULL nu0/S/gamma0); n_lines < 0; T, P_atm, dnu,
  * cutoff, mass_amu not > 0 or not finite; N < 1 or N > 2^30; precision unknown.
  * HK_ERR_UNSUPPORTED: precision == HK_FP32.
- * Asynchronous on prm->stream.  nu0 must be ascending when lines_sorted = 1 (see hk_opacity_check). */
+ * Asynchronous on prm->stream (synchronises once when lines_sorted = 0).  nu0 must be ascending when
+ * lines_sorted = 1 (see hk_lines_check_sorted). */
 int hk_opacity(const hk_lines *lines, int64_t n_lines, double T, double P_atm, double nu_min, double nu_max,
                double dnu, double cutoff, double *kappa_out, const hk_params *prm);
+
+/* End-to-end form with HOST buffers (what bench.py's `e2e` times): copies the line arrays host -> device, runs
+ * hk_opacity and, when k_host_out != NULL, hk_kdist(bin_width, n_g), copies kappa (when kappa_host_out != NULL) and the
+ * k-table device -> host, and waits for the stream.  Every array of lines_host is a HOST pointer (pinned memory makes
+ * the copies asynchronous to the host but is not required); kappa_host_out: host [N] or NULL; k_host_out: host
+ * [n_bins*n_g] or NULL (then bin_width and n_g are ignored); at least one output is required.  Device memory comes from
+ * the library's pool.  Errors as hk_opacity / hk_kdist.  Synchronous. */
+int hk_opacity_host(const hk_lines *lines_host, int64_t n_lines, double T, double P_atm, double nu_min, double nu_max,
+                    double dnu, double cutoff, double *kappa_host_out, double bin_width, int n_g, double *k_host_out,
+                    const hk_params *prm);
 
 /* Synchronous check that a device nu0 array is ascending (what lines_sorted = 1 promises).
  * Returns HK_OK, HK_ERR_UNSORTED, or an error.  Blocks until the stream is idle. */
@@ -118,7 +131,8 @@ int hk_voigt_K(const double *x, const double *y, int64_t n, double *out, int pre
 
 /* Persistent-context form for T-P sweeps ("repeat this calculation for multiple combinations of
  * temperature and pressure"): the line list is bound once, scratch is kept between calls.
- * hk_create copies nothing: the hk_lines device arrays must outlive the context. */
+ * hk_create copies nothing when nu0 is ascending: the hk_lines device arrays must outlive the context; with
+ * lines_sorted = 0 and an unordered list the context owns an ordered copy (made once). */
 typedef struct hk_ctx hk_ctx;
 int hk_create(const hk_lines *lines, int64_t n_lines, const hk_params *prm, hk_ctx **out);
 int hk_opacity_ctx(hk_ctx *ctx, double T, double P_atm, double q_ratio, double nu_min, double nu_max, double dnu,

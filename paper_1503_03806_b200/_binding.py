@@ -56,6 +56,9 @@ def load_library():
     L.hk_opacity.restype = C.c_int
     L.hk_opacity.argtypes = [C.POINTER(_hk_lines), _i64, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double,
                              C.c_double, C.c_void_p, C.POINTER(_hk_params)]
+    L.hk_opacity_host.restype = C.c_int
+    L.hk_opacity_host.argtypes = [C.POINTER(_hk_lines), _i64, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double,
+                                  C.c_double, C.c_void_p, C.c_double, C.c_int, C.c_void_p, C.POINTER(_hk_params)]
     L.hk_lines_check_sorted.restype = C.c_int
     L.hk_lines_check_sorted.argtypes = [C.c_void_p, _i64, C.c_void_p]
     L.hk_count_evals.restype = _i64
@@ -287,22 +290,51 @@ class Context:
             pass
 
 
-def opacity_host(nu0, S, gamma0, T, P_atm, nu_min, nu_max, dnu, cutoff, mass_amu=18.0, E_low=None, q_ratio=1.0,
-                 bin_width=None, n_g=20, kappa_out=None):
-    """End-to-end call with HOST buffers: pinned host line arrays -> device, hk_opacity (+ hk_kdist when bin_width is
-    given), result -> pinned host.  Returns (kappa_host, k_host or None).  Synchronous."""
+def _host_ptr(t, name, allow_none=False):
+    if t is None:
+        if allow_none:
+            return None
+        raise ValueError(f"{name} is required")
+    import torch
+    if isinstance(t, np.ndarray):
+        if t.dtype != np.float64 or not t.flags.c_contiguous:
+            raise TypeError(f"{name} must be a contiguous float64 array")
+        return t.ctypes.data
+    if not (isinstance(t, torch.Tensor) and not t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise TypeError(f"{name} must be a contiguous float64 HOST tensor or numpy array")
+    return t.data_ptr()
+
+
+def hk_opacity_host(nu0, S, gamma0, T, P_atm, nu_min, nu_max, dnu, cutoff, mass_amu=18.0, n_T=None, E_low=None, q_ratio=1.0,
+                    lines_sorted=True, bin_width=None, n_g=20, kappa_out=None, k_out=None, want_kappa=True, stream=None):
+    """End-to-end call with HOST buffers (hk_opacity_host of include/hk.h): host line arrays -> device, hk_opacity
+    (+ hk_kdist when bin_width is given), kappa / k-table -> host.  Buffers are host torch tensors (pinned for
+    asynchronous copies) or numpy arrays.  Returns (kappa_host or None, k_host or None).  Synchronous."""
     torch = _torch()
-    dev = torch.device("cuda")
-    up = lambda a: None if a is None else a.to(dev, non_blocking=True)
-    lines = Lines(up(nu0), up(S), up(gamma0), None, up(E_low))
-    kappa = hk_opacity(lines, T, P_atm, nu_min, nu_max, dnu, cutoff, mass_amu=mass_amu, q_ratio=q_ratio)
-    k_host = None
+    L = load_library()
+    N = hk_grid_size(nu_min, nu_max, dnu)
+    n = int(nu0.shape[0])
+    for name, t in (("S", S), ("gamma0", gamma0), ("n_T", n_T), ("E_low", E_low)):
+        if t is not None and int(t.shape[0]) != n:
+            raise ValueError(f"{name} has {int(t.shape[0])} entries, nu0 has {n}")
+    if want_kappa and kappa_out is None and N >= 1:
+        kappa_out = torch.empty(N, dtype=torch.float64, pin_memory=True)
+    if kappa_out is not None and N >= 1 and int(kappa_out.shape[0]) != N:
+        raise ValueError(f"kappa_out has {int(kappa_out.shape[0])} entries, the grid has {N}")
     if bin_width is not None:
-        k = hk_kdist(kappa, dnu, bin_width, n_g)
-        k_host = torch.empty(k.shape, dtype=k.dtype, pin_memory=True)
-        k_host.copy_(k, non_blocking=True)
-    if kappa_out is None:
-        kappa_out = torch.empty(kappa.shape, dtype=kappa.dtype, pin_memory=True)
-    kappa_out.copy_(kappa, non_blocking=True)
-    torch.cuda.current_stream().synchronize()
-    return kappa_out, k_host
+        ppb = int(round(bin_width / dnu))
+        if ppb < 1 or N < 1 or N % ppb or n_g < 1:
+            raise HKError(-1, "hk_opacity_host")
+        if k_out is None:
+            k_out = torch.empty((N // ppb, n_g), dtype=torch.float64, pin_memory=True)
+        elif tuple(k_out.shape) != (N // ppb, n_g):
+            raise ValueError(f"k_out has shape {tuple(k_out.shape)}, expected {(N // ppb, n_g)}")
+    else:
+        k_out = None
+    cl = _hk_lines(_host_ptr(nu0, "nu0"), _host_ptr(S, "S"), _host_ptr(gamma0, "gamma0"), _host_ptr(n_T, "n_T", True),
+                   _host_ptr(E_low, "E_low", True))
+    prm = _hk_params(float(mass_amu), float(q_ratio), HK_FP64, int(bool(lines_sorted)), _stream_ptr(stream))
+    _check(L.hk_opacity_host(C.byref(cl), n, T, P_atm, nu_min, nu_max, dnu, cutoff, _host_ptr(kappa_out, "kappa_out", True),
+                             float(bin_width or 0.0), int(n_g), _host_ptr(k_out, "k_out", True), C.byref(prm)),
+           "hk_opacity_host")
+    return kappa_out, k_out

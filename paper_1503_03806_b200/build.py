@@ -6,8 +6,9 @@ import shutil
 import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SRC = [os.path.join(HERE, "csrc", "hk_kernels.cu")]
-DEPS = SRC + [os.path.join(HERE, "csrc", "hk_voigt.cuh"), os.path.join(HERE, "..", "include", "hk.h")]
+SRC = [os.path.join(HERE, "csrc", "hk_kernels.cu"), os.path.join(HERE, "csrc", "hk_sort.cu")]
+DEPS = SRC + [os.path.join(HERE, "csrc", "hk_voigt.cuh"), os.path.join(HERE, "csrc", "hk_internal.h"),
+              os.path.join(HERE, "..", "include", "hk.h")]
 LIB = os.path.join(HERE, "libhk.so")
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

@@ -1,0 +1,21 @@
+// hk_internal.h — helpers shared by the translation units of libhk.so (not part of the C ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/hk.h"
+
+namespace hk {
+
+// records the CUDA error text for hk_last_cuda_error() and maps it to HK_ERR_NOMEM / HK_ERR_CUDA
+int cuda_fail(cudaError_t e, const char *what);
+
+// Stream-ordered allocations from the library's own memory pool (one per device, created on first use, release
+// threshold = unlimited so that scratch freed by one call is reused by the next instead of going back to the driver).
+int pool_alloc(void **p, size_t bytes, cudaStream_t st);
+void pool_free(void *p, cudaStream_t st);
+
+// hk_sort.cu
+int sort_lines_copy(const hk_lines *in, int64_t n, cudaStream_t st, hk_lines *out, void **buf);
+
+}  // namespace hk

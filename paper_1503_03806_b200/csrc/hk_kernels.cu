@@ -17,6 +17,7 @@
 #include <new>
 
 #include "../../include/hk.h"
+#include "hk_internal.h"
 #include "hk_voigt.cuh"
 
 namespace hk {
@@ -735,7 +736,7 @@ static thread_local cudaEvent_t g_ev[4] = {nullptr, nullptr, nullptr, nullptr}; 
 static thread_local bool g_ev_pending = false;
 static int g_timing = 0;
 
-static int cuda_fail(cudaError_t e, const char *what)
+int cuda_fail(cudaError_t e, const char *what)
 {
   snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", what, cudaGetErrorString(e));
   return e == cudaErrorMemoryAllocation ? HK_ERR_NOMEM : HK_ERR_CUDA;
@@ -747,6 +748,42 @@ static int cuda_fail(cudaError_t e, const char *what)
   } while (0)
 
 static bool pos_finite(double v) { return v > 0.0 && isfinite(v); }
+
+// the library's own stream-ordered memory pool, one per device (hk_internal.h)
+static int lib_pool(cudaMemPool_t *out)
+{
+  static cudaMemPool_t pools[64] = {};
+  int dev = 0;
+  HK_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) return HK_ERR_UNSUPPORTED;
+  if (!pools[dev]) {
+    cudaMemPoolProps props = {};
+    props.allocType = cudaMemAllocationTypePinned;
+    props.handleTypes = cudaMemHandleTypeNone;
+    props.location.type = cudaMemLocationTypeDevice;
+    props.location.id = dev;
+    cudaMemPool_t mp = nullptr;
+    HK_CUDA(cudaMemPoolCreate(&mp, &props));
+    uint64_t keep = UINT64_MAX;
+    HK_CUDA(cudaMemPoolSetAttribute(mp, cudaMemPoolAttrReleaseThreshold, &keep));
+    pools[dev] = mp;
+  }
+  *out = pools[dev];
+  return HK_OK;
+}
+int pool_alloc(void **p, size_t bytes, cudaStream_t st)
+{
+  *p = nullptr;
+  cudaMemPool_t mp = nullptr;
+  int rc = lib_pool(&mp);
+  if (rc != HK_OK) return rc;
+  HK_CUDA(cudaMallocFromPoolAsync(p, bytes ? bytes : 16, mp, st));
+  return HK_OK;
+}
+void pool_free(void *p, cudaStream_t st)
+{
+  if (p) cudaFreeAsync(p, st);
+}
 
 #ifndef HK_P
 #define HK_P 8
@@ -773,20 +810,15 @@ struct Scratch {
   int cap_tiles = 0;
 };
 
-static void dev_free(void *p, cudaStream_t st, bool pooled)
-{
-  if (!p) return;
-  if (pooled) cudaFreeAsync(p, st); else cudaFree(p);
-}
-
-static int scratch_reserve(Scratch &s, int64_t n_lines, int n_tiles, cudaStream_t st, bool pooled)
+static int scratch_reserve(Scratch &s, int64_t n_lines, int n_tiles, cudaStream_t st)
 {
   if (n_lines > s.cap_lines) {
-    dev_free(s.ma, st, pooled);
+    pool_free(s.ma, st);
     s.ma = nullptr; s.cap_lines = 0;
     const size_t n = (size_t)n_lines;
     void *p = nullptr;
-    if (pooled) HK_CUDA(cudaMallocAsync(&p, n * kBytesPerLine, st)); else HK_CUDA(cudaMalloc(&p, n * kBytesPerLine));
+    int rc = pool_alloc(&p, n * kBytesPerLine, st);
+    if (rc != HK_OK) return rc;
     s.ma = (MetaA *)p;
     s.mb = (MetaB *)((char *)p + n * 16);
     s.base = (LineBase *)((char *)p + n * 32);
@@ -795,11 +827,12 @@ static int scratch_reserve(Scratch &s, int64_t n_lines, int n_tiles, cudaStream_
     s.cap_lines = n_lines;
   }
   if (n_tiles > s.cap_tiles) {
-    dev_free(s.plan, st, pooled);
+    pool_free(s.plan, st);
     s.plan = nullptr; s.cap_tiles = 0;
     void *p = nullptr;
     const size_t bytes = (size_t)n_tiles * sizeof(int2) + 16;
-    if (pooled) HK_CUDA(cudaMallocAsync(&p, bytes, st)); else HK_CUDA(cudaMalloc(&p, bytes));
+    int rc = pool_alloc(&p, bytes, st);
+    if (rc != HK_OK) return rc;
     s.plan = (int2 *)p;
     s.queue = (int *)((char *)p + (size_t)n_tiles * sizeof(int2));
     s.cap_tiles = n_tiles;
@@ -807,10 +840,10 @@ static int scratch_reserve(Scratch &s, int64_t n_lines, int n_tiles, cudaStream_
   return HK_OK;
 }
 
-static void scratch_release(Scratch &s, cudaStream_t st, bool pooled)
+static void scratch_release(Scratch &s, cudaStream_t st)
 {
-  dev_free(s.ma, st, pooled);
-  dev_free(s.plan, st, pooled);
+  pool_free(s.ma, st);
+  pool_free(s.plan, st);
   s = Scratch();
 }
 
@@ -854,15 +887,14 @@ static int validate(const hk_lines *lines, int64_t n_lines, double T, double P_a
 }
 
 static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double P_atm, double q_ratio, double mass_amu,
-                       double nu_min, double dnu, double cutoff, int64_t N, double *kappa_out, Scratch &s, cudaStream_t st,
-                       bool pooled)
+                       double nu_min, double dnu, double cutoff, int64_t N, double *kappa_out, Scratch &s, cudaStream_t st)
 {
   if (n_lines == 0) {
     HK_CUDA(cudaMemsetAsync(kappa_out, 0, (size_t)N * sizeof(double), st));
     return HK_OK;
   }
   const int n_tiles = (int)((N + kTile - 1) / kTile);
-  int rc = scratch_reserve(s, n_lines, n_tiles, st, pooled);
+  int rc = scratch_reserve(s, n_lines, n_tiles, st);
   if (rc != HK_OK) return rc;
 
   cudaEvent_t *ev = g_ev;
@@ -911,11 +943,25 @@ static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double 
 using namespace hk;
 
 struct hk_ctx {
-  hk_lines lines;
+  hk_lines lines;      // what the kernels read: the caller's arrays, or the library's ordered copy
+  void *sorted_buf;    // the ordered copy (NULL when the caller's list was already ascending)
   int64_t n_lines;
   hk_params prm;
   Scratch scratch;
 };
+
+// Resolves the line list the kernels will read: the caller's arrays when they are ascending (promised by lines_sorted = 1,
+// or found so by the device check), else an ordered copy (*buf, to be released with pool_free).
+static int ordered_lines(const hk_lines *lines, int64_t n_lines, const hk_params *prm, hk_lines *out, void **buf)
+{
+  *out = *lines;
+  *buf = nullptr;
+  if (prm->lines_sorted || n_lines < 2) return HK_OK;
+  int rc = hk_lines_check_sorted(lines->nu0, n_lines, prm->stream);
+  if (rc == HK_OK) return HK_OK;
+  if (rc != HK_ERR_UNSORTED) return rc;
+  return sort_lines_copy(lines, n_lines, (cudaStream_t)prm->stream, out, buf);
+}
 
 extern "C" {
 
@@ -933,35 +979,85 @@ int hk_opacity(const hk_lines *lines, int64_t n_lines, double T, double P_atm, d
   int64_t N = 0;
   int rc = validate(lines, n_lines, T, P_atm, nu_min, nu_max, dnu, cutoff, kappa_out, prm, &N);
   if (rc != HK_OK) return rc;
-  if (!prm->lines_sorted && n_lines > 1) {
-    rc = hk_lines_check_sorted(lines->nu0, n_lines, prm->stream);
-    if (rc == HK_ERR_UNSORTED) return HK_ERR_UNSUPPORTED;  // TODO(round 1): device sort of a copy
-    if (rc != HK_OK) return rc;
+  cudaStream_t st = (cudaStream_t)prm->stream;
+  hk_lines use;
+  void *sorted_buf = nullptr;
+  rc = ordered_lines(lines, n_lines, prm, &use, &sorted_buf);
+  if (rc != HK_OK) return rc;
+  Scratch s;
+  rc = run_opacity(&use, n_lines, T, P_atm, prm->q_ratio, prm->mass_amu, nu_min, dnu, cutoff, N, kappa_out, s, st);
+  scratch_release(s, st);
+  pool_free(sorted_buf, st);
+  return rc;
+}
+
+int hk_opacity_host(const hk_lines *lines_host, int64_t n_lines, double T, double P_atm, double nu_min, double nu_max,
+                    double dnu, double cutoff, double *kappa_host_out, double bin_width, int n_g, double *k_host_out,
+                    const hk_params *prm)
+{
+  if (!lines_host || !prm || n_lines < 0 || (!kappa_host_out && !k_host_out)) return HK_ERR_INVALID;
+  if (n_lines > 0 && (!lines_host->nu0 || !lines_host->S || !lines_host->gamma0)) return HK_ERR_INVALID;
+  const int64_t N = hk_grid_size(nu_min, nu_max, dnu);
+  if (N < 1 || N > (1LL << 30)) return HK_ERR_INVALID;
+  int64_t n_bins = 0;
+  if (k_host_out) {
+    if (!pos_finite(bin_width) || n_g < 1 || n_g > 128) return HK_ERR_INVALID;
+    const double ppb_d = nearbyint(bin_width / dnu);
+    if (ppb_d < 1.0 || fmod((double)N, ppb_d) != 0.0) return HK_ERR_INVALID;
+    n_bins = N / (int64_t)ppb_d;
   }
   cudaStream_t st = (cudaStream_t)prm->stream;
-  Scratch s;
-  rc = run_opacity(lines, n_lines, T, P_atm, prm->q_ratio, prm->mass_amu, nu_min, dnu, cutoff, N, kappa_out, s, st, true);
-  scratch_release(s, st, true);
-  return rc;
+  const double *src[5] = {lines_host->nu0, lines_host->S, lines_host->gamma0, lines_host->n_T, lines_host->E_low};
+  const size_t fbytes = ((size_t)n_lines * sizeof(double) + 255) & ~(size_t)255;
+  const size_t kappa_bytes = ((size_t)N * sizeof(double) + 255) & ~(size_t)255;
+  void *dev = nullptr;
+  int rc = pool_alloc(&dev, 5 * fbytes + kappa_bytes + (size_t)n_bins * n_g * sizeof(double), st);
+  if (rc != HK_OK) return rc;
+  const double *dptr[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+  cudaError_t e = cudaSuccess;
+  for (int f = 0; f < 5 && e == cudaSuccess; ++f) {
+    if (!src[f] || n_lines == 0) continue;
+    double *d = (double *)((char *)dev + f * fbytes);
+    e = cudaMemcpyAsync(d, src[f], (size_t)n_lines * sizeof(double), cudaMemcpyHostToDevice, st);
+    dptr[f] = d;
+  }
+  double *d_kappa = (double *)((char *)dev + 5 * fbytes);
+  double *d_k = (double *)((char *)dev + 5 * fbytes + kappa_bytes);
+  if (e == cudaSuccess) {
+    hk_lines dl = {dptr[0], dptr[1], dptr[2], dptr[3], dptr[4]};
+    rc = hk_opacity(&dl, n_lines, T, P_atm, nu_min, nu_max, dnu, cutoff, d_kappa, prm);
+    if (rc == HK_OK && k_host_out) rc = hk_kdist(d_kappa, N, dnu, bin_width, n_g, d_k, prm->stream);
+    if (rc == HK_OK && kappa_host_out)
+      e = cudaMemcpyAsync(kappa_host_out, d_kappa, (size_t)N * sizeof(double), cudaMemcpyDeviceToHost, st);
+    if (rc == HK_OK && e == cudaSuccess && k_host_out)
+      e = cudaMemcpyAsync(k_host_out, d_k, (size_t)n_bins * n_g * sizeof(double), cudaMemcpyDeviceToHost, st);
+  }
+  pool_free(dev, st);
+  const cudaError_t es = cudaStreamSynchronize(st);
+  if (rc != HK_OK) return rc;
+  if (e != cudaSuccess) return cuda_fail(e, "hk_opacity_host copy");
+  if (es != cudaSuccess) return cuda_fail(es, "hk_opacity_host synchronize");
+  return HK_OK;
 }
 
 int hk_create(const hk_lines *lines, int64_t n_lines, const hk_params *prm, hk_ctx **out)
 {
   if (!lines || !prm || !out || n_lines < 0) return HK_ERR_INVALID;
   if (n_lines > 0 && (!lines->nu0 || !lines->S || !lines->gamma0)) return HK_ERR_INVALID;
+  if (n_lines > 2000000000LL) return HK_ERR_UNSUPPORTED;
   if (!pos_finite(prm->mass_amu)) return HK_ERR_INVALID;
   if (prm->precision == HK_FP32) return HK_ERR_UNSUPPORTED;
   if (prm->precision != HK_FP64) return HK_ERR_INVALID;
-  if (!prm->lines_sorted && n_lines > 1) {
-    int rc = hk_lines_check_sorted(lines->nu0, n_lines, prm->stream);
-    if (rc == HK_ERR_UNSORTED) return HK_ERR_UNSUPPORTED;
-    if (rc != HK_OK) return rc;
-  }
   hk_ctx *c = new (std::nothrow) hk_ctx();
   if (!c) return HK_ERR_NOMEM;
-  c->lines = *lines;
+  int rc = ordered_lines(lines, n_lines, prm, &c->lines, &c->sorted_buf);
+  if (rc != HK_OK) {
+    delete c;
+    return rc;
+  }
   c->n_lines = n_lines;
   c->prm = *prm;
+  c->prm.lines_sorted = 1;
   *out = c;
   return HK_OK;
 }
@@ -976,14 +1072,16 @@ int hk_opacity_ctx(hk_ctx *ctx, double T, double P_atm, double q_ratio, double n
   int rc = validate(&ctx->lines, ctx->n_lines, T, P_atm, nu_min, nu_max, dnu, cutoff, kappa_out, &p, &N);
   if (rc != HK_OK) return rc;
   return run_opacity(&ctx->lines, ctx->n_lines, T, P_atm, q_ratio, p.mass_amu, nu_min, dnu, cutoff, N, kappa_out,
-                     ctx->scratch, (cudaStream_t)p.stream, false);
+                     ctx->scratch, (cudaStream_t)p.stream);
 }
 
 int hk_destroy(hk_ctx *ctx)
 {
   if (!ctx) return HK_ERR_INVALID;
-  cudaStreamSynchronize((cudaStream_t)ctx->prm.stream);
-  scratch_release(ctx->scratch, (cudaStream_t)ctx->prm.stream, false);
+  cudaStream_t st = (cudaStream_t)ctx->prm.stream;
+  scratch_release(ctx->scratch, st);
+  pool_free(ctx->sorted_buf, st);
+  cudaStreamSynchronize(st);
   delete ctx;
   return HK_OK;
 }
@@ -994,7 +1092,7 @@ int hk_lines_check_sorted(const double *nu0_device, int64_t n_lines, void *strea
   if (n_lines < 2) return HK_OK;
   cudaStream_t st = (cudaStream_t)stream;
   int *flag = nullptr;
-  HK_CUDA(cudaMallocAsync(&flag, sizeof(int), st));
+  { void *pf = nullptr; int rcp = pool_alloc(&pf, sizeof(int), st); if (rcp != HK_OK) return rcp; flag = (int *)pf; }
   HK_CUDA(cudaMemsetAsync(flag, 0, sizeof(int), st));
   check_sorted_kernel<<<(unsigned)((n_lines + 255) / 256), 256, 0, st>>>(nu0_device, n_lines, flag);
   int h = 0;
@@ -1147,7 +1245,7 @@ int hk_fp64_peak(double *inst_per_s_out, void *stream)
   HK_CUDA(cudaGetDevice(&dev));
   HK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
   double *buf = nullptr;
-  HK_CUDA(cudaMallocAsync(&buf, 64, st));
+  { void *pb = nullptr; int rcp = pool_alloc(&pb, 64, st); if (rcp != HK_OK) return rcp; buf = (double *)pb; }
   cudaEvent_t e0, e1;
   HK_CUDA(cudaEventCreate(&e0));
   HK_CUDA(cudaEventCreate(&e1));

@@ -178,3 +178,48 @@ def test_config2_pressure_sweep_sampled_points():
         ref = oracle.opacity_points(wl.nu0, wl.S, wl.gamma0, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, js)
         _check(got[js], ref, ref_max=got.max())
     ctx.close()
+
+
+def test_unsorted_input_is_sorted_on_a_copy():
+    import torch
+    wl = workloads.small(seed=21, n_lines=5000, nu_max=150.0, cutoff=25.0, with_E=True, sorted_by_nu0=False)
+    assert np.any(np.diff(wl.nu0) < 0)
+    T, P, q = 1200.0, 0.5, wl.q_ratio(1200.0)
+    lines = hk.Lines.from_numpy(wl.nu0, wl.S, wl.gamma0, E_low=wl.E_low)
+    before = [t.clone() for t in (lines.nu0, lines.S, lines.gamma0, lines.E_low)]
+    got = hk.hk_opacity(lines, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, q_ratio=q, lines_sorted=False)
+    ctx = hk.Context(lines, lines_sorted=False)
+    got_ctx = ctx.opacity(T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, q_ratio=q)
+    torch.cuda.synchronize()
+    ctx.close()
+    for a, b in zip(before, (lines.nu0, lines.S, lines.gamma0, lines.E_low)):
+        assert torch.equal(a, b)                                     # inputs are never modified
+    idx = np.argsort(wl.nu0, kind="stable")
+    ref = oracle.opacity(wl.nu0[idx], wl.S[idx], wl.gamma0[idx], T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff,
+                         E_low=wl.E_low[idx], q_ratio=q)
+    _check(got.cpu().numpy(), ref)
+    assert torch.equal(got, got_ctx)
+    # an ordered list passed with lines_sorted=False takes the no-copy path and gives the same bits as lines_sorted=True
+    s = hk.Lines.from_numpy(wl.nu0[idx], wl.S[idx], wl.gamma0[idx], E_low=wl.E_low[idx])
+    a = hk.hk_opacity(s, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, q_ratio=q, lines_sorted=False)
+    b = hk.hk_opacity(s, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, q_ratio=q, lines_sorted=True)
+    assert torch.equal(a, b) and torch.equal(a, got)
+
+
+def test_host_buffer_form_matches_device_form():
+    import torch
+    wl = workloads.small(seed=5, n_lines=1500, nu_max=200.0, cutoff=25.0)
+    T, P = 1500.0, 1.0
+    lines = hk.Lines.from_numpy(wl.nu0, wl.S, wl.gamma0)
+    kap = hk.hk_opacity(lines, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff)
+    ktab = hk.hk_kdist(kap, wl.dnu, wl.bin_width, wl.n_g)
+    pin = lambda a: torch.as_tensor(a).pin_memory()
+    hk_kap, hk_k = hk.hk_opacity_host(pin(wl.nu0), pin(wl.S), pin(wl.gamma0), T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff,
+                                      bin_width=wl.bin_width, n_g=wl.n_g)
+    assert torch.equal(hk_kap, kap.cpu()) and torch.equal(hk_k, ktab.cpu())
+    # pageable numpy buffers, k-table only
+    none_kap, k2 = hk.hk_opacity_host(wl.nu0, wl.S, wl.gamma0, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff,
+                                      bin_width=wl.bin_width, n_g=wl.n_g, want_kappa=False)
+    assert none_kap is None and torch.equal(k2, ktab.cpu())
+    with pytest.raises(hk.HKError):
+        hk.hk_opacity_host(wl.nu0, wl.S, wl.gamma0, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, want_kappa=False)
