@@ -1,0 +1,231 @@
+// hk_kdist.cu — a5 + a6: per-bin ascending sort of kappa and resampling at Gauss-Legendre nodes (the k-distribution;
+// eqs. 14-15, per-bin result PAPER.md:219; the paper sorts the whole grid with Thrust and a bin key).
+//
+// One CTA per bin.  The bin is padded with +inf to n = T*E points (a power of two) and sorted by a bitonic network held in
+// REGISTERS: thread t owns the E consecutive elements t*E .. t*E+E-1.  Every merge phase (block size k) is the "flip"
+// step (partner i ^ (k-1)) followed by half-cleaners (partner i ^ j, j = k/4 .. 1), all ascending, so no direction flags:
+//   partner in the same thread (j < E)            -> compile-time register pairs
+//   partner in the same warp   (j < 32 E)         -> SHFL.BFLY
+//   partner in another warp    (j >= 32 E)        -> through shared memory (n = 1024, E = 8: 3 of the 55 steps)
+// kappa >= 0 (or +inf), no NaN: plain FP64 compares order the values.  HBM-bound in principle (8 B/point read once,
+// 8 n_g B/bin written); in practice bound by the compare-exchange count, n log^2 n / 4 per bin.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+
+#include "hk_internal.h"
+
+namespace hk {
+
+constexpr unsigned kFullMask = 0xffffffffu;
+
+struct KdistArgs {
+  const double *kappa;
+  double *k_out;
+  int ppb;   // points per bin
+  int n;     // padded size, T*E
+  int n_g;
+  double g[128];
+};
+
+__device__ __forceinline__ void ce(double &a, double &b)  // ascending compare-exchange
+{
+  const bool sw = a > b;
+  const double lo = sw ? b : a, hi = sw ? a : b;
+  a = lo;
+  b = hi;
+}
+
+// in-thread half-cleaners j = J, J/2, ..., 1 on E registers
+template <int E, int J>
+__device__ __forceinline__ void clean_regs(double (&v)[E])
+{
+  if constexpr (J >= 1) {
+#pragma unroll
+    for (int r = 0; r < E; ++r)
+      if ((r & J) == 0) ce(v[r], v[r | J]);
+    clean_regs<E, J / 2>(v);
+  }
+}
+// in-thread flip of block size K <= E
+template <int E, int K>
+__device__ __forceinline__ void flip_regs(double (&v)[E])
+{
+#pragma unroll
+  for (int r = 0; r < E; ++r)
+    if ((r & (K / 2)) == 0) ce(v[r], v[r ^ (K - 1)]);
+}
+// sorts the E registers of one thread (phases k = 2 .. E)
+template <int E, int K>
+__device__ __forceinline__ void sort_regs(double (&v)[E])
+{
+  if constexpr (K <= E) {
+    flip_regs<E, K>(v);
+    clean_regs<E, K / 4>(v);
+    sort_regs<E, K * 2>(v);
+  }
+}
+
+// shared-memory index of element i: E doubles of a thread, then 2 doubles of padding (128-bit accesses of the blocked
+// layout are then conflict-free per quarter warp)
+template <int E>
+__device__ __forceinline__ int pad(int i)
+{
+  return i + 2 * (i / E);
+}
+
+template <int E, int MAXT>
+__global__ void __launch_bounds__(MAXT) kdist_kernel(const __grid_constant__ KdistArgs a)
+{
+  extern __shared__ __align__(16) double s[];
+  const int T = blockDim.x, t = threadIdx.x;
+  const int bin = blockIdx.x;
+  const double *src = a.kappa + (int64_t)bin * a.ppb;
+  const double inf = __longlong_as_double(0x7ff0000000000000LL);
+
+  double v[E];
+  const int i0 = t * E;
+  if (i0 + E <= a.ppb && (reinterpret_cast<uintptr_t>(src + i0) & 15) == 0) {
+#pragma unroll
+    for (int r = 0; r < E; r += 2) {
+      const double2 d = *reinterpret_cast<const double2 *>(src + i0 + r);
+      v[r] = d.x;
+      v[r + 1] = d.y;
+    }
+  } else {
+#pragma unroll
+    for (int r = 0; r < E; ++r) v[r] = (i0 + r < a.ppb) ? src[i0 + r] : inf;
+  }
+
+  sort_regs<E, 2>(v);
+
+  for (int m = 2; m <= T; m <<= 1) {  // merge phase of block size k = m*E elements = m threads
+    // ---- steps whose partner sits in another warp: through shared memory ----
+    if (m > 32) {
+      __syncthreads();  // previous readers of s are done
+#pragma unroll
+      for (int r = 0; r < E; r += 2) *reinterpret_cast<double2 *>(&s[pad<E>(i0 + r)]) = make_double2(v[r], v[r + 1]);
+      __syncthreads();
+      const int k = m * E;
+      for (int q = 0; q < E / 2; ++q) {  // flip: i in the lower half of its block, partner i ^ (k-1)
+        const int p = t + T * q;
+        const int i = ((p & ~(k / 2 - 1)) << 1) | (p & (k / 2 - 1));
+        const int x = pad<E>(i), y = pad<E>(i ^ (k - 1));
+        const double u = s[x], w = s[y];
+        if (u > w) { s[x] = w; s[y] = u; }
+      }
+      __syncthreads();
+      for (int jj = m >> 2; jj >= 32; jj >>= 1) {
+        const int j = jj * E;
+        for (int q = 0; q < E / 2; ++q) {
+          const int p = t + T * q;
+          const int i = ((p & ~(j - 1)) << 1) | (p & (j - 1));
+          const int x = pad<E>(i), y = pad<E>(i | j);
+          const double u = s[x], w = s[y];
+          if (u > w) { s[x] = w; s[y] = u; }
+        }
+        __syncthreads();
+      }
+#pragma unroll
+      for (int r = 0; r < E; r += 2) {
+        const double2 d = *reinterpret_cast<const double2 *>(&s[pad<E>(i0 + r)]);
+        v[r] = d.x;
+        v[r + 1] = d.y;
+      }
+    } else {
+      // flip inside the warp: partner thread t ^ (m-1), its register E-1-r; the lower thread keeps the minimum
+      const bool keep_min = (t & (m >> 1)) == 0;
+#pragma unroll
+      for (int r = 0; r < E / 2; ++r) {
+        const double oa = __shfl_xor_sync(kFullMask, v[E - 1 - r], m - 1);
+        const double ob = __shfl_xor_sync(kFullMask, v[r], m - 1);
+        v[r] = ((v[r] > oa) == keep_min) ? oa : v[r];
+        v[E - 1 - r] = ((v[E - 1 - r] > ob) == keep_min) ? ob : v[E - 1 - r];
+      }
+    }
+    // ---- half-cleaners inside the warp ----
+    for (int jj = min(m >> 2, 16); jj >= 1; jj >>= 1) {
+      const bool keep_min = (t & jj) == 0;
+#pragma unroll
+      for (int r = 0; r < E; ++r) {
+        const double o = __shfl_xor_sync(kFullMask, v[r], jj);
+        const bool take = (v[r] > o) == keep_min;
+        v[r] = take ? o : v[r];
+      }
+    }
+    // ---- half-cleaners inside the thread ----
+    clean_regs<E, E / 2>(v);
+  }
+
+  // ---- a6: y_k = (k + 1/2)/ppb, linear interpolation at the Gauss-Legendre nodes, clamped at the ends ----
+  __syncthreads();
+#pragma unroll
+  for (int r = 0; r < E; r += 2) *reinterpret_cast<double2 *>(&s[pad<E>(i0 + r)]) = make_double2(v[r], v[r + 1]);
+  __syncthreads();
+  for (int q = t; q < a.n_g; q += T) {
+    const double p = __dadd_rn(__dmul_rn(a.g[q], (double)a.ppb), -0.5);
+    double val;
+    if (p <= 0.0) val = s[pad<E>(0)];
+    else if (p >= (double)(a.ppb - 1)) val = s[pad<E>(a.ppb - 1)];
+    else {
+      const int k = (int)floor(p);
+      const double f = p - (double)k;
+      const double s0 = s[pad<E>(k)], s1 = s[pad<E>(k + 1)];
+      val = s0 + f * (s1 - s0);
+    }
+    a.k_out[(int64_t)bin * a.n_g + q] = val;
+  }
+}
+
+template <int E, int MAXT>
+static int launch_kdist(const KdistArgs &a, int64_t n_bins, cudaStream_t st)
+{
+  const int T = a.n / E;
+  const size_t smem = (size_t)(a.n + 2 * T) * sizeof(double);
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(kdist_kernel<E, MAXT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (16384 + 2048) * 8);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(kdist_kernel)");
+    attr_set = true;
+  }
+  kdist_kernel<E, MAXT><<<(unsigned)n_bins, T, smem, st>>>(a);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return cuda_fail(e, "kdist_kernel launch");
+  return HK_OK;
+}
+
+}  // namespace hk
+
+using namespace hk;
+
+extern "C" int hk_kdist(const double *kappa, int64_t n_points, double dnu, double bin_width, int n_g, double *k_out,
+                        void *stream)
+{
+  if (!kappa || !k_out || n_points < 1 || !(dnu > 0.0) || !isfinite(dnu) || !(bin_width > 0.0) || !isfinite(bin_width) ||
+      n_g < 1 || n_g > 128)
+    return HK_ERR_INVALID;
+  const double ratio = bin_width / dnu;
+  const double ppb_d = nearbyint(ratio);
+  if (ppb_d < 1.0 || fabs(ratio - ppb_d) > 1e-9 * ppb_d) return HK_ERR_INVALID;
+  if (ppb_d > 16384.0) return HK_ERR_UNSUPPORTED;
+  const int ppb = (int)ppb_d;
+  if (n_points % ppb != 0) return HK_ERR_INVALID;
+  const int64_t n_bins = n_points / ppb;
+  if (n_bins > 2147483647LL) return HK_ERR_UNSUPPORTED;
+  KdistArgs a;
+  a.kappa = kappa;
+  a.k_out = k_out;
+  a.ppb = ppb;
+  a.n_g = n_g;
+  int n = 64;
+  while (n < ppb) n <<= 1;
+  a.n = n;
+  double wts[128];
+  int rc = hk_gauss_legendre(n_g, a.g, wts);
+  if (rc != HK_OK) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (n <= 256) return launch_kdist<2, 128>(a, n_bins, st);   // T = 32 .. 128
+  if (n == 512) return launch_kdist<4, 128>(a, n_bins, st);   // T = 128
+  if (n == 1024) return launch_kdist<8, 128>(a, n_bins, st);  // T = 128
+  return launch_kdist<16, 1024>(a, n_bins, st);                // T = 128 .. 1024
+}

@@ -7,7 +7,7 @@
 //                         streamed through a shared-memory ring by 1-D TMA bulk copies (producer warp, full/empty
 //                         mbarriers), regime chosen per (line, warp span) or per (line, 32-point group)
 //   a4                    coalesced kappa store from the same kernel ("without additional write-outs")
-//   a5/a6 kdist_kernel    per-bin shared-memory sort + resampling at Gauss-Legendre nodes
+//   a5/a6 kdist_kernel    (hk_kdist.cu) per-bin register/shuffle bitonic sort + resampling at Gauss-Legendre nodes
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdint.h>
@@ -661,51 +661,6 @@ __global__ void __launch_bounds__(128) voigt_K_kernel(const double *x, const dou
   if (live) out[i] = v;
 }
 
-// ------------------------------------------------------------------------------------------------------
-// a5 + a6: per-bin sort and resampling.  One CTA per bin; the bin is loaded into shared memory, padded with +inf
-// to a power of two, sorted by a bitonic network, and read at the Gauss-Legendre nodes.
-// ------------------------------------------------------------------------------------------------------
-struct KdistArgs {
-  const double *kappa;
-  double *k_out;
-  int ppb, ppb2, n_g;
-  double g[128];
-};
-
-__global__ void __launch_bounds__(512) kdist_kernel(const __grid_constant__ KdistArgs a)
-{
-  extern __shared__ __align__(16) double s[];
-  const int bin = blockIdx.x;
-  const double *src = a.kappa + (int64_t)bin * a.ppb;
-  for (int i = threadIdx.x; i < a.ppb2; i += blockDim.x)
-    s[i] = i < a.ppb ? src[i] : __longlong_as_double(0x7ff0000000000000LL);
-  __syncthreads();
-  for (int k = 2; k <= a.ppb2; k <<= 1) {
-    for (int j = k >> 1; j > 0; j >>= 1) {
-      for (int t = threadIdx.x; t < (a.ppb2 >> 1); t += blockDim.x) {
-        const int i = ((t & ~(j - 1)) << 1) | (t & (j - 1));  // index with bit j clear
-        const int p = i | j;
-        const double u = s[i], v = s[p];
-        const bool up = (i & k) == 0;
-        if ((u > v) == up) { s[i] = v; s[p] = u; }
-      }
-      __syncthreads();
-    }
-  }
-  for (int q = threadIdx.x; q < a.n_g; q += blockDim.x) {
-    const double p = __dadd_rn(__dmul_rn(a.g[q], (double)a.ppb), -0.5);
-    double v;
-    if (p <= 0.0) v = s[0];
-    else if (p >= (double)(a.ppb - 1)) v = s[a.ppb - 1];
-    else {
-      const int k = (int)floor(p);
-      const double f = p - (double)k;
-      v = s[k] + f * (s[k + 1] - s[k]);
-    }
-    a.k_out[(int64_t)bin * a.n_g + q] = v;
-  }
-}
-
 __global__ void __launch_bounds__(256) check_sorted_kernel(const double *nu0, int64_t n, int *flag)
 {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -1191,38 +1146,6 @@ int hk_gauss_legendre(int n_g, double *g, double *w)
     w[n_g - 1 - i] = (double)wt;
     w[i] = (double)wt;
   }
-  return HK_OK;
-}
-
-int hk_kdist(const double *kappa, int64_t n_points, double dnu, double bin_width, int n_g, double *k_out, void *stream)
-{
-  if (!kappa || !k_out || n_points < 1 || !pos_finite(dnu) || !pos_finite(bin_width) || n_g < 1 || n_g > 128)
-    return HK_ERR_INVALID;
-  const double ratio = bin_width / dnu;
-  const double ppb_d = nearbyint(ratio);
-  if (ppb_d < 1.0 || fabs(ratio - ppb_d) > 1e-9 * ppb_d) return HK_ERR_INVALID;
-  if (ppb_d > 16384.0) return HK_ERR_UNSUPPORTED;
-  const int ppb = (int)ppb_d;
-  if (n_points % ppb != 0) return HK_ERR_INVALID;
-  const int64_t n_bins = n_points / ppb;
-  if (n_bins > 2147483647LL) return HK_ERR_UNSUPPORTED;
-  KdistArgs a;
-  a.kappa = kappa; a.k_out = k_out; a.ppb = ppb; a.n_g = n_g;
-  int p2 = 2;
-  while (p2 < ppb) p2 <<= 1;
-  a.ppb2 = p2;
-  double wts[128];
-  int rc = hk_gauss_legendre(n_g, a.g, wts);
-  if (rc != HK_OK) return rc;
-  const size_t smem = (size_t)p2 * sizeof(double);
-  static bool attr_set = false;
-  if (!attr_set) {
-    HK_CUDA(cudaFuncSetAttribute(kdist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 16384 * 8));
-    attr_set = true;
-  }
-  int threads = p2 / 2 < 64 ? 64 : (p2 / 2 > 512 ? 512 : p2 / 2);
-  kdist_kernel<<<(unsigned)n_bins, threads, smem, (cudaStream_t)stream>>>(a);
-  HK_CUDA(cudaGetLastError());
   return HK_OK;
 }
 
