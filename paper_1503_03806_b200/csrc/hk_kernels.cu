@@ -9,11 +9,13 @@
 //   a4                    coalesced kappa store from the same kernel ("without additional write-outs")
 //   a5/a6 kdist_kernel    (hk_kdist.cu) per-bin register/shuffle bitonic sort + resampling at Gauss-Legendre nodes
 #include <cuda_runtime.h>
+#include <limits.h>
 #include <math.h>
 #include <stdint.h>
 #include <stdio.h>
 #include <string.h>
 
+#include <algorithm>
 #include <new>
 
 #include "../../include/hk.h"
@@ -73,7 +75,29 @@ struct PrepArgs {
   LineBase *base;
   LineGH2 *gh2;
   LineCore *core;
+  int nb;         // number of plan blocks of kPlanBlock grid points, ceil(N / kPlanBlock)
+  int *first_hi;  // [nb+1]  first_hi[b] = first line i with jhi_i >= b*kPlanBlock   (n if none)
+  int *first_lo;  // [nb+1]  first_lo[b] = first line i with jlo_i >= b*kPlanBlock   (n if none)
+  int *queue;     // tile-ticket counter of a3, reset here
 };
+
+constexpr int kPlanBlock = 256;  // granularity of the line-range lookup and of the cost model of a2
+
+// index window of a line: sub, sub, IEEE divide, ceil/floor — no multiply-add, nothing to contract (A4)
+__device__ __forceinline__ void line_window(double nu0, const PrepArgs &a, int &jlo, int &jhi)
+{
+  double lo = ceil(__ddiv_rn(__dsub_rn(__dsub_rn(nu0, a.cutoff), a.nu_min), a.dnu));
+  double hi = floor(__ddiv_rn(__dsub_rn(__dadd_rn(nu0, a.cutoff), a.nu_min), a.dnu));
+  if (!(lo > 0.0)) lo = 0.0;
+  if (!(hi < (double)(a.N - 1))) hi = (double)(a.N - 1);
+  if (lo > 2.0e9) lo = 2.0e9;
+  if (hi < -2.0e9) hi = -2.0e9;
+  jlo = (int)lo;
+  jhi = (int)hi;
+}
+// floor(j / kPlanBlock) for any sign
+__device__ __forceinline__ int plan_block_floor(int j) { return j >> 8; }
+static_assert(kPlanBlock == 256, "plan_block_floor shifts by 8");
 
 // grid-unit radius outside which x^2 + y^2 >= R holds: sqrt(R alpha^2 - gamma^2)/dnu, rounded outward
 __device__ __forceinline__ float radius_grid(double R, double a2, double g2, double inv_dnu, double margin)
@@ -88,6 +112,7 @@ __global__ void __launch_bounds__(256) line_prep_kernel(PrepArgs a)
 {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= a.n) return;
+  if (i == 0) *a.queue = 0;
   const double nu0 = a.nu0[i];
   double alpha = nu0 * a.vth;
   if (!(alpha > 0.0)) alpha = 0.0;  // nu0 <= 0: Lorentzian (A9)
@@ -116,17 +141,26 @@ __global__ void __launch_bounds__(256) line_prep_kernel(PrepArgs a)
   k.xc2 = alpha > 0.0 ? core_xc2(k.y) : 0.0;
   k.erfcx_y = k.xc2 > 0.0 ? erfcx(k.y) : 0.0;
   k.Acore = amp * g.inv_alpha * kInvSqrtPi;
-  // index window: sub, sub, IEEE divide, ceil/floor — no multiply-add, nothing to contract (A4)
-  double lo = ceil(__ddiv_rn(__dsub_rn(__dsub_rn(nu0, a.cutoff), a.nu_min), a.dnu));
-  double hi = floor(__ddiv_rn(__dsub_rn(__dadd_rn(nu0, a.cutoff), a.nu_min), a.dnu));
-  if (!(lo > 0.0)) lo = 0.0;
-  if (!(hi < (double)(a.N - 1))) hi = (double)(a.N - 1);
-  if (lo > 2.0e9) lo = 2.0e9;
-  if (hi < -2.0e9) hi = -2.0e9;
   MetaA ma;
   MetaB mb;
-  ma.jlo = (int)lo;
-  ma.jhi = (int)hi;
+  line_window(nu0, a, ma.jlo, ma.jhi);
+  {
+    // a2, line-parallel half: the list is ordered by nu0, so jlo and jhi are non-decreasing in i and line i is the
+    // "first line with jhi >= b*kPlanBlock" exactly for the blocks b with jhi_{i-1} < b*kPlanBlock <= jhi_i (same for jlo).
+    // Each entry of first_hi / first_lo has exactly one writer; the last line also fills the blocks beyond its window.
+    int plo = INT_MIN, phi = INT_MIN;
+    if (i > 0) line_window(a.nu0[i - 1], a, plo, phi);
+    const int n = (int)a.n;
+    int b0 = i > 0 ? max(plan_block_floor(phi) + 1, 0) : 0, b1 = min(plan_block_floor(ma.jhi), a.nb);
+    for (int b = b0; b <= b1; ++b) a.first_hi[b] = (int)i;
+    if (i == n - 1)
+      for (int b = max(plan_block_floor(ma.jhi) + 1, 0); b <= a.nb; ++b) a.first_hi[b] = n;
+    b0 = i > 0 ? max(plan_block_floor(plo) + 1, 0) : 0;
+    b1 = min(plan_block_floor(ma.jlo), a.nb);
+    for (int b = b0; b <= b1; ++b) a.first_lo[b] = (int)i;
+    if (i == n - 1)
+      for (int b = max(plan_block_floor(ma.jlo) + 1, 0); b <= a.nb; ++b) a.first_lo[b] = n;
+  }
   const double inv_dnu = 1.0 / a.dnu;
   double c = (nu0 - a.nu_min) * inv_dnu;
   c = fmin(fmax(c, -3.0e9), 3.0e9);
@@ -142,30 +176,6 @@ __global__ void __launch_bounds__(256) line_prep_kernel(PrepArgs a)
   a.base[i] = b;
   a.gh2[i] = g;
   a.core[i] = k;
-}
-
-// a2: lines are sorted by nu0, so jlo and jhi are non-decreasing in i.  Tile t owns points [t*tile, (t+1)*tile).
-// plan[t] = [first i with jhi >= tile_lo, first i with jlo > tile_hi).  Thread 0 also resets the tile queue of a3.
-__global__ void __launch_bounds__(128) tile_plan_kernel(const MetaA *meta, int64_t n, int n_tiles, int tile, int N,
-                                                        int2 *plan, int *queue)
-{
-  int t = blockIdx.x * blockDim.x + threadIdx.x;
-  if (t == 0) *queue = 0;
-  if (t >= n_tiles) return;
-  const int tlo = t * tile;
-  const int thi = min(N, tlo + tile) - 1;
-  int64_t lo = 0, hi = n;
-  while (lo < hi) {
-    int64_t mid = lo + ((hi - lo) >> 1);
-    if (meta[mid].jhi < tlo) lo = mid + 1; else hi = mid;
-  }
-  const int64_t L0 = lo;
-  hi = n;
-  while (lo < hi) {
-    int64_t mid = lo + ((hi - lo) >> 1);
-    if (meta[mid].jlo <= thi) lo = mid + 1; else hi = mid;
-  }
-  plan[t] = make_int2((int)L0, (int)lo);
 }
 
 // ------------------------------------------------------------------------------------------------------
@@ -243,7 +253,9 @@ struct __align__(16) StageHdr {
   int tile_lo;  // first grid point of the tile this chunk belongs to; < 0: no more work
   int cnt;      // lines in the chunk (0 for a tile no line touches)
   int flags;    // 1: first chunk of its tile, 2: last chunk of its tile
-  int pad;
+  int ws;       // points per warp span in this tile (<= 32 P)
+  int tile_hi;  // one past the last grid point of the tile
+  int pad[3];
 };
 
 template <int P, int WARPS>
@@ -261,6 +273,7 @@ struct __align__(128) VoigtSmem {
   int issued;        // chunks handed to the TMA engine so far (ticket that orders the refills)
   // refill cursor: owned by whoever holds ticket `issued`
   int cur_tile, cur_L0, cur_nl, cur_c, cur_nchunks, cur_stop;
+  int descending;  // tiles are handed out from the top of the grid (heavier tiles first)
 };
 
 struct VoigtArgs {
@@ -269,10 +282,10 @@ struct VoigtArgs {
   const LineBase *base;
   const LineGH2 *gh2;
   const LineCore *core;
-  const int2 *plan;
-  const int *order;  // tiles in the order they are handed out (descending cost), or NULL: ascending index
-  int *queue;
-  int n_tiles;
+  const int *first_hi;  // a2 lookup tables (see PrepArgs)
+  const int *first_lo;
+  int *queue;           // tile tickets (reset by a1)
+  int nb, n_tiles;
   double nu_min, dnu;
   int N;
   double *kappa;
@@ -337,12 +350,11 @@ struct SpanMasks {
   unsigned m1, m2, m3, e1, e2, mn;
 };
 template <int P>
-__device__ __forceinline__ SpanMasks classify32(const MetaA *ma, const MetaB *mb, int l, int cnt, int slo)
+__device__ __forceinline__ SpanMasks classify32(const MetaA *ma, const MetaB *mb, int l, int cnt, int slo, int shi)
 {
-  const int shi = slo + 32 * P - 1;
   const MetaA A = ma[l];
   const MetaB B = mb[l];
-  const bool act = (l < cnt) && (A.jhi >= slo) && (A.jlo <= shi);
+  const bool act = (l < cnt) && (shi >= slo) && (A.jhi >= slo) && (A.jlo <= shi);
   const bool inside = (A.jlo <= slo) && (A.jhi >= shi);
   const float dist = fmaxf(fmaxf((float)slo - A.c, A.c - (float)shi), 0.0f);
   const bool w1 = dist >= B.r1, w2 = dist >= B.r2, w3 = dist >= A.r3;
@@ -365,8 +377,8 @@ __device__ __forceinline__ SpanMasks classify32(const MetaA *ma, const MetaB *mb
 // first pass masked (same predicate on the same d^2).  Everything else goes through near_span (rule per group).
 template <int P>
 __device__ __noinline__ void near_pass(const MetaA *ma, const MetaB *mb, const LineBase *base, const LineGH2 *gh2,
-                                       const LineCore *core, int cnt, int slo, double nu_min, double dnu, const double *En_tab,
-                                       double *sk)
+                                       const LineCore *core, int cnt, int slo, int shi_act, double nu_min, double dnu,
+                                       const double *En_tab, double *sk)
 {
   const int lane = threadIdx.x & 31;
   const double En = lane < kTerms ? En_tab[lane] : 0.0;
@@ -377,7 +389,7 @@ __device__ __noinline__ void near_pass(const MetaA *ma, const MetaB *mb, const L
   for (int k = 0; k < P; ++k) accn[k] = 0.0;
 #pragma unroll 1
   for (int b0 = 0; b0 < cnt; b0 += 32) {
-    const SpanMasks M = classify32<P>(ma, mb, b0 + lane, cnt, slo);
+    const SpanMasks M = classify32<P>(ma, mb, b0 + lane, cnt, slo, shi_act);
 #pragma unroll 1
     for (unsigned m = M.mn; m; m &= m - 1) {
       const int i = b0 + (__ffs(m) - 1);
@@ -425,6 +437,15 @@ __device__ __noinline__ void near_pass(const MetaA *ma, const MetaB *mb, const L
   for (int k = 0; k < P; ++k) sk[32 * k + lane] += accn[k];
 }
 
+// lines that can touch the grid points [lo, hi): jhi >= lo and jlo < hi, looked up at plan-block granularity (a superset
+// by at most the lines that end or begin inside the two boundary blocks; classify32 masks them out)
+__device__ __forceinline__ int2 tile_lines(const VoigtArgs &a, int lo, int hi)
+{
+  const int L0 = a.first_hi[lo / kPlanBlock];
+  const int L1 = a.first_lo[min((hi + kPlanBlock - 1) / kPlanBlock, a.nb)];
+  return make_int2(L0, max(L1, L0));
+}
+
 // Hands the next chunk of lines (ring sequence number n) to the TMA engine: stage n % STAGES gets a header and, if the chunk
 // holds lines, five bulk copies completing on the stage's `full` mbarrier.  Pulls a new tile from the queue when the current
 // one is exhausted; after the last tile one stop header is posted and nothing more.  Called by one thread at a time, in
@@ -439,14 +460,14 @@ __device__ __forceinline__ void issue_chunk(VoigtSmem<P, WARPS> &S, const VoigtA
     const int ticket = atomicAdd(a.queue, 1);
     if (ticket >= a.n_tiles) {
       S.cur_stop = 1;
-      StageHdr h;
-      h.tile_lo = -1; h.cnt = 0; h.flags = 0; h.pad = 0;
+      StageHdr h = {};
+      h.tile_lo = -1;
       S.hdr[stage] = h;
       mbar_expect_tx(&S.full[stage], 0u);
       return;
     }
-    const int tile = a.order ? a.order[ticket] : ticket;
-    const int2 pl = a.plan[tile];
+    const int tile = S.descending ? a.n_tiles - 1 - ticket : ticket;
+    const int2 pl = tile_lines(a, tile * TILE, min((tile + 1) * TILE, a.N));
     const int nl = pl.y - pl.x;
     S.cur_tile = tile;
     S.cur_L0 = pl.x;
@@ -456,11 +477,12 @@ __device__ __forceinline__ void issue_chunk(VoigtSmem<P, WARPS> &S, const VoigtA
   }
   const int c = S.cur_c;
   const int cnt = min(CH, S.cur_nl - c * CH);
-  StageHdr h;
+  StageHdr h = {};
   h.tile_lo = S.cur_tile * TILE;
+  h.tile_hi = min(h.tile_lo + TILE, a.N);
+  h.ws = 32 * P;
   h.cnt = cnt > 0 ? cnt : 0;
   h.flags = (c == 0 ? 1 : 0) | (c == S.cur_nchunks - 1 ? 2 : 0);
-  h.pad = 0;
   S.hdr[stage] = h;
   S.cur_c = c + 1;
   const uint32_t nb = (uint32_t)h.cnt;
@@ -492,6 +514,13 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) voigt_kernel(const __grid_co
       S.done[s] = 0;
     }
     S.cur_tile = 0; S.cur_L0 = 0; S.cur_nl = 0; S.cur_c = 0; S.cur_nchunks = 0; S.cur_stop = 0;
+    {
+      // heavier tiles first: compare the line counts of the first and the last tile; on a tie take the top of the grid
+      // first (alpha grows with nu0, and with it the number of core points per line)
+      constexpr int TILE = WARPS * 32 * P;
+      const int2 f = tile_lines(a, 0, min(TILE, a.N)), l = tile_lines(a, (a.n_tiles - 1) * TILE, a.N);
+      S.descending = (l.y - l.x) >= (f.y - f.x);
+    }
     mbar_fence_init();
     for (int n = 0; n < STAGES; ++n) issue_chunk<P, WARPS>(S, a, n);  // fill the ring
     S.issued = STAGES;
@@ -499,7 +528,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) voigt_kernel(const __grid_co
   __syncthreads();  // the only CTA-wide barrier
 
   double *sk = S.sk[warp];  // this warp's accumulators between chunks (zero at the start of a tile)
-  int slo = 0;
+  int slo = 0, shi = -1;  // this warp's span of the current tile, inclusive (empty if shi < slo)
   int stage = 0;
   uint32_t phase = 0;
 
@@ -507,7 +536,10 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) voigt_kernel(const __grid_co
     mbar_wait(&S.full[stage], phase);
     const StageHdr h = S.hdr[stage];
     if (h.tile_lo < 0) break;
-    if (h.flags & 1) slo = h.tile_lo + warp * (32 * P);
+    if (h.flags & 1) {
+      slo = h.tile_lo + warp * h.ws;
+      shi = min(slo + h.ws, h.tile_hi) - 1;
+    }
     const LineBase *sbase = S.base[stage];
     const LineGH2 *sgh2 = S.gh2[stage];
     unsigned any_near = 0;
@@ -519,7 +551,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) voigt_kernel(const __grid_co
       for (int k = 0; k < P; ++k) acc[k] = sk[32 * k + lane];
 #pragma unroll 1
       for (int b0 = 0; b0 < h.cnt; b0 += 32) {
-        const SpanMasks M = classify32<P>(S.ma[stage], S.mb[stage], b0 + lane, h.cnt, slo);
+        const SpanMasks M = classify32<P>(S.ma[stage], S.mb[stage], b0 + lane, h.cnt, slo, shi);
         any_near |= M.mn;
         // ---- 1-point rule ----
 #pragma unroll 1
@@ -586,14 +618,15 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) voigt_kernel(const __grid_co
       for (int k = 0; k < P; ++k) sk[32 * k + lane] = acc[k];
     }
     // ---- near pass: 6-point rule and series, accumulating in sk ----
-    if (any_near) near_pass<P>(S.ma[stage], S.mb[stage], sbase, sgh2, S.core[stage], h.cnt, slo, a.nu_min, a.dnu, S.En, sk);
+    if (any_near)
+      near_pass<P>(S.ma[stage], S.mb[stage], sbase, sgh2, S.core[stage], h.cnt, slo, shi, a.nu_min, a.dnu, S.En, sk);
     if (h.flags & 2) {
 #pragma unroll
       for (int k = 0; k < P; ++k) {
         const int j = slo + lane + 32 * k;
         const double v = sk[32 * k + lane];
         sk[32 * k + lane] = 0.0;
-        if (j < a.N) a.kappa[j] = v;
+        if (j <= shi) a.kappa[j] = v;
       }
     }
     // ---- release the stage; the last warp out refills it (ring sequence number n + STAGES), in ticket order ----
@@ -759,13 +792,14 @@ struct Scratch {
   LineBase *base = nullptr;
   LineGH2 *gh2 = nullptr;
   LineCore *core = nullptr;
-  int2 *plan = nullptr;      // one allocation: plan[n_tiles] | queue
+  int *first_hi = nullptr;   // one allocation: first_hi[nb+1] | first_lo[nb+1] | queue
+  int *first_lo = nullptr;
   int *queue = nullptr;
   int64_t cap_lines = 0;
-  int cap_tiles = 0;
+  int cap_blocks = 0;
 };
 
-static int scratch_reserve(Scratch &s, int64_t n_lines, int n_tiles, cudaStream_t st)
+static int scratch_reserve(Scratch &s, int64_t n_lines, int nb, cudaStream_t st)
 {
   if (n_lines > s.cap_lines) {
     pool_free(s.ma, st);
@@ -781,16 +815,16 @@ static int scratch_reserve(Scratch &s, int64_t n_lines, int n_tiles, cudaStream_
     s.core = (LineCore *)((char *)p + n * 96);
     s.cap_lines = n_lines;
   }
-  if (n_tiles > s.cap_tiles) {
-    pool_free(s.plan, st);
-    s.plan = nullptr; s.cap_tiles = 0;
+  if (nb > s.cap_blocks) {
+    pool_free(s.first_hi, st);
+    s.first_hi = nullptr; s.cap_blocks = 0;
     void *p = nullptr;
-    const size_t bytes = (size_t)n_tiles * sizeof(int2) + 16;
-    int rc = pool_alloc(&p, bytes, st);
+    int rc = pool_alloc(&p, ((size_t)2 * (nb + 1) + 4) * sizeof(int), st);
     if (rc != HK_OK) return rc;
-    s.plan = (int2 *)p;
-    s.queue = (int *)((char *)p + (size_t)n_tiles * sizeof(int2));
-    s.cap_tiles = n_tiles;
+    s.first_hi = (int *)p;
+    s.first_lo = s.first_hi + (nb + 1);
+    s.queue = s.first_lo + (nb + 1);
+    s.cap_blocks = nb;
   }
   return HK_OK;
 }
@@ -798,7 +832,7 @@ static int scratch_reserve(Scratch &s, int64_t n_lines, int n_tiles, cudaStream_
 static void scratch_release(Scratch &s, cudaStream_t st)
 {
   pool_free(s.ma, st);
-  pool_free(s.plan, st);
+  pool_free(s.first_hi, st);
   s = Scratch();
 }
 
@@ -848,9 +882,14 @@ static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double 
     HK_CUDA(cudaMemsetAsync(kappa_out, 0, (size_t)N * sizeof(double), st));
     return HK_OK;
   }
-  const int n_tiles = (int)((N + kTile - 1) / kTile);
-  int rc = scratch_reserve(s, n_lines, n_tiles, st);
+  const int nb = (int)((N + kPlanBlock - 1) / kPlanBlock);
+  int rc = scratch_reserve(s, n_lines, nb, st);
   if (rc != HK_OK) return rc;
+  int grid = 0;
+  rc = voigt_grid(&grid);
+  if (rc != HK_OK) return rc;
+  const int n_tiles = (int)((N + kTile - 1) / kTile);
+  if (grid > n_tiles) grid = n_tiles;
 
   cudaEvent_t *ev = g_ev;
   if (g_timing) {
@@ -869,21 +908,15 @@ static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double 
   pa.nu_min = nu_min; pa.dnu = dnu; pa.cutoff = cutoff; pa.N = (int)N;
   pa.margin = 2.0 + 2.4e-7 * (double)N;
   pa.ma = s.ma; pa.mb = s.mb; pa.base = s.base; pa.gh2 = s.gh2; pa.core = s.core;
+  pa.nb = nb; pa.first_hi = s.first_hi; pa.first_lo = s.first_lo; pa.queue = s.queue;
   line_prep_kernel<<<(unsigned)((n_lines + 255) / 256), 256, 0, st>>>(pa);
   HK_CUDA(cudaGetLastError());
   if (g_timing) HK_CUDA(cudaEventRecord(ev[1], st));
-  tile_plan_kernel<<<(n_tiles + 127) / 128, 128, 0, st>>>(s.ma, n_lines, n_tiles, kTile, (int)N, s.plan, s.queue);
-  HK_CUDA(cudaGetLastError());
-  if (g_timing) HK_CUDA(cudaEventRecord(ev[2], st));
+  if (g_timing) HK_CUDA(cudaEventRecord(ev[2], st));  // a2 has no kernel of its own any more: stage [1] reads 0
   VoigtArgs va;
-  va.ma = s.ma; va.mb = s.mb; va.base = s.base; va.gh2 = s.gh2; va.core = s.core; va.plan = s.plan; va.queue = s.queue;
-  va.order = nullptr;
-  va.n_tiles = n_tiles;
+  va.ma = s.ma; va.mb = s.mb; va.base = s.base; va.gh2 = s.gh2; va.core = s.core;
+  va.first_hi = s.first_hi; va.first_lo = s.first_lo; va.queue = s.queue; va.nb = nb; va.n_tiles = n_tiles;
   va.nu_min = nu_min; va.dnu = dnu; va.N = (int)N; va.kappa = kappa_out;
-  int grid = 0;
-  rc = voigt_grid(&grid);
-  if (rc != HK_OK) return rc;
-  if (grid > n_tiles) grid = n_tiles;
   voigt_kernel<kP, kWarps, kMinB><<<grid, kWarps * 32, sizeof(VoigtSmemT), st>>>(va);
   HK_CUDA(cudaGetLastError());
   if (g_timing) {
