@@ -415,7 +415,11 @@ __device__ __noinline__ void near_pass(const MetaA *ma, const MetaB *mb, const L
         const bool keep = ((unsigned)(jrel + 32 * k) <= wlen) && !(q < qc);
         accn[k] += keep ? v : 0.0;
       }
+#ifdef HK_EXP_NO_SERIES
+      if (false) {
+#else
       if (dist < B.r6) {
+#endif
         const double inv_alpha = gh2[i].inv_alpha;
         const CoreLine C = core_setup(kc.y, kc.erfcx_y, En);
 #pragma unroll 1
@@ -618,6 +622,9 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) voigt_kernel(const __grid_co
       for (int k = 0; k < P; ++k) sk[32 * k + lane] = acc[k];
     }
     // ---- near pass: 6-point rule and series, accumulating in sk ----
+#ifdef HK_EXP_NO_NEAR
+    any_near = 0;
+#endif
     if (any_near)
       near_pass<P>(S.ma[stage], S.mb[stage], sbase, sgh2, S.core[stage], h.cnt, slo, shi, a.nu_min, a.dnu, S.En, sk);
     if (h.flags & 2) {
