@@ -152,9 +152,11 @@ int hk_regime_census(const double *nu0_host, const double *gamma0_host, int64_t 
                      double mass_amu, double nu_min, int64_t N, double dnu, double cutoff, int64_t counts_out[5]);
 
 /* Per-stage device time of the last hk_opacity / hk_opacity_ctx call on this thread, in milliseconds, measured
- * with CUDA events on the call's stream: [0] line prep, [1] tile plan, [2] Voigt accumulation + kappa store.
- * Enabled by hk_set_timing(1) (off by default).  The timed call stays asynchronous: it only records the events;
- * hk_last_stage_ms() waits for the last one (synchronous) and must be called before the next timed call. */
+ * with CUDA events on the call's stream: [0] line prep (a1, with the lookup tables of a2), [1] Voigt accumulation, far
+ * kernel (1- and 2-point rule, writes kappa), [2] Voigt accumulation, near kernel (3-, 6-point rule and series, adds to
+ * kappa); a3 + a4 = [1] + [2].  Enabled by hk_set_timing(1) (off by default).  The timed call stays asynchronous: it only
+ * records the events; hk_last_stage_ms() waits for the last one (synchronous) and must be called before the next timed
+ * call. */
 int hk_set_timing(int on);
 int hk_last_stage_ms(float ms_out[3]);
 

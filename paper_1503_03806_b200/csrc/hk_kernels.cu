@@ -47,12 +47,13 @@ struct __align__(16) LineGH2 {
   double e2, f2, A1a2, inv_alpha;  // gamma^2 - alpha^2/2; 2 alpha^2 gamma^2; A1 alpha^2; 1/alpha (0 if alpha == 0)
 };
 struct __align__(16) LineCore {
-  double y, erfcx_y, Acore, xc2;  // gamma/alpha; erfcx(y); amp/(alpha sqrt(pi)); series where x^2 < xc2
+  double y, erfcx_y, Acore, inv_y;  // gamma/alpha; erfcx(y); amp/(alpha sqrt(pi)); alpha/gamma.  alpha = 0: y = 1e150
 };
 static_assert(sizeof(MetaA) == 16 && sizeof(MetaB) == 16 && sizeof(LineBase) == 32 && sizeof(LineGH2) == 32 &&
                   sizeof(LineCore) == 32,
               "record size");
 constexpr size_t kBytesPerLine = sizeof(MetaA) + sizeof(MetaB) + sizeof(LineBase) + sizeof(LineGH2) + sizeof(LineCore);
+constexpr size_t kRingBytesPerLine = sizeof(MetaA) + sizeof(MetaB) + sizeof(LineBase) + sizeof(LineGH2);  // far kernel
 
 constexpr double kCLight = 2.99792458e10;   // cm/s
 constexpr double kBoltz = 1.380649e-16;     // erg/K
@@ -78,6 +79,7 @@ struct PrepArgs {
   int nb;         // number of plan blocks of kPlanBlock grid points, ceil(N / kPlanBlock)
   int *first_hi;  // [nb+1]  first_hi[b] = first line i with jhi_i >= b*kPlanBlock   (n if none)
   int *first_lo;  // [nb+1]  first_lo[b] = first line i with jlo_i >= b*kPlanBlock   (n if none)
+  int *first_c;   // [nb+1]  first_c[b]  = first line i centred at or beyond grid point b*kPlanBlock   (n if none)
   int *queue;     // tile-ticket counter of a3, reset here
 };
 
@@ -94,6 +96,12 @@ __device__ __forceinline__ void line_window(double nu0, const PrepArgs &a, int &
   if (hi < -2.0e9) hi = -2.0e9;
   jlo = (int)lo;
   jhi = (int)hi;
+}
+// floor of the line centre in grid units, clamped to the int range (monotone in nu0)
+__device__ __forceinline__ int line_centre_index(double nu0, const PrepArgs &a)
+{
+  const double c = floor((nu0 - a.nu_min) * (1.0 / a.dnu));
+  return (int)fmin(fmax(c, -2.0e9), 2.0e9);
 }
 // floor(j / kPlanBlock) for any sign
 __device__ __forceinline__ int plan_block_floor(int j) { return j >> 8; }
@@ -137,9 +145,9 @@ __global__ void __launch_bounds__(256) line_prep_kernel(PrepArgs a)
   g.A1a2 = b.A1 * a2;
   g.inv_alpha = alpha > 0.0 ? 1.0 / alpha : 0.0;
   LineCore k;
-  k.y = gamma * g.inv_alpha;
-  k.xc2 = alpha > 0.0 ? core_xc2(k.y) : 0.0;
-  k.erfcx_y = k.xc2 > 0.0 ? erfcx(k.y) : 0.0;
+  k.y = alpha > 0.0 ? gamma * g.inv_alpha : 1.0e150;  // series region x^2 < 44 - y^2: none for alpha = 0
+  k.inv_y = alpha > 0.0 ? alpha / gamma : 0.0;
+  k.erfcx_y = core_xc2(k.y) > 0.0 ? erfcx(k.y) : 0.0;
   k.Acore = amp * g.inv_alpha * kInvSqrtPi;
   MetaA ma;
   MetaB mb;
@@ -148,8 +156,12 @@ __global__ void __launch_bounds__(256) line_prep_kernel(PrepArgs a)
     // a2, line-parallel half: the list is ordered by nu0, so jlo and jhi are non-decreasing in i and line i is the
     // "first line with jhi >= b*kPlanBlock" exactly for the blocks b with jhi_{i-1} < b*kPlanBlock <= jhi_i (same for jlo).
     // Each entry of first_hi / first_lo has exactly one writer; the last line also fills the blocks beyond its window.
-    int plo = INT_MIN, phi = INT_MIN;
-    if (i > 0) line_window(a.nu0[i - 1], a, plo, phi);
+    int plo = INT_MIN, phi = INT_MIN, pc = INT_MIN;
+    if (i > 0) {
+      line_window(a.nu0[i - 1], a, plo, phi);
+      pc = line_centre_index(a.nu0[i - 1], a);
+    }
+    const int jc = line_centre_index(nu0, a);
     const int n = (int)a.n;
     int b0 = i > 0 ? max(plan_block_floor(phi) + 1, 0) : 0, b1 = min(plan_block_floor(ma.jhi), a.nb);
     for (int b = b0; b <= b1; ++b) a.first_hi[b] = (int)i;
@@ -160,6 +172,11 @@ __global__ void __launch_bounds__(256) line_prep_kernel(PrepArgs a)
     for (int b = b0; b <= b1; ++b) a.first_lo[b] = (int)i;
     if (i == n - 1)
       for (int b = max(plan_block_floor(ma.jlo) + 1, 0); b <= a.nb; ++b) a.first_lo[b] = n;
+    b0 = i > 0 ? max(plan_block_floor(pc) + 1, 0) : 0;
+    b1 = min(plan_block_floor(jc), a.nb);
+    for (int b = b0; b <= b1; ++b) a.first_c[b] = (int)i;
+    if (i == n - 1)
+      for (int b = max(plan_block_floor(jc) + 1, 0); b <= a.nb; ++b) a.first_c[b] = n;
   }
   const double inv_dnu = 1.0 / a.dnu;
   double c = (nu0 - a.nu_min) * inv_dnu;
@@ -226,25 +243,31 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
 }
 
 // ------------------------------------------------------------------------------------------------------
-// a3 + a4: Voigt accumulation.  Persistent CTAs of WARPS warps, all of them consumers.
+// a3 + a4: Voigt accumulation, in two kernels that split the (line, 256-point span) pairs between them by ONE test,
+// classify32(): does the whole span lie at or beyond the line's 2-point radius?
 //
-// Work unit = tile of WARPS*32*P consecutive grid points, pulled from an atomic queue.  Consumer warp w owns the span
-// [tile_lo + w*32P, +32P), lane l the points span_lo + l + 32k (k < P): stores are coalesced, every 32 consecutive points
-// ("group") belong to one k, and a thread carries P independent dependency chains.
+//   voigt_far_kernel   every pair whose span lies wholly in the far wing (r^2 >= 3200: 1- or 2-point Gauss-Hermite rule,
+//                      97 % of all evaluations of config 1), and writes kappa;
+//   voigt_near_kernel  every other pair (3-point, 6-point rule, series), rule chosen per 32-point group, and adds to kappa.
 //
-// The producer warp streams the lines of the tile's plan range through a STAGES-deep shared-memory ring in chunks of CH
-// lines: five 1-D TMA bulk copies per chunk (the five record spans) completing on the stage's `full` mbarrier; each
-// consumer warp releases the stage on its `empty` mbarrier.  No CTA-wide barrier exists after start-up: warps drift apart by
-// up to STAGES-1 chunks, and the ring keeps flowing across tile boundaries (each stage carries a header naming its tile).
+// Why two: the far work of a chunk of lines is the same for every warp of a CTA, the near work is not (it falls on the one
+// warp whose span holds the line centres; in a dense list, config 3, on the same warp for hundreds of consecutive chunks),
+// and warps that share a line ring can drift apart by only STAGES-1 chunks.  Kept apart, the far kernel streams lines through
+// a shared ring in lockstep at full rate, and the near work is spread over 4x as many independent 64-point units.
+// Each grid point has one owner per kernel and a fixed summation order: results are bitwise reproducible.
 //
-// A consumer warp handles a chunk 32 lines at a time.  First it CLASSIFIES them, lane = line: from the span's distance to
-// the line centre (float, grid units, conservative radii from a1) each lane picks the rule valid on the whole span, and four
-// ballots turn that into bit masks (1-, 2-, 3-point rule, near).  Then it walks each mask: a branch-free loop over the lines
-// of one rule, parameters broadcast from shared memory, an unrolled P-point body accumulating in registers.  The regime
-// decision thus costs ~1 instruction per (line, span) instead of a branch ladder, and the per-rule loops have no divergence.
-// Spans that reach inside the 3-point radius or straddle a cutoff edge take the near path: the rule is chosen per 32-point
-// group (still warp-uniform), the series only on groups that hold core points, accumulated in a per-warp shared-memory
-// strip (dynamic k without spilling the register accumulators).  Summation order is fixed: bitwise deterministic.
+// Far kernel.  Persistent CTAs of WARPS warps, all of them consumers.  Work unit = tile of WARPS*32*P consecutive grid
+// points, pulled from an atomic queue.  Warp w owns the span [tile_lo + w*32P, +32P), lane l the points span_lo + l + 32k
+// (k < P): stores are coalesced, every 32 consecutive points ("group") belong to one k, and a thread carries P independent
+// dependency chains.  The lines of the tile's range are streamed through a STAGES-deep shared-memory ring in chunks of CH
+// lines: four 1-D TMA bulk copies per chunk (the four record spans) completing on the stage's `full` mbarrier; the last
+// warp out of a stage refills it (ticket-ordered).  No CTA-wide barrier exists after start-up, and the ring keeps flowing
+// across tile boundaries (each stage carries a header naming its tile).
+// A warp handles a chunk 32 lines at a time.  First it CLASSIFIES them, lane = line: from the span's distance to the line
+// centre (float, grid units, conservative radii from a1) each lane picks the rule valid on the whole span, and ballots turn
+// that into bit masks.  Then it walks each mask: a branch-free loop over the lines of one rule, parameters broadcast from
+// shared memory, an unrolled P-point body accumulating in registers: ~1 instruction per (line, span) for the regime
+// decision, no divergence in the loops.
 // ------------------------------------------------------------------------------------------------------
 constexpr int CH = 128;     // lines per ring stage: 128 lines x 128 B
 constexpr int STAGES = 4;
@@ -264,9 +287,6 @@ struct __align__(128) VoigtSmem {
   MetaB mb[STAGES][CH];
   LineBase base[STAGES][CH];
   LineGH2 gh2[STAGES][CH];
-  LineCore core[STAGES][CH];
-  double sk[WARPS][32 * P];
-  double En[kTerms];  // exp(-a^2 n^2), n = 1..16: lane constants of the series
   StageHdr hdr[STAGES];
   uint64_t full[STAGES];
   int done[STAGES];  // warps that have finished with the stage's current chunk
@@ -284,161 +304,41 @@ struct VoigtArgs {
   const LineCore *core;
   const int *first_hi;  // a2 lookup tables (see PrepArgs)
   const int *first_lo;
-  int *queue;           // tile tickets (reset by a1)
+  const int *first_c;
+  int *queue;           // tile tickets of the far kernel (reset by a1)
   int nb, n_tiles;
   double nu_min, dnu;
   int N;
   double *kappa;
+  double r2_slope, r2_offset;  // near kernel: no line centred beyond r2_slope*j + r2_offset grid units of point j reaches it inside its 2-point radius
 };
 
-// near path of a3 for one (line, warp span): rule per 32-point group (warp-uniform), accumulated in the warp's shared-memory
-// strip sk[32k + lane].  Warp-collective (SHFL in the series).
-template <int P>
-__device__ __forceinline__ void near_span(const MetaA *pa, const MetaB *pm, const LineBase *pb, const LineGH2 *pg,
-                                       const LineCore *pk, int slo, int lane, double x0, double dnu, double En, double *sk)
-{
-  const MetaA ma = *pa;
-  const MetaB mb = *pm;
-  const LineBase b = *pb;
-  const LineGH2 g = *pg;
-  const float dist = fmaxf(fmaxf((float)slo - ma.c, ma.c - (float)(slo + 32 * P - 1)), 0.0f);
-  const double d0 = x0 - b.nu0;
-  Gh6 G6;
-  LineCore kc;
-  CoreLine C;
-  if (dist < ma.r3) {  // some group may need the 6-point rule or the series
-    G6 = gh6_consts(b.A1, b.g2, b.a2);
-    kc = *pk;
-    if (dist < mb.r6) C = core_setup(kc.y, kc.erfcx_y, En);
-  }
-#pragma unroll 1
-  for (int k = 0; k < P; ++k) {
-    const int glo = slo + 32 * k, ghi = glo + 31;
-    if (ghi < ma.jlo || glo > ma.jhi) continue;
-    const int j = glo + lane;
-    const bool inwin = (j >= ma.jlo) && (j <= ma.jhi);
-    const double d = fma((double)(32 * k), dnu, d0);
-    const float dg = fmaxf(fmaxf((float)glo - ma.c, ma.c - (float)ghi), 0.0f);
-    double v;
-    if (dg >= mb.r2) {
-      v = dg >= mb.r1 ? gh1_acc(0.0, d, b.A1, b.g2) : gh2_acc(0.0, d, b.A1, g.e2, g.f2, g.A1a2);
-    } else if (dg >= ma.r3) {
-      const double c3 = b.A1 * (1.0 / 3.0);
-      v = gh3_acc(0.0, d, b.g2, fma(-1.5, b.a2, b.g2), 6.0 * b.a2 * b.g2, 2.0 * c3, c3, b.A1 * b.a2);
-    } else {
-      v = gh6_val(d * d, G6);
-      if (dg < mb.r6) {  // the series region reaches into this group
-        const double x = fabs(d) * g.inv_alpha;
-        const double ks = core_K(fmin(x, 6.7), C);
-        if (x * x < kc.xc2) v = kc.Acore * ks;
-        else if (mb.rg > 0.0f) v = fma(kc.Acore, exp(-x * x), v);
-      } else if (dg < mb.rg) {
-        const double x = d * g.inv_alpha;
-        v = fma(kc.Acore, exp(-x * x), v);
-      }
-    }
-    sk[32 * k + lane] += inwin ? v : 0.0;
-  }
-}
-
-// lane = line classification of 32 lines of a chunk against the warp span [slo, slo + 32P).  Bit masks of the lines that
-//   m1, m2, m3 : take the 1-, 2-, 3-point rule on the whole span, span inside the line's window ("far")
-//   e1, e2     : take the 1- or 2-point rule on the whole span, but a cutoff edge of the line falls inside the span ("edge")
-//   mn         : everything else that touches the span ("near": span reaches inside the 3-point radius, or an edge span
-//                closer than the 2-point radius)
+// lane = line classification of 32 lines against the 256-point span [slo, shi] (both kernels call this, on the same
+// records, with the same float arithmetic: it is what splits the pairs between them).  Bit masks of the lines that
+//   m1, m2 : take the 1- / 2-point rule on the whole span, span inside the line's window             (far kernel)
+//   e1, e2 : likewise, but a cutoff edge of the line falls inside the span: masked to the window      (far kernel)
+//   mn     : touch the span, and the span reaches inside the 2-point radius                           (near kernel)
 struct SpanMasks {
-  unsigned m1, m2, m3, e1, e2, mn;
+  unsigned m1, m2, e1, e2, mn;
 };
-template <int P>
-__device__ __forceinline__ SpanMasks classify32(const MetaA *ma, const MetaB *mb, int l, int cnt, int slo, int shi)
+__device__ __forceinline__ SpanMasks classify_regs(const MetaA &A, const MetaB &B, bool live, int slo, int shi)
 {
-  const MetaA A = ma[l];
-  const MetaB B = mb[l];
-  const bool act = (l < cnt) && (shi >= slo) && (A.jhi >= slo) && (A.jlo <= shi);
+  const bool act = live && (shi >= slo) && (A.jhi >= slo) && (A.jlo <= shi);
   const bool inside = (A.jlo <= slo) && (A.jhi >= shi);
   const float dist = fmaxf(fmaxf((float)slo - A.c, A.c - (float)shi), 0.0f);
-  const bool w1 = dist >= B.r1, w2 = dist >= B.r2, w3 = dist >= A.r3;
+  const bool w1 = dist >= B.r1, w2 = dist >= B.r2;
   SpanMasks M;
   M.m1 = __ballot_sync(kFull, act && inside && w1);
   M.m2 = __ballot_sync(kFull, act && inside && !w1 && w2);
-  M.m3 = __ballot_sync(kFull, act && inside && !w2 && w3);
   M.e1 = __ballot_sync(kFull, act && !inside && w1);
   M.e2 = __ballot_sync(kFull, act && !inside && !w1 && w2);
-  M.mn = __ballot_sync(kFull, act && (!w3 || (!inside && !w2)));
+  M.mn = __ballot_sync(kFull, act && !w2);
   return M;
 }
-
-// near pass over one chunk: kept out of line (one call per chunk) so that the 6-point and series state never competes for
-// registers with the far loops; the span's accumulators live in the shared-memory strip sk across the call.
-//
-// Fast path (span reaches inside the 3-point radius, y >= 1e-8): the 6-point rule, valid wherever r^2 >= 44, on all P
-// groups at once (unrolled, P independent chains), masked to the window and to the points outside the series region
-// d^2 >= qc = xc2 alpha^2; then the series on the groups that hold series points, adding amp*K at exactly the points the
-// first pass masked (same predicate on the same d^2).  Everything else goes through near_span (rule per group).
-template <int P>
-__device__ __noinline__ void near_pass(const MetaA *ma, const MetaB *mb, const LineBase *base, const LineGH2 *gh2,
-                                       const LineCore *core, int cnt, int slo, int shi_act, double nu_min, double dnu,
-                                       const double *En_tab, double *sk)
+__device__ __forceinline__ SpanMasks classify32(const MetaA *ma, const MetaB *mb, int l, int cnt, int slo, int shi)
 {
-  const int lane = threadIdx.x & 31;
-  const double En = lane < kTerms ? En_tab[lane] : 0.0;
-  const double x0 = __dadd_rn(nu_min, __dmul_rn((double)(slo + lane), dnu));
-  const int shi = slo + 32 * P - 1;
-  double accn[P];
-#pragma unroll
-  for (int k = 0; k < P; ++k) accn[k] = 0.0;
-#pragma unroll 1
-  for (int b0 = 0; b0 < cnt; b0 += 32) {
-    const SpanMasks M = classify32<P>(ma, mb, b0 + lane, cnt, slo, shi_act);
-#pragma unroll 1
-    for (unsigned m = M.mn; m; m &= m - 1) {
-      const int i = b0 + (__ffs(m) - 1);
-      const MetaA A = ma[i];
-      const MetaB B = mb[i];
-      const float dist = fmaxf(fmaxf((float)slo - A.c, A.c - (float)shi), 0.0f);
-      if (!(dist < A.r3) || B.rg > 0.0f) {
-        near_span<P>(ma + i, mb + i, base + i, gh2 + i, core + i, slo, lane, x0, dnu, En, sk);
-        continue;
-      }
-      const LineBase b = base[i];
-      const LineCore kc = core[i];
-      const Gh6 G6 = gh6_consts(b.A1, b.g2, b.a2);
-      const double qc = kc.xc2 * b.a2;
-      const double d0 = x0 - b.nu0;
-      const unsigned wlen = (unsigned)(A.jhi - A.jlo);
-      const int jrel = slo + lane - A.jlo;
-#pragma unroll
-      for (int k = 0; k < P; ++k) {
-        const double d = fma((double)(32 * k), dnu, d0);
-        const double q = d * d;
-        const double v = gh6_val(q, G6);
-        const bool keep = ((unsigned)(jrel + 32 * k) <= wlen) && !(q < qc);
-        accn[k] += keep ? v : 0.0;
-      }
-#ifdef HK_EXP_NO_SERIES
-      if (false) {
-#else
-      if (dist < B.r6) {
-#endif
-        const double inv_alpha = gh2[i].inv_alpha;
-        const CoreLine C = core_setup(kc.y, kc.erfcx_y, En);
-#pragma unroll 1
-        for (int k = 0; k < P; ++k) {
-          const int glo = slo + 32 * k, ghi = glo + 31;
-          const float dg = fmaxf(fmaxf((float)glo - A.c, A.c - (float)ghi), 0.0f);
-          if (!(dg < B.r6) || ghi < A.jlo || glo > A.jhi) continue;
-          const double d = fma((double)(32 * k), dnu, d0);
-          const double q = d * d;
-          const double x = fabs(d) * inv_alpha;
-          const double ks = core_K(fmin(x, 6.7), C);
-          const bool take = ((unsigned)(jrel + 32 * k) <= wlen) && (q < qc);
-          sk[32 * k + lane] += take ? kc.Acore * ks : 0.0;
-        }
-      }
-    }
-  }
-#pragma unroll
-  for (int k = 0; k < P; ++k) sk[32 * k + lane] += accn[k];
+  const bool live = l < cnt;
+  return classify_regs(ma[live ? l : 0], mb[live ? l : 0], live, slo, shi);
 }
 
 // lines that can touch the grid points [lo, hi): jhi >= lo and jlo < hi, looked up at plan-block granularity (a superset
@@ -451,7 +351,7 @@ __device__ __forceinline__ int2 tile_lines(const VoigtArgs &a, int lo, int hi)
 }
 
 // Hands the next chunk of lines (ring sequence number n) to the TMA engine: stage n % STAGES gets a header and, if the chunk
-// holds lines, five bulk copies completing on the stage's `full` mbarrier.  Pulls a new tile from the queue when the current
+// holds lines, four bulk copies completing on the stage's `full` mbarrier.  Pulls a new tile from the queue when the current
 // one is exhausted; after the last tile one stop header is posted and nothing more.  Called by one thread at a time, in
 // order of n (ticket S.issued).
 template <int P, int WARPS>
@@ -491,27 +391,23 @@ __device__ __forceinline__ void issue_chunk(VoigtSmem<P, WARPS> &S, const VoigtA
   S.cur_c = c + 1;
   const uint32_t nb = (uint32_t)h.cnt;
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // the stage's previous readers (generic proxy) come first
-  mbar_expect_tx(&S.full[stage], nb * (uint32_t)kBytesPerLine);  // release: the header store above is visible to the waiters
+  mbar_expect_tx(&S.full[stage], nb * (uint32_t)kRingBytesPerLine);  // release: the header store above is visible to the waiters
   if (nb) {
     const int first = S.cur_L0 + c * CH;
     bulk_g2s(&S.ma[stage][0], a.ma + first, nb * 16u, &S.full[stage]);
     bulk_g2s(&S.mb[stage][0], a.mb + first, nb * 16u, &S.full[stage]);
     bulk_g2s(&S.base[stage][0], a.base + first, nb * 32u, &S.full[stage]);
     bulk_g2s(&S.gh2[stage][0], a.gh2 + first, nb * 32u, &S.full[stage]);
-    bulk_g2s(&S.core[stage][0], a.core + first, nb * 32u, &S.full[stage]);
   }
 }
 
 template <int P, int WARPS, int MINB>
-__global__ void __launch_bounds__(WARPS * 32, MINB) voigt_kernel(const __grid_constant__ VoigtArgs a)
+__global__ void __launch_bounds__(WARPS * 32, MINB) voigt_far_kernel(const __grid_constant__ VoigtArgs a)
 {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   VoigtSmem<P, WARPS> &S = *reinterpret_cast<VoigtSmem<P, WARPS> *>(smem_raw);
 
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-#pragma unroll
-  for (int k = 0; k < P; ++k) S.sk[warp][32 * k + lane] = 0.0;
-  if (warp == 1 && lane < kTerms) S.En[lane] = core_lane_const();
   if (threadIdx.x == 0) {
     for (int s = 0; s < STAGES; ++s) {
       mbar_init(&S.full[s], 1);
@@ -519,8 +415,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) voigt_kernel(const __grid_co
     }
     S.cur_tile = 0; S.cur_L0 = 0; S.cur_nl = 0; S.cur_c = 0; S.cur_nchunks = 0; S.cur_stop = 0;
     {
-      // heavier tiles first: compare the line counts of the first and the last tile; on a tie take the top of the grid
-      // first (alpha grows with nu0, and with it the number of core points per line)
+      // heavier tiles first: compare the line counts of the first and the last tile
       constexpr int TILE = WARPS * 32 * P;
       const int2 f = tile_lines(a, 0, min(TILE, a.N)), l = tile_lines(a, (a.n_tiles - 1) * TILE, a.N);
       S.descending = (l.y - l.x) >= (f.y - f.x);
@@ -531,10 +426,13 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) voigt_kernel(const __grid_co
   }
   __syncthreads();  // the only CTA-wide barrier
 
-  double *sk = S.sk[warp];  // this warp's accumulators between chunks (zero at the start of a tile)
   int slo = 0, shi = -1;  // this warp's span of the current tile, inclusive (empty if shi < slo)
   int stage = 0;
   uint32_t phase = 0;
+  double x0 = 0.0;
+  double acc[P];  // kappa of this thread's P points, carried in registers over all chunks of a tile
+#pragma unroll
+  for (int k = 0; k < P; ++k) acc[k] = 0.0;
 
   for (int n = 0;; ++n) {
     mbar_wait(&S.full[stage], phase);
@@ -543,97 +441,69 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) voigt_kernel(const __grid_co
     if (h.flags & 1) {
       slo = h.tile_lo + warp * h.ws;
       shi = min(slo + h.ws, h.tile_hi) - 1;
+      x0 = __dadd_rn(a.nu_min, __dmul_rn((double)(slo + lane), a.dnu));  // nu_j exactly as defined (A6)
     }
     const LineBase *sbase = S.base[stage];
     const LineGH2 *sgh2 = S.gh2[stage];
-    unsigned any_near = 0;
-    {
-      // ---- far pass: register accumulators ----
-      const double x0 = __dadd_rn(a.nu_min, __dmul_rn((double)(slo + lane), a.dnu));  // nu_j exactly as defined (A6)
-      double acc[P];
-#pragma unroll
-      for (int k = 0; k < P; ++k) acc[k] = sk[32 * k + lane];
 #pragma unroll 1
-      for (int b0 = 0; b0 < h.cnt; b0 += 32) {
-        const SpanMasks M = classify32<P>(S.ma[stage], S.mb[stage], b0 + lane, h.cnt, slo, shi);
-        any_near |= M.mn;
-        // ---- 1-point rule ----
+    for (int b0 = 0; b0 < h.cnt; b0 += 32) {
+      const SpanMasks M = classify32(S.ma[stage] + b0, S.mb[stage] + b0, lane, h.cnt - b0, slo, shi);
+      // ---- 1-point rule ----
 #pragma unroll 1
-        for (unsigned m = M.m1; m; m &= m - 1) {
-          const LineBase *pb = sbase + b0 + (__ffs(m) - 1);
-          const double nu0 = pb->nu0, A1 = pb->A1, g2 = pb->g2;
-          const double d0 = x0 - nu0;
+      for (unsigned m = M.m1; m; m &= m - 1) {
+        const LineBase *pb = sbase + b0 + (__ffs(m) - 1);
+        const double nu0 = pb->nu0, A1 = pb->A1, g2 = pb->g2;
+        const double d0 = x0 - nu0;
 #pragma unroll
-          for (int k = 0; k < P; ++k) acc[k] = gh1_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), A1, g2);
-        }
-        // ---- 2-point rule ----
+        for (int k = 0; k < P; ++k) acc[k] = gh1_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), A1, g2);
+      }
+      // ---- 2-point rule ----
 #pragma unroll 1
-        for (unsigned m = M.m2; m; m &= m - 1) {
-          const int i = b0 + (__ffs(m) - 1);
-          const double nu0 = sbase[i].nu0, A1 = sbase[i].A1;
-          const double e2 = sgh2[i].e2, f2 = sgh2[i].f2, A1a2 = sgh2[i].A1a2;
-          const double d0 = x0 - nu0;
+      for (unsigned m = M.m2; m; m &= m - 1) {
+        const int i = b0 + (__ffs(m) - 1);
+        const double nu0 = sbase[i].nu0, A1 = sbase[i].A1;
+        const double e2 = sgh2[i].e2, f2 = sgh2[i].f2, A1a2 = sgh2[i].A1a2;
+        const double d0 = x0 - nu0;
 #pragma unroll
-          for (int k = 0; k < P; ++k) acc[k] = gh2_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), A1, e2, f2, A1a2);
-        }
-        // ---- 3-point rule ----
+        for (int k = 0; k < P; ++k) acc[k] = gh2_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), A1, e2, f2, A1a2);
+      }
+      // ---- the same rules on spans that hold a cutoff edge: masked to the line's window ----
 #pragma unroll 1
-        for (unsigned m = M.m3; m; m &= m - 1) {
-          const LineBase *pb = sbase + b0 + (__ffs(m) - 1);
-          const double nu0 = pb->nu0, A1 = pb->A1, g2 = pb->g2, a2 = pb->a2;
-          const double d0 = x0 - nu0;
-          const double e3 = fma(-1.5, a2, g2), f3 = 6.0 * a2 * g2;
-          const double c3 = A1 * (1.0 / 3.0), c0 = 2.0 * c3, c3a = A1 * a2;
+      for (unsigned m = M.e1; m; m &= m - 1) {
+        const int i = b0 + (__ffs(m) - 1);
+        const int jlo = S.ma[stage][i].jlo, jhi = S.ma[stage][i].jhi;
+        const double nu0 = sbase[i].nu0, A1 = sbase[i].A1, g2 = sbase[i].g2;
+        const double d0 = x0 - nu0;
+        const unsigned wlen = (unsigned)(jhi - jlo);
+        const int jrel = slo + lane - jlo;
 #pragma unroll
-          for (int k = 0; k < P; ++k) acc[k] = gh3_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), g2, e3, f3, c0, c3, c3a);
-        }
-        // ---- 1- and 2-point rule on spans that hold a cutoff edge: same rules, masked to the line's window ----
-#pragma unroll 1
-        for (unsigned m = M.e1; m; m &= m - 1) {
-          const int i = b0 + (__ffs(m) - 1);
-          const int jlo = S.ma[stage][i].jlo, jhi = S.ma[stage][i].jhi;
-          const double nu0 = sbase[i].nu0, A1 = sbase[i].A1, g2 = sbase[i].g2;
-          const double d0 = x0 - nu0;
-          const unsigned wlen = (unsigned)(jhi - jlo);
-          const int jrel = slo + lane - jlo;
-#pragma unroll
-          for (int k = 0; k < P; ++k) {
-            const double t = gh1_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), A1, g2);
-            acc[k] = ((unsigned)(jrel + 32 * k) <= wlen) ? t : acc[k];
-          }
-        }
-#pragma unroll 1
-        for (unsigned m = M.e2; m; m &= m - 1) {
-          const int i = b0 + (__ffs(m) - 1);
-          const int jlo = S.ma[stage][i].jlo, jhi = S.ma[stage][i].jhi;
-          const double nu0 = sbase[i].nu0, A1 = sbase[i].A1;
-          const double e2 = sgh2[i].e2, f2 = sgh2[i].f2, A1a2 = sgh2[i].A1a2;
-          const double d0 = x0 - nu0;
-          const unsigned wlen = (unsigned)(jhi - jlo);
-          const int jrel = slo + lane - jlo;
-#pragma unroll
-          for (int k = 0; k < P; ++k) {
-            const double t = gh2_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), A1, e2, f2, A1a2);
-            acc[k] = ((unsigned)(jrel + 32 * k) <= wlen) ? t : acc[k];
-          }
+        for (int k = 0; k < P; ++k) {
+          const double t = gh1_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), A1, g2);
+          acc[k] = ((unsigned)(jrel + 32 * k) <= wlen) ? t : acc[k];
         }
       }
+#pragma unroll 1
+      for (unsigned m = M.e2; m; m &= m - 1) {
+        const int i = b0 + (__ffs(m) - 1);
+        const int jlo = S.ma[stage][i].jlo, jhi = S.ma[stage][i].jhi;
+        const double nu0 = sbase[i].nu0, A1 = sbase[i].A1;
+        const double e2 = sgh2[i].e2, f2 = sgh2[i].f2, A1a2 = sgh2[i].A1a2;
+        const double d0 = x0 - nu0;
+        const unsigned wlen = (unsigned)(jhi - jlo);
+        const int jrel = slo + lane - jlo;
 #pragma unroll
-      for (int k = 0; k < P; ++k) sk[32 * k + lane] = acc[k];
+        for (int k = 0; k < P; ++k) {
+          const double t = gh2_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), A1, e2, f2, A1a2);
+          acc[k] = ((unsigned)(jrel + 32 * k) <= wlen) ? t : acc[k];
+        }
+      }
     }
-    // ---- near pass: 6-point rule and series, accumulating in sk ----
-#ifdef HK_EXP_NO_NEAR
-    any_near = 0;
-#endif
-    if (any_near)
-      near_pass<P>(S.ma[stage], S.mb[stage], sbase, sgh2, S.core[stage], h.cnt, slo, shi, a.nu_min, a.dnu, S.En, sk);
-    if (h.flags & 2) {
+    if (h.flags & 2) {  // a4: the tile is complete
 #pragma unroll
       for (int k = 0; k < P; ++k) {
         const int j = slo + lane + 32 * k;
-        const double v = sk[32 * k + lane];
-        sk[32 * k + lane] = 0.0;
-        if (j <= shi) a.kappa[j] = v;
+        if (j <= shi) a.kappa[j] = acc[k];
+        acc[k] = 0.0;
       }
     }
     // ---- release the stage; the last warp out refills it (ring sequence number n + STAGES), in ticket order ----
@@ -662,6 +532,162 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) voigt_kernel(const __grid_co
       stage = 0;
       phase ^= 1u;
     }
+  }
+}
+
+// Near kernel.  CTA = one 256-point span (a plan block), kNearWarps warps, lane l of every warp on the points
+// plo + l + 32k (k < 8).  The CTA walks the lines centred within the block's bound on the 2-point radius (a2 table
+// first_c) 32 per warp at a time, classifies them against the span exactly as the far kernel does (classify32), and
+// compacts the lines the far kernel left out, in line order, into a shared-memory list with their records.  The list is
+// dealt round-robin to the warps.  A line whose span stays outside the 3-point radius takes the 3-point rule on all 8
+// groups (unrolled, register accumulators, masked to the window); any other line gets its rule per 32-point group, warp-
+// uniformly (3-, 6-point rule, series on the groups that hold core points), accumulated in the warp's shared-memory strip.
+// At the end the warps' sums are added in a fixed order to the kappa the far kernel wrote.
+constexpr int kNearP = kPlanBlock / 32;
+constexpr int kNearWarps = 4;
+constexpr int kNearCap = 256;  // list entries; a round adds at most 32 per warp
+
+struct __align__(16) NearSmem {
+  MetaA ma[kNearCap];
+  MetaB mb[kNearCap];
+  LineBase base[kNearCap];
+  LineGH2 gh2[kNearCap];
+  LineCore core[kNearCap];
+  double sk[kNearWarps][kPlanBlock];
+  int counts[kNearWarps];
+};
+
+// rule per 32-point group for one listed line, accumulated in the warp's strip sk[32k + lane].  Warp-collective.
+__device__ __noinline__ void near_groups(const MetaA *pa, const MetaB *pm, const LineBase *pb, const LineGH2 *pg,
+                                         const LineCore *pk, int plo, int lane, double x0, double dnu, double En, double *sk)
+{
+  const MetaA ma = *pa;
+  const MetaB mb = *pm;
+  const LineBase b = *pb;
+  const LineGH2 g = *pg;
+  const LineCore kc = *pk;
+  const float dist = fmaxf(fmaxf((float)plo - ma.c, ma.c - (float)(plo + kPlanBlock - 1)), 0.0f);
+  const double d0 = x0 - b.nu0;
+  const Gh6 G6 = gh6_consts(b.A1, b.g2, b.a2);
+  const double xc2 = core_xc2(kc.y);
+  CoreLine C;
+  if (dist < mb.r6) C = core_setup(kc.y, kc.inv_y, kc.erfcx_y, En);
+#pragma unroll 1
+  for (int k = 0; k < kNearP; ++k) {
+    const int glo = plo + 32 * k, ghi = glo + 31;
+    if (ghi < ma.jlo || glo > ma.jhi) continue;
+    const int j = glo + lane;
+    const bool inwin = (j >= ma.jlo) && (j <= ma.jhi);
+    const double d = fma((double)(32 * k), dnu, d0);
+    const float dg = fmaxf(fmaxf((float)glo - ma.c, ma.c - (float)ghi), 0.0f);
+    double v;
+    if (dg >= mb.r2) {
+      v = dg >= mb.r1 ? gh1_acc(0.0, d, b.A1, b.g2) : gh2_acc(0.0, d, b.A1, g.e2, g.f2, g.A1a2);
+    } else if (dg >= ma.r3) {
+      const double c3 = b.A1 * (1.0 / 3.0);
+      v = gh3_acc(0.0, d, b.g2, fma(-1.5, b.a2, b.g2), 6.0 * b.a2 * b.g2, 2.0 * c3, c3, b.A1 * b.a2);
+    } else {
+      v = gh6_val(d * d, G6);
+      if (dg < mb.r6) {  // the series region reaches into this group
+        const double x = fabs(d) * g.inv_alpha;
+        const double ks = core_K(fmin(x, 6.7), C);
+        if (x * x < xc2) v = kc.Acore * ks;
+        else if (mb.rg > 0.0f) v = fma(kc.Acore, exp(-x * x), v);
+      } else if (dg < mb.rg) {
+        const double x = d * g.inv_alpha;
+        v = fma(kc.Acore, exp(-x * x), v);
+      }
+    }
+    sk[32 * k + lane] += inwin ? v : 0.0;
+  }
+}
+
+__global__ void __launch_bounds__(kNearWarps * 32, 4) voigt_near_kernel(const __grid_constant__ VoigtArgs a)
+{
+  __shared__ NearSmem S;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int b = blockIdx.x;
+  const int plo = b * kPlanBlock, phi = min(plo + kPlanBlock, a.N) - 1;  // the span classify32 sees
+  // lines that can be "near" for this span: centre within R of it, and window touching it
+  const double R = fmax(fma(a.r2_slope, (double)phi, a.r2_offset), 4.0);
+  const double clo = (double)plo - R, chi = (double)phi + R;
+  int L0 = a.first_hi[b], L1 = a.first_lo[min(b + 1, a.nb)];
+  if (clo > 0.0) L0 = max(L0, a.first_c[min((int)(clo * (1.0 / kPlanBlock)), a.nb)]);
+  if (chi < (double)a.nb * kPlanBlock - 1.0) L1 = min(L1, a.first_c[min((int)(chi * (1.0 / kPlanBlock)) + 1, a.nb)]);
+  if (L1 <= L0) return;  // uniform over the CTA
+
+  const double En = core_lane_const();
+  const double x0 = __dadd_rn(a.nu_min, __dmul_rn((double)(plo + lane), a.dnu));
+  double *sk = S.sk[warp];
+#pragma unroll
+  for (int k = 0; k < kNearP; ++k) sk[32 * k + lane] = 0.0;
+  double acc[kNearP];
+#pragma unroll
+  for (int k = 0; k < kNearP; ++k) acc[k] = 0.0;
+  int list_n = 0;
+  bool any = false;
+
+  for (int base0 = L0; base0 < L1; base0 += 32 * kNearWarps) {
+    // ---- classify 32 lines per warp, compact the near ones into the list in line order ----
+    const int b0 = base0 + 32 * warp;
+    const int i = b0 + lane;
+    const bool live = i < L1;
+    const MetaA A = a.ma[live ? i : L0];
+    const MetaB B = a.mb[live ? i : L0];
+    const SpanMasks M = classify_regs(A, B, live, plo, phi);
+    if (lane == 0) S.counts[warp] = __popc(M.mn);
+    __syncthreads();
+    int off = list_n, total = 0;
+#pragma unroll
+    for (int w = 0; w < kNearWarps; ++w) {
+      const int c = S.counts[w];
+      if (w < warp) off += c;
+      total += c;
+    }
+    if ((M.mn >> lane) & 1u) {
+      const int slot = off + __popc(M.mn & ((1u << lane) - 1u));
+      S.ma[slot] = A;
+      S.mb[slot] = B;
+      S.base[slot] = a.base[i];
+      S.gh2[slot] = a.gh2[i];
+      S.core[slot] = a.core[i];
+    }
+    list_n += total;
+    __syncthreads();
+    // ---- work the list off when it may not hold another round, and at the end ----
+    if (list_n > kNearCap - 32 * kNearWarps || base0 + 32 * kNearWarps >= L1) {
+      any |= list_n > 0;
+#pragma unroll 1
+      for (int e = warp; e < list_n; e += kNearWarps) {
+        const MetaA ea = S.ma[e];
+        const float dist = fmaxf(fmaxf((float)plo - ea.c, ea.c - (float)phi), 0.0f);
+        if (dist >= ea.r3) {  // 3-point rule on the whole span
+          const LineBase lb = S.base[e];
+          const double d0 = x0 - lb.nu0;
+          const double e3 = fma(-1.5, lb.a2, lb.g2), f3 = 6.0 * lb.a2 * lb.g2;
+          const double c3 = lb.A1 * (1.0 / 3.0), c0 = 2.0 * c3, c3a = lb.A1 * lb.a2;
+          const unsigned wlen = (unsigned)(ea.jhi - ea.jlo);
+          const int jrel = plo + lane - ea.jlo;
+#pragma unroll
+          for (int k = 0; k < kNearP; ++k) {
+            const double t = gh3_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), lb.g2, e3, f3, c0, c3, c3a);
+            acc[k] = ((unsigned)(jrel + 32 * k) <= wlen) ? t : acc[k];
+          }
+        } else {
+          near_groups(S.ma + e, S.mb + e, S.base + e, S.gh2 + e, S.core + e, plo, lane, x0, a.dnu, En, sk);
+        }
+      }
+      list_n = 0;
+      __syncthreads();  // the list is free again
+    }
+  }
+  if (!any) return;  // uniform over the CTA
+#pragma unroll
+  for (int k = 0; k < kNearP; ++k) sk[32 * k + lane] += acc[k];
+  __syncthreads();
+  for (int p = threadIdx.x; p < kPlanBlock; p += kNearWarps * 32) {
+    const int j = plo + p;
+    if (j <= phi) a.kappa[j] += (S.sk[0][p] + S.sk[1][p]) + (S.sk[2][p] + S.sk[3][p]);
   }
 }
 
@@ -694,7 +720,7 @@ __global__ void __launch_bounds__(128) voigt_K_kernel(const double *x, const dou
     const int src = __ffs(need) - 1;
     need &= need - 1;
     const double ys = __shfl_sync(kFull, yi, src), xs = __shfl_sync(kFull, xi, src);
-    const CoreLine C = core_setup(ys, erfcx(ys), En);
+    const CoreLine C = core_setup(ys, 1.0 / ys, erfcx(ys), En);
     const double kc = core_K(fmin(xs, 6.7), C);
     if (lane == src) v = kc;
   }
@@ -799,8 +825,9 @@ struct Scratch {
   LineBase *base = nullptr;
   LineGH2 *gh2 = nullptr;
   LineCore *core = nullptr;
-  int *first_hi = nullptr;   // one allocation: first_hi[nb+1] | first_lo[nb+1] | queue
+  int *first_hi = nullptr;   // one allocation: first_hi[nb+1] | first_lo[nb+1] | first_c[nb+1] | queue
   int *first_lo = nullptr;
+  int *first_c = nullptr;
   int *queue = nullptr;
   int64_t cap_lines = 0;
   int cap_blocks = 0;
@@ -826,11 +853,12 @@ static int scratch_reserve(Scratch &s, int64_t n_lines, int nb, cudaStream_t st)
     pool_free(s.first_hi, st);
     s.first_hi = nullptr; s.cap_blocks = 0;
     void *p = nullptr;
-    int rc = pool_alloc(&p, ((size_t)2 * (nb + 1) + 4) * sizeof(int), st);
+    int rc = pool_alloc(&p, ((size_t)3 * (nb + 1) + 4) * sizeof(int), st);
     if (rc != HK_OK) return rc;
     s.first_hi = (int *)p;
     s.first_lo = s.first_hi + (nb + 1);
-    s.queue = s.first_lo + (nb + 1);
+    s.first_c = s.first_lo + (nb + 1);
+    s.queue = s.first_c + (nb + 1);
     s.cap_blocks = nb;
   }
   return HK_OK;
@@ -852,9 +880,9 @@ static int voigt_grid(int *grid_out)
   if (dev != cached_dev) {
     int sms = 0, per_sm = 0;
     HK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    HK_CUDA(cudaFuncSetAttribute(voigt_kernel<kP, kWarps, kMinB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    HK_CUDA(cudaFuncSetAttribute(voigt_far_kernel<kP, kWarps, kMinB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  (int)sizeof(VoigtSmemT)));
-    HK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, voigt_kernel<kP, kWarps, kMinB>, kWarps * 32,
+    HK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, voigt_far_kernel<kP, kWarps, kMinB>, kWarps * 32,
                                                           sizeof(VoigtSmemT)));
     if (per_sm < 1) per_sm = 1;
     cached_grid = sms * per_sm;
@@ -915,16 +943,31 @@ static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double 
   pa.nu_min = nu_min; pa.dnu = dnu; pa.cutoff = cutoff; pa.N = (int)N;
   pa.margin = 2.0 + 2.4e-7 * (double)N;
   pa.ma = s.ma; pa.mb = s.mb; pa.base = s.base; pa.gh2 = s.gh2; pa.core = s.core;
-  pa.nb = nb; pa.first_hi = s.first_hi; pa.first_lo = s.first_lo; pa.queue = s.queue;
+  pa.nb = nb; pa.first_hi = s.first_hi; pa.first_lo = s.first_lo; pa.first_c = s.first_c; pa.queue = s.queue;
   line_prep_kernel<<<(unsigned)((n_lines + 255) / 256), 256, 0, st>>>(pa);
   HK_CUDA(cudaGetLastError());
   if (g_timing) HK_CUDA(cudaEventRecord(ev[1], st));
-  if (g_timing) HK_CUDA(cudaEventRecord(ev[2], st));  // a2 has no kernel of its own any more: stage [1] reads 0
   VoigtArgs va;
   va.ma = s.ma; va.mb = s.mb; va.base = s.base; va.gh2 = s.gh2; va.core = s.core;
-  va.first_hi = s.first_hi; va.first_lo = s.first_lo; va.queue = s.queue; va.nb = nb; va.n_tiles = n_tiles;
+  va.first_hi = s.first_hi; va.first_lo = s.first_lo; va.first_c = s.first_c; va.queue = s.queue;
+  va.nb = nb; va.n_tiles = n_tiles;
   va.nu_min = nu_min; va.dnu = dnu; va.N = (int)N; va.kappa = kappa_out;
-  voigt_kernel<kP, kWarps, kMinB><<<grid, kWarps * 32, sizeof(VoigtSmemT), st>>>(va);
+  {
+    // bound on the 2-point radius (grid units) of any line that can be near grid point j: r2 <= s*alpha/dnu + margin with
+    // alpha = vth*nu0 and nu0 <= nu_j + r2*dnu, s = sqrt(kR2)  =>  r2 <= (s*vth*(nu_min/dnu + j) + margin)/(1 - s*vth)
+    const double sv = sqrt(kR2) * pa.vth;
+    if (sv < 0.5) {
+      va.r2_slope = sv / (1.0 - sv);
+      va.r2_offset = (sv * fmax(nu_min / dnu, 0.0) + pa.margin + 4.0) / (1.0 - sv);
+    } else {  // absurdly hot / light: no useful bound, the near kernel scans every line that touches the span
+      va.r2_slope = 0.0;
+      va.r2_offset = 4.0e9;
+    }
+  }
+  voigt_far_kernel<kP, kWarps, kMinB><<<grid, kWarps * 32, sizeof(VoigtSmemT), st>>>(va);
+  HK_CUDA(cudaGetLastError());
+  if (g_timing) HK_CUDA(cudaEventRecord(ev[2], st));
+  voigt_near_kernel<<<nb, kNearWarps * 32, 0, st>>>(va);
   HK_CUDA(cudaGetLastError());
   if (g_timing) {
     HK_CUDA(cudaEventRecord(ev[3], st));

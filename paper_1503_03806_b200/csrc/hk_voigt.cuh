@@ -153,13 +153,13 @@ __device__ __forceinline__ double core_lane_const()
 }
 
 // All 32 lanes must call (warp-collective).  En = core_lane_const().
-__device__ __forceinline__ CoreLine core_setup(double y, double erfcx_y, double En)
+__device__ __forceinline__ CoreLine core_setup(double y, double inv_y, double erfcx_y, double En)
 {
   CoreLine c;
   const int lane = threadIdx.x & 31;
   const double n = (double)(lane + 1);
   c.y = y;
-  c.inv_y = 1.0 / y;
+  c.inv_y = inv_y;
   c.erfcx_y = erfcx_y;
   c.W = En * rcp_nr2(fma(kA * kA * n, n, y * y));
   double t = c.W;
