@@ -54,7 +54,8 @@ def tp_table(wl, world):
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs (B200_PROFILING.md)."""
+    """nvidia-smi clocks / throttle reasons sampled every 50 ms while the two timed regions (device-timed steps, then the
+    e2e steps) run (B200_PROFILING.md)."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
@@ -65,7 +66,7 @@ class ClockSampler:
 
     def start(self):
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200",
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "50",
                                           "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
         except OSError:
             self.proc = None
@@ -224,8 +225,6 @@ def run_ours(args):
     ms_kdist = sum(e[1].elapsed_time(e[2]) for e in ev)
     ms_total = ms_opacity + ms_kdist
     stage /= args.steps
-    clocks = sampler.stop() if rank == 0 else None
-
     # ---- e2e: host buffers in, host buffers out, through the public API -----------------------------------------------
     pin = lambda a: torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64)).pin_memory()
     h_nu0, h_S, h_g0 = pin(wl.nu0), pin(wl.S), pin(wl.gamma0)
@@ -241,6 +240,7 @@ def run_ours(args):
                            bin_width=wl.bin_width, n_g=wl.n_g, kappa_out=h_kappa, k_out=h_ktab)
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
+    clocks = sampler.stop() if rank == 0 else None
     h2d = 3 * 8 * wl.n_lines
     d2h = 8 * N + 8 * (N // ppb) * wl.n_g
 
@@ -296,7 +296,7 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     args = ap.parse_args()
