@@ -43,6 +43,9 @@ WORKLOAD = "BASELINE.json configs[1]: 1e5 lines, 3e6 grid points, cutoff 100 cm^
 # FP64-pipe thread-instructions the method needs per line-point evaluation, by regime (counted from
 # the formulas of hk_voigt.cuh with the Newton reciprocal; these are the algorithmic figures, not the executed SASS).
 FP64_INST_PER_EVAL = {"gh1": 5.0, "gh2": 7.0, "gh3": 11.0, "gh6": 22.0, "series": 150.0}
+# --precision fp32: FP32-pipe thread-instructions per evaluation of the two rules the far kernel runs in float, two points per
+# reciprocal (hk_voigt.cuh gh1_acc2f / gh2_acc2f: 8 and 13 per pair, + 1 MUFU.RCP per pair)
+FP32_INST_PER_EVAL = {"gh1": 4.0, "gh2": 6.5}
 
 
 def tp_table(wl, world):
@@ -191,11 +194,14 @@ def run_ours(args):
     flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
     stream = torch.cuda.current_stream()
 
+    prec = hk.HK_FP32 if args.precision == "fp32" else hk.HK_FP64
+
     def step():
-        hk.hk_opacity(lines, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, mass_amu=wl.mass_amu, out=kappa)
+        hk.hk_opacity(lines, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, mass_amu=wl.mass_amu, out=kappa, precision=prec)
         hk.hk_kdist(kappa, wl.dnu, wl.bin_width, wl.n_g, out=ktab)
 
     fp64_peak = hk.hk_fp64_peak()                                        # DFMA thread-instructions/s, measured live
+    fp32_peak = hk.hk_fp32_peak()                                        # FFMA, likewise
     for _ in range(max(args.warmup, 3)):
         step()
     barrier()
@@ -213,7 +219,7 @@ def run_ours(args):
     for i in range(args.steps):
         flush.zero_()
         ev[i][0].record(stream)
-        hk.hk_opacity(lines, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, mass_amu=wl.mass_amu, out=kappa)
+        hk.hk_opacity(lines, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, mass_amu=wl.mass_amu, out=kappa, precision=prec)
         ev[i][1].record(stream)
         hk.hk_kdist(kappa, wl.dnu, wl.bin_width, wl.n_g, out=ktab)
         ev[i][2].record(stream)
@@ -232,12 +238,12 @@ def run_ours(args):
     h_ktab = torch.empty((N // ppb, wl.n_g), dtype=torch.float64, pin_memory=True)
     for _ in range(2):
         hk.hk_opacity_host(h_nu0, h_S, h_g0, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, mass_amu=wl.mass_amu,
-                        bin_width=wl.bin_width, n_g=wl.n_g, kappa_out=h_kappa, k_out=h_ktab)
+                           bin_width=wl.bin_width, n_g=wl.n_g, kappa_out=h_kappa, k_out=h_ktab, precision=prec)
     barrier()
     t0 = time.perf_counter()
     for _ in range(args.steps):
         hk.hk_opacity_host(h_nu0, h_S, h_g0, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, mass_amu=wl.mass_amu,
-                           bin_width=wl.bin_width, n_g=wl.n_g, kappa_out=h_kappa, k_out=h_ktab)
+                           bin_width=wl.bin_width, n_g=wl.n_g, kappa_out=h_kappa, k_out=h_ktab, precision=prec)
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
     clocks = sampler.stop() if rank == 0 else None
@@ -245,10 +251,11 @@ def run_ours(args):
     d2h = 8 * N + 8 * (N // ppb) * wl.n_g
 
     # ---- max over ranks ------------------------------------------------------------------------------------------------
-    red = torch.tensor([ms_total, ms_opacity, ms_kdist, e2e_s * 1e3, stage[1] + stage[2]], dtype=torch.float64, device="cuda")
+    red = torch.tensor([ms_total, ms_opacity, ms_kdist, e2e_s * 1e3, stage[1] + stage[2], stage[1]], dtype=torch.float64,
+                       device="cuda")
     if world > 1:
         dist.all_reduce(red, op=dist.ReduceOp.MAX)
-    ms_total, ms_opacity, ms_kdist, e2e_ms, ms_voigt = [float(v) for v in red.cpu()]
+    ms_total, ms_opacity, ms_kdist, e2e_ms, ms_voigt, ms_far = [float(v) for v in red.cpu()]
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -257,17 +264,30 @@ def run_ours(args):
     K = args.steps
     value = world * n_evals * K / (ms_total * 1e-3)
     # roofline of the dominant kernel (voigt_kernel, a3+a4): ALU-bound on the FP64 pipe
-    census = hk.hk_regime_census(wl.nu0, wl.gamma0, T, P, wl.mass_amu, wl.nu_min, N, wl.dnu, wl.cutoff)
-    alg_inst = sum(FP64_INST_PER_EVAL[k] * census[k] for k in FP64_INST_PER_EVAL)
-    achieved = 2.0 * alg_inst / (ms_voigt * 1e-3) / 1e12                # FMA-equivalent TFLOP/s (1 FP64 instruction = 2 flop)
-    peak = 2.0 * fp64_peak / 1e12
+    census = hk.hk_regime_census(wl.nu0, wl.gamma0, T, P, wl.mass_amu, wl.nu_min, N, wl.dnu, wl.cutoff, precision=prec)
+    if prec == hk.HK_FP32:
+        # the FP32 variant's dominant kernel is the far kernel alone (1-/2-point rules in float, FP32 pipe)
+        alg_inst = sum(FP32_INST_PER_EVAL[k] * census[k] for k in FP32_INST_PER_EVAL)
+        achieved = 2.0 * alg_inst / (ms_far * 1e-3) / 1e12
+        peak = 2.0 * fp32_peak / 1e12
+        roof_kernel, roof_ms = "voigt_far_kernel<FP32> (a3 far wings + a4)", ms_far
+        roof_note = ("FP32-pipe thread-instructions x2 of the 1-/2-point rules (regime census x per-eval figure, two points per "
+                     "MUFU.RCP); peak = hk_fp32_peak FFMA microbenchmark measured live in this run; the near kernel "
+                     "(3-/6-point rules, series) stays FP64 and is reported in stage_ms")
+    else:
+        alg_inst = sum(FP64_INST_PER_EVAL[k] * census[k] for k in FP64_INST_PER_EVAL)
+        achieved = 2.0 * alg_inst / (ms_voigt * 1e-3) / 1e12            # FMA-equivalent TFLOP/s (1 FP64 instruction = 2 flop)
+        peak = 2.0 * fp64_peak / 1e12
+        roof_kernel, roof_ms = "voigt_far_kernel + voigt_near_kernel (a3+a4)", ms_voigt
+        roof_note = ("FP64-pipe thread-instructions x2; algorithmic instructions = regime census x per-eval figure "
+                     "(DESIGN.md); peak = hk_fp64_peak DFMA microbenchmark measured live in this run")
     cpu_v, cpu_dt, cpu_ne, cpu_desc, cores = oracle_sample(wl, T, P, 15.0) if world == 1 else (None, 0, 0, "", 0)
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic",
-        "config": {"workload": WORKLOAD, "n_lines": wl.n_lines, "n_points": N, "line_point_evals": n_evals,
+        "dtype": "f32" if prec == hk.HK_FP32 else "f64", "data": "synthetic",
+        "config": {"workload": WORKLOAD + (" [optional FP32 variant, bar 1e-4]" if prec == hk.HK_FP32 else ""), "n_lines": wl.n_lines, "n_points": N, "line_point_evals": n_evals,
                    "parallelism": f"tp-pairs x{world} (no collective)", "api": "hk_opacity + hk_kdist (C ABI, one-shot form)",
                    "l2": "flushed between steps by a 512 MiB memset outside the per-step CUDA events",
                    "T_K": T, "P_atm": P},
@@ -278,11 +298,9 @@ def run_ours(args):
         "e2e": {"value": world * n_evals * K / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": e2e_ms / K},
         "gpu_launches": 4 * K,   # line_prep, voigt_far, voigt_near, kdist
-        "roofline": {"kernel": "voigt_far_kernel + voigt_near_kernel (a3+a4)", "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                     "frac": achieved / peak, "traffic": None,
-                     "note": "FP64-pipe thread-instructions x2; algorithmic instructions = regime census x per-eval figure "
-                             "(DESIGN.md); peak = hk_fp64_peak DFMA microbenchmark measured live in this run",
-                     "regime_census": census, "ms": ms_voigt},
+        "roofline": {"kernel": roof_kernel, "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                     "frac": achieved / peak, "traffic": None, "note": roof_note, "regime_census": census, "ms": roof_ms,
+                     "fp64_peak_tflops": 2.0 * fp64_peak / 1e12, "fp32_peak_tflops": 2.0 * fp32_peak / 1e12},
         "clocks": clocks,
     }
     if cpu_v is not None:
@@ -299,6 +317,8 @@ def main():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--precision", choices=["fp64", "fp32"], default="fp64",
+                    help="fp64 (BASELINE.json config 1, the default) or the optional FP32 variant (bar 1e-4)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -45,7 +45,7 @@ extern "C" {
 #define HK_ERR_UNSUPPORTED (-5) /* valid request outside the implemented range (e.g. points per bin > 16384) */
 
 #define HK_FP64 0
-#define HK_FP32 1               /* reserved: optional FP32 variant (not implemented: returns HK_ERR_UNSUPPORTED) */
+#define HK_FP32 1               /* optional FP32 variant (north_star; bar 1e-4): see hk_opacity */
 
 /* Line list, structure of arrays, all DEVICE pointers, n_lines entries each.
  * These are the fields of a HITRAN/HITEMP record that the simplified broadening law of
@@ -61,7 +61,7 @@ typedef struct {
 typedef struct {
   double mass_amu;      /* molecular mass m (one species per call), amu; > 0                          */
   double q_ratio;       /* Q(296 K)/Q(T) of eq. 18; used only when E_low != NULL                      */
-  int precision;        /* HK_FP64                                                                    */
+  int precision;        /* HK_FP64 (bar 1e-6) or HK_FP32 (bar 1e-4): arithmetic of the far-wing rules, see hk_opacity */
   int lines_sorted;     /* 1: caller guarantees nu0 ascending, as HITRAN/HITEMP files are (not re-checked; see
                            hk_lines_check_sorted()).  0: the library checks on the device (synchronises the
                            stream) and, if needed, works on a copy ordered by nu0; inputs are never modified */
@@ -85,11 +85,17 @@ int64_t hk_grid_size(double nu_min, double nu_max, double dnu);
  * K = Re w(x+iy) is evaluated to <= 2.5e-7 relative error: Algorithm-916-type series for x^2+y^2 < 44,
  * 6/3/2/1-point Gauss-Hermite rules beyond 44 / 280 / 3200 / 6e6.
  *
+ * prm->precision = HK_FP32 (north_star's optional FP32 variant, max relative error <= 1e-4): the same ladder with the
+ * switches at 44 / 64 / 300 / 4e4 (each rule <= 4e-5 from exact K); the 1- and 2-point rules — every (line, 256-point
+ * span) pair beyond the 2-point radius, ~99 % of all evaluations — run in FP32 (distances from an integer + fraction
+ * split of the line centre in grid units, a float partial sum per 32 lines added to FP64 accumulators); the 3-/6-point
+ * rules and the series near the centre stay FP64, as do line prep, the index windows and kappa_out.  Line amplitudes
+ * S gamma/(pi m) below 1e-38 flush to zero in this mode.
+ *
  * kappa_out: device, N doubles, overwritten.  Lines outside [nu_min, nu_max) still contribute if within the
  * cutoff.  n_lines == 0 gives kappa == 0.
  * HK_ERR_INVALID: NULL lines/prm/kappa_out or (n_lines > 0 and NULL nu0/S/gamma0); n_lines < 0; T, P_atm, dnu,
  * cutoff, mass_amu not > 0 or not finite; N < 1 or N > 2^30; precision unknown.
- * HK_ERR_UNSUPPORTED: precision == HK_FP32.
  * Asynchronous on prm->stream (synchronises once when lines_sorted = 0).  nu0 must be ascending when
  * lines_sorted = 1 (see hk_lines_check_sorted). */
 int hk_opacity(const hk_lines *lines, int64_t n_lines, double T, double P_atm, double nu_min, double nu_max,
@@ -126,7 +132,8 @@ int hk_kdist(const double *kappa, int64_t n_points, double dnu, double bin_width
 int hk_gauss_legendre(int n_g, double *g, double *w);
 
 /* Test hook: out[i] = K(x[i], y[i]) = Re w(x+iy) through the device Voigt routine of hk_opacity (same regime
- * switches).  x, y, out: device [n]; y > 0.  Asynchronous. */
+ * switches; precision = HK_FP32: the FP32 variant's switches and float 1-/2-point rules).  x, y, out: device [n];
+ * y > 0.  HK_ERR_INVALID: NULL, n < 0, unknown precision.  Asynchronous. */
 int hk_voigt_K(const double *x, const double *y, int64_t n, double *out, int precision, void *stream);
 
 /* Persistent-context form for T-P sweeps ("repeat this calculation for multiple combinations of
@@ -143,13 +150,17 @@ int hk_destroy(hk_ctx *ctx);
  * thread-instructions per second (the "alu" roofline denominator of bench.py, measured live).  Synchronous. */
 int hk_fp64_peak(double *inst_per_s_out, void *stream);
 
+/* Likewise for the FP32 pipe (dependent FFMA; the roofline denominator of the FP32 variant).  Synchronous. */
+int hk_fp32_peak(double *inst_per_s_out, void *stream);
+
 /* Measurement helper (roofline numerator of bench.py): how many line-point evaluations of the workload fall in each
- * regime of the device Voigt routine, decided per POINT on r^2 = x^2 + y^2 exactly as hk_voigt_K does:
+ * regime of the device Voigt routine (switches of `precision`), decided per POINT on r^2 = x^2 + y^2 as hk_voigt_K does:
  * counts_out[0..4] = 1-point, 2-point, 3-point, 6-point Gauss-Hermite, series.  Their sum equals hk_count_evals().
  * gamma = gamma0 * P_atm * (296/T)^0.5 (n_T = 0.5), alpha = (nu0/c) sqrt(2 k_B T/m).  HOST arrays, host arithmetic,
- * O(n_lines).  HK_ERR_INVALID on NULL or non-positive T, P_atm, mass_amu, dnu, cutoff, N. */
+ * O(n_lines).  HK_ERR_INVALID on NULL, non-positive T, P_atm, mass_amu, dnu, cutoff, N, or unknown precision. */
 int hk_regime_census(const double *nu0_host, const double *gamma0_host, int64_t n_lines, double T, double P_atm,
-                     double mass_amu, double nu_min, int64_t N, double dnu, double cutoff, int64_t counts_out[5]);
+                     double mass_amu, double nu_min, int64_t N, double dnu, double cutoff, int precision,
+                     int64_t counts_out[5]);
 
 /* Per-stage device time of the last hk_opacity / hk_opacity_ctx call on this thread, in milliseconds, measured
  * with CUDA events on the call's stream: [0] line prep (a1, with the lookup tables of a2), [1] Voigt accumulation, far

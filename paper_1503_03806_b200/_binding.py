@@ -67,7 +67,7 @@ def load_library():
     L.hk_kdist.argtypes = [C.c_void_p, _i64, C.c_double, C.c_double, C.c_int, C.c_void_p, C.c_void_p]
     L.hk_regime_census.restype = C.c_int
     L.hk_regime_census.argtypes = [_dp, _dp, _i64, C.c_double, C.c_double, C.c_double, C.c_double, _i64, C.c_double,
-                                   C.c_double, C.POINTER(_i64)]
+                                   C.c_double, C.c_int, C.POINTER(_i64)]
     L.hk_gauss_legendre.restype = C.c_int
     L.hk_gauss_legendre.argtypes = [C.c_int, _dp, _dp]
     L.hk_voigt_K.restype = C.c_int
@@ -80,6 +80,8 @@ def load_library():
     L.hk_destroy.argtypes = [C.c_void_p]
     L.hk_fp64_peak.restype = C.c_int
     L.hk_fp64_peak.argtypes = [_dp, C.c_void_p]
+    L.hk_fp32_peak.restype = C.c_int
+    L.hk_fp32_peak.argtypes = [_dp, C.c_void_p]
     L.hk_set_timing.restype = C.c_int
     L.hk_set_timing.argtypes = [C.c_int]
     L.hk_last_stage_ms.restype = C.c_int
@@ -171,7 +173,7 @@ def hk_count_evals(nu0_host, nu_min: float, N: int, dnu: float, cutoff: float) -
     return int(load_library().hk_count_evals(a.ctypes.data_as(_dp), a.size, nu_min, int(N), dnu, cutoff))
 
 
-def hk_regime_census(nu0_host, gamma0_host, T, P_atm, mass_amu, nu_min, N, dnu, cutoff) -> dict:
+def hk_regime_census(nu0_host, gamma0_host, T, P_atm, mass_amu, nu_min, N, dnu, cutoff, precision=HK_FP64) -> dict:
     """Line-point evaluations per regime of the device Voigt routine (bench.py's roofline numerator).  Host arrays."""
     a = np.ascontiguousarray(nu0_host, dtype=np.float64)
     g = np.ascontiguousarray(gamma0_host, dtype=np.float64)
@@ -179,7 +181,7 @@ def hk_regime_census(nu0_host, gamma0_host, T, P_atm, mass_amu, nu_min, N, dnu, 
         raise ValueError("nu0 and gamma0 differ in length")
     c = (_i64 * 5)()
     _check(load_library().hk_regime_census(a.ctypes.data_as(_dp), g.ctypes.data_as(_dp), a.size, T, P_atm, mass_amu, nu_min,
-                                           int(N), dnu, cutoff, c), "hk_regime_census")
+                                           int(N), dnu, cutoff, int(precision), c), "hk_regime_census")
     return dict(zip(("gh1", "gh2", "gh3", "gh6", "series"), (int(v) for v in c)))
 
 
@@ -249,6 +251,13 @@ def hk_fp64_peak(stream=None) -> float:
     return v.value
 
 
+def hk_fp32_peak(stream=None) -> float:
+    """Measured FP32 FMA thread-instructions per second of this GPU (roofline denominator of the FP32 variant)."""
+    v = C.c_double(0.0)
+    _check(load_library().hk_fp32_peak(C.byref(v), _stream_ptr(stream)), "hk_fp32_peak")
+    return v.value
+
+
 def hk_set_timing(on: bool) -> None:
     _check(load_library().hk_set_timing(int(bool(on))), "hk_set_timing")
 
@@ -262,11 +271,11 @@ def hk_last_stage_ms():
 class Context:
     """hk_create / hk_opacity_ctx / hk_destroy: line list bound once, scratch kept across (T,P) calls."""
 
-    def __init__(self, lines: Lines, mass_amu=18.0, lines_sorted=True, stream=None):
+    def __init__(self, lines: Lines, mass_amu=18.0, lines_sorted=True, stream=None, precision=HK_FP64):
         self._lines = lines      # keep the tensors alive
         self._h = C.c_void_p()
         cl = lines._c()
-        prm = _hk_params(float(mass_amu), 1.0, HK_FP64, int(bool(lines_sorted)), _stream_ptr(stream))
+        prm = _hk_params(float(mass_amu), 1.0, int(precision), int(bool(lines_sorted)), _stream_ptr(stream))
         _check(load_library().hk_create(C.byref(cl), lines.n, C.byref(prm), C.byref(self._h)), "hk_create")
 
     def opacity(self, T, P_atm, nu_min, nu_max, dnu, cutoff, q_ratio=1.0, out=None):
@@ -306,7 +315,8 @@ def _host_ptr(t, name, allow_none=False):
 
 
 def hk_opacity_host(nu0, S, gamma0, T, P_atm, nu_min, nu_max, dnu, cutoff, mass_amu=18.0, n_T=None, E_low=None, q_ratio=1.0,
-                    lines_sorted=True, bin_width=None, n_g=20, kappa_out=None, k_out=None, want_kappa=True, stream=None):
+                    lines_sorted=True, bin_width=None, n_g=20, kappa_out=None, k_out=None, want_kappa=True, stream=None,
+                    precision=HK_FP64):
     """End-to-end call with HOST buffers (hk_opacity_host of include/hk.h): host line arrays -> device, hk_opacity
     (+ hk_kdist when bin_width is given), kappa / k-table -> host.  Buffers are host torch tensors (pinned for
     asynchronous copies) or numpy arrays.  Returns (kappa_host or None, k_host or None).  Synchronous."""
@@ -333,7 +343,7 @@ def hk_opacity_host(nu0, S, gamma0, T, P_atm, nu_min, nu_max, dnu, cutoff, mass_
         k_out = None
     cl = _hk_lines(_host_ptr(nu0, "nu0"), _host_ptr(S, "S"), _host_ptr(gamma0, "gamma0"), _host_ptr(n_T, "n_T", True),
                    _host_ptr(E_low, "E_low", True))
-    prm = _hk_params(float(mass_amu), float(q_ratio), HK_FP64, int(bool(lines_sorted)), _stream_ptr(stream))
+    prm = _hk_params(float(mass_amu), float(q_ratio), int(precision), int(bool(lines_sorted)), _stream_ptr(stream))
     _check(L.hk_opacity_host(C.byref(cl), n, T, P_atm, nu_min, nu_max, dnu, cutoff, _host_ptr(kappa_out, "kappa_out", True),
                              float(bin_width or 0.0), int(n_g), _host_ptr(k_out, "k_out", True), C.byref(prm)),
            "hk_opacity_host")

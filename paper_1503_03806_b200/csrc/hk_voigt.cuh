@@ -27,6 +27,12 @@ constexpr double kR1 = 6.0e6;   // 1-point rule from here   (max rel. error 2.5e
 constexpr double kR2 = 3200.0;  // 2-point rule             (2.4e-7)
 constexpr double kR3 = 280.0;   // 3-point rule             (2.4e-7)
 constexpr double kRc = 44.0;    // 6-point rule from here (3.7e-8); series below
+// FP32 variant (hk_params.precision = HK_FP32; north_star: "optional FP32 path", bar 1e-4): the same ladder with the
+// switches moved in to where each rule is <= 4e-5 from exact K (1-point 1.5/x^2, 2-point
+// 2.8e-5 at 300, 3-point 2.2e-5 at 64); the 1- and 2-point rules (the far kernel: ~99 % of all evaluations) run in FP32.
+constexpr double kR1f = 4.0e4;  // 1-point rule from here   (3.8e-5)
+constexpr double kR2f = 300.0;  // 2-point rule             (2.8e-5)
+constexpr double kR3f = 64.0;   // 3-point rule             (2.2e-5)
 constexpr double kXgCapSq = 270.0;  // the Gaussian term is never added beyond the 6-point region (exp(-270) = 5e-118)
 constexpr double kTinyY = 1.0e-8;   // below this damping the wing rules miss a visible exp(-x^2) beyond r^2 = 44
 
@@ -95,6 +101,31 @@ __device__ __forceinline__ double gh3_acc(double acc, double d, double g2, doubl
   double B = fma(c3, E, c3a);
   double num = fma(c0, D, B * R);
   return fma(num, rcp_nr(R * D), acc);
+}
+// ---- FP32 wing rules (far kernel of the FP32 variant): TWO points per reciprocal, 1/(D0 D1) by one MUFU.RCP (1 ulp),
+// so that the MUFU unit (16 lanes/SM) does not bound the FP32 pipe (128 lanes/SM).  d^4 products stay far inside the
+// float range: the 2-point rule is only used for |d| < 200 alpha.
+__device__ __forceinline__ float rcpf(float x)
+{
+  float r;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+__device__ __forceinline__ void gh1_acc2f(float &a0, float &a1, float d0, float d1, float A1, float g2)
+{
+  const float D0 = fmaf(d0, d0, g2), D1 = fmaf(d1, d1, g2);
+  const float t = A1 * rcpf(D0 * D1);
+  a0 = fmaf(t, D1, a0);
+  a1 = fmaf(t, D0, a1);
+}
+__device__ __forceinline__ void gh2_acc2f(float &a0, float &a1, float d0, float d1, float A1, float e2, float f2, float A1a2)
+{
+  const float E0 = fmaf(d0, d0, e2), E1 = fmaf(d1, d1, e2);
+  const float D0 = fmaf(E0, E0, f2), D1 = fmaf(E1, E1, f2);
+  const float B0 = fmaf(A1, E0, A1a2), B1 = fmaf(A1, E1, A1a2);
+  const float r = rcpf(D0 * D1);
+  a0 = fmaf(B0 * D1, r, a0);
+  a1 = fmaf(B1 * D0, r, a1);
 }
 // per-line constants of one +-t pair of the 6-point rule: E = q + e, value = (cE * E + c0) / (E^2 + f)
 struct GhPair {

@@ -15,6 +15,7 @@ import oracle
 import paper_1503_03806_b200 as hk
 
 TOL = 3.0e-7
+TOL32 = 5.0e-5      # FP32 variant: every rule <= 4e-5 from exact K (hk_voigt.cuh), float rounding of the 1-/2-point rules
 
 
 def _dev(a):
@@ -22,9 +23,9 @@ def _dev(a):
     return torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64)).cuda()
 
 
-def _K(x, y):
+def _K(x, y, precision=hk.HK_FP64):
     import torch
-    out = hk.hk_voigt_K(_dev(x), _dev(y))
+    out = hk.hk_voigt_K(_dev(x), _dev(y), precision=precision)
     torch.cuda.synchronize()
     return out.cpu().numpy()
 
@@ -78,3 +79,28 @@ def test_tiny_damping_widens_the_series_region():
         k = _K(x, np.full_like(x, y))
         ref = oracle.faddeeva_re(x, np.full_like(x, y))
         assert np.abs(k / ref - 1.0).max() < TOL, y
+
+
+def test_fp32_variant_golden_table_and_switches(golden_dir):
+    d = np.genfromtxt(os.path.join(golden_dir, "faddeeva_golden.csv"), delimiter=",", comments="#", usecols=(1, 2, 3))
+    k = _K(d[:, 0], d[:, 1], hk.HK_FP32)
+    rel = np.abs(k / d[:, 2] - 1.0)
+    assert rel.max() < TOL32, (rel.max(), d[np.argmax(rel)])
+    assert rel.max() > 1e-6                                          # the relaxed ladder really is in use
+    th = np.concatenate([10 ** np.linspace(-9, -1, 60), np.linspace(0.1, np.pi / 2, 60)])
+    for R in (44.0, 64.0, 300.0, 4.0e4):
+        for s in (1 - 1e-9, 1 + 1e-9, 0.999, 1.001):
+            r = np.sqrt(R * s)
+            x, y = r * np.cos(th), r * np.sin(th)
+            assert np.abs(_K(x, y, hk.HK_FP32) / oracle.faddeeva_re(x, y) - 1.0).max() < TOL32, (R, s)
+    rng = np.random.default_rng(22)
+    n = 200_000
+    x = np.concatenate([10 ** rng.uniform(-3, 7.5, n // 2), rng.uniform(0, 60, n // 2)])
+    y = np.concatenate([10 ** rng.uniform(-8, 4, n // 2), 10 ** rng.uniform(-7, 1.3, n // 2)])
+    rel = np.abs(_K(x, y, hk.HK_FP32) / oracle.faddeeva_re(x, y) - 1.0)
+    i = np.argmax(rel)
+    assert rel.max() < TOL32, (rel.max(), x[i], y[i])
+    x = np.linspace(0.0, 12.0, 600)
+    for yy in (1e-9, 1e-12, 1e-15):                                  # tiny damping: the Gaussian term beyond the series
+        rel = np.abs(_K(x, np.full_like(x, yy), hk.HK_FP32) / oracle.faddeeva_re(x, np.full_like(x, yy)) - 1.0)
+        assert rel.max() < TOL32, yy
