@@ -156,3 +156,75 @@ def kdist(kappa, ppb: int, n_g: int):
     if rc != 0:
         raise ValueError(f"orc_kdist: error {rc}")
     return out
+
+
+# ---------------------------------------------------------------------------------------------------------
+# SURVEY.md §8(f) "next" rows: Chebyshev resampling (f1) and the transmission function (f2).  Plain numpy, FP64.
+# ---------------------------------------------------------------------------------------------------------
+KAPPA_FLOOR = 1.0e-300   # DESIGN.md reading C1: ln(kappa) is taken of max(kappa, 1e-300) (the paper is silent on kappa = 0)
+
+
+def cheb_design(ppb: int, n_c: int):
+    """A[k][n] = T_n(2 y_k - 1) at the cell centres y_k = (k + 1/2)/ppb (A7), by the recurrence
+    T_0 = 1, T_1 = t, T_{n+1} = 2 t T_n - T_{n-1}  ("exploit the recurrence relations")."""
+    t = 2.0 * ((np.arange(ppb) + 0.5) / ppb) - 1.0
+    A = np.empty((ppb, n_c))
+    A[:, 0] = 1.0
+    if n_c > 1:
+        A[:, 1] = t
+    for n in range(2, n_c):
+        A[:, n] = 2.0 * t * A[:, n - 1] - A[:, n - 2]
+    return A
+
+
+def kdist_cheb(kappa, ppb: int, n_c: int):
+    """C[n_bins, n_c]: least-squares fit of ln kappa(y) of every bin with n_c Chebyshev polynomials, solved through the
+    Q-R decomposition of the design matrix ("solving A C = D ... we implement Q-R decomposition")."""
+    kappa = _arr(kappa)
+    if kappa.size % ppb:
+        raise ValueError("n_points is not a multiple of ppb")
+    A = cheb_design(ppb, n_c)
+    Q, R = np.linalg.qr(A)                                    # library primitive (LAPACK Householder QR), thin form
+    out = np.empty((kappa.size // ppb, n_c))
+    for b in range(kappa.size // ppb):
+        s = np.sort(kappa[b * ppb:(b + 1) * ppb])             # kappa(y) of the bin (eqs. 14-15)
+        D = np.log(np.maximum(s, KAPPA_FLOOR))
+        out[b] = np.linalg.solve(R, Q.T @ D)                  # R C = Q^T D
+    return out
+
+
+def cheb_eval(C, y):
+    """kappa(y) = exp(sum_n C_n T_n(2y - 1)) for every bin (rows of C) at the abscissae y in [0,1]."""
+    C = np.atleast_2d(_arr(C))
+    y = _arr(y)
+    t = 2.0 * y - 1.0
+    T = np.empty((y.size, C.shape[1]))
+    T[:, 0] = 1.0
+    if C.shape[1] > 1:
+        T[:, 1] = t
+    for n in range(2, C.shape[1]):
+        T[:, n] = 2.0 * t * T[:, n - 1] - T[:, n - 2]
+    return np.exp(C @ T.T)
+
+
+def transmission_kdist(k_table, mcol):
+    """T[b][m] = int_0^1 exp(-kappa(y) m~) dy (eq. 5, second equality) by the Gauss-Legendre rule whose nodes
+    the k-table holds: sum_q w_q exp(-k[b][q] m~_m)."""
+    k_table = np.atleast_2d(_arr(k_table))
+    mcol = _arr(mcol)
+    _, w = gauss_legendre(k_table.shape[1])
+    return np.einsum("q,bqm->bm", w, np.exp(-k_table[:, :, None] * mcol[None, None, :]))
+
+
+def transmission_direct(kappa, ppb: int, mcol):
+    """T[b][m] = (1/Delta x) int exp(-kappa(x) m~) dx over the bin (eq. 5, first equality), on the grid: the mean of
+    exp(-kappa_j m~_m) over the bin's ppb points (each point stands for delta x)."""
+    kappa = _arr(kappa)
+    mcol = _arr(mcol)
+    if kappa.size % ppb:
+        raise ValueError("n_points is not a multiple of ppb")
+    kb = kappa.reshape(-1, ppb)
+    out = np.empty((kb.shape[0], mcol.size))
+    for b in range(kb.shape[0]):
+        out[b] = np.exp(-kb[b][:, None] * mcol[None, :]).mean(axis=0)
+    return out

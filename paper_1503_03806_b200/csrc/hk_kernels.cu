@@ -666,14 +666,22 @@ struct __align__(16) NearSmem {
   int counts[kNearWarps];
 };
 
-// rule per 32-point group for one listed line, accumulated in the warp's strip sk[32k + lane].  Warp-collective.
-__device__ __noinline__ void near_groups(const MetaA *pa, const MetaB *pm, const LineBase *pb, const LineGH2 *pg,
-                                         const LineCore *pk, int plo, int lane, double x0, double dnu, double En, double *sk)
+// distance (grid units, float) of the 32-point group [glo, glo+31] from a line centre; both halves of the near kernel's
+// work on a listed line (3-point rule in registers / inner rules below) split the groups by the SAME test dg >= r3
+__device__ __forceinline__ float group_dist(int glo, float c)
+{
+  return fmaxf(fmaxf((float)glo - c, c - (float)(glo + 31)), 0.0f);
+}
+
+// inner groups of one listed line (those closer to its centre than the 3-point radius): 6-point rule, series on the groups
+// that hold core points, Gaussian term of a tiny-y line; accumulated in the warp's strip sk[32k + lane].  Warp-collective.
+__device__ __noinline__ void near_inner(const MetaA *pa, const MetaB *pm, const LineBase *pb, const LineGH2 *pg,
+                                        const LineCore *pk, int plo, int lane, double x0, double dnu, double En, double *sk)
 {
   const MetaA ma = *pa;
   const MetaB mb = *pm;
   const LineBase b = *pb;
-  const LineGH2 g = *pg;
+  const double inv_alpha = pg->inv_alpha;
   const LineCore kc = *pk;
   const float dist = fmaxf(fmaxf((float)plo - ma.c, ma.c - (float)(plo + kPlanBlock - 1)), 0.0f);
   const double d0 = x0 - b.nu0;
@@ -685,27 +693,20 @@ __device__ __noinline__ void near_groups(const MetaA *pa, const MetaB *pm, const
   for (int k = 0; k < kNearP; ++k) {
     const int glo = plo + 32 * k, ghi = glo + 31;
     if (ghi < ma.jlo || glo > ma.jhi) continue;
+    const float dg = group_dist(glo, ma.c);
+    if (dg >= ma.r3) continue;  // taken by the 3-point rule in the caller
     const int j = glo + lane;
     const bool inwin = (j >= ma.jlo) && (j <= ma.jhi);
     const double d = fma((double)(32 * k), dnu, d0);
-    const float dg = fmaxf(fmaxf((float)glo - ma.c, ma.c - (float)ghi), 0.0f);
-    double v;
-    if (dg >= mb.r2) {
-      v = dg >= mb.r1 ? gh1_acc(0.0, d, b.A1, b.g2) : gh2_acc(0.0, d, b.A1, g.e2, g.f2, g.A1a2);
-    } else if (dg >= ma.r3) {
-      const double c3 = b.A1 * (1.0 / 3.0);
-      v = gh3_acc(0.0, d, b.g2, fma(-1.5, b.a2, b.g2), 6.0 * b.a2 * b.g2, 2.0 * c3, c3, b.A1 * b.a2);
-    } else {
-      v = gh6_val(d * d, G6);
-      if (dg < mb.r6) {  // the series region reaches into this group
-        const double x = fabs(d) * g.inv_alpha;
-        const double ks = core_K(fmin(x, 6.7), C);
-        if (x * x < xc2) v = kc.Acore * ks;
-        else if (mb.rg > 0.0f) v = fma(kc.Acore, exp(-x * x), v);
-      } else if (dg < mb.rg) {
-        const double x = d * g.inv_alpha;
-        v = fma(kc.Acore, exp(-x * x), v);
-      }
+    double v = gh6_val(d * d, G6);
+    if (dg < mb.r6) {  // the series region reaches into this group
+      const double x = fabs(d) * inv_alpha;
+      const double ks = core_K(fmin(x, 6.7), C);
+      if (x * x < xc2) v = kc.Acore * ks;
+      else if (mb.rg > 0.0f) v = fma(kc.Acore, exp(-x * x), v);
+    } else if (dg < mb.rg) {
+      const double x = d * inv_alpha;
+      v = fma(kc.Acore, exp(-x * x), v);
     }
     sk[32 * k + lane] += inwin ? v : 0.0;
   }
@@ -769,8 +770,8 @@ __global__ void __launch_bounds__(kNearWarps * 32, 4) voigt_near_kernel(const __
 #pragma unroll 1
       for (int e = warp; e < list_n; e += kNearWarps) {
         const MetaA ea = S.ma[e];
-        const float dist = fmaxf(fmaxf((float)plo - ea.c, ea.c - (float)phi), 0.0f);
-        if (dist >= ea.r3) {  // 3-point rule on the whole span
+        bool inner = false;  // some group lies inside the 3-point radius (warp-uniform)
+        {  // 3-point rule, unrolled over the 8 groups in registers, on every group at or beyond the 3-point radius
           const LineBase lb = S.base[e];
           const double d0 = x0 - lb.nu0;
           const double e3 = fma(-1.5, lb.a2, lb.g2), f3 = 6.0 * lb.a2 * lb.g2;
@@ -780,11 +781,13 @@ __global__ void __launch_bounds__(kNearWarps * 32, 4) voigt_near_kernel(const __
 #pragma unroll
           for (int k = 0; k < kNearP; ++k) {
             const double t = gh3_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), lb.g2, e3, f3, c0, c3, c3a);
-            acc[k] = ((unsigned)(jrel + 32 * k) <= wlen) ? t : acc[k];
+            const bool far3 = group_dist(plo + 32 * k, ea.c) >= ea.r3;
+            acc[k] = (far3 && (unsigned)(jrel + 32 * k) <= wlen) ? t : acc[k];
+            inner |= !far3;
           }
-        } else {
-          near_groups(S.ma + e, S.mb + e, S.base + e, S.gh2 + e, S.core + e, plo, lane, x0, a.dnu, En, sk);
         }
+        if (inner)
+          near_inner(S.ma + e, S.mb + e, S.base + e, S.gh2 + e, S.core + e, plo, lane, x0, a.dnu, En, sk);
       }
       list_n = 0;
       __syncthreads();  // the list is free again
