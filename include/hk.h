@@ -11,7 +11,8 @@
  *       parallel with kappa accumulated in registers;
  *   (2) the k-distribution of kappa in fixed-width bins: per-bin ascending sort, equal delta-y = 1/N_nu
  *       (eqs. 14-15), resampled at n_g Gauss-Legendre nodes on (0,1)
- *       (BASELINE.json north_star; the paper's Chebyshev fit, is not on this path).
+ *       (BASELINE.json north_star); the paper's own Chebyshev fit is hk_kdist_cheb, and the
+ *       transmission function of eq. 5 is hk_transmission / hk_transmission_direct.
  *
  * Conventions
  *   - Every pointer marked "device" is a CUDA device pointer (e.g. torch .data_ptr()); "host" is host memory.
@@ -126,6 +127,42 @@ int64_t hk_count_evals(const double *nu0_host, int64_t n_lines, double nu_min, i
  * HK_ERR_INVALID: NULL pointers, n_points < 1, dnu or bin_width not > 0, bin_width/dnu not an integer within 1e-9,
  * n_points not a multiple of ppb, n_g < 1 or > 128.   HK_ERR_UNSUPPORTED: ppb > 16384.   Asynchronous. */
 int hk_kdist(const double *kappa, int64_t n_points, double dnu, double bin_width, int n_g, double *k_out, void *stream);
+
+/* the paper's own resampling: per bin, least-squares fit of ln kappa(y) with n_c
+ * Chebyshev polynomials of t = 2y - 1 at the cell centres y_k = (k + 1/2)/ppb of the sorted bin,
+ *   minimise sum_k ( sum_n C_n T_n(2 y_k - 1) - ln max(s_k, 1e-300) )^2 ,
+ * "solving A C = D" by Q-R decomposition.  The design matrix A is the same for every bin, so it is factored once per
+ * (ppb, n_c) (Householder Q-R in long double on the host; P = R^-1 Q^T kept on the device for the life of the process;
+ * that first call synchronises), and each bin costs its sort plus the product C = P D in the sort kernel.  The paper is
+ * silent on kappa = 0: ln is taken of max(kappa, 1e-300).
+ * coef_out: device [n_bins*n_c], row-major by bin, overwritten.  k_out: device [n_bins*n_g] or NULL — when given, the
+ * Gauss-Legendre k-table of hk_kdist is written by the same launch (n_g is ignored when k_out is NULL).
+ * HK_ERR_INVALID: as hk_kdist, or NULL coef_out, n_c < 1, n_c > 64, n_c > ppb.  HK_ERR_UNSUPPORTED: ppb > 16384. */
+int hk_kdist_cheb(const double *kappa, int64_t n_points, double dnu, double bin_width, int n_c, double *coef_out, int n_g,
+                  double *k_out, void *stream);
+
+/* The projection matrix hk_kdist_cheb uses, P[n][k] (row-major, n_c x ppb) with C = P D: host arithmetic only (no GPU
+ * needed), for inspection and tests.  P_host_out: HOST [n_c*ppb].  HK_ERR_INVALID: NULL, n_c < 1 or > 64, ppb < n_c or
+ * > 16384. */
+int hk_cheb_projection(int ppb, int n_c, double *P_host_out);
+
+/* kappa_y_out[b][i] = exp( sum_n coef[b][n] T_n(2 y_i - 1) ): the resampled k-distribution function of every bin at the
+ * abscissae y (device [n_y], in [0,1]), by the Clenshaw recurrence.  coef: device [n_bins*n_c]; kappa_y_out: device
+ * [n_bins*n_y], overwritten.  HK_ERR_INVALID: NULL, n_bins < 1, n_c < 1 or > 64, n_y < 1.  Asynchronous. */
+int hk_cheb_eval(const double *coef, int64_t n_bins, int n_c, const double *y, int n_y, double *kappa_y_out, void *stream);
+
+/* transmission function of every bin for n_m column masses m~ [g cm^-2] (eq. 5, PAPER.md:74-80;
+ * "computing T for 1000 values of m~"):
+ *   hk_transmission         T[b][m] = int_0^1 exp(-kappa(y) m~) dy = sum_q w_q exp(-k_table[b][q] m~_m)   (Lebesgue side)
+ *                           with the n_g-point Gauss-Legendre weights whose nodes hk_kdist sampled;
+ *   hk_transmission_direct  T[b][m] = (1/Delta x) int exp(-kappa(x) m~) dx = mean over the bin's ppb grid points of
+ *                           exp(-kappa_j m~_m)                                                              (Riemann side).
+ * k_table: device [n_bins*n_g]; kappa: device [n_points], finite; mcol: device [n_m], >= 0; T_out: device [n_bins*n_m],
+ * row-major by bin, overwritten.  HK_ERR_INVALID: NULL, n_bins < 1, n_g < 1 or > 128, n_m < 1, or the bin arguments as
+ * in hk_kdist.  Asynchronous. */
+int hk_transmission(const double *k_table, int64_t n_bins, int n_g, const double *mcol, int n_m, double *T_out, void *stream);
+int hk_transmission_direct(const double *kappa, int64_t n_points, double dnu, double bin_width, const double *mcol, int n_m,
+                           double *T_out, void *stream);
 
 /* n_g Gauss-Legendre nodes g (ascending) and weights w on (0,1), sum w = 1.  HOST arrays of n_g doubles.
  * HK_ERR_INVALID for n_g < 1, n_g > 4096 or NULL. */

@@ -65,6 +65,16 @@ def load_library():
     L.hk_count_evals.argtypes = [_dp, _i64, C.c_double, _i64, C.c_double, C.c_double]
     L.hk_kdist.restype = C.c_int
     L.hk_kdist.argtypes = [C.c_void_p, _i64, C.c_double, C.c_double, C.c_int, C.c_void_p, C.c_void_p]
+    L.hk_kdist_cheb.restype = C.c_int
+    L.hk_kdist_cheb.argtypes = [C.c_void_p, _i64, C.c_double, C.c_double, C.c_int, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
+    L.hk_cheb_projection.restype = C.c_int
+    L.hk_cheb_projection.argtypes = [C.c_int, C.c_int, _dp]
+    L.hk_cheb_eval.restype = C.c_int
+    L.hk_cheb_eval.argtypes = [C.c_void_p, _i64, C.c_int, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
+    L.hk_transmission.restype = C.c_int
+    L.hk_transmission.argtypes = [C.c_void_p, _i64, C.c_int, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
+    L.hk_transmission_direct.restype = C.c_int
+    L.hk_transmission_direct.argtypes = [C.c_void_p, _i64, C.c_double, C.c_double, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
     L.hk_regime_census.restype = C.c_int
     L.hk_regime_census.argtypes = [_dp, _dp, _i64, C.c_double, C.c_double, C.c_double, C.c_double, _i64, C.c_double,
                                    C.c_double, C.c_int, C.POINTER(_i64)]
@@ -223,6 +233,62 @@ def hk_kdist(kappa, dnu, bin_width, n_g, out=None, stream=None):
         out = torch.empty((n // ppb, n_g), dtype=torch.float64, device=kappa.device)
     _check(L.hk_kdist(_dev_ptr(kappa, "kappa"), n, dnu, bin_width, int(n_g), _dev_ptr(out, "out"), _stream_ptr(stream)),
            "hk_kdist")
+    return out
+
+
+def hk_kdist_cheb(kappa, dnu, bin_width, n_c=20, n_g=None, stream=None):
+    """Chebyshev coefficients [n_bins, n_c] of ln kappa(y) per bin (hk_kdist_cheb); with n_g also the Gauss-Legendre k-table
+    [n_bins, n_g] from the same launch.  Returns coef, or (coef, k_table)."""
+    torch = _torch()
+    n = int(kappa.numel())
+    ppb = int(round(bin_width / dnu))
+    if ppb < 1 or n % ppb or n_c < 1:
+        raise HKError(-1, "hk_kdist_cheb")
+    coef = torch.empty((n // ppb, n_c), dtype=torch.float64, device=kappa.device)
+    ktab = None if n_g is None else torch.empty((n // ppb, n_g), dtype=torch.float64, device=kappa.device)
+    _check(load_library().hk_kdist_cheb(_dev_ptr(kappa, "kappa"), n, dnu, bin_width, int(n_c), _dev_ptr(coef, "coef"),
+                                        int(n_g or 0), _dev_ptr(ktab, "k_out", True), _stream_ptr(stream)), "hk_kdist_cheb")
+    return coef if ktab is None else (coef, ktab)
+
+
+def hk_cheb_projection(ppb: int, n_c: int):
+    """P[n_c, ppb] with C = P D, the host-side Q-R product hk_kdist_cheb uploads (host arithmetic, no GPU needed)."""
+    P = np.empty((int(n_c), int(ppb)))
+    _check(load_library().hk_cheb_projection(int(ppb), int(n_c), P.ctypes.data_as(_dp)), "hk_cheb_projection")
+    return P
+
+
+def hk_cheb_eval(coef, y, stream=None):
+    """kappa(y) [n_bins, n_y] reconstructed from Chebyshev coefficients [n_bins, n_c] (hk_cheb_eval)."""
+    torch = _torch()
+    n_bins, n_c = (int(v) for v in coef.shape)
+    out = torch.empty((n_bins, int(y.numel())), dtype=torch.float64, device=coef.device)
+    _check(load_library().hk_cheb_eval(_dev_ptr(coef, "coef"), n_bins, n_c, _dev_ptr(y, "y"), int(y.numel()),
+                                       _dev_ptr(out, "out"), _stream_ptr(stream)), "hk_cheb_eval")
+    return out
+
+
+def hk_transmission(k_table, mcol, stream=None):
+    """T[n_bins, n_m] = sum_q w_q exp(-k_table[b][q] m~) (hk_transmission; eq. 5 on the k-distribution side)."""
+    torch = _torch()
+    n_bins, n_g = (int(v) for v in k_table.shape)
+    out = torch.empty((n_bins, int(mcol.numel())), dtype=torch.float64, device=k_table.device)
+    _check(load_library().hk_transmission(_dev_ptr(k_table, "k_table"), n_bins, n_g, _dev_ptr(mcol, "mcol"), int(mcol.numel()),
+                                          _dev_ptr(out, "out"), _stream_ptr(stream)), "hk_transmission")
+    return out
+
+
+def hk_transmission_direct(kappa, dnu, bin_width, mcol, stream=None):
+    """T[n_bins, n_m] = mean over each bin's grid points of exp(-kappa_j m~) (hk_transmission_direct; eq. 5, Riemann side)."""
+    torch = _torch()
+    n = int(kappa.numel())
+    ppb = int(round(bin_width / dnu))
+    if ppb < 1 or n % ppb:
+        raise HKError(-1, "hk_transmission_direct")
+    out = torch.empty((n // ppb, int(mcol.numel())), dtype=torch.float64, device=kappa.device)
+    _check(load_library().hk_transmission_direct(_dev_ptr(kappa, "kappa"), n, dnu, bin_width, _dev_ptr(mcol, "mcol"),
+                                                 int(mcol.numel()), _dev_ptr(out, "out"), _stream_ptr(stream)),
+           "hk_transmission_direct")
     return out
 
 

@@ -7,7 +7,7 @@ import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = [os.path.join(HERE, "csrc", "hk_kernels.cu"), os.path.join(HERE, "csrc", "hk_sort.cu"),
-       os.path.join(HERE, "csrc", "hk_kdist.cu")]
+       os.path.join(HERE, "csrc", "hk_kdist.cu"), os.path.join(HERE, "csrc", "hk_resample.cu")]
 DEPS = SRC + [os.path.join(HERE, "csrc", "hk_voigt.cuh"), os.path.join(HERE, "csrc", "hk_internal.h"),
               os.path.join(HERE, "..", "include", "hk.h")]
 LIB = os.path.join(HERE, "libhk.so")

@@ -18,4 +18,8 @@ void pool_free(void *p, cudaStream_t st);
 // hk_sort.cu
 int sort_lines_copy(const hk_lines *in, int64_t n, cudaStream_t st, hk_lines *out, void **buf);
 
+// hk_resample.cu: device copy of the projection matrix P[n_c][ppb] of the Chebyshev least-squares fit on the current device
+// (factored on the host and uploaded on first use — synchronous — then cached for the life of the process)
+int cheb_projection_device(int ppb, int n_c, const double **P_out);
+
 }  // namespace hk

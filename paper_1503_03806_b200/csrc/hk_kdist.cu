@@ -25,6 +25,9 @@ struct KdistArgs {
   int ppb;   // points per bin
   int n;     // padded size, T*E
   int n_g;
+  const double *cheb_P;  // f1 (hk_kdist_cheb): projection matrix [n_c][ppb] of the Chebyshev least-squares fit, or NULL
+  double *cheb_out;      // [n_bins][n_c]
+  int n_c;
   double g[128];
 };
 
@@ -162,7 +165,7 @@ __global__ void __launch_bounds__(MAXT) kdist_kernel(const __grid_constant__ Kdi
 #pragma unroll
   for (int r = 0; r < E; r += 2) *reinterpret_cast<double2 *>(&s[pad<E>(i0 + r)]) = make_double2(v[r], v[r + 1]);
   __syncthreads();
-  for (int q = t; q < a.n_g; q += T) {
+  for (int q = t; a.k_out && q < a.n_g; q += T) {
     const double p = __dadd_rn(__dmul_rn(a.g[q], (double)a.ppb), -0.5);
     double val;
     if (p <= 0.0) val = s[pad<E>(0)];
@@ -174,6 +177,32 @@ __global__ void __launch_bounds__(MAXT) kdist_kernel(const __grid_constant__ Kdi
       val = s0 + f * (s1 - s0);
     }
     a.k_out[(int64_t)bin * a.n_g + q] = val;
+  }
+  // ---- f1: Chebyshev coefficients of ln kappa(y), C = P D with D_k = ln max(s_k, 1e-300) (the Q-R
+  // factorisation behind P is done once on the host, hk_resample.cu).  Thread t holds s_k for k = tE .. tE+E-1 in registers;
+  // per coefficient: E products per thread, a butterfly over the warp, then the warps' partial sums in a fixed order.
+  if (a.cheb_P) {
+    double d[E];
+#pragma unroll
+    for (int r = 0; r < E; ++r) d[r] = (i0 + r < a.ppb) ? log(fmax(v[r], 1.0e-300)) : 0.0;
+    __syncthreads();  // the resampling above is done with s
+    const int nw = (T + 31) >> 5, warp = t >> 5, lane = t & 31;
+    for (int n = 0; n < a.n_c; ++n) {
+      const double *Pn = a.cheb_P + (int64_t)n * a.ppb;
+      double acc = 0.0;
+#pragma unroll
+      for (int r = 0; r < E; ++r)
+        if (i0 + r < a.ppb) acc = fma(Pn[i0 + r], d[r], acc);
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(kFullMask, acc, o);
+      if (lane == 0) s[warp * a.n_c + n] = acc;
+    }
+    __syncthreads();
+    for (int n = t; n < a.n_c; n += T) {
+      double c = 0.0;
+      for (int w = 0; w < nw; ++w) c += s[w * a.n_c + n];
+      a.cheb_out[(int64_t)bin * a.n_c + n] = c;
+    }
   }
 }
 
@@ -198,11 +227,11 @@ static int launch_kdist(const KdistArgs &a, int64_t n_bins, cudaStream_t st)
 
 using namespace hk;
 
-extern "C" int hk_kdist(const double *kappa, int64_t n_points, double dnu, double bin_width, int n_g, double *k_out,
-                        void *stream)
+static int kdist_common(const double *kappa, int64_t n_points, double dnu, double bin_width, int n_g, double *k_out, int n_c,
+                        double *coef_out, void *stream)
 {
-  if (!kappa || !k_out || n_points < 1 || !(dnu > 0.0) || !isfinite(dnu) || !(bin_width > 0.0) || !isfinite(bin_width) ||
-      n_g < 1 || n_g > 128)
+  if (!kappa || (!k_out && !coef_out) || n_points < 1 || !(dnu > 0.0) || !isfinite(dnu) || !(bin_width > 0.0) || !isfinite(bin_width) ||
+      (k_out && (n_g < 1 || n_g > 128)) || (coef_out && (n_c < 1 || n_c > 64)))
     return HK_ERR_INVALID;
   const double ratio = bin_width / dnu;
   const double ppb_d = nearbyint(ratio);
@@ -212,20 +241,42 @@ extern "C" int hk_kdist(const double *kappa, int64_t n_points, double dnu, doubl
   if (n_points % ppb != 0) return HK_ERR_INVALID;
   const int64_t n_bins = n_points / ppb;
   if (n_bins > 2147483647LL) return HK_ERR_UNSUPPORTED;
+  if (coef_out && n_c > ppb) return HK_ERR_INVALID;  // more coefficients than points: the fit is not determined
   KdistArgs a;
   a.kappa = kappa;
   a.k_out = k_out;
   a.ppb = ppb;
-  a.n_g = n_g;
+  a.n_g = k_out ? n_g : 0;
+  a.cheb_P = nullptr;
+  a.cheb_out = coef_out;
+  a.n_c = coef_out ? n_c : 0;
+  if (coef_out) {
+    int rcp = cheb_projection_device(ppb, n_c, &a.cheb_P);
+    if (rcp != HK_OK) return rcp;
+  }
   int n = 64;
   while (n < ppb) n <<= 1;
   a.n = n;
   double wts[128];
-  int rc = hk_gauss_legendre(n_g, a.g, wts);
+  int rc = k_out ? hk_gauss_legendre(n_g, a.g, wts) : HK_OK;
   if (rc != HK_OK) return rc;
   cudaStream_t st = (cudaStream_t)stream;
   if (n <= 256) return launch_kdist<2, 128>(a, n_bins, st);   // T = 32 .. 128
   if (n == 512) return launch_kdist<4, 128>(a, n_bins, st);   // T = 128
   if (n == 1024) return launch_kdist<8, 128>(a, n_bins, st);  // T = 128
   return launch_kdist<16, 1024>(a, n_bins, st);                // T = 128 .. 1024
+}
+
+extern "C" int hk_kdist(const double *kappa, int64_t n_points, double dnu, double bin_width, int n_g, double *k_out,
+                        void *stream)
+{
+  if (!k_out) return HK_ERR_INVALID;
+  return kdist_common(kappa, n_points, dnu, bin_width, n_g, k_out, 0, nullptr, stream);
+}
+
+extern "C" int hk_kdist_cheb(const double *kappa, int64_t n_points, double dnu, double bin_width, int n_c, double *coef_out,
+                             int n_g, double *k_out, void *stream)
+{
+  if (!coef_out) return HK_ERR_INVALID;
+  return kdist_common(kappa, n_points, dnu, bin_width, n_g, k_out, n_c, coef_out, stream);
 }

@@ -81,3 +81,22 @@ def test_compute_call_without_gpu_fails_loudly():
         hk.hk_fp64_peak()
     with pytest.raises(RuntimeError):
         hk.Lines.from_numpy([1.0], [1.0], [0.05])
+
+
+@pytest.mark.parametrize("ppb,n_c", [(1000, 20), (10000, 20), (37, 5), (64, 8), (20, 20)])
+def test_cheb_projection_host_against_the_oracle(ppb, n_c):
+    # host logic of hk_kdist_cheb (Householder Q-R in long double): C = P D must be the least-squares solution
+    import oracle
+    from paper_1503_03806_b200.build import build_library
+    build_library()
+    P = hk.hk_cheb_projection(ppb, n_c)
+    assert P.shape == (n_c, ppb)
+    A = oracle.cheb_design(ppb, n_c)
+    tol = 1e-9 if n_c < ppb else 1e-4         # as many polynomials as equispaced points: interpolation, cond(A) ~ 1e9
+    assert np.abs(P @ A - np.eye(n_c)).max() < tol                                   # left inverse of the design matrix
+    rng = np.random.default_rng(ppb)
+    kappa = np.sort(10 ** rng.uniform(-8, 4, ppb))
+    C = oracle.kdist_cheb(kappa, ppb, n_c)[0]
+    assert np.abs(P @ np.log(kappa) - C).max() < tol * max(1.0, np.abs(C).max())
+    with pytest.raises(hk.HKError):
+        hk.hk_cheb_projection(10, 20)
