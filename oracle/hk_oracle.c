@@ -267,14 +267,23 @@ double orc_voigt_V(double dv, double alpha, double gamma)
 }
 
 /* kappa_out[k] = kappa(nu_{js[k]}) for an arbitrary list of grid indices.  Lines may come in any order. */
-int orc_opacity_points(const double *nu0, const double *S, const double *gamma0, const double *n_T, const double *E_low,
-                       int64_t n_lines, double T, double P_atm, double nu_min, int64_t N, double dnu, double cutoff,
-                       double mass_amu, double q_ratio, const int64_t *js, int64_t n_js, double *kappa_out)
+/* Full line physics: eq. 20 with the natural width A21/(4 pi c), air and self
+ * broadening, P_self = self_fraction * P ("in equal proportions (P_self = 0.5 P)"), P0 = 1 atm:
+ *     gamma = A21/(4 pi c) + (T/T0)^(-n) [ gamma_air (P - P_self)/P0 + gamma_self P_self/P0 ]
+ * and eq. 21: nu0 -> nu0 + delta P/P0, the shifted centre replacing nu0 everywhere after it (profile
+ * centre, Doppler width, window, eq. 18: DESIGN.md reading C2).  NULL gamma_self: no self term (P_self = 0); NULL A21:
+ * no natural width; NULL delta: no shift.  abundance X multiplies the species' opacity (kappa = sum_s X_s kappa_s,
+ * PAPER.md:133-135). */
+int orc_opacity_points_full(const double *nu0_in, const double *S, const double *gamma0, const double *gamma_self,
+                            const double *A21, const double *delta, const double *n_T, const double *E_low,
+                            int64_t n_lines, double T, double P_atm, double self_fraction, double abundance, double nu_min,
+                            int64_t N, double dnu, double cutoff, double mass_amu, double q_ratio, const int64_t *js,
+                            int64_t n_js, double *kappa_out)
 {
     if (n_lines < 0 || !(T > 0.0) || !(P_atm > 0.0) || !(dnu > 0.0) || !(cutoff > 0.0) || N <= 0 || !(mass_amu > 0.0) ||
         n_js < 0 || (n_js > 0 && (!js || !kappa_out)))
         return ORC_ERR_INVALID;
-    if (n_lines > 0 && (!nu0 || !S || !gamma0)) return ORC_ERR_INVALID;
+    if (n_lines > 0 && (!nu0_in || !S || !gamma0)) return ORC_ERR_INVALID;
     for (int64_t k = 0; k < n_js; k++)
         if (js[k] < 0 || js[k] >= N) return ORC_ERR_INVALID;
     double m_g = mass_amu * ORC_AMU;
@@ -284,12 +293,16 @@ int orc_opacity_points(const double *nu0, const double *S, const double *gamma0,
 #pragma omp parallel for schedule(static)
     for (int64_t i = 0; i < n_lines; i++) {
         double nT = n_T ? n_T[i] : 0.5;
-        L[i].nu0 = nu0[i];
-        L[i].alpha = nu0[i] * vth;
-        L[i].gamma = gamma0[i] * P_atm * pow(ORC_T0 / T, nT);
-        double s = E_low ? orc_line_strength(S[i], nu0[i], E_low[i], T, q_ratio) : S[i];
-        L[i].amp = s / m_g;
-        orc_window(nu0[i], nu_min, N, dnu, cutoff, &L[i].jlo, &L[i].jhi);
+        double nu0 = delta ? nu0_in[i] + delta[i] * P_atm : nu0_in[i];                    /* eq. 21, P0 = 1 atm */
+        double P_self = gamma_self ? self_fraction * P_atm : 0.0;
+        double press = gamma0[i] * (P_atm - P_self) + (gamma_self ? gamma_self[i] * P_self : 0.0);
+        L[i].nu0 = nu0;
+        L[i].alpha = nu0 * vth;
+        L[i].gamma = pow(ORC_T0 / T, nT) * press;                                          /* eq. 20, pressure terms */
+        if (A21) L[i].gamma += A21[i] / (4.0 * 3.14159265358979323846 * ORC_C_LIGHT);     /* natural width */
+        double s = E_low ? orc_line_strength(S[i], nu0, E_low[i], T, q_ratio) : S[i];
+        L[i].amp = abundance * s / m_g;
+        orc_window(nu0, nu_min, N, dnu, cutoff, &L[i].jlo, &L[i].jhi);
         L[i].src = i;
     }
     int sorted = 1;
@@ -316,6 +329,14 @@ int orc_opacity_points(const double *nu0, const double *S, const double *gamma0,
     }
     free(L);
     return ORC_OK;
+}
+
+int orc_opacity_points(const double *nu0, const double *S, const double *gamma0, const double *n_T, const double *E_low,
+                       int64_t n_lines, double T, double P_atm, double nu_min, int64_t N, double dnu, double cutoff,
+                       double mass_amu, double q_ratio, const int64_t *js, int64_t n_js, double *kappa_out)
+{
+    return orc_opacity_points_full(nu0, S, gamma0, NULL, NULL, NULL, n_T, E_low, n_lines, T, P_atm, 0.0, 1.0, nu_min, N, dnu,
+                                   cutoff, mass_amu, q_ratio, js, n_js, kappa_out);
 }
 
 /* kappa_out[j - j_begin] for j in [j_begin, j_end). */

@@ -98,3 +98,66 @@ def test_transmission_invariants_and_lebesgue_equals_riemann():
     # numpy brute force of the definition
     ref = np.array([[np.mean(np.exp(-kap[b * ppb:(b + 1) * ppb] * mm)) for mm in m] for b in range(2)])
     assert np.abs(Td / ref - 1.0).max() < 1e-13
+
+
+# ---- f3: full line physics (eqs. 20-21) and species mixing -------------------------
+def _draw(n=60, seed=4):
+    rng = np.random.default_rng(seed)
+    nu0 = np.sort(rng.uniform(5.0, 95.0, n))
+    return (nu0, 10 ** rng.uniform(-22, -19, n), rng.uniform(0.02, 0.1, n), rng.uniform(0.1, 0.5, n),
+            10 ** rng.uniform(-2, 2, n), rng.uniform(-0.02, 0.02, n), rng.uniform(0.3, 0.8, n))
+
+
+GRID = (0.0, 100.0, 0.01, 25.0)
+
+
+def test_full_physics_reduces_to_the_simple_law():
+    nu0, S, ga, gs, A, dl, nT = _draw()
+    base = oracle.opacity(nu0, S, ga, 900.0, 2.0, *GRID, n_T=nT)
+    assert np.array_equal(oracle.opacity_full(nu0, S, ga, 900.0, 2.0, *GRID, n_T=nT), base)
+    # gamma_self == gamma_air: the self fraction drops out of eq. 20
+    for f in (0.0, 0.5, 1.0):
+        k = oracle.opacity_full(nu0, S, ga, 900.0, 2.0, *GRID, n_T=nT, gamma_self=ga, self_fraction=f)
+        assert np.abs(k / base - 1.0).max() < 1e-13
+    # self_fraction = 0: air only; = 1: the simple law with gamma_self in place of gamma_air
+    k0 = oracle.opacity_full(nu0, S, ga, 900.0, 2.0, *GRID, n_T=nT, gamma_self=gs, self_fraction=0.0)
+    assert np.abs(k0 / base - 1.0).max() < 1e-13
+    k1 = oracle.opacity_full(nu0, S, ga, 900.0, 2.0, *GRID, n_T=nT, gamma_self=gs, self_fraction=1.0)
+    assert np.abs(k1 / oracle.opacity(nu0, S, gs, 900.0, 2.0, *GRID, n_T=nT) - 1.0).max() < 1e-13
+    # equal proportions: the pressure term is the mean of the two coefficients
+    kh = oracle.opacity_full(nu0, S, ga, 900.0, 2.0, *GRID, n_T=nT, gamma_self=gs, self_fraction=0.5)
+    assert np.abs(kh / oracle.opacity(nu0, S, 0.5 * (ga + gs), 900.0, 2.0, *GRID, n_T=nT) - 1.0).max() < 1e-12
+
+
+def test_natural_width_adds_to_the_lorentz_width():
+    # a line at nu0 -> 0 is a pure Lorentzian (alpha = 0): peak = amp/(pi gamma), so gamma is read off the peak
+    c, amu = 2.99792458e10, 1.66053906660e-24
+    S, ga, A, T, P = 1e-20, 0.05, 3.0e9, 296.0, 1e-3
+    k = oracle.opacity_full([0.0], [S], [ga], T, P, 0.0, 10.0, 0.01, 25.0, A21=[A])
+    gamma = ga * P + A / (4 * np.pi * c)
+    assert abs(k[0] / (S / (18.0 * amu) / (np.pi * gamma)) - 1.0) < 1e-13
+    assert A / (4 * np.pi * c) > 0.1 * ga * P                                    # the natural width matters in this case
+    j = 137
+    lor = S / (18.0 * amu) * gamma / (np.pi * ((j * 0.01) ** 2 + gamma ** 2))
+    assert abs(k[j] / lor - 1.0) < 1e-13
+
+
+def test_pressure_shift_is_a_translation_of_the_centre():
+    nu0, S, ga, gs, A, dl, nT = _draw()
+    P = 7.0
+    k = oracle.opacity_full(nu0, S, ga, 1200.0, P, *GRID, delta=dl)
+    ref = oracle.opacity(nu0 + dl * P, S, ga, 1200.0, P, *GRID)                  # the shifted list is no longer ordered
+    assert np.any(np.diff(nu0 + dl * P) < 0)
+    assert np.abs(k / ref - 1.0).max() < 1e-13
+    one = oracle.opacity_full([50.0], [1e-20], [0.05], 300.0, 10.0, *GRID, delta=[-0.031])
+    assert np.argmax(one) == 5000 - 31
+
+
+def test_abundance_weight_and_mixing_is_linear():
+    nu0, S, ga, gs, A, dl, nT = _draw()
+    kw = dict(gamma_self=gs, A21=A, delta=dl, n_T=nT)
+    k1 = oracle.opacity_full(nu0, S, ga, 800.0, 0.5, *GRID, **kw)
+    kx = oracle.opacity_full(nu0, S, ga, 800.0, 0.5, *GRID, abundance=0.25, **kw)
+    assert np.abs(kx / (0.25 * k1) - 1.0).max() < 1e-14
+    js = np.array([0, 17, 5000, 9999])
+    assert np.array_equal(oracle.opacity_full(nu0, S, ga, 800.0, 0.5, *GRID, js=js, **kw), k1[js])
