@@ -57,6 +57,10 @@ typedef struct {
   const double *gamma0; /* Lorentz HWHM at 296 K and 1 atm, cm^-1/atm                                */
   const double *n_T;    /* temperature exponent n_coll of eq. 20, or NULL for 0.5 on every line      */
   const double *E_low;  /* lower-state energy, cm^-1, or NULL: no S(T) scaling (eq. 18 not applied)  */
+  /* full line physics of eqs. 20-21; each may be NULL (term absent): */
+  const double *gamma_self; /* self-broadening HWHM alpha_self at 296 K, 1 atm, cm^-1/atm (gamma0 is then alpha_air) */
+  const double *A21;        /* Einstein A coefficient, s^-1: natural width A21/(4 pi c)                      */
+  const double *delta;      /* pressure-induced shift delta_shift, cm^-1/atm (eq. 21)                        */
 } hk_lines;
 
 typedef struct {
@@ -67,6 +71,12 @@ typedef struct {
                            hk_lines_check_sorted()).  0: the library checks on the device (synchronises the
                            stream) and, if needed, works on a copy ordered by nu0; inputs are never modified */
   void *stream;         /* cudaStream_t, or NULL                                                      */
+  double self_fraction; /* P_self/P of eq. 20 (the paper takes 0.5), in [0,1]; used only when
+                           gamma_self != NULL                                                         */
+  double abundance;     /* X_s: the species' opacity is multiplied by it (kappa = sum_s X_s kappa_s);
+                           0 means 1, so that a zero-initialised tail keeps the one-species behaviour          */
+  int accumulate;       /* 0: kappa_out is overwritten.  1: X_s kappa_s is ADDED to kappa_out — the species are summed
+                           BEFORE the sort, as PAPER.md:135 requires; the first species of a mixture passes 0     */
 } hk_params;
 
 /* N = llround((nu_max - nu_min)/dnu): number of grid points nu_j = nu_min + j*dnu, j < N. Host only. */
@@ -86,6 +96,16 @@ int64_t hk_grid_size(double nu_min, double nu_max, double dnu);
  * K = Re w(x+iy) is evaluated to <= 2.5e-7 relative error: Algorithm-916-type series for x^2+y^2 < 44,
  * 6/3/2/1-point Gauss-Hermite rules beyond 44 / 280 / 3200 / 6e6.
  *
+ * Full line physics, active per optional array of hk_lines:
+ *   gamma_i = A21_i/(4 pi c) + (296/T)^n_i [ gamma0_i (P - P_self) + gamma_self_i P_self ],  P_self = self_fraction * P   eq. 20
+ *   nu0_i  -> nu0_i + delta_i * P_atm                                                                                    eq. 21
+ * (P0 = 1 atm).  The shifted centre replaces nu0 everywhere downstream (profile centre, Doppler width, window, eq. 18).
+ * Shifted centres are in general no longer ascending: with delta != NULL the library shifts a copy, checks it on the
+ * device (synchronises the stream) and orders it when needed, whatever lines_sorted says.
+ * Mixtures: call once per species with prm->abundance = X_s and prm->accumulate = 1 from the second species on; the
+ * k-distribution of the sum is then taken by hk_kdist (adding k-distributions instead would be the correlated-k
+ * approximation).
+ *
  * prm->precision = HK_FP32 (north_star's optional FP32 variant, max relative error <= 1e-4): the same ladder with the
  * switches at 44 / 64 / 300 / 4e4 (each rule <= 4e-5 from exact K); the 1- and 2-point rules — every (line, 256-point
  * span) pair beyond the 2-point radius, ~99 % of all evaluations — run in FP32 (distances from an integer + fraction
@@ -96,7 +116,8 @@ int64_t hk_grid_size(double nu_min, double nu_max, double dnu);
  * kappa_out: device, N doubles, overwritten.  Lines outside [nu_min, nu_max) still contribute if within the
  * cutoff.  n_lines == 0 gives kappa == 0.
  * HK_ERR_INVALID: NULL lines/prm/kappa_out or (n_lines > 0 and NULL nu0/S/gamma0); n_lines < 0; T, P_atm, dnu,
- * cutoff, mass_amu not > 0 or not finite; N < 1 or N > 2^30; precision unknown.
+ * cutoff, mass_amu not > 0 or not finite; N < 1 or N > 2^30; precision unknown; abundance < 0 or not finite;
+ * self_fraction outside [0,1] when gamma_self != NULL.
  * Asynchronous on prm->stream (synchronises once when lines_sorted = 0).  nu0 must be ascending when
  * lines_sorted = 1 (see hk_lines_check_sorted). */
 int hk_opacity(const hk_lines *lines, int64_t n_lines, double T, double P_atm, double nu_min, double nu_max,
@@ -107,7 +128,8 @@ int hk_opacity(const hk_lines *lines, int64_t n_lines, double T, double P_atm, d
  * k-table device -> host, and waits for the stream.  Every array of lines_host is a HOST pointer (pinned memory makes
  * the copies asynchronous to the host but is not required); kappa_host_out: host [N] or NULL; k_host_out: host
  * [n_bins*n_g] or NULL (then bin_width and n_g are ignored); at least one output is required.  Device memory comes from
- * the library's pool.  Errors as hk_opacity / hk_kdist.  Synchronous. */
+ * the library's pool.  With prm->accumulate = 1 kappa_host_out is also an INPUT (the running sum of the mixture, copied
+ * host -> device first) and must not be NULL.  Errors as hk_opacity / hk_kdist.  Synchronous. */
 int hk_opacity_host(const hk_lines *lines_host, int64_t n_lines, double T, double P_atm, double nu_min, double nu_max,
                     double dnu, double cutoff, double *kappa_host_out, double bin_width, int n_g, double *k_host_out,
                     const hk_params *prm);
@@ -176,7 +198,9 @@ int hk_voigt_K(const double *x, const double *y, int64_t n, double *out, int pre
 /* Persistent-context form for T-P sweeps ("repeat this calculation for multiple combinations of
  * temperature and pressure"): the line list is bound once, scratch is kept between calls.
  * hk_create copies nothing when nu0 is ascending: the hk_lines device arrays must outlive the context; with
- * lines_sorted = 0 and an unordered list the context owns an ordered copy (made once). */
+ * lines_sorted = 0 and an unordered list the context owns an ordered copy (made once).  A list with a pressure shift
+ * (delta != NULL) would have to be re-ordered at every pressure: hk_create returns HK_ERR_UNSUPPORTED for it (use
+ * hk_opacity).  self_fraction, abundance and accumulate are taken from prm at hk_create. */
 typedef struct hk_ctx hk_ctx;
 int hk_create(const hk_lines *lines, int64_t n_lines, const hk_params *prm, hk_ctx **out);
 int hk_opacity_ctx(hk_ctx *ctx, double T, double P_atm, double q_ratio, double nu_min, double nu_max, double dnu,

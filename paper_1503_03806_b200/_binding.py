@@ -24,12 +24,18 @@ class HKError(RuntimeError):
 
 
 class _hk_lines(C.Structure):
-    _fields_ = [("nu0", C.c_void_p), ("S", C.c_void_p), ("gamma0", C.c_void_p), ("n_T", C.c_void_p), ("E_low", C.c_void_p)]
+    _fields_ = [("nu0", C.c_void_p), ("S", C.c_void_p), ("gamma0", C.c_void_p), ("n_T", C.c_void_p), ("E_low", C.c_void_p),
+                ("gamma_self", C.c_void_p), ("A21", C.c_void_p), ("delta", C.c_void_p)]
 
 
 class _hk_params(C.Structure):
     _fields_ = [("mass_amu", C.c_double), ("q_ratio", C.c_double), ("precision", C.c_int), ("lines_sorted", C.c_int),
-                ("stream", C.c_void_p)]
+                ("stream", C.c_void_p), ("self_fraction", C.c_double), ("abundance", C.c_double), ("accumulate", C.c_int)]
+
+
+def _params(mass_amu, q_ratio, precision, lines_sorted, stream, self_fraction=0.5, abundance=1.0, accumulate=False):
+    return _hk_params(float(mass_amu), float(q_ratio), int(precision), int(bool(lines_sorted)), _stream_ptr(stream),
+                      float(self_fraction), float(abundance), int(bool(accumulate)))
 
 
 _lib = None
@@ -153,12 +159,15 @@ class Lines:
     gamma0: object
     n_T: object = None
     E_low: object = None
+    gamma_self: object = None      # eq. 20: self broadening (gamma0 is then the air-broadening coefficient)
+    A21: object = None             # eq. 20: Einstein A (natural width)
+    delta: object = None           # eq. 21: pressure shift
 
     @staticmethod
-    def from_numpy(nu0, S, gamma0, n_T=None, E_low=None, device="cuda"):
+    def from_numpy(nu0, S, gamma0, n_T=None, E_low=None, gamma_self=None, A21=None, delta=None, device="cuda"):
         torch = _torch()
         f = lambda a: None if a is None else torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64)).to(device)
-        return Lines(f(nu0), f(S), f(gamma0), f(n_T), f(E_low))
+        return Lines(f(nu0), f(S), f(gamma0), f(n_T), f(E_low), f(gamma_self), f(A21), f(delta))
 
     @property
     def n(self) -> int:
@@ -166,12 +175,14 @@ class Lines:
 
     def _c(self):
         n = self.n
-        for name in ("S", "gamma0", "n_T", "E_low"):
+        for name in ("S", "gamma0", "n_T", "E_low", "gamma_self", "A21", "delta"):
             t = getattr(self, name)
             if t is not None and int(t.numel()) != n:
                 raise ValueError(f"{name} has {int(t.numel())} entries, nu0 has {n}")
         return _hk_lines(_dev_ptr(self.nu0, "nu0"), _dev_ptr(self.S, "S"), _dev_ptr(self.gamma0, "gamma0"),
-                         _dev_ptr(self.n_T, "n_T", True), _dev_ptr(self.E_low, "E_low", True))
+                         _dev_ptr(self.n_T, "n_T", True), _dev_ptr(self.E_low, "E_low", True),
+                         _dev_ptr(self.gamma_self, "gamma_self", True), _dev_ptr(self.A21, "A21", True),
+                         _dev_ptr(self.delta, "delta", True))
 
 
 def hk_grid_size(nu_min: float, nu_max: float, dnu: float) -> int:
@@ -203,19 +214,20 @@ def hk_gauss_legendre(n_g: int):
 
 
 def hk_opacity(lines: Lines, T, P_atm, nu_min, nu_max, dnu, cutoff, mass_amu=18.0, q_ratio=1.0, lines_sorted=True,
-               out=None, stream=None, precision=HK_FP64):
-    """kappa[N] on the device (hk_opacity of include/hk.h).  Asynchronous on the current (or given) torch stream."""
+               out=None, stream=None, precision=HK_FP64, self_fraction=0.5, abundance=1.0, accumulate=False):
+    """kappa[N] on the device (hk_opacity of include/hk.h).  Asynchronous on the current (or given) torch stream.
+    accumulate=True adds abundance * kappa of this species to `out` (mixtures)."""
     torch = _torch()
     L = load_library()
     N = hk_grid_size(nu_min, nu_max, dnu)
     if out is None:
-        if N < 1:
+        if N < 1 or accumulate:
             raise HKError(-1, "hk_opacity")
         out = torch.empty(N, dtype=torch.float64, device=lines.nu0.device)
     elif N >= 1 and int(out.numel()) != N:       # (N < 1: let the library report HK_ERR_INVALID)
         raise ValueError(f"out has {int(out.numel())} entries, the grid has {N}")
     cl = lines._c()
-    prm = _hk_params(float(mass_amu), float(q_ratio), int(precision), int(bool(lines_sorted)), _stream_ptr(stream))
+    prm = _params(mass_amu, q_ratio, precision, lines_sorted, stream, self_fraction, abundance, accumulate)
     _check(L.hk_opacity(C.byref(cl), lines.n, T, P_atm, nu_min, nu_max, dnu, cutoff, _dev_ptr(out, "out"), C.byref(prm)),
            "hk_opacity")
     return out
@@ -337,11 +349,12 @@ def hk_last_stage_ms():
 class Context:
     """hk_create / hk_opacity_ctx / hk_destroy: line list bound once, scratch kept across (T,P) calls."""
 
-    def __init__(self, lines: Lines, mass_amu=18.0, lines_sorted=True, stream=None, precision=HK_FP64):
+    def __init__(self, lines: Lines, mass_amu=18.0, lines_sorted=True, stream=None, precision=HK_FP64, self_fraction=0.5,
+                 abundance=1.0, accumulate=False):
         self._lines = lines      # keep the tensors alive
         self._h = C.c_void_p()
         cl = lines._c()
-        prm = _hk_params(float(mass_amu), 1.0, int(precision), int(bool(lines_sorted)), _stream_ptr(stream))
+        prm = _params(mass_amu, 1.0, precision, lines_sorted, stream, self_fraction, abundance, accumulate)
         _check(load_library().hk_create(C.byref(cl), lines.n, C.byref(prm), C.byref(self._h)), "hk_create")
 
     def opacity(self, T, P_atm, nu_min, nu_max, dnu, cutoff, q_ratio=1.0, out=None):
@@ -382,7 +395,8 @@ def _host_ptr(t, name, allow_none=False):
 
 def hk_opacity_host(nu0, S, gamma0, T, P_atm, nu_min, nu_max, dnu, cutoff, mass_amu=18.0, n_T=None, E_low=None, q_ratio=1.0,
                     lines_sorted=True, bin_width=None, n_g=20, kappa_out=None, k_out=None, want_kappa=True, stream=None,
-                    precision=HK_FP64):
+                    precision=HK_FP64, gamma_self=None, A21=None, delta=None, self_fraction=0.5, abundance=1.0,
+                    accumulate=False):
     """End-to-end call with HOST buffers (hk_opacity_host of include/hk.h): host line arrays -> device, hk_opacity
     (+ hk_kdist when bin_width is given), kappa / k-table -> host.  Buffers are host torch tensors (pinned for
     asynchronous copies) or numpy arrays.  Returns (kappa_host or None, k_host or None).  Synchronous."""
@@ -390,7 +404,8 @@ def hk_opacity_host(nu0, S, gamma0, T, P_atm, nu_min, nu_max, dnu, cutoff, mass_
     L = load_library()
     N = hk_grid_size(nu_min, nu_max, dnu)
     n = int(nu0.shape[0])
-    for name, t in (("S", S), ("gamma0", gamma0), ("n_T", n_T), ("E_low", E_low)):
+    for name, t in (("S", S), ("gamma0", gamma0), ("n_T", n_T), ("E_low", E_low), ("gamma_self", gamma_self), ("A21", A21),
+                    ("delta", delta)):
         if t is not None and int(t.shape[0]) != n:
             raise ValueError(f"{name} has {int(t.shape[0])} entries, nu0 has {n}")
     if want_kappa and kappa_out is None and N >= 1:
@@ -408,8 +423,9 @@ def hk_opacity_host(nu0, S, gamma0, T, P_atm, nu_min, nu_max, dnu, cutoff, mass_
     else:
         k_out = None
     cl = _hk_lines(_host_ptr(nu0, "nu0"), _host_ptr(S, "S"), _host_ptr(gamma0, "gamma0"), _host_ptr(n_T, "n_T", True),
-                   _host_ptr(E_low, "E_low", True))
-    prm = _hk_params(float(mass_amu), float(q_ratio), int(precision), int(bool(lines_sorted)), _stream_ptr(stream))
+                   _host_ptr(E_low, "E_low", True), _host_ptr(gamma_self, "gamma_self", True), _host_ptr(A21, "A21", True),
+                   _host_ptr(delta, "delta", True))
+    prm = _params(mass_amu, q_ratio, precision, lines_sorted, stream, self_fraction, abundance, accumulate)
     _check(L.hk_opacity_host(C.byref(cl), n, T, P_atm, nu_min, nu_max, dnu, cutoff, _host_ptr(kappa_out, "kappa_out", True),
                              float(bin_width or 0.0), int(n_g), _host_ptr(k_out, "k_out", True), C.byref(prm)),
            "hk_opacity_host")

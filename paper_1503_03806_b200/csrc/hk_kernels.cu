@@ -73,6 +73,8 @@ constexpr double kT0 = 296.0;               // K
 
 struct PrepArgs {
   const double *nu0, *S, *gamma0, *n_T, *E_low;
+  const double *gamma_self, *A21;  // eq. 20 (either may be NULL); the shift of eq. 21 is applied before a1
+  double self_fraction, abundance;
   int64_t n;
   double T, P_atm, tfac_half;  // (296/T)^0.5 for n_T == NULL
   double vth;                  // sqrt(2 kB T/m)/c : alpha = nu0*vth
@@ -137,14 +139,21 @@ __global__ void __launch_bounds__(256) line_prep_kernel(PrepArgs a)
   double alpha = nu0 * a.vth;
   if (!(alpha > 0.0)) alpha = 0.0;  // nu0 <= 0: Lorentzian (A9)
   const double tfac = a.n_T ? pow(kT0 / a.T, a.n_T[i]) : a.tfac_half;
-  const double gamma = a.gamma0[i] * a.P_atm * tfac;
+  double gamma;
+  if (a.gamma_self) {  // eq. 20: air and self broadening, P0 = 1 atm
+    const double P_self = a.self_fraction * a.P_atm;
+    gamma = tfac * (a.gamma0[i] * (a.P_atm - P_self) + a.gamma_self[i] * P_self);
+  } else {
+    gamma = a.gamma0[i] * a.P_atm * tfac;
+  }
+  if (a.A21) gamma += a.A21[i] * (1.0 / (4.0 * kPi * kCLight));  // natural width
   double S = a.S[i];
   if (a.E_low) {  // eq. 18, PAPER.md:170 (T0 in the last denominator: DESIGN.md G1)
     const double boltz = exp(-kC2 * a.E_low[i] * (1.0 / a.T - 1.0 / kT0));
     const double stim = (nu0 == 0.0) ? kT0 / a.T : (-expm1(-kC2 * nu0 / a.T)) / (-expm1(-kC2 * nu0 / kT0));
     S = S * a.q_ratio * boltz * stim;
   }
-  const double amp = S * a.inv_mg;
+  const double amp = S * a.inv_mg * a.abundance;
   const double g2 = gamma * gamma, a2 = alpha * alpha;
   LineBase b;
   b.nu0 = nu0;
@@ -349,6 +358,7 @@ struct VoigtArgs {
   double nu_min, dnu;
   float dnu_f;
   int N;
+  int accumulate;  // 1: add to kappa (species of a mixture after the first), 0: overwrite
   double *kappa;
   double r2_slope, r2_offset;  // near kernel: no line centred beyond r2_slope*j + r2_offset grid units of point j reaches it inside its 2-point radius
 };
@@ -611,7 +621,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) voigt_far_kernel(const __gri
 #pragma unroll
       for (int k = 0; k < P; ++k) {
         const int j = slo + lane + 32 * k;
-        if (j <= shi) a.kappa[j] = acc[k];
+        if (j <= shi) a.kappa[j] = a.accumulate ? a.kappa[j] + acc[k] : acc[k];
         acc[k] = 0.0;
       }
     }
@@ -854,6 +864,14 @@ __global__ void __launch_bounds__(128) voigt_K_kernel(const double *x, const dou
   if (live) out[i] = v;
 }
 
+// eq. 21: nu0 -> nu0 + delta P/P0, P0 = 1 atm
+__global__ void __launch_bounds__(256) shift_centres_kernel(const double *nu0, const double *delta, double P_atm, int64_t n,
+                                                            double *out)
+{
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) out[i] = __dadd_rn(nu0[i], __dmul_rn(delta[i], P_atm));
+}
+
 __global__ void __launch_bounds__(256) check_sorted_kernel(const double *nu0, int64_t n, int *flag)
 {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -1052,6 +1070,8 @@ static int validate(const hk_lines *lines, int64_t n_lines, double T, double P_a
   if (!isfinite(nu_min) || !isfinite(nu_max)) return HK_ERR_INVALID;
   if (prm->precision != HK_FP64 && prm->precision != HK_FP32) return HK_ERR_INVALID;
   if (lines->E_low && !pos_finite(prm->q_ratio)) return HK_ERR_INVALID;
+  if (!(prm->abundance >= 0.0) || !isfinite(prm->abundance)) return HK_ERR_INVALID;
+  if (lines->gamma_self && !(prm->self_fraction >= 0.0 && prm->self_fraction <= 1.0)) return HK_ERR_INVALID;
   const int64_t N = hk_grid_size(nu_min, nu_max, dnu);
   if (N < 1 || N > (1LL << 30)) return HK_ERR_INVALID;
   *N_out = N;
@@ -1059,12 +1079,12 @@ static int validate(const hk_lines *lines, int64_t n_lines, double T, double P_a
 }
 
 static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double P_atm, double q_ratio, double mass_amu,
-                       double nu_min, double dnu, double cutoff, int64_t N, double *kappa_out, Scratch &s, int precision,
+                       double nu_min, double dnu, double cutoff, int64_t N, double *kappa_out, Scratch &s, const hk_params &prm,
                        cudaStream_t st)
 {
-  const bool f32 = precision == HK_FP32;
+  const bool f32 = prm.precision == HK_FP32;
   if (n_lines == 0) {
-    HK_CUDA(cudaMemsetAsync(kappa_out, 0, (size_t)N * sizeof(double), st));
+    if (!prm.accumulate) HK_CUDA(cudaMemsetAsync(kappa_out, 0, (size_t)N * sizeof(double), st));
     return HK_OK;
   }
   const int nb = (int)((N + kPlanBlock - 1) / kPlanBlock);
@@ -1084,6 +1104,8 @@ static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double 
   }
   PrepArgs pa;
   pa.nu0 = lines->nu0; pa.S = lines->S; pa.gamma0 = lines->gamma0; pa.n_T = lines->n_T; pa.E_low = lines->E_low;
+  pa.gamma_self = lines->gamma_self; pa.A21 = lines->A21;
+  pa.self_fraction = prm.self_fraction; pa.abundance = prm.abundance > 0.0 ? prm.abundance : 1.0;
   pa.n = n_lines;
   pa.T = T; pa.P_atm = P_atm; pa.tfac_half = pow(kT0 / T, 0.5);
   const double m_g = mass_amu * kAmu;
@@ -1104,7 +1126,7 @@ static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double 
   va.dnu_f = (float)dnu;
   va.first_hi = s.first_hi; va.first_lo = s.first_lo; va.first_c = s.first_c; va.queue = s.queue;
   va.nb = nb; va.n_tiles = n_tiles;
-  va.nu_min = nu_min; va.dnu = dnu; va.N = (int)N; va.kappa = kappa_out;
+  va.nu_min = nu_min; va.dnu = dnu; va.N = (int)N; va.kappa = kappa_out; va.accumulate = prm.accumulate ? 1 : 0;
   {
     // bound on the 2-point radius (grid units) of any line that can be near grid point j: r2 <= s*alpha/dnu + margin with
     // alpha = vth*nu0 and nu0 <= nu_j + r2*dnu, s = sqrt(kR2)  =>  r2 <= (s*vth*(nu_min/dnu + j) + margin)/(1 - s*vth)
@@ -1172,15 +1194,30 @@ int hk_opacity(const hk_lines *lines, int64_t n_lines, double T, double P_atm, d
   int rc = validate(lines, n_lines, T, P_atm, nu_min, nu_max, dnu, cutoff, kappa_out, prm, &N);
   if (rc != HK_OK) return rc;
   cudaStream_t st = (cudaStream_t)prm->stream;
+  hk_lines eff = *lines;
+  hk_params pe = *prm;
+  void *shift_buf = nullptr;
+  if (lines->delta && n_lines > 0) {  // eq. 21: shifted centres on a copy; their order is re-checked
+    rc = pool_alloc(&shift_buf, (size_t)n_lines * sizeof(double), st);
+    if (rc != HK_OK) return rc;
+    shift_centres_kernel<<<(unsigned)((n_lines + 255) / 256), 256, 0, st>>>(lines->nu0, lines->delta, P_atm, n_lines,
+                                                                            (double *)shift_buf);
+    eff.nu0 = (const double *)shift_buf;
+    pe.lines_sorted = 0;
+  }
+  eff.delta = nullptr;
   hk_lines use;
   void *sorted_buf = nullptr;
-  rc = ordered_lines(lines, n_lines, prm, &use, &sorted_buf);
-  if (rc != HK_OK) return rc;
+  rc = ordered_lines(&eff, n_lines, &pe, &use, &sorted_buf);
+  if (rc != HK_OK) {
+    pool_free(shift_buf, st);
+    return rc;
+  }
   Scratch s;
-  rc = run_opacity(&use, n_lines, T, P_atm, prm->q_ratio, prm->mass_amu, nu_min, dnu, cutoff, N, kappa_out, s,
-                   prm->precision, st);
+  rc = run_opacity(&use, n_lines, T, P_atm, prm->q_ratio, prm->mass_amu, nu_min, dnu, cutoff, N, kappa_out, s, *prm, st);
   scratch_release(s, st);
   pool_free(sorted_buf, st);
+  pool_free(shift_buf, st);
   return rc;
 }
 
@@ -1189,6 +1226,7 @@ int hk_opacity_host(const hk_lines *lines_host, int64_t n_lines, double T, doubl
                     const hk_params *prm)
 {
   if (!lines_host || !prm || n_lines < 0 || (!kappa_host_out && !k_host_out)) return HK_ERR_INVALID;
+  if (prm->accumulate && !kappa_host_out) return HK_ERR_INVALID;  // the running sum of a mixture is read from it
   if (n_lines > 0 && (!lines_host->nu0 || !lines_host->S || !lines_host->gamma0)) return HK_ERR_INVALID;
   const int64_t N = hk_grid_size(nu_min, nu_max, dnu);
   if (N < 1 || N > (1LL << 30)) return HK_ERR_INVALID;
@@ -1200,24 +1238,28 @@ int hk_opacity_host(const hk_lines *lines_host, int64_t n_lines, double T, doubl
     n_bins = N / (int64_t)ppb_d;
   }
   cudaStream_t st = (cudaStream_t)prm->stream;
-  const double *src[5] = {lines_host->nu0, lines_host->S, lines_host->gamma0, lines_host->n_T, lines_host->E_low};
+  constexpr int NF = 8;
+  const double *src[NF] = {lines_host->nu0, lines_host->S, lines_host->gamma0, lines_host->n_T, lines_host->E_low,
+                           lines_host->gamma_self, lines_host->A21, lines_host->delta};
   const size_t fbytes = ((size_t)n_lines * sizeof(double) + 255) & ~(size_t)255;
   const size_t kappa_bytes = ((size_t)N * sizeof(double) + 255) & ~(size_t)255;
   void *dev = nullptr;
-  int rc = pool_alloc(&dev, 5 * fbytes + kappa_bytes + (size_t)n_bins * n_g * sizeof(double), st);
+  int rc = pool_alloc(&dev, NF * fbytes + kappa_bytes + (size_t)n_bins * n_g * sizeof(double), st);
   if (rc != HK_OK) return rc;
-  const double *dptr[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+  const double *dptr[NF] = {};
   cudaError_t e = cudaSuccess;
-  for (int f = 0; f < 5 && e == cudaSuccess; ++f) {
+  for (int f = 0; f < NF && e == cudaSuccess; ++f) {
     if (!src[f] || n_lines == 0) continue;
     double *d = (double *)((char *)dev + f * fbytes);
     e = cudaMemcpyAsync(d, src[f], (size_t)n_lines * sizeof(double), cudaMemcpyHostToDevice, st);
     dptr[f] = d;
   }
-  double *d_kappa = (double *)((char *)dev + 5 * fbytes);
-  double *d_k = (double *)((char *)dev + 5 * fbytes + kappa_bytes);
+  double *d_kappa = (double *)((char *)dev + NF * fbytes);
+  double *d_k = (double *)((char *)dev + NF * fbytes + kappa_bytes);
+  if (e == cudaSuccess && prm->accumulate && kappa_host_out)  // a mixture's running sum lives in the caller's host buffer
+    e = cudaMemcpyAsync(d_kappa, kappa_host_out, (size_t)N * sizeof(double), cudaMemcpyHostToDevice, st);
   if (e == cudaSuccess) {
-    hk_lines dl = {dptr[0], dptr[1], dptr[2], dptr[3], dptr[4]};
+    hk_lines dl = {dptr[0], dptr[1], dptr[2], dptr[3], dptr[4], dptr[5], dptr[6], dptr[7]};
     rc = hk_opacity(&dl, n_lines, T, P_atm, nu_min, nu_max, dnu, cutoff, d_kappa, prm);
     if (rc == HK_OK && k_host_out) rc = hk_kdist(d_kappa, N, dnu, bin_width, n_g, d_k, prm->stream);
     if (rc == HK_OK && kappa_host_out)
@@ -1240,6 +1282,7 @@ int hk_create(const hk_lines *lines, int64_t n_lines, const hk_params *prm, hk_c
   if (n_lines > 2000000000LL) return HK_ERR_UNSUPPORTED;
   if (!pos_finite(prm->mass_amu)) return HK_ERR_INVALID;
   if (prm->precision != HK_FP64 && prm->precision != HK_FP32) return HK_ERR_INVALID;
+  if (lines->delta) return HK_ERR_UNSUPPORTED;  // the order of shifted centres depends on P: use hk_opacity
   hk_ctx *c = new (std::nothrow) hk_ctx();
   if (!c) return HK_ERR_NOMEM;
   int rc = ordered_lines(lines, n_lines, prm, &c->lines, &c->sorted_buf);
@@ -1264,7 +1307,7 @@ int hk_opacity_ctx(hk_ctx *ctx, double T, double P_atm, double q_ratio, double n
   int rc = validate(&ctx->lines, ctx->n_lines, T, P_atm, nu_min, nu_max, dnu, cutoff, kappa_out, &p, &N);
   if (rc != HK_OK) return rc;
   return run_opacity(&ctx->lines, ctx->n_lines, T, P_atm, q_ratio, p.mass_amu, nu_min, dnu, cutoff, N, kappa_out,
-                     ctx->scratch, p.precision, (cudaStream_t)p.stream);
+                     ctx->scratch, p, (cudaStream_t)p.stream);
 }
 
 int hk_destroy(hk_ctx *ctx)

@@ -32,11 +32,11 @@ __global__ void __launch_bounds__(256) gather_fields_kernel(const int *perm, int
 }
 
 // Stable ascending sort by nu0.  `buf` receives one allocation holding the ordered copies (freed by the caller with
-// pool_free); `out` points into it (n_T / E_low stay NULL when the input has none).
+// pool_free); `out` points into it (optional fields stay NULL when the input has none).
 int sort_lines_copy(const hk_lines *in, int64_t n, cudaStream_t st, hk_lines *out, void **buf)
 {
   *buf = nullptr;
-  const int nf = 3 + (in->n_T ? 1 : 0) + (in->E_low ? 1 : 0);
+  const int nf = 3 + (in->n_T ? 1 : 0) + (in->E_low ? 1 : 0) + (in->gamma_self ? 1 : 0) + (in->A21 ? 1 : 0);
   const size_t fbytes = ((size_t)n * sizeof(double) + 255) & ~(size_t)255;
   const size_t ibytes = ((size_t)n * sizeof(int) + 255) & ~(size_t)255;
   size_t tmp_bytes = 0;
@@ -61,8 +61,17 @@ int sort_lines_copy(const hk_lines *in, int64_t n, cudaStream_t st, hk_lines *ou
     double *dS = (double *)((char *)keep + fbytes), *dG = (double *)((char *)keep + 2 * fbytes);
     double *dN = in->n_T ? (double *)((char *)keep + 3 * fbytes) : nullptr;
     double *dE = in->E_low ? (double *)((char *)keep + (size_t)(3 + (in->n_T ? 1 : 0)) * fbytes) : nullptr;
+    int used = 3 + (in->n_T ? 1 : 0) + (in->E_low ? 1 : 0);
+    double *dGs = in->gamma_self ? (double *)((char *)keep + (size_t)(used++) * fbytes) : nullptr;
+    double *dA = in->A21 ? (double *)((char *)keep + (size_t)(used++) * fbytes) : nullptr;
     gather_fields_kernel<<<blocks, 256, 0, st>>>(idx_out, n, in->S, in->gamma0, in->n_T, in->E_low, dS, dG, dN, dE);
+    if (dGs || dA)
+      gather_fields_kernel<<<blocks, 256, 0, st>>>(idx_out, n, in->gamma_self, in->A21, nullptr, nullptr, dGs, dA, nullptr,
+                                                   nullptr);
     e = cudaGetLastError();
+    out->gamma_self = dGs;
+    out->A21 = dA;
+    out->delta = nullptr;  // eq. 21 is applied to nu0 before the list is ordered
     out->nu0 = f;
     out->S = dS;
     out->gamma0 = dG;
