@@ -169,7 +169,7 @@ __device__ __forceinline__ double gh6_val(double q, const Gh6 &g)
 //   W_n = exp(-a^2 n^2)/(a^2 n^2 + y^2),  S1 = sum_n W_n,  p = exp(2 a x)
 // (exp(-(an-x)^2) + exp(-(an+x)^2) = exp(-x^2) exp(-a^2 n^2) (p^n + p^-n)).  y is a per-line constant: lane n-1 of the
 // warp holds W_n and the series loop broadcasts it with SHFL; C_n = p^n + p^-n advances by the three-term recurrence
-// C_{n+1} = (p + 1/p) C_n - C_{n-1} (forward-stable: the growing solution dominates), so a term is 2 DFMA + 1 SHFL.
+// C_{n+2} = ((p + 1/p)^2 - 2) C_n - C_{n-2} (forward-stable: the growing solution dominates), so a term is 2 DFMA + 1 SHFL.
 // p^16 <= exp(1.4 * 6.64 * 16) = 4e64: no overflow for x <= sqrt(44).
 struct CoreLine {
   double y, inv_y, erfcx_y, S1, W;  // W is lane-dependent: W_{lane+1} (0 for lane >= 16)
@@ -205,16 +205,22 @@ __device__ __forceinline__ double core_K(double x, const CoreLine &c)
 {
   const double ex2 = exp(-x * x);
   const double p = exp(2.0 * kA * x);
-  const double s2c = p + rcp_nr2(p);  // 2 cosh(2 a x)
-  double Cm = 2.0, C = s2c, sum = 0.0;
+  const double s2c = p + rcp_nr2(p);  // 2 cosh(2 a x) = C_1
+  // C_n = p^n + p^-n in two independent chains (odd and even n) with the step-2 recurrence C_{n+2} = (C_1^2 - 2) C_n - C_{n-2},
+  // C_{-1} = C_1, C_0 = 2, C_2 = C_1^2 - 2: the dependent-DFMA path is 8 long instead of 16 (this loop is latency-bound at
+  // the near kernel's 4 warps per scheduler)
+  const double t2 = fma(s2c, s2c, -2.0);
+  double Com = s2c, Co = s2c, Cem = 2.0, Ce = t2, so = 0.0, se = 0.0;
 #pragma unroll
-  for (int n = 0; n < kTerms; ++n) {
-    const double w = __shfl_sync(kFull, c.W, n);
-    sum = fma(w, C, sum);
-    const double Cn = fma(s2c, C, -Cm);
-    Cm = C;
-    C = Cn;
+  for (int i = 0; i < kTerms / 2; ++i) {
+    const double wo = __shfl_sync(kFull, c.W, 2 * i), we = __shfl_sync(kFull, c.W, 2 * i + 1);
+    so = fma(wo, Co, so);
+    se = fma(we, Ce, se);
+    const double Con = fma(t2, Co, -Com), Cen = fma(t2, Ce, -Cem);
+    Com = Co; Co = Con;
+    Cem = Ce; Ce = Cen;
   }
+  const double sum = so + se;
   const double s = sinpi(x * c.y * kInvPi);  // x y <= 44; sinpi has no slow range-reduction path
   const double s2 = s * s;
   const double c2 = fma(-2.0, s2, 1.0);
