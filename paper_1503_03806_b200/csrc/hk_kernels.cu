@@ -673,6 +673,7 @@ struct __align__(16) NearSmem {
   LineGH2 gh2[kNearCap];
   LineCore core[kNearCap];
   double sk[kNearWarps][kPlanBlock];
+  double W[kNearWarps][kTerms];  // series weights of the line a warp is working on
   int counts[kNearWarps];
 };
 
@@ -686,7 +687,8 @@ __device__ __forceinline__ float group_dist(int glo, float c)
 // inner groups of one listed line (those closer to its centre than the 3-point radius): 6-point rule, series on the groups
 // that hold core points, Gaussian term of a tiny-y line; accumulated in the warp's strip sk[32k + lane].  Warp-collective.
 __device__ __noinline__ void near_inner(const MetaA *pa, const MetaB *pm, const LineBase *pb, const LineGH2 *pg,
-                                        const LineCore *pk, int plo, int lane, double x0, double dnu, double En, double *sk)
+                                        const LineCore *pk, int plo, int lane, double x0, double dnu, double En, double *sk,
+                                        double *Wsm, unsigned inner)
 {
   const MetaA ma = *pa;
   const MetaB mb = *pm;
@@ -698,25 +700,31 @@ __device__ __noinline__ void near_inner(const MetaA *pa, const MetaB *pm, const 
   const Gh6 G6 = gh6_consts(b.A1, b.g2, b.a2);
   const double xc2 = core_xc2(kc.y);
   CoreLine C;
-  if (dist < mb.r6) C = core_setup(kc.y, kc.inv_y, kc.erfcx_y, En);
+  if (dist < mb.r6) C = core_setup(kc.y, kc.inv_y, kc.erfcx_y, En, Wsm);
 #pragma unroll 1
-  for (int k = 0; k < kNearP; ++k) {
-    const int glo = plo + 32 * k, ghi = glo + 31;
-    if (ghi < ma.jlo || glo > ma.jhi) continue;
+  for (unsigned m = inner; m; m &= m - 1) {  // groups inside the 3-point radius that touch the line's window
+    const int k = __ffs(m) - 1;
+    const int glo = plo + 32 * k;
     const float dg = group_dist(glo, ma.c);
-    if (dg >= ma.r3) continue;  // taken by the 3-point rule in the caller
     const int j = glo + lane;
     const bool inwin = (j >= ma.jlo) && (j <= ma.jhi);
     const double d = fma((double)(32 * k), dnu, d0);
-    double v = gh6_val(d * d, G6);
+    double v = 0.0;
     if (dg < mb.r6) {  // the series region reaches into this group
       const double x = fabs(d) * inv_alpha;
+      const bool core = x * x < xc2;
       const double ks = core_K(fmin(x, 6.7), C);
-      if (x * x < xc2) v = kc.Acore * ks;
-      else if (mb.rg > 0.0f) v = fma(kc.Acore, exp(-x * x), v);
-    } else if (dg < mb.rg) {
-      const double x = d * inv_alpha;
-      v = fma(kc.Acore, exp(-x * x), v);
+      if (!__all_sync(kFull, core || !inwin)) {  // some point of the group lies outside the series region
+        v = gh6_val(d * d, G6);
+        if (mb.rg > 0.0f) v = fma(kc.Acore, exp(-x * x), v);
+      }
+      if (core) v = kc.Acore * ks;
+    } else {
+      v = gh6_val(d * d, G6);
+      if (dg < mb.rg) {
+        const double x = d * inv_alpha;
+        v = fma(kc.Acore, exp(-x * x), v);
+      }
     }
     sk[32 * k + lane] += inwin ? v : 0.0;
   }
@@ -780,7 +788,7 @@ __global__ void __launch_bounds__(kNearWarps * 32, 4) voigt_near_kernel(const __
 #pragma unroll 1
       for (int e = warp; e < list_n; e += kNearWarps) {
         const MetaA ea = S.ma[e];
-        bool inner = false;  // some group lies inside the 3-point radius (warp-uniform)
+        unsigned inner = 0u;  // groups inside the 3-point radius that touch the window (warp-uniform bit mask)
         {  // 3-point rule, unrolled over the 8 groups in registers, on every group at or beyond the 3-point radius
           const LineBase lb = S.base[e];
           const double d0 = x0 - lb.nu0;
@@ -793,11 +801,12 @@ __global__ void __launch_bounds__(kNearWarps * 32, 4) voigt_near_kernel(const __
             const double t = gh3_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), lb.g2, e3, f3, c0, c3, c3a);
             const bool far3 = group_dist(plo + 32 * k, ea.c) >= ea.r3;
             acc[k] = (far3 && (unsigned)(jrel + 32 * k) <= wlen) ? t : acc[k];
-            inner |= !far3;
+            const int glo = plo + 32 * k;
+            if (!far3 && glo + 31 >= ea.jlo && glo <= ea.jhi) inner |= 1u << k;
           }
         }
         if (inner)
-          near_inner(S.ma + e, S.mb + e, S.base + e, S.gh2 + e, S.core + e, plo, lane, x0, a.dnu, En, sk);
+          near_inner(S.ma + e, S.mb + e, S.base + e, S.gh2 + e, S.core + e, plo, lane, x0, a.dnu, En, sk, S.W[warp], inner);
       }
       list_n = 0;
       __syncthreads();  // the list is free again
@@ -851,13 +860,14 @@ __global__ void __launch_bounds__(128) voigt_K_kernel(const double *x, const dou
     if (tiny_gauss) v += exp(-q);
   }
   const bool incore = live && (q < core_xc2(yi));
+  __shared__ double Wsm[4][kTerms];
   const double En = core_lane_const();
   unsigned need = __ballot_sync(kFull, incore);
   while (need) {  // the series is warp-collective with a warp-uniform y: serve one lane at a time
     const int src = __ffs(need) - 1;
     need &= need - 1;
     const double ys = __shfl_sync(kFull, yi, src), xs = __shfl_sync(kFull, xi, src);
-    const CoreLine C = core_setup(ys, 1.0 / ys, erfcx(ys), En);
+    const CoreLine C = core_setup(ys, 1.0 / ys, erfcx(ys), En, Wsm[threadIdx.x >> 5]);
     const double kc = core_K(fmin(xs, 6.7), C);
     if (lane == src) v = kc;
   }

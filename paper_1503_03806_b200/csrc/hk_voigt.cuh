@@ -168,11 +168,12 @@ __device__ __forceinline__ double gh6_val(double q, const Gh6 &g)
 //                        + (a/pi) y sum_{n=1..16} W_n (p^n + p^-n) ],
 //   W_n = exp(-a^2 n^2)/(a^2 n^2 + y^2),  S1 = sum_n W_n,  p = exp(2 a x)
 // (exp(-(an-x)^2) + exp(-(an+x)^2) = exp(-x^2) exp(-a^2 n^2) (p^n + p^-n)).  y is a per-line constant: lane n-1 of the
-// warp holds W_n and the series loop broadcasts it with SHFL; C_n = p^n + p^-n advances by the three-term recurrence
+// warp computes W_n into a 16-entry shared-memory table and the series loop reads it by broadcast (one LDS.128 per two terms); C_n = p^n + p^-n advances by the three-term recurrence
 // C_{n+2} = ((p + 1/p)^2 - 2) C_n - C_{n-2} (forward-stable: the growing solution dominates), so a term is 2 DFMA + 1 SHFL.
 // p^16 <= exp(1.4 * 6.64 * 16) = 4e64: no overflow for x <= sqrt(44).
 struct CoreLine {
-  double y, inv_y, erfcx_y, S1, W;  // W is lane-dependent: W_{lane+1} (0 for lane >= 16)
+  double y, inv_y, erfcx_y, S1;
+  const double *W;  // the warp's shared-memory table W_1 .. W_16 (read by broadcast in the series loop)
 };
 
 // exp(-a^2 n^2) for n = lane + 1 (0 beyond the 16 terms): a per-lane constant, computed once per kernel
@@ -183,8 +184,8 @@ __device__ __forceinline__ double core_lane_const()
   return lane < kTerms ? exp(-kA * kA * n * n) : 0.0;
 }
 
-// All 32 lanes must call (warp-collective).  En = core_lane_const().
-__device__ __forceinline__ CoreLine core_setup(double y, double inv_y, double erfcx_y, double En)
+// All 32 lanes must call (warp-collective).  En = core_lane_const(); Wsm = kTerms doubles of shared memory owned by the warp.
+__device__ __forceinline__ CoreLine core_setup(double y, double inv_y, double erfcx_y, double En, double *Wsm)
 {
   CoreLine c;
   const int lane = threadIdx.x & 31;
@@ -192,15 +193,19 @@ __device__ __forceinline__ CoreLine core_setup(double y, double inv_y, double er
   c.y = y;
   c.inv_y = inv_y;
   c.erfcx_y = erfcx_y;
-  c.W = En * rcp_nr2(fma(kA * kA * n, n, y * y));
-  double t = c.W;
+  c.W = Wsm;
+  const double W = En * rcp_nr2(fma(kA * kA * n, n, y * y));
+  __syncwarp();  // readers of the previous line's table are done
+  if (lane < kTerms) Wsm[lane] = W;
+  double t = W;
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(kFull, t, o);
   c.S1 = t;
+  __syncwarp();
   return c;
 }
 
-// All 32 lanes must call with the same CoreLine (warp-collective: SHFL inside).  0 <= x <= 6.7.
+// Lanes of a warp call with the same CoreLine.  0 <= x <= 6.7.
 __device__ __forceinline__ double core_K(double x, const CoreLine &c)
 {
   const double ex2 = exp(-x * x);
@@ -213,7 +218,7 @@ __device__ __forceinline__ double core_K(double x, const CoreLine &c)
   double Com = s2c, Co = s2c, Cem = 2.0, Ce = t2, so = 0.0, se = 0.0;
 #pragma unroll
   for (int i = 0; i < kTerms / 2; ++i) {
-    const double wo = __shfl_sync(kFull, c.W, 2 * i), we = __shfl_sync(kFull, c.W, 2 * i + 1);
+    const double wo = c.W[2 * i], we = c.W[2 * i + 1];
     so = fma(wo, Co, so);
     se = fma(we, Ce, se);
     const double Con = fma(t2, Co, -Com), Cen = fma(t2, Ce, -Cem);
