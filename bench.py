@@ -46,6 +46,10 @@ FP64_INST_PER_EVAL = {"gh1": 5.0, "gh2": 7.0, "gh3": 11.0, "gh6": 22.0, "series"
 # --precision fp32: FP32-pipe thread-instructions per evaluation of the two rules the far kernel runs in float, two points per
 # reciprocal (hk_voigt.cuh gh1_acc2f / gh2_acc2f: 8 and 13 per pair, + 1 MUFU.RCP per pair)
 FP32_INST_PER_EVAL = {"gh1": 4.0, "gh2": 6.5}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the roofline kernel(s), from the committed `ncu --set full` captures
+# of this command (profiles/r01c_voigt_{far,near,far32}_kernel_ncu_full.txt): far 9.76 MB + near 36.90 MB read, ~0 written
+# (kappa, 24 MB, stays in the 126 MB L2 between the two kernels); FP32 far kernel 6.52 MB.  Not memory-bound: context only.
+NCU_DRAM_BYTES = {"fp64": 9.761e6 + 36.898e6 + 0.020e6, "fp32": 6.518e6}
 
 
 def tp_table(wl, world):
@@ -299,7 +303,9 @@ def run_ours(args):
                 "ms_per_step": e2e_ms / K},
         "gpu_launches": 4 * K,   # line_prep, voigt_far, voigt_near, kdist
         "roofline": {"kernel": roof_kernel, "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                     "frac": achieved / peak, "traffic": None, "note": roof_note, "regime_census": census, "ms": roof_ms,
+                     "frac": achieved / peak, "traffic": NCU_DRAM_BYTES[args.precision],
+                     "traffic_note": "DRAM bytes per launch from the committed ncu --set full capture (profiles/r01c_*), not live",
+                     "note": roof_note, "regime_census": census, "ms": roof_ms,
                      "fp64_peak_tflops": 2.0 * fp64_peak / 1e12, "fp32_peak_tflops": 2.0 * fp32_peak / 1e12},
         "clocks": clocks,
     }
