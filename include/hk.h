@@ -155,7 +155,8 @@ int hk_kdist(const double *kappa, int64_t n_points, double dnu, double bin_width
  *   minimise sum_k ( sum_n C_n T_n(2 y_k - 1) - ln max(s_k, 1e-300) )^2 ,
  * "solving A C = D" by Q-R decomposition.  The design matrix A is the same for every bin, so it is factored once per
  * (ppb, n_c) (Householder Q-R in long double on the host; P = R^-1 Q^T kept on the device for the life of the process;
- * that first call synchronises), and each bin costs its sort plus the product C = P D in the sort kernel.  The paper is
+ * that first call synchronises); each call is the sort kernel, which also stores ln of the sorted values in a scratch
+ * array from the library's pool, and one projection kernel C = D P^T.  The paper is
  * silent on kappa = 0: ln is taken of max(kappa, 1e-300).
  * coef_out: device [n_bins*n_c], row-major by bin, overwritten.  k_out: device [n_bins*n_g] or NULL — when given, the
  * Gauss-Legendre k-table of hk_kdist is written by the same launch (n_g is ignored when k_out is NULL).

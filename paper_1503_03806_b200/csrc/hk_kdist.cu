@@ -25,9 +25,7 @@ struct KdistArgs {
   int ppb;   // points per bin
   int n;     // padded size, T*E
   int n_g;
-  const double *cheb_P;  // f1 (hk_kdist_cheb): projection matrix [n_c][ppb] of the Chebyshev least-squares fit, or NULL
-  double *cheb_out;      // [n_bins][n_c]
-  int n_c;
+  double *ln_out;  // f1 (hk_kdist_cheb): ln max(s_k, 1e-300) of every sorted bin, [n_bins][ppb] scratch, or NULL
   double g[128];
 };
 
@@ -77,7 +75,7 @@ __device__ __forceinline__ int pad(int i)
   return i + 2 * (i / E);
 }
 
-template <int E, int MAXT>
+template <int E, int MAXT, bool CHEB>
 __global__ void __launch_bounds__(MAXT) kdist_kernel(const __grid_constant__ KdistArgs a)
 {
   extern __shared__ __align__(16) double s[];
@@ -178,49 +176,118 @@ __global__ void __launch_bounds__(MAXT) kdist_kernel(const __grid_constant__ Kdi
     }
     a.k_out[(int64_t)bin * a.n_g + q] = val;
   }
-  // ---- f1: Chebyshev coefficients of ln kappa(y), C = P D with D_k = ln max(s_k, 1e-300) (the Q-R
-  // factorisation behind P is done once on the host, hk_resample.cu).  Thread t holds s_k for k = tE .. tE+E-1 in registers;
-  // per coefficient: E products per thread, a butterfly over the warp, then the warps' partial sums in a fixed order.
-  if (a.cheb_P) {
-    double d[E];
+  // ---- f1: D_k = ln max(s_k, 1e-300) of the sorted bin, for the Chebyshev least-squares fit (cheb_project_kernel)
+  if constexpr (CHEB) {
+    double *dst = a.ln_out + (int64_t)bin * a.ppb;
 #pragma unroll
-    for (int r = 0; r < E; ++r) d[r] = (i0 + r < a.ppb) ? log(fmax(v[r], 1.0e-300)) : 0.0;
-    __syncthreads();  // the resampling above is done with s
-    const int nw = (T + 31) >> 5, warp = t >> 5, lane = t & 31;
-    for (int n = 0; n < a.n_c; ++n) {
-      const double *Pn = a.cheb_P + (int64_t)n * a.ppb;
-      double acc = 0.0;
-#pragma unroll
-      for (int r = 0; r < E; ++r)
-        if (i0 + r < a.ppb) acc = fma(Pn[i0 + r], d[r], acc);
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(kFullMask, acc, o);
-      if (lane == 0) s[warp * a.n_c + n] = acc;
-    }
-    __syncthreads();
-    for (int n = t; n < a.n_c; n += T) {
-      double c = 0.0;
-      for (int w = 0; w < nw; ++w) c += s[w * a.n_c + n];
-      a.cheb_out[(int64_t)bin * a.n_c + n] = c;
-    }
+    for (int r = 0; r < E; ++r)
+      if (i0 + r < a.ppb) dst[i0 + r] = log(fmax(v[r], 1.0e-300));
   }
 }
 
-template <int E, int MAXT>
-static int launch_kdist(const KdistArgs &a, int64_t n_bins, cudaStream_t st)
+// f1: C = D P^T, the Chebyshev coefficients of ln kappa(y) of every bin (the Q-R factorisation behind
+// P is done once on the host, hk_resample.cu).  D [n_bins][ppb] (written by kdist_kernel), P [n_c][ppb], C [n_bins][n_c].
+// A plain FP64 contraction of 2 n_bins ppb n_c flop (1.2e8 at config 1: microseconds of the FP64 pipe, so no tensor-core
+// path); what matters is that P is read once per 8 bins, not once per bin, and that enough CTAs are in flight to hide the
+// staging: CTA = 8 bins x all coefficients, D and P staged through (dynamic) shared memory in chunks of up to 256 points
+// (few, long stages: every load of a stage is in flight at once); thread t owns bin t % 8 and the coefficients t / 8,
+// t / 8 + 16, ...; fixed summation order.
+constexpr int kCpBins = 8, kCpChunk = 256, kCpMaxNc = 64, kCpGroups = 128 / kCpBins;
+__global__ void __launch_bounds__(128) cheb_project_kernel(const double *D, const double *P, int64_t n_bins, int ppb, int n_c,
+                                                           double *C)
+{
+  extern __shared__ __align__(16) double cp_smem[];
+  const int KC = min(kCpChunk, ppb), ld = KC + 1;
+  double *Ds = cp_smem;               // [kCpBins][ld]
+  double *Ps = cp_smem + kCpBins * ld;  // [n_c][ld]
+  const int t = threadIdx.x, bl = t % kCpBins, cg = t / kCpBins;
+  const int64_t b0 = (int64_t)blockIdx.x * kCpBins;
+  const int nb = (int)min((int64_t)kCpBins, n_bins - b0);
+  constexpr int U = kCpMaxNc / kCpGroups;
+  double acc[U];
+#pragma unroll
+  for (int u = 0; u < U; ++u) acc[u] = 0.0;
+  for (int k0 = 0; k0 < ppb; k0 += KC) {
+    const int kc = min(KC, ppb - k0);
+    __syncthreads();
+    // thread t stages columns t and t + 128 of every row; loads go to registers in batches of 8 rows before any store, so
+    // that a batch is one round trip to L2.  Every CTA stages the same rows of P at about the same time: each starts at
+    // another row, so that their requests spread over the L2 slices instead of queueing on one line.
+    constexpr int H = kCpChunk / 128;
+    {
+      double tmp[kCpBins][H];
+#pragma unroll
+      for (int r = 0; r < kCpBins; ++r)
+#pragma unroll
+        for (int h = 0; h < H; ++h) {
+          const int c = t + 128 * h;
+          tmp[r][h] = (r < nb && c < kc) ? D[(b0 + r) * ppb + k0 + c] : 0.0;
+        }
+#pragma unroll
+      for (int r = 0; r < kCpBins; ++r)
+#pragma unroll
+        for (int h = 0; h < H; ++h)
+          if (t + 128 * h < KC) Ds[r * ld + t + 128 * h] = tmp[r][h];
+    }
+    const int r_first = (int)(blockIdx.x % (unsigned)n_c);
+    for (int r0 = 0; r0 < n_c; r0 += 8) {
+      double tmp[8][H];
+      int row[8];
+#pragma unroll
+      for (int q = 0; q < 8; ++q) {
+        const int rr = min(r0 + q, n_c - 1) + r_first;
+        row[q] = rr < n_c ? rr : rr - n_c;
+#pragma unroll
+        for (int h = 0; h < H; ++h) {
+          const int c = t + 128 * h;
+          tmp[q][h] = c < kc ? __ldg(P + (int64_t)row[q] * ppb + k0 + c) : 0.0;
+        }
+      }
+#pragma unroll
+      for (int q = 0; q < 8; ++q)
+#pragma unroll
+        for (int h = 0; h < H; ++h)
+          if (r0 + q < n_c && t + 128 * h < KC) Ps[row[q] * ld + t + 128 * h] = tmp[q][h];
+    }
+    __syncthreads();
+#pragma unroll 8
+    for (int kk = 0; kk < kc; ++kk) {
+      const double dv = Ds[bl * ld + kk];
+#pragma unroll
+      for (int u = 0; u < U; ++u)
+        if (cg + kCpGroups * u < n_c) acc[u] = fma(Ps[(cg + kCpGroups * u) * ld + kk], dv, acc[u]);
+    }
+  }
+  if (bl < nb) {
+#pragma unroll
+    for (int u = 0; u < U; ++u)
+      if (cg + kCpGroups * u < n_c) C[(b0 + bl) * n_c + cg + kCpGroups * u] = acc[u];
+  }
+}
+
+template <int E, int MAXT, bool CHEB>
+static int launch_kdist_t(const KdistArgs &a, int64_t n_bins, cudaStream_t st)
 {
   const int T = a.n / E;
   const size_t smem = (size_t)(a.n + 2 * T) * sizeof(double);
   static bool attr_set = false;
   if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(kdist_kernel<E, MAXT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (16384 + 2048) * 8);
+    cudaError_t e = cudaFuncSetAttribute(kdist_kernel<E, MAXT, CHEB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (16384 + 2048) * 8);
     if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(kdist_kernel)");
     attr_set = true;
   }
-  kdist_kernel<E, MAXT><<<(unsigned)n_bins, T, smem, st>>>(a);
+  kdist_kernel<E, MAXT, CHEB><<<(unsigned)n_bins, T, smem, st>>>(a);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return cuda_fail(e, "kdist_kernel launch");
   return HK_OK;
+}
+
+// the plain k-distribution (a5 + a6) and the variant with the Chebyshev epilogue are separate instantiations: the epilogue's
+// registers do not weigh on the hot path
+template <int E, int MAXT>
+static int launch_kdist(const KdistArgs &a, int64_t n_bins, cudaStream_t st)
+{
+  return a.ln_out ? launch_kdist_t<E, MAXT, true>(a, n_bins, st) : launch_kdist_t<E, MAXT, false>(a, n_bins, st);
 }
 
 }  // namespace hk
@@ -247,24 +314,46 @@ static int kdist_common(const double *kappa, int64_t n_points, double dnu, doubl
   a.k_out = k_out;
   a.ppb = ppb;
   a.n_g = k_out ? n_g : 0;
-  a.cheb_P = nullptr;
-  a.cheb_out = coef_out;
-  a.n_c = coef_out ? n_c : 0;
+  a.ln_out = nullptr;
+  cudaStream_t st = (cudaStream_t)stream;
+  const double *P = nullptr;
+  void *ln_buf = nullptr;
   if (coef_out) {
-    int rcp = cheb_projection_device(ppb, n_c, &a.cheb_P);
+    int rcp = cheb_projection_device(ppb, n_c, &P);
     if (rcp != HK_OK) return rcp;
+    rcp = pool_alloc(&ln_buf, (size_t)n_points * sizeof(double), st);
+    if (rcp != HK_OK) return rcp;
+    a.ln_out = (double *)ln_buf;
   }
   int n = 64;
   while (n < ppb) n <<= 1;
   a.n = n;
   double wts[128];
   int rc = k_out ? hk_gauss_legendre(n_g, a.g, wts) : HK_OK;
-  if (rc != HK_OK) return rc;
-  cudaStream_t st = (cudaStream_t)stream;
-  if (n <= 256) return launch_kdist<2, 128>(a, n_bins, st);   // T = 32 .. 128
-  if (n == 512) return launch_kdist<4, 128>(a, n_bins, st);   // T = 128
-  if (n == 1024) return launch_kdist<8, 128>(a, n_bins, st);  // T = 128
-  return launch_kdist<16, 1024>(a, n_bins, st);                // T = 128 .. 1024
+  if (rc == HK_OK) {
+    if (n <= 256) rc = launch_kdist<2, 128>(a, n_bins, st);        // T = 32 .. 128
+    else if (n == 512) rc = launch_kdist<4, 128>(a, n_bins, st);   // T = 128
+    else if (n == 1024) rc = launch_kdist<8, 128>(a, n_bins, st);  // T = 128
+    else rc = launch_kdist<16, 1024>(a, n_bins, st);               // T = 128 .. 1024
+  }
+  if (rc == HK_OK && coef_out) {
+    const size_t cp_bytes = (size_t)(kCpBins + n_c) * (size_t)((ppb < kCpChunk ? ppb : kCpChunk) + 1) * sizeof(double);
+    static bool cp_attr = false;
+    cudaError_t e = cudaSuccess;
+    if (!cp_attr) {
+      e = cudaFuncSetAttribute(cheb_project_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                               (int)((kCpBins + kCpMaxNc) * (kCpChunk + 1) * sizeof(double)));
+      cp_attr = e == cudaSuccess;
+    }
+    if (e == cudaSuccess) {
+      cheb_project_kernel<<<(unsigned)((n_bins + kCpBins - 1) / kCpBins), 128, cp_bytes, st>>>(a.ln_out, P, n_bins, ppb, n_c,
+                                                                                                coef_out);
+      e = cudaGetLastError();
+    }
+    if (e != cudaSuccess) rc = cuda_fail(e, "cheb_project_kernel launch");
+  }
+  pool_free(ln_buf, st);
+  return rc;
 }
 
 extern "C" int hk_kdist(const double *kappa, int64_t n_points, double dnu, double bin_width, int n_g, double *k_out,
