@@ -56,6 +56,10 @@ def lib():
         L.orc_opacity_points_full.restype = C.c_int
         L.orc_opacity_points_full.argtypes = [_dp] * 8 + [_i64, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double,
                                               _i64, C.c_double, C.c_double, C.c_double, C.c_double, C.POINTER(_i64), _i64, _dp]
+        L.orc_opacity_points_rel.restype = C.c_int
+        L.orc_opacity_points_rel.argtypes = [_dp] * 8 + [_i64, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double,
+                                             _i64, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double,
+                                             C.POINTER(_i64), _i64, _dp]
         L.orc_kdist.restype = C.c_int
         L.orc_kdist.argtypes = [_dp, _i64, _i64, C.c_int, _dp]
         _lib = L
@@ -150,20 +154,22 @@ def opacity_points(nu0, S, gamma0, T, P_atm, nu_min, nu_max, dnu, cutoff, js, ma
 
 
 def opacity_full(nu0, S, gamma_air, T, P_atm, nu_min, nu_max, dnu, cutoff, mass_amu=18.0, gamma_self=None, A21=None,
-                 delta=None, n_T=None, E_low=None, q_ratio=1.0, self_fraction=0.5, abundance=1.0, js=None):
+                 delta=None, n_T=None, E_low=None, q_ratio=1.0, self_fraction=0.5, abundance=1.0, js=None,
+                 cutoff_widths=0.0):
     """kappa with the full line physics of eqs. 20-21 (PAPER.md:185-189) and an abundance weight (PAPER.md:133-135);
-    on the whole grid, or at the grid indices `js`."""
+    on the whole grid, or at the grid indices `js`.  cutoff_widths > 0: line i is truncated at
+    min(cutoff, cutoff_widths * gamma_i) ("500 Lorentz widths", PAPER.md:207, 253)."""
     f = lambda a: None if a is None else _arr(a)
     nu0, S, gamma_air = _arr(nu0), _arr(S), _arr(gamma_air)
     gamma_self, A21, delta, n_T, E_low = f(gamma_self), f(A21), f(delta), f(n_T), f(E_low)
     N = grid_size(nu_min, nu_max, dnu)
     js = np.arange(N, dtype=np.int64) if js is None else np.ascontiguousarray(js, dtype=np.int64)
     out = np.empty(js.size, dtype=np.float64)
-    rc = lib().orc_opacity_points_full(_p(nu0), _p(S), _p(gamma_air), _p(gamma_self), _p(A21), _p(delta), _p(n_T), _p(E_low),
-                                       nu0.size, T, P_atm, self_fraction, abundance, nu_min, N, dnu, cutoff, mass_amu,
-                                       q_ratio, js.ctypes.data_as(C.POINTER(_i64)), js.size, _p(out))
+    rc = lib().orc_opacity_points_rel(_p(nu0), _p(S), _p(gamma_air), _p(gamma_self), _p(A21), _p(delta), _p(n_T), _p(E_low),
+                                      nu0.size, T, P_atm, self_fraction, abundance, nu_min, N, dnu, cutoff, cutoff_widths,
+                                      mass_amu, q_ratio, js.ctypes.data_as(C.POINTER(_i64)), js.size, _p(out))
     if rc != 0:
-        raise ValueError(f"orc_opacity_points_full: error {rc}")
+        raise ValueError(f"orc_opacity_points_rel: error {rc}")
     return out
 
 

@@ -267,6 +267,12 @@ double orc_voigt_V(double dv, double alpha, double gamma)
 }
 
 /* kappa_out[k] = kappa(nu_{js[k]}) for an arbitrary list of grid indices.  Lines may come in any order. */
+int orc_opacity_points_rel(const double *nu0_in, const double *S, const double *gamma0, const double *gamma_self,
+                           const double *A21, const double *delta, const double *n_T, const double *E_low,
+                           int64_t n_lines, double T, double P_atm, double self_fraction, double abundance, double nu_min,
+                           int64_t N, double dnu, double cutoff, double cutoff_widths, double mass_amu, double q_ratio,
+                           const int64_t *js, int64_t n_js, double *kappa_out);
+
 /* Full line physics: eq. 20 with the natural width A21/(4 pi c), air and self
  * broadening, P_self = self_fraction * P ("in equal proportions (P_self = 0.5 P)"), P0 = 1 atm:
  *     gamma = A21/(4 pi c) + (T/T0)^(-n) [ gamma_air (P - P_self)/P0 + gamma_self P_self/P0 ]
@@ -279,6 +285,20 @@ int orc_opacity_points_full(const double *nu0_in, const double *S, const double 
                             int64_t n_lines, double T, double P_atm, double self_fraction, double abundance, double nu_min,
                             int64_t N, double dnu, double cutoff, double mass_amu, double q_ratio, const int64_t *js,
                             int64_t n_js, double *kappa_out)
+{
+    return orc_opacity_points_rel(nu0_in, S, gamma0, gamma_self, A21, delta, n_T, E_low, n_lines, T, P_atm, self_fraction,
+                                  abundance, nu_min, N, dnu, cutoff, 0.0, mass_amu, q_ratio, js, n_js, kappa_out);
+}
+
+/* The same with a RELATIVE line-wing cutoff ("an ad hoc cutoff of 500 Lorentz widths"):
+ * cutoff_widths > 0 truncates line i at min(cutoff, cutoff_widths * gamma_i), gamma_i the Lorentz half-width of eq. 20
+ * (reading C5: the absolute cutoff stays as an upper bound; pass a large one for a purely relative cutoff).
+ * cutoff_widths == 0: the absolute cutoff alone. */
+int orc_opacity_points_rel(const double *nu0_in, const double *S, const double *gamma0, const double *gamma_self,
+                           const double *A21, const double *delta, const double *n_T, const double *E_low,
+                           int64_t n_lines, double T, double P_atm, double self_fraction, double abundance, double nu_min,
+                           int64_t N, double dnu, double cutoff, double cutoff_widths, double mass_amu, double q_ratio,
+                           const int64_t *js, int64_t n_js, double *kappa_out)
 {
     if (n_lines < 0 || !(T > 0.0) || !(P_atm > 0.0) || !(dnu > 0.0) || !(cutoff > 0.0) || N <= 0 || !(mass_amu > 0.0) ||
         n_js < 0 || (n_js > 0 && (!js || !kappa_out)))
@@ -302,7 +322,9 @@ int orc_opacity_points_full(const double *nu0_in, const double *S, const double 
         if (A21) L[i].gamma += A21[i] / (4.0 * 3.14159265358979323846 * ORC_C_LIGHT);     /* natural width */
         double s = E_low ? orc_line_strength(S[i], nu0, E_low[i], T, q_ratio) : S[i];
         L[i].amp = abundance * s / m_g;
-        orc_window(nu0, nu_min, N, dnu, cutoff, &L[i].jlo, &L[i].jhi);
+        double cut = cutoff;
+        if (cutoff_widths > 0.0 && cutoff_widths * L[i].gamma < cut) cut = cutoff_widths * L[i].gamma;
+        orc_window(nu0, nu_min, N, dnu, cut, &L[i].jlo, &L[i].jhi);
         L[i].src = i;
     }
     int sorted = 1;

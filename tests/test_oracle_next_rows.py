@@ -161,3 +161,30 @@ def test_abundance_weight_and_mixing_is_linear():
     assert np.abs(kx / (0.25 * k1) - 1.0).max() < 1e-14
     js = np.array([0, 17, 5000, 9999])
     assert np.array_equal(oracle.opacity_full(nu0, S, ga, 800.0, 0.5, *GRID, js=js, **kw), k1[js])
+
+
+# ---- f4: relative line-wing cutoff --------------------------------------------------------------------
+def test_relative_cutoff_support_and_reductions():
+    nu0, S, ga, gs, A, dl, nT = _draw(n=40, seed=9)
+    T, P, W = 296.0, 1.0, 40.0                     # gamma_i = ga_i at 296 K, 1 atm (simple law): W gamma = 0.8 .. 4 cm^-1
+    k_abs = oracle.opacity(nu0, S, ga, T, P, *GRID)
+    # a relative cutoff wider than the absolute one never binds
+    assert np.array_equal(oracle.opacity_full(nu0, S, ga, T, P, *GRID, cutoff_widths=1e6), k_abs)
+    assert np.array_equal(oracle.opacity_full(nu0, S, ga, T, P, *GRID, cutoff_widths=0.0), k_abs)
+    # single lines: the support is |nu_j - nu0| <= W gamma exactly (brute force on the grid), the values inside are untouched
+    nu = np.arange(10000) * 0.01
+    for i in (0, 7, 23):
+        k = oracle.opacity_full(nu0[i:i + 1], S[i:i + 1], ga[i:i + 1], T, P, 0.0, 100.0, 0.01, 1e4, cutoff_widths=W)
+        full = oracle.opacity(nu0[i:i + 1], S[i:i + 1], ga[i:i + 1], T, P, 0.0, 100.0, 0.01, 1e4)
+        lo = np.ceil(((nu0[i] - W * ga[i]) - 0.0) / 0.01)
+        hi = np.floor(((nu0[i] + W * ga[i]) - 0.0) / 0.01)
+        inside = (np.arange(10000) >= lo) & (np.arange(10000) <= hi)
+        assert np.array_equal(k != 0.0, inside) and np.array_equal(k[inside], full[inside])
+        assert abs(inside.sum() - 2 * W * ga[i] / 0.01) <= 2
+    # the sum over lines of the single-line results is the multi-line result (each line keeps its own cutoff)
+    parts = sum(oracle.opacity_full(nu0[i:i + 1], S[i:i + 1], ga[i:i + 1], T, P, *GRID, cutoff_widths=W) for i in range(40))
+    allk = oracle.opacity_full(nu0, S, ga, T, P, *GRID, cutoff_widths=W)
+    assert np.abs(allk - parts).max() <= 1e-12 * allk.max()
+    # the absolute cutoff stays an upper bound: min(cutoff, W gamma)
+    capped = oracle.opacity_full(nu0[:1], S[:1], ga[:1], T, P, 0.0, 100.0, 0.01, 3.0, cutoff_widths=W)
+    assert np.count_nonzero(capped) == np.count_nonzero(oracle.opacity(nu0[:1], S[:1], ga[:1], T, P, 0.0, 100.0, 0.01, 3.0))
