@@ -75,6 +75,10 @@ typedef struct {
                            gamma_self != NULL                                                         */
   double abundance;     /* X_s: the species' opacity is multiplied by it (kappa = sum_s X_s kappa_s);
                            0 means 1, so that a zero-initialised tail keeps the one-species behaviour          */
+  double cutoff_widths; /* relative line-wing cutoff ("500 Lorentz widths"): > 0 truncates line i at
+                           min(cutoff, cutoff_widths * gamma_i), gamma_i the Lorentz half-width of eq. 20 at (T, P);
+                           0: the absolute cutoff alone.  The absolute `cutoff` stays the upper bound (and sizes the line
+                           ranges the kernels scan: keep it near cutoff_widths * max gamma for speed)            */
   int accumulate;       /* 0: kappa_out is overwritten.  1: X_s kappa_s is ADDED to kappa_out — the species are summed
                            BEFORE the sort, as PAPER.md:135 requires; the first species of a mixture passes 0     */
 } hk_params;
@@ -88,7 +92,8 @@ int64_t hk_grid_size(double nu_min, double nu_max, double dnu);
  *   alpha_i = (nu0_i/c) sqrt(2 k_B T/m)  [= Gamma_D/sqrt(ln 2)]
  *   S_i(T)  = S_i, or eq. 18 (T0 = 296 K in the last denominator) when E_low != NULL, with
  *             c2 = hc/k_B = 1.4388 cm K
- *   window  : line i contributes to j_lo(i) <= j <= j_hi(i),
+ *   window  : line i contributes to j_lo(i) <= j <= j_hi(i)  (cutoff -> min(cutoff, cutoff_widths*gamma_i) when
+ *             prm->cutoff_widths > 0),
  *             j_lo = max(0, ceil(((nu0-cutoff)-nu_min)/dnu)), j_hi = min(N-1, floor(((nu0+cutoff)-nu_min)/dnu))
  *             (inclusive, decided in index space; hard truncation, no renormalisation)
  *   kappa_j = sum_{i in window} (S_i(T)/(m*amu)) * K(x_ij, y_i)/(alpha_i sqrt(pi)),  x = (nu_j-nu0)/alpha, y = gamma/alpha
@@ -116,7 +121,8 @@ int64_t hk_grid_size(double nu_min, double nu_max, double dnu);
  * kappa_out: device, N doubles, overwritten.  Lines outside [nu_min, nu_max) still contribute if within the
  * cutoff.  n_lines == 0 gives kappa == 0.
  * HK_ERR_INVALID: NULL lines/prm/kappa_out or (n_lines > 0 and NULL nu0/S/gamma0); n_lines < 0; T, P_atm, dnu,
- * cutoff, mass_amu not > 0 or not finite; N < 1 or N > 2^30; precision unknown; abundance < 0 or not finite;
+ * cutoff, mass_amu not > 0 or not finite; N < 1 or N > 2^30; precision unknown; abundance or cutoff_widths < 0 or
+ * not finite;
  * self_fraction outside [0,1] when gamma_self != NULL.
  * Asynchronous on prm->stream (synchronises once when lines_sorted = 0).  nu0 must be ascending when
  * lines_sorted = 1 (see hk_lines_check_sorted). */

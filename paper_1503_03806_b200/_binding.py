@@ -30,12 +30,14 @@ class _hk_lines(C.Structure):
 
 class _hk_params(C.Structure):
     _fields_ = [("mass_amu", C.c_double), ("q_ratio", C.c_double), ("precision", C.c_int), ("lines_sorted", C.c_int),
-                ("stream", C.c_void_p), ("self_fraction", C.c_double), ("abundance", C.c_double), ("accumulate", C.c_int)]
+                ("stream", C.c_void_p), ("self_fraction", C.c_double), ("abundance", C.c_double), ("cutoff_widths", C.c_double),
+                ("accumulate", C.c_int)]
 
 
-def _params(mass_amu, q_ratio, precision, lines_sorted, stream, self_fraction=0.5, abundance=1.0, accumulate=False):
+def _params(mass_amu, q_ratio, precision, lines_sorted, stream, self_fraction=0.5, abundance=1.0, accumulate=False,
+            cutoff_widths=0.0):
     return _hk_params(float(mass_amu), float(q_ratio), int(precision), int(bool(lines_sorted)), _stream_ptr(stream),
-                      float(self_fraction), float(abundance), int(bool(accumulate)))
+                      float(self_fraction), float(abundance), float(cutoff_widths), int(bool(accumulate)))
 
 
 _lib = None
@@ -214,7 +216,8 @@ def hk_gauss_legendre(n_g: int):
 
 
 def hk_opacity(lines: Lines, T, P_atm, nu_min, nu_max, dnu, cutoff, mass_amu=18.0, q_ratio=1.0, lines_sorted=True,
-               out=None, stream=None, precision=HK_FP64, self_fraction=0.5, abundance=1.0, accumulate=False):
+               out=None, stream=None, precision=HK_FP64, self_fraction=0.5, abundance=1.0, accumulate=False,
+               cutoff_widths=0.0):
     """kappa[N] on the device (hk_opacity of include/hk.h).  Asynchronous on the current (or given) torch stream.
     accumulate=True adds abundance * kappa of this species to `out` (mixtures)."""
     torch = _torch()
@@ -227,7 +230,7 @@ def hk_opacity(lines: Lines, T, P_atm, nu_min, nu_max, dnu, cutoff, mass_amu=18.
     elif N >= 1 and int(out.numel()) != N:       # (N < 1: let the library report HK_ERR_INVALID)
         raise ValueError(f"out has {int(out.numel())} entries, the grid has {N}")
     cl = lines._c()
-    prm = _params(mass_amu, q_ratio, precision, lines_sorted, stream, self_fraction, abundance, accumulate)
+    prm = _params(mass_amu, q_ratio, precision, lines_sorted, stream, self_fraction, abundance, accumulate, cutoff_widths)
     _check(L.hk_opacity(C.byref(cl), lines.n, T, P_atm, nu_min, nu_max, dnu, cutoff, _dev_ptr(out, "out"), C.byref(prm)),
            "hk_opacity")
     return out
@@ -350,11 +353,11 @@ class Context:
     """hk_create / hk_opacity_ctx / hk_destroy: line list bound once, scratch kept across (T,P) calls."""
 
     def __init__(self, lines: Lines, mass_amu=18.0, lines_sorted=True, stream=None, precision=HK_FP64, self_fraction=0.5,
-                 abundance=1.0, accumulate=False):
+                 abundance=1.0, accumulate=False, cutoff_widths=0.0):
         self._lines = lines      # keep the tensors alive
         self._h = C.c_void_p()
         cl = lines._c()
-        prm = _params(mass_amu, 1.0, precision, lines_sorted, stream, self_fraction, abundance, accumulate)
+        prm = _params(mass_amu, 1.0, precision, lines_sorted, stream, self_fraction, abundance, accumulate, cutoff_widths)
         _check(load_library().hk_create(C.byref(cl), lines.n, C.byref(prm), C.byref(self._h)), "hk_create")
 
     def opacity(self, T, P_atm, nu_min, nu_max, dnu, cutoff, q_ratio=1.0, out=None):
@@ -396,7 +399,7 @@ def _host_ptr(t, name, allow_none=False):
 def hk_opacity_host(nu0, S, gamma0, T, P_atm, nu_min, nu_max, dnu, cutoff, mass_amu=18.0, n_T=None, E_low=None, q_ratio=1.0,
                     lines_sorted=True, bin_width=None, n_g=20, kappa_out=None, k_out=None, want_kappa=True, stream=None,
                     precision=HK_FP64, gamma_self=None, A21=None, delta=None, self_fraction=0.5, abundance=1.0,
-                    accumulate=False):
+                    accumulate=False, cutoff_widths=0.0):
     """End-to-end call with HOST buffers (hk_opacity_host of include/hk.h): host line arrays -> device, hk_opacity
     (+ hk_kdist when bin_width is given), kappa / k-table -> host.  Buffers are host torch tensors (pinned for
     asynchronous copies) or numpy arrays.  Returns (kappa_host or None, k_host or None).  Synchronous."""
@@ -425,7 +428,7 @@ def hk_opacity_host(nu0, S, gamma0, T, P_atm, nu_min, nu_max, dnu, cutoff, mass_
     cl = _hk_lines(_host_ptr(nu0, "nu0"), _host_ptr(S, "S"), _host_ptr(gamma0, "gamma0"), _host_ptr(n_T, "n_T", True),
                    _host_ptr(E_low, "E_low", True), _host_ptr(gamma_self, "gamma_self", True), _host_ptr(A21, "A21", True),
                    _host_ptr(delta, "delta", True))
-    prm = _params(mass_amu, q_ratio, precision, lines_sorted, stream, self_fraction, abundance, accumulate)
+    prm = _params(mass_amu, q_ratio, precision, lines_sorted, stream, self_fraction, abundance, accumulate, cutoff_widths)
     _check(L.hk_opacity_host(C.byref(cl), n, T, P_atm, nu_min, nu_max, dnu, cutoff, _host_ptr(kappa_out, "kappa_out", True),
                              float(bin_width or 0.0), int(n_g), _host_ptr(k_out, "k_out", True), C.byref(prm)),
            "hk_opacity_host")

@@ -75,6 +75,7 @@ struct PrepArgs {
   const double *nu0, *S, *gamma0, *n_T, *E_low;
   const double *gamma_self, *A21;  // eq. 20 (either may be NULL); the shift of eq. 21 is applied before a1
   double self_fraction, abundance;
+  double cutoff_widths;  // > 0: line i is truncated at min(cutoff, cutoff_widths * gamma_i)
   int64_t n;
   double T, P_atm, tfac_half;  // (296/T)^0.5 for n_T == NULL
   double vth;                  // sqrt(2 kB T/m)/c : alpha = nu0*vth
@@ -100,10 +101,10 @@ struct PrepArgs {
 constexpr int kPlanBlock = 256;  // granularity of the line-range lookup and of the cost model of a2
 
 // index window of a line: sub, sub, IEEE divide, ceil/floor — no multiply-add, nothing to contract (A4)
-__device__ __forceinline__ void line_window(double nu0, const PrepArgs &a, int &jlo, int &jhi)
+__device__ __forceinline__ void line_window(double nu0, double cutoff, const PrepArgs &a, int &jlo, int &jhi)
 {
-  double lo = ceil(__ddiv_rn(__dsub_rn(__dsub_rn(nu0, a.cutoff), a.nu_min), a.dnu));
-  double hi = floor(__ddiv_rn(__dsub_rn(__dadd_rn(nu0, a.cutoff), a.nu_min), a.dnu));
+  double lo = ceil(__ddiv_rn(__dsub_rn(__dsub_rn(nu0, cutoff), a.nu_min), a.dnu));
+  double hi = floor(__ddiv_rn(__dsub_rn(__dadd_rn(nu0, cutoff), a.nu_min), a.dnu));
   if (!(lo > 0.0)) lo = 0.0;
   if (!(hi < (double)(a.N - 1))) hi = (double)(a.N - 1);
   if (lo > 2.0e9) lo = 2.0e9;
@@ -172,27 +173,33 @@ __global__ void __launch_bounds__(256) line_prep_kernel(PrepArgs a)
   k.Acore = amp * g.inv_alpha * kInvSqrtPi;
   MetaA ma;
   MetaB mb;
-  line_window(nu0, a, ma.jlo, ma.jhi);
+  // relative cutoff: the line's own window is narrower than the window of the absolute cutoff; the a2 tables are built from
+  // the latter (qlo, qhi: non-decreasing in i, a superset), classify32 masks with the former
+  double cut = a.cutoff;
+  if (a.cutoff_widths > 0.0) cut = fmin(cut, __dmul_rn(a.cutoff_widths, gamma));
+  line_window(nu0, cut, a, ma.jlo, ma.jhi);
+  int qlo, qhi;
+  line_window(nu0, a.cutoff, a, qlo, qhi);
   {
     // a2, line-parallel half: the list is ordered by nu0, so jlo and jhi are non-decreasing in i and line i is the
     // "first line with jhi >= b*kPlanBlock" exactly for the blocks b with jhi_{i-1} < b*kPlanBlock <= jhi_i (same for jlo).
     // Each entry of first_hi / first_lo has exactly one writer; the last line also fills the blocks beyond its window.
     int plo = INT_MIN, phi = INT_MIN, pc = INT_MIN;
     if (i > 0) {
-      line_window(a.nu0[i - 1], a, plo, phi);
+      line_window(a.nu0[i - 1], a.cutoff, a, plo, phi);
       pc = line_centre_index(a.nu0[i - 1], a);
     }
     const int jc = line_centre_index(nu0, a);
     const int n = (int)a.n;
-    int b0 = i > 0 ? max(plan_block_floor(phi) + 1, 0) : 0, b1 = min(plan_block_floor(ma.jhi), a.nb);
+    int b0 = i > 0 ? max(plan_block_floor(phi) + 1, 0) : 0, b1 = min(plan_block_floor(qhi), a.nb);
     for (int b = b0; b <= b1; ++b) a.first_hi[b] = (int)i;
     if (i == n - 1)
-      for (int b = max(plan_block_floor(ma.jhi) + 1, 0); b <= a.nb; ++b) a.first_hi[b] = n;
+      for (int b = max(plan_block_floor(qhi) + 1, 0); b <= a.nb; ++b) a.first_hi[b] = n;
     b0 = i > 0 ? max(plan_block_floor(plo) + 1, 0) : 0;
-    b1 = min(plan_block_floor(ma.jlo), a.nb);
+    b1 = min(plan_block_floor(qlo), a.nb);
     for (int b = b0; b <= b1; ++b) a.first_lo[b] = (int)i;
     if (i == n - 1)
-      for (int b = max(plan_block_floor(ma.jlo) + 1, 0); b <= a.nb; ++b) a.first_lo[b] = n;
+      for (int b = max(plan_block_floor(qlo) + 1, 0); b <= a.nb; ++b) a.first_lo[b] = n;
     b0 = i > 0 ? max(plan_block_floor(pc) + 1, 0) : 0;
     b1 = min(plan_block_floor(jc), a.nb);
     for (int b = b0; b <= b1; ++b) a.first_c[b] = (int)i;
@@ -1081,6 +1088,7 @@ static int validate(const hk_lines *lines, int64_t n_lines, double T, double P_a
   if (prm->precision != HK_FP64 && prm->precision != HK_FP32) return HK_ERR_INVALID;
   if (lines->E_low && !pos_finite(prm->q_ratio)) return HK_ERR_INVALID;
   if (!(prm->abundance >= 0.0) || !isfinite(prm->abundance)) return HK_ERR_INVALID;
+  if (!(prm->cutoff_widths >= 0.0) || !isfinite(prm->cutoff_widths)) return HK_ERR_INVALID;
   if (lines->gamma_self && !(prm->self_fraction >= 0.0 && prm->self_fraction <= 1.0)) return HK_ERR_INVALID;
   const int64_t N = hk_grid_size(nu_min, nu_max, dnu);
   if (N < 1 || N > (1LL << 30)) return HK_ERR_INVALID;
@@ -1116,6 +1124,7 @@ static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double 
   pa.nu0 = lines->nu0; pa.S = lines->S; pa.gamma0 = lines->gamma0; pa.n_T = lines->n_T; pa.E_low = lines->E_low;
   pa.gamma_self = lines->gamma_self; pa.A21 = lines->A21;
   pa.self_fraction = prm.self_fraction; pa.abundance = prm.abundance > 0.0 ? prm.abundance : 1.0;
+  pa.cutoff_widths = prm.cutoff_widths;
   pa.n = n_lines;
   pa.T = T; pa.P_atm = P_atm; pa.tfac_half = pow(kT0 / T, 0.5);
   const double m_g = mass_amu * kAmu;

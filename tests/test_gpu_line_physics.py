@@ -105,3 +105,30 @@ def test_context_rejects_a_pressure_shift_and_bad_fractions():
     ctx.close()
     _check(got, oracle.opacity_full(wl.nu0, wl.S, wl.gamma0, 1000.0, 1.0, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff,
                                     gamma_self=ex["gamma_self"], self_fraction=0.3), BAR)
+
+
+@pytest.mark.parametrize("T,P,W,cap", [(1500.0, 1.0, 500.0, 25.0), (296.0, 1.0, 40.0, 25.0), (1000.0, 30.0, 20.0, 100.0),
+                                         (2000.0, 0.01, 500.0, 3.0)])
+def test_relative_cutoff_in_lorentz_widths(T, P, W, cap):
+    # line i truncated at min(cap, W gamma_i); windows are no longer ordered like the centres
+    import torch
+    wl = workloads.small(seed=71, n_lines=2500, nu_max=300.0, cutoff=cap)
+    ex = _fields(wl, 72)
+    lines = hk.Lines.from_numpy(wl.nu0, wl.S, wl.gamma0, gamma_self=ex["gamma_self"])
+    ref = oracle.opacity_full(wl.nu0, wl.S, wl.gamma0, T, P, wl.nu_min, wl.nu_max, wl.dnu, cap, gamma_self=ex["gamma_self"],
+                              cutoff_widths=W)
+    ref_abs = oracle.opacity_full(wl.nu0, wl.S, wl.gamma0, T, P, wl.nu_min, wl.nu_max, wl.dnu, cap, gamma_self=ex["gamma_self"])
+    for prec, bar in ((hk.HK_FP64, BAR), (hk.HK_FP32, BAR32)):
+        got = hk.hk_opacity(lines, T, P, wl.nu_min, wl.nu_max, wl.dnu, cap, cutoff_widths=W, precision=prec)
+        torch.cuda.synchronize()
+        _check(got.cpu().numpy(), ref, bar)
+    if W * 0.02 * P * (296.0 / T) ** 0.5 < cap:
+        assert not np.array_equal(ref, ref_abs)                      # the relative cutoff binds for some line
+    # single line: bit-exact support (index work in FP64 on both sides)
+    one = hk.Lines.from_numpy(wl.nu0[100:101], wl.S[100:101], wl.gamma0[100:101])
+    got1 = hk.hk_opacity(one, 296.0, 1.0, wl.nu_min, wl.nu_max, wl.dnu, cap, cutoff_widths=W).cpu().numpy()
+    ref1 = oracle.opacity_full(wl.nu0[100:101], wl.S[100:101], wl.gamma0[100:101], 296.0, 1.0, wl.nu_min, wl.nu_max, wl.dnu, cap,
+                               cutoff_widths=W)
+    assert np.array_equal(got1 != 0.0, ref1 != 0.0)
+    with pytest.raises(hk.HKError):
+        hk.hk_opacity(one, 296.0, 1.0, wl.nu_min, wl.nu_max, wl.dnu, cap, cutoff_widths=-1.0)
