@@ -42,6 +42,7 @@ WORKLOAD = "BASELINE.json configs[1]: 1e5 lines, 3e6 grid points, cutoff 100 cm^
 
 # FP64-pipe thread-instructions the method needs per line-point evaluation, by regime (counted from
 # the formulas of hk_voigt.cuh with the Newton reciprocal; these are the algorithmic figures, not the executed SASS).
+# gh1 = the 1-point rule with the shifted denominator (from r^2 >= max(3600, 4100 y)), gh2 the shell between 3200 and that.
 FP64_INST_PER_EVAL = {"gh1": 5.0, "gh2": 7.0, "gh3": 11.0, "gh6": 22.0, "series": 150.0}
 # --precision fp32: FP32-pipe thread-instructions per evaluation of the two rules the far kernel runs in float, two points per
 # reciprocal (hk_voigt.cuh gh1_acc2f / gh2_acc2f: 8 and 13 per pair, + 1 MUFU.RCP per pair)

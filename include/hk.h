@@ -99,7 +99,8 @@ int64_t hk_grid_size(double nu_min, double nu_max, double dnu);
  *   kappa_j = sum_{i in window} (S_i(T)/(m*amu)) * K(x_ij, y_i)/(alpha_i sqrt(pi)),  x = (nu_j-nu0)/alpha, y = gamma/alpha
  *
  * K = Re w(x+iy) is evaluated to <= 2.5e-7 relative error: Algorithm-916-type series for x^2+y^2 < 44,
- * 6/3/2/1-point Gauss-Hermite rules beyond 44 / 280 / 3200 / 6e6.
+ * 6/3/2-point Gauss-Hermite rules beyond 44 / 280 / 3200, and from max(3600, 4100 y) the 1-point rule with the
+ * shifted denominator x^2 + y^2 - 3/2.
  *
  * Full line physics, active per optional array of hk_lines:
  *   gamma_i = A21_i/(4 pi c) + (296/T)^n_i [ gamma0_i (P - P_self) + gamma_self_i P_self ],  P_self = self_fraction * P   eq. 20
@@ -112,7 +113,7 @@ int64_t hk_grid_size(double nu_min, double nu_max, double dnu);
  * approximation).
  *
  * prm->precision = HK_FP32 (north_star's optional FP32 variant, max relative error <= 1e-4): the same ladder with the
- * switches at 44 / 64 / 300 / 4e4 (each rule <= 4e-5 from exact K); the 1- and 2-point rules — every (line, 256-point
+ * switches at 44 / 64 / 300 / max(400, 400 y) (each rule <= 4e-5 from exact K); the 1- and 2-point rules — every (line, 256-point
  * span) pair beyond the 2-point radius, ~99 % of all evaluations — run in FP32 (distances from an integer + fraction
  * split of the line centre in grid units, a float partial sum per 32 lines added to FP64 accumulators); the 3-/6-point
  * rules and the series near the centre stay FP64, as do line prep, the index windows and kappa_out.  Line amplitudes

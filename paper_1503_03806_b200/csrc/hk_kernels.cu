@@ -84,7 +84,8 @@ struct PrepArgs {
   double nu_min, dnu, cutoff;
   int N;
   double margin;  // grid units added to every regime radius: covers the float rounding of c and of the span ends
-  double R1, R2, R3;  // switch radii on r^2 of the 1-, 2-, 3-point rule (kR1.. for FP64, kR1f.. for the FP32 variant)
+  double R2, R3;      // switch radii on r^2 of the 2-, 3-point rule (kR2.. for FP64, kR2f.. for the FP32 variant)
+  int f32_ladder;     // the 1-point rule's switch is r1_sq(y, f32_ladder)
   LineF32 *f32;       // FP32 variant only (else NULL)
   MetaA *ma;
   MetaB *mb;
@@ -210,7 +211,7 @@ __global__ void __launch_bounds__(256) line_prep_kernel(PrepArgs a)
   double c = (nu0 - a.nu_min) * inv_dnu;
   c = fmin(fmax(c, -3.0e9), 3.0e9);
   ma.c = (float)c;
-  mb.r1 = radius_grid(a.R1, a2, g2, inv_dnu, a.margin);
+  mb.r1 = alpha > 0.0 ? radius_grid(r1_sq(k.y, a.f32_ladder != 0), a2, g2, inv_dnu, a.margin) : 0.0f;
   mb.r2 = radius_grid(a.R2, a2, g2, inv_dnu, a.margin);
   ma.r3 = radius_grid(a.R3, a2, g2, inv_dnu, a.margin);
   mb.r6 = radius_grid(kRc, a2, g2, inv_dnu, a.margin);
@@ -528,7 +529,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) voigt_far_kernel(const __gri
 #pragma unroll
           for (int k = 0; k < P; k += 2)
             gh1_acc2f(af[k], af[k + 1], (k == 0 ? d0 : fmaf((float)(32 * k), a.dnu_f, d0)),
-                      fmaf((float)(32 * k + 32), a.dnu_f, d0), w, L.g2);
+                      fmaf((float)(32 * k + 32), a.dnu_f, d0), w, fmaf(-1.5f, L.a2, L.g2));
         }
 #pragma unroll 1
         for (unsigned m = M.m2; m; m &= m - 1) {
@@ -557,7 +558,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) voigt_far_kernel(const __gri
           for (int k = 0; k < P; k += 2) {
             float t0 = 0.0f, t1 = 0.0f;
             const float da = (k == 0 ? d0 : fmaf((float)(32 * k), a.dnu_f, d0)), db = fmaf((float)(32 * k + 32), a.dnu_f, d0);
-            if (one) gh1_acc2f(t0, t1, da, db, w, L.g2);
+            if (one) gh1_acc2f(t0, t1, da, db, w, fmaf(-1.5f, L.a2, L.g2));
             else gh2_acc2f(t0, t1, da, db, w, L.e2, L.f2, wa2);
             af[k] += ((unsigned)(jrel + 32 * k) <= wlen) ? t0 : 0.0f;
             af[k + 1] += ((unsigned)(jrel + 32 * k + 32) <= wlen) ? t1 : 0.0f;
@@ -577,7 +578,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) voigt_far_kernel(const __gri
 #pragma unroll 1
       for (unsigned m = M.m1; m; m &= m - 1) {
         const LineBase *pb = sbase + b0 + (__ffs(m) - 1);
-        const double nu0 = pb->nu0, A1 = pb->A1, g2 = pb->g2;
+        const double nu0 = pb->nu0, A1 = pb->A1, g2 = fma(-1.5, pb->a2, pb->g2);  // shifted denominator (kR1a)
         const double d0 = x0 - nu0;
 #pragma unroll
         for (int k = 0; k < P; ++k) acc[k] = gh1_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), A1, g2);
@@ -597,7 +598,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) voigt_far_kernel(const __gri
       for (unsigned m = M.e1; m; m &= m - 1) {
         const int i = b0 + (__ffs(m) - 1);
         const int jlo = S.ma[stage][i].jlo, jhi = S.ma[stage][i].jhi;
-        const double nu0 = sbase[i].nu0, A1 = sbase[i].A1, g2 = sbase[i].g2;
+        const double nu0 = sbase[i].nu0, A1 = sbase[i].A1, g2 = fma(-1.5, sbase[i].a2, sbase[i].g2);
         const double d0 = x0 - nu0;
         const unsigned wlen = (unsigned)(jhi - jlo);
         const int jrel = slo + lane - jlo;
@@ -833,7 +834,7 @@ __global__ void __launch_bounds__(kNearWarps * 32, 4) voigt_near_kernel(const __
 template <bool F32>
 __global__ void __launch_bounds__(128) voigt_K_kernel(const double *x, const double *y, int64_t n, double *out)
 {
-  constexpr double R1 = F32 ? kR1f : kR1, R2 = F32 ? kR2f : kR2, R3 = F32 ? kR3f : kR3;
+  constexpr double R2 = F32 ? kR2f : kR2, R3 = F32 ? kR3f : kR3;
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const bool live = i < n;
   const double xi = live ? fabs(x[i]) : 1.0e3, yi = live ? y[i] : 1.0;
@@ -843,13 +844,13 @@ __global__ void __launch_bounds__(128) voigt_K_kernel(const double *x, const dou
   const double r2 = q + g2;
   double v;
   const bool tiny_gauss = q < gauss_xg2(yi);  // only the 6-point branch adds the Gaussian term (as line_prep arranges)
-  if (r2 >= R1 && !tiny_gauss) {
+  if (r2 >= r1_sq(yi, F32) && !tiny_gauss) {
     if constexpr (F32) {  // the far kernel's float arithmetic; the partner point of the pair is a dummy
       float v0 = 0.0f, v1 = 0.0f;
-      gh1_acc2f(v0, v1, (float)xi, 1.0f, (float)A1, (float)g2);
+      gh1_acc2f(v0, v1, (float)xi, 1.0f, (float)A1, fmaf(-1.5f, (float)a2, (float)g2));
       v = (double)v0;
     } else {
-      v = gh1_acc(0.0, xi, A1, g2);
+      v = gh1_acc(0.0, xi, A1, fma(-1.5, a2, g2));
     }
   } else if (r2 >= R2 && !tiny_gauss) {
     if constexpr (F32) {
@@ -1133,7 +1134,7 @@ static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double 
   pa.q_ratio = q_ratio;
   pa.nu_min = nu_min; pa.dnu = dnu; pa.cutoff = cutoff; pa.N = (int)N;
   pa.margin = 2.0 + 2.4e-7 * (double)N;
-  pa.R1 = f32 ? kR1f : kR1; pa.R2 = f32 ? kR2f : kR2; pa.R3 = f32 ? kR3f : kR3;
+  pa.R2 = f32 ? kR2f : kR2; pa.R3 = f32 ? kR3f : kR3; pa.f32_ladder = f32 ? 1 : 0;
   pa.f32 = f32 ? s.f32 : nullptr;
   pa.ma = s.ma; pa.mb = s.mb; pa.base = s.base; pa.gh2 = s.gh2; pa.core = s.core;
   pa.nb = nb; pa.first_hi = s.first_hi; pa.first_lo = s.first_lo; pa.first_c = s.first_c; pa.queue = s.queue;
@@ -1376,8 +1377,7 @@ int hk_regime_census(const double *nu0_host, const double *gamma0_host, int64_t 
                      int64_t counts_out[5])
 {
   if (precision != HK_FP64 && precision != HK_FP32) return HK_ERR_INVALID;
-  const double R1 = precision == HK_FP32 ? kR1f : kR1, R2 = precision == HK_FP32 ? kR2f : kR2,
-               R3 = precision == HK_FP32 ? kR3f : kR3;
+  const double R2 = precision == HK_FP32 ? kR2f : kR2, R3 = precision == HK_FP32 ? kR3f : kR3;
   if (!nu0_host || !gamma0_host || !counts_out || n_lines < 0 || N < 1 || !pos_finite(T) || !pos_finite(P_atm) ||
       !pos_finite(mass_amu) || !pos_finite(dnu) || !pos_finite(cutoff))
     return HK_ERR_INVALID;
@@ -1405,7 +1405,9 @@ int hk_regime_census(const double *nu0_host, const double *gamma0_host, int64_t 
     const double gamma = gamma0_host[i] * P_atm * tfac, a2 = alpha * alpha, g2 = gamma * gamma, y = gamma / alpha;
     auto rho = [&](double R) { const double t = R * a2 - g2; return t > 0.0 ? sqrt(t) : 0.0; };
     const double xc2 = core_xc2(y);
-    const int64_t n1 = within(nu0, rho(R1), jl, jh), n2 = within(nu0, rho(R2), jl, jh), n3 = within(nu0, rho(R3), jl, jh);
+    const double R1 = r1_sq(y, precision == HK_FP32);
+    const int64_t n2 = within(nu0, rho(R2), jl, jh), n3 = within(nu0, rho(R3), jl, jh);
+    const int64_t n1 = std::max(within(nu0, rho(R1), jl, jh), n2);  // the 2-point rule fills [R2, R1) when R1 > R2
     const int64_t nc = xc2 > 0.0 ? within(nu0, sqrt(xc2) * alpha, jl, jh) : 0;
     const int64_t ncore = nc < n3 ? nc : n3;
     c[0] += tot - n1; c[1] += n1 - n2; c[2] += n2 - n3; c[3] += n3 - ncore; c[4] += ncore;

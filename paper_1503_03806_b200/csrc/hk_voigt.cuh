@@ -5,7 +5,7 @@
 // is evaluated in one of five regimes chosen on r^2 = x^2 + y^2 (PAPER.md:197 gives the three-regime
 // structure and calls its switch points "trial-and-error"; DESIGN.md §4 derives these):
 //
-//   r^2 >= 6.0e6 : 1-point Gauss-Hermite  (a Lorentzian)                      5 FP64 + 1 MUFU per point
+//   r^2 >= max(3600, 4100 y) : 1-point rule with shifted denominator          5 FP64 + 1 MUFU per point
 //   r^2 >= 3200  : 2-point Gauss-Hermite                                       7 FP64 + 1 MUFU
 //   r^2 >= 280   : 3-point Gauss-Hermite ("third-order", Letchworth & Benner) 11 FP64 + 1 MUFU
 //   r^2 >= 44    : 6-point Gauss-Hermite                                      22 FP64 + 3 MUFU
@@ -23,14 +23,18 @@
 
 namespace hk {
 
-constexpr double kR1 = 6.0e6;   // 1-point rule from here   (max rel. error 2.5e-7 on the ring)
+// 1-point rule with the shifted denominator, K = (y/sqrt(pi)) / (x^2 + y^2 - 3/2)  (V = A1/(d^2 + gamma^2 - 1.5 alpha^2)):
+// the second term of w(z) ~ (i/sqrt(pi)) (1/z)(1 + 1/(2 z^2) + 3/(4 z^4) + ...) folded into the Lorentzian's denominator.  Its
+// relative error is 1.5/x^4 + 2 y^2/r^4 (checked against the oracle: tests/test_rule_accuracy.py), so it serves from
+// r^2 >= max(kR1a, kR1b y) at the cost of the plain 1-point rule (which needs r^2 >= 6e6 for the same accuracy).
+constexpr double kR1a = 3600.0, kR1b = 4100.0;  // 1.2e-7 + 1.2e-7 <= 2.4e-7
 constexpr double kR2 = 3200.0;  // 2-point rule             (2.4e-7)
 constexpr double kR3 = 280.0;   // 3-point rule             (2.4e-7)
 constexpr double kRc = 44.0;    // 6-point rule from here (3.7e-8); series below
 // FP32 variant (hk_params.precision = HK_FP32; north_star: "optional FP32 path", bar 1e-4): the same ladder with the
 // switches moved in to where each rule is <= 4e-5 from exact K (1-point 1.5/x^2, 2-point
 // 2.8e-5 at 300, 3-point 2.2e-5 at 64); the 1- and 2-point rules (the far kernel: ~99 % of all evaluations) run in FP32.
-constexpr double kR1f = 4.0e4;  // 1-point rule from here   (3.8e-5)
+constexpr double kR1fa = 400.0, kR1fb = 400.0;  // shifted 1-point rule from r^2 >= max(400, 400 y)   (9.4e-6 + 1.3e-5)
 constexpr double kR2f = 300.0;  // 2-point rule             (2.8e-5)
 constexpr double kR3f = 64.0;   // 3-point rule             (2.2e-5)
 constexpr double kXgCapSq = 270.0;  // the Gaussian term is never added beyond the 6-point region (exp(-270) = 5e-118)
@@ -51,6 +55,13 @@ constexpr double kAoverPi = 0.2228169203286534700764373;  // a/pi
 constexpr double kT6sq0 = 0.1901635091934881328718554, kW6_0 = 0.4088284695560292260885378;
 constexpr double kT6sq1 = 1.784492748543251591186722, kW6_1 = 0.08861574604191452748085588;
 constexpr double kT6sq2 = 5.525343742263260275941422, kW6_2 = 0.002555784402056246430606291;
+
+// r^2 from which the (shifted) 1-point rule serves a line of damping y
+__device__ __host__ __forceinline__ double r1_sq(double y, bool f32)
+{
+  const double a = f32 ? kR1fa : kR1a, b = (f32 ? kR1fb : kR1b) * y;
+  return a > b ? a : b;
+}
 
 constexpr unsigned kFull = 0xffffffffu;
 
@@ -76,7 +87,7 @@ __device__ __forceinline__ double rcp_nr2(double x)
 }
 
 // ---- wing rules: contribution amp * V(d) added to acc --------------------------------------------------
-// 1-point: A1/(d^2+g2), A1 = amp*gamma/pi
+// 1-point: A1/(d^2+g2s), A1 = amp*gamma/pi, g2s = gamma^2 - 1.5 alpha^2 (shifted denominator, see kR1a)
 __device__ __forceinline__ double gh1_acc(double acc, double d, double A1, double g2)
 {
   double D = fma(d, d, g2);

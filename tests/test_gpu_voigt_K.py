@@ -104,3 +104,19 @@ def test_fp32_variant_golden_table_and_switches(golden_dir):
     for yy in (1e-9, 1e-12, 1e-15):                                  # tiny damping: the Gaussian term beyond the series
         rel = np.abs(_K(x, np.full_like(x, yy), hk.HK_FP32) / oracle.faddeeva_re(x, np.full_like(x, yy)) - 1.0)
         assert rel.max() < TOL32, yy
+
+
+def test_shifted_one_point_rule_along_its_switch_curve():
+    # the 1-point rule with the shifted denominator serves from r^2 = max(3600, 4100 y) (FP64) / max(400, 400 y) (FP32):
+    # both sides of that curve for dampings from Doppler- to Lorentz-dominated, and far beyond it
+    y = np.concatenate([10 ** np.linspace(-8, 3, 120), [0.5, 0.878, 0.879, 1.0, 22.0]])
+    for prec, a, b, tol in ((hk.HK_FP64, 3600.0, 4100.0, TOL), (hk.HK_FP32, 400.0, 400.0, TOL32)):
+        R = np.maximum(a, b * y)
+        for s in (1 - 1e-9, 1 + 1e-9, 0.99, 1.01, 3.0, 100.0, 1e4):
+            r2 = R * s
+            ok = r2 > y * y
+            x = np.sqrt(r2[ok] - y[ok] ** 2)
+            k = _K(x, y[ok], prec)
+            ref = oracle.faddeeva_re(x, y[ok])
+            rel = np.abs(k / ref - 1.0)
+            assert rel.max() < tol, (prec, s, rel.max(), x[np.argmax(rel)], y[ok][np.argmax(rel)])
