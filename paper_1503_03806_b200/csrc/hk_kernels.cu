@@ -581,7 +581,9 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) voigt_far_kernel(const __gri
         const double nu0 = pb->nu0, A1 = pb->A1, g2 = fma(-1.5, pb->a2, pb->g2);  // shifted denominator (kR1a)
         const double d0 = x0 - nu0;
 #pragma unroll
-        for (int k = 0; k < P; ++k) acc[k] = gh1_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), A1, g2);
+        for (int k = 0; k < P; k += 2)
+          gh1_acc2(acc[k], acc[k + 1], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), fma((double)(32 * k + 32), a.dnu, d0),
+                   A1, g2);
       }
       // ---- 2-point rule ----
 #pragma unroll 1

@@ -93,6 +93,15 @@ __device__ __forceinline__ double gh1_acc(double acc, double d, double A1, doubl
   double D = fma(d, d, g2);
   return fma(A1, rcp_nr(D), acc);
 }
+// the same for TWO points with one reciprocal, 1/(D0 D1): 10 FP64 + 1 MUFU per pair — the FP64 count of two gh1_acc, half
+// the MUFU.RCP64H (the XU unit, 16 lanes/SM, is the far kernel's second-busiest pipe)
+__device__ __forceinline__ void gh1_acc2(double &a0, double &a1, double d0, double d1, double A1, double g2)
+{
+  const double D0 = fma(d0, d0, g2), D1 = fma(d1, d1, g2);
+  const double t = A1 * rcp_nr(D0 * D1);
+  a0 = fma(t, D1, a0);
+  a1 = fma(t, D0, a1);
+}
 // 2-point (t^2 = 1/2, wn = 1/2): A1 (E + alpha^2)/(E^2 + f2), E = d^2 + e2, e2 = g2 - a2/2, f2 = 2 a2 g2
 __device__ __forceinline__ double gh2_acc(double acc, double d, double A1, double e2, double f2, double A1a2)
 {
