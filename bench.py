@@ -50,7 +50,7 @@ FP32_INST_PER_EVAL = {"gh1": 4.0, "gh2": 6.5}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the roofline kernel(s), from the committed `ncu --set full` captures
 # of this command (profiles/r01c_voigt_{far,near,far32}_kernel_ncu_full.txt): far 9.76 MB + near 36.90 MB read, ~0 written
 # (kappa, 24 MB, stays in the 126 MB L2 between the two kernels); FP32 far kernel 6.52 MB.  Not memory-bound: context only.
-NCU_DRAM_BYTES = {"fp64": 9.761e6 + 36.898e6 + 0.020e6, "fp32": 6.518e6}
+NCU_DRAM_BYTES = {"fp64": 9.719e6 + 36.894e6 + 0.020e6, "fp32": 6.518e6}
 
 
 def tp_table(wl, world):
