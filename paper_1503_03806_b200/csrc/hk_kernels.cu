@@ -1,13 +1,18 @@
 // hk_kernels.cu — sm_100a kernels and the C ABI of include/hk.h.
 //
 // Steps:
-//   a1 line_prep_kernel   per line: alpha, gamma, S(T), amplitude, index window, regime radii
-//   a2 tile_plan_kernel   per grid tile: range of sorted lines whose window touches the tile
-//   a3 voigt_kernel       kappa_j = sum_i amp_i V_i(nu_j): grid-point-owned register accumulation, persistent CTAs, lines
-//                         streamed through a shared-memory ring by 1-D TMA bulk copies (producer warp, full/empty
-//                         mbarriers), regime chosen per (line, warp span) or per (line, 32-point group)
-//   a4                    coalesced kappa store from the same kernel ("without additional write-outs")
+//   a1 line_prep_kernel   per line: alpha, gamma (eq. 20), S(T) (eq. 18), amplitude, index window (absolute or relative
+//                         cutoff), regime radii, packed records
+//   a2 (same kernel)      per 256-point block: first line ending / beginning / centred there (lookup tables: a tile's line
+//                         range is two reads)
+//   a3 voigt_far_kernel   far wings (1-/2-point rule) of kappa_j = sum_i amp_i V_i(nu_j): grid-point-owned register
+//                         accumulation, persistent CTAs on a tile queue, lines streamed through a shared-memory ring by 1-D
+//                         TMA bulk copies completing on mbarriers; FP64, or the FP32 variant (template parameter)
+//      voigt_near_kernel  line cores and near wings (3-, 6-point rule, series), one CTA per 256-point span, adds to kappa
+//   a4                    coalesced kappa store from the far kernel ("without additional write-outs")
 //   a5/a6 kdist_kernel    (hk_kdist.cu) per-bin register/shuffle bitonic sort + resampling at Gauss-Legendre nodes
+// eq. 20/21 line physics, mixtures and the relative cutoff live in a1 and the host code below;
+// Chebyshev resampling and the transmission function in hk_kdist.cu / hk_resample.cu.
 #include <cuda_runtime.h>
 #include <limits.h>
 #include <math.h>
