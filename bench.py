@@ -318,6 +318,34 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_stage_times(args):
+    """--stage-times: per-stage device times (hk_set_timing) of hk_opacity on configs 1, 2 (its highest pressure) and 3 cut to
+    1e7 lines, in both precisions — the figures profiles/ and DESIGN.md quote beside the bench line.  One GPU; not a bench line."""
+    import torch
+    import paper_1503_03806_b200 as hk
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --stage-times: no CUDA device")
+    for cfg, n_lines, reps in ((1, None, 10), (2, None, 5), (3, 10_000_000, 3)):
+        wl = workloads.config(cfg) if n_lines is None else workloads.config(cfg, n_lines=n_lines)
+        T, P = wl.T[0], (wl.P_atm[-1] if cfg == 2 else wl.P_atm[0])
+        lines = hk.Lines.from_numpy(wl.nu0, wl.S, wl.gamma0)
+        ne = hk.hk_count_evals(wl.nu0, wl.nu_min, wl.n_points, wl.dnu, wl.cutoff)
+        for prec, name in ((hk.HK_FP64, "fp64"), (hk.HK_FP32, "fp32")):
+            ctx = hk.Context(lines, precision=prec)
+            out = ctx.opacity(T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff)
+            hk.hk_set_timing(True)
+            st = np.zeros(3)
+            for _ in range(reps):
+                ctx.opacity(T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, out=out)
+                st += np.array(hk.hk_last_stage_ms())
+            hk.hk_set_timing(False)
+            st /= reps
+            ctx.close()
+            print(json.dumps({"config": cfg, "n_lines": wl.n_lines, "T_K": T, "P_atm": P, "precision": name,
+                              "line_prep_ms": st[0], "voigt_far_ms": st[1], "voigt_near_ms": st[2],
+                              "opacity_ms": float(st.sum()), "evals_per_s": ne / (st.sum() * 1e-3)}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -326,8 +354,12 @@ def main():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--precision", choices=["fp64", "fp32"], default="fp64",
                     help="fp64 (BASELINE.json config 1, the default) or the optional FP32 variant (bar 1e-4)")
+    ap.add_argument("--stage-times", action="store_true",
+                    help="print per-stage device times of configs 1, 2, 3 (1e7 lines) in both precisions and exit")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.stage_times:
+        run_stage_times(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)
