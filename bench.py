@@ -288,6 +288,15 @@ def run_ours(args):
                      "(DESIGN.md); peak = hk_fp64_peak DFMA microbenchmark measured live in this run")
     cpu_v, cpu_dt, cpu_ne, cpu_desc, cores = oracle_sample(wl, T, P, 15.0) if world == 1 else (None, 0, 0, "", 0)
 
+    # HBM-bound steps: a5+a6 reads kappa once and writes the k-table; a4 is the kappa store inside the far kernel
+    hbm_peak, hbm_src = 6650.0, "of fallback (6.65 TB/s, B200_PROFILING.md)"
+    try:
+        hbm_peak = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"])
+        hbm_src = "of measured (MEASURED_PEAKS.json hbm_gbs)"
+    except (OSError, KeyError, ValueError):
+        pass
+    kdist_bytes = 8.0 * N + 8.0 * (N // ppb) * wl.n_g
+    kdist_gbs = kdist_bytes / (ms_kdist / K * 1e-3) / 1e9
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -308,6 +317,10 @@ def run_ours(args):
                      "traffic_note": "DRAM bytes per launch from the committed ncu --set full capture (profiles/r01c_*), not live",
                      "note": roof_note, "regime_census": census, "ms": roof_ms,
                      "fp64_peak_tflops": 2.0 * fp64_peak / 1e12, "fp32_peak_tflops": 2.0 * fp32_peak / 1e12},
+        "kdist_hbm": {"kernel": "kdist_kernel (a5+a6)", "bound": "hbm", "achieved": kdist_gbs, "peak": hbm_peak, "unit": "GB/s",
+                      "frac": kdist_gbs / hbm_peak, "algorithmic_bytes": kdist_bytes, "peak_source": hbm_src,
+                      "note": "8 B/point read + 8 n_g B/bin written; the kernel is bound by the bitonic network's "
+                              "compare-exchange count, not by HBM (profiles/r01b_kdist_kernel_ncu_full.txt)"},
         "clocks": clocks,
     }
     if cpu_v is not None:
