@@ -132,3 +132,23 @@ def test_relative_cutoff_in_lorentz_widths(T, P, W, cap):
     assert np.array_equal(got1 != 0.0, ref1 != 0.0)
     with pytest.raises(hk.HKError):
         hk.hk_opacity(one, 296.0, 1.0, wl.nu_min, wl.nu_max, wl.dnu, cap, cutoff_widths=-1.0)
+
+
+def test_host_buffer_form_with_every_optional_field():
+    import torch
+    wl = workloads.small(seed=81, n_lines=1200, nu_max=120.0, cutoff=25.0, with_E=True)
+    ex = _fields(wl, 82)
+    T, P, q = 900.0, 20.0, wl.q_ratio(900.0)
+    lines = hk.Lines.from_numpy(wl.nu0, wl.S, wl.gamma0, E_low=wl.E_low, **ex)
+    for prec in (hk.HK_FP64, hk.HK_FP32):
+        dev = hk.hk_opacity(lines, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, q_ratio=q, self_fraction=0.4, abundance=0.6,
+                            cutoff_widths=300.0, precision=prec)
+        kt = hk.hk_kdist(dev, wl.dnu, wl.bin_width, wl.n_g)
+        hk_kap, hk_k = hk.hk_opacity_host(wl.nu0, wl.S, wl.gamma0, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, E_low=wl.E_low,
+                                          q_ratio=q, self_fraction=0.4, abundance=0.6, cutoff_widths=300.0, precision=prec,
+                                          bin_width=wl.bin_width, n_g=wl.n_g, **ex)
+        assert torch.equal(hk_kap, dev.cpu()) and torch.equal(hk_k, kt.cpu())
+    ref = oracle.opacity_full(wl.nu0, wl.S, wl.gamma0, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, E_low=wl.E_low, q_ratio=q,
+                              self_fraction=0.4, abundance=0.6, cutoff_widths=300.0, **ex)
+    _check(hk.hk_opacity(lines, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, q_ratio=q, self_fraction=0.4, abundance=0.6,
+                         cutoff_widths=300.0).cpu().numpy(), ref, BAR)
