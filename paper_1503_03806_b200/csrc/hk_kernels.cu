@@ -372,6 +372,7 @@ struct VoigtArgs {
   float dnu_f;
   int N;
   int accumulate;  // 1: add to kappa (species of a mixture after the first), 0: overwrite
+  int block0;      // near kernel: first 256-point span of this launch (the near kernel may run as several launches)
   double *kappa;
   double r2_slope, r2_offset;  // near kernel: no line centred beyond r2_slope*j + r2_offset grid units of point j reaches it inside its 2-point radius
 };
@@ -749,7 +750,7 @@ __global__ void __launch_bounds__(kNearWarps * 32, 4) voigt_near_kernel(const __
 {
   __shared__ NearSmem S;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int b = blockIdx.x;
+  const int b = a.block0 + (int)blockIdx.x;
   const int plo = b * kPlanBlock, phi = min(plo + kPlanBlock, a.N) - 1;  // the span classify32 sees
   // lines that can be "near" for this span: centre within R of it, and window touching it
   const double R = fmax(fma(a.r2_slope, (double)phi, a.r2_offset), 4.0);
@@ -1108,13 +1109,27 @@ static int validate(const hk_lines *lines, int64_t n_lines, double T, double P_a
   return HK_OK;
 }
 
+// The near kernel in `n` launches over consecutive ranges of spans, an event after each: kappa[0, hi[i]) is final once
+// done[i] has passed — hk_opacity_host copies kappa back range by range while the later ranges are still being computed.
+constexpr int kMaxNearChunks = 8;
+struct NearChunks {
+  int n = 1;
+  cudaEvent_t done[kMaxNearChunks] = {};
+  int64_t hi[kMaxNearChunks] = {};  // one past the last grid point of range i
+};
+
 static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double P_atm, double q_ratio, double mass_amu,
                        double nu_min, double dnu, double cutoff, int64_t N, double *kappa_out, Scratch &s, const hk_params &prm,
-                       cudaStream_t st)
+                       cudaStream_t st, NearChunks *chunks = nullptr)
 {
   const bool f32 = prm.precision == HK_FP32;
   if (n_lines == 0) {
     if (!prm.accumulate) HK_CUDA(cudaMemsetAsync(kappa_out, 0, (size_t)N * sizeof(double), st));
+    if (chunks) {
+      chunks->n = 1;
+      chunks->hi[0] = N;
+      HK_CUDA(cudaEventRecord(chunks->done[0], st));
+    }
     return HK_OK;
   }
   const int nb = (int)((N + kPlanBlock - 1) / kPlanBlock);
@@ -1175,8 +1190,18 @@ static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double 
   else voigt_far_kernel<kP, kWarps, kMinB, false><<<grid, kWarps * 32, sizeof(VoigtSmemT), st>>>(va);
   HK_CUDA(cudaGetLastError());
   if (g_timing) HK_CUDA(cudaEventRecord(ev[2], st));
-  voigt_near_kernel<<<nb, kNearWarps * 32, 0, st>>>(va);
-  HK_CUDA(cudaGetLastError());
+  const int nch = chunks ? std::max(1, std::min(chunks->n, std::min(kMaxNearChunks, nb))) : 1;
+  for (int c = 0; c < nch; ++c) {
+    const int b_lo = (int)((int64_t)nb * c / nch), b_hi = (int)((int64_t)nb * (c + 1) / nch);
+    va.block0 = b_lo;
+    voigt_near_kernel<<<b_hi - b_lo, kNearWarps * 32, 0, st>>>(va);
+    HK_CUDA(cudaGetLastError());
+    if (chunks) {
+      chunks->hi[c] = std::min<int64_t>((int64_t)b_hi * kPlanBlock, N);
+      HK_CUDA(cudaEventRecord(chunks->done[c], st));
+    }
+  }
+  if (chunks) chunks->n = nch;
   if (g_timing) {
     HK_CUDA(cudaEventRecord(ev[3], st));
     g_ev_pending = true;  // resolved by hk_last_stage_ms(): the call itself stays asynchronous
@@ -1219,8 +1244,8 @@ int64_t hk_grid_size(double nu_min, double nu_max, double dnu)
   return (int64_t)llround(n);
 }
 
-int hk_opacity(const hk_lines *lines, int64_t n_lines, double T, double P_atm, double nu_min, double nu_max, double dnu,
-               double cutoff, double *kappa_out, const hk_params *prm)
+static int opacity_impl(const hk_lines *lines, int64_t n_lines, double T, double P_atm, double nu_min, double nu_max,
+                        double dnu, double cutoff, double *kappa_out, const hk_params *prm, NearChunks *chunks)
 {
   int64_t N = 0;
   int rc = validate(lines, n_lines, T, P_atm, nu_min, nu_max, dnu, cutoff, kappa_out, prm, &N);
@@ -1246,11 +1271,42 @@ int hk_opacity(const hk_lines *lines, int64_t n_lines, double T, double P_atm, d
     return rc;
   }
   Scratch s;
-  rc = run_opacity(&use, n_lines, T, P_atm, prm->q_ratio, prm->mass_amu, nu_min, dnu, cutoff, N, kappa_out, s, *prm, st);
+  rc = run_opacity(&use, n_lines, T, P_atm, prm->q_ratio, prm->mass_amu, nu_min, dnu, cutoff, N, kappa_out, s, *prm, st,
+                   chunks);
   scratch_release(s, st);
   pool_free(sorted_buf, st);
   pool_free(shift_buf, st);
   return rc;
+}
+
+int hk_opacity(const hk_lines *lines, int64_t n_lines, double T, double P_atm, double nu_min, double nu_max, double dnu,
+               double cutoff, double *kappa_out, const hk_params *prm)
+{
+  return opacity_impl(lines, n_lines, T, P_atm, nu_min, nu_max, dnu, cutoff, kappa_out, prm, nullptr);
+}
+
+// copy stream and events of hk_opacity_host, one set per host thread (re-made when the thread changes device)
+struct HostCopy {
+  int dev = -1;
+  cudaStream_t copy = nullptr;
+  cudaEvent_t done[kMaxNearChunks] = {};
+  cudaEvent_t copied = nullptr;
+};
+static thread_local HostCopy g_hc;
+static int host_copy_get(HostCopy **out)
+{
+  int dev = 0;
+  HK_CUDA(cudaGetDevice(&dev));
+  HostCopy &h = g_hc;
+  if (h.dev != dev) {
+    h = HostCopy();  // a set made on another device is abandoned (a thread that hops devices is not the case served)
+    HK_CUDA(cudaStreamCreateWithFlags(&h.copy, cudaStreamNonBlocking));
+    for (int i = 0; i < kMaxNearChunks; ++i) HK_CUDA(cudaEventCreateWithFlags(&h.done[i], cudaEventDisableTiming));
+    HK_CUDA(cudaEventCreateWithFlags(&h.copied, cudaEventDisableTiming));
+    h.dev = dev;
+  }
+  *out = &h;
+  return HK_OK;
 }
 
 int hk_opacity_host(const hk_lines *lines_host, int64_t n_lines, double T, double P_atm, double nu_min, double nu_max,
@@ -1270,6 +1326,11 @@ int hk_opacity_host(const hk_lines *lines_host, int64_t n_lines, double T, doubl
     n_bins = N / (int64_t)ppb_d;
   }
   cudaStream_t st = (cudaStream_t)prm->stream;
+  HostCopy *hc = nullptr;
+  {
+    int rch = host_copy_get(&hc);
+    if (rch != HK_OK) return rch;
+  }
   constexpr int NF = 8;
   const double *src[NF] = {lines_host->nu0, lines_host->S, lines_host->gamma0, lines_host->n_T, lines_host->E_low,
                            lines_host->gamma_self, lines_host->A21, lines_host->delta};
@@ -1292,13 +1353,31 @@ int hk_opacity_host(const hk_lines *lines_host, int64_t n_lines, double T, doubl
     e = cudaMemcpyAsync(d_kappa, kappa_host_out, (size_t)N * sizeof(double), cudaMemcpyHostToDevice, st);
   if (e == cudaSuccess) {
     hk_lines dl = {dptr[0], dptr[1], dptr[2], dptr[3], dptr[4], dptr[5], dptr[6], dptr[7]};
-    rc = hk_opacity(&dl, n_lines, T, P_atm, nu_min, nu_max, dnu, cutoff, d_kappa, prm);
-    if (rc == HK_OK && k_host_out) rc = hk_kdist(d_kappa, N, dnu, bin_width, n_g, d_k, prm->stream);
-    if (rc == HK_OK && kappa_host_out)
-      e = cudaMemcpyAsync(kappa_host_out, d_kappa, (size_t)N * sizeof(double), cudaMemcpyDeviceToHost, st);
+    // kappa goes back range by range on a second stream while the near kernel still works on the later ranges: the
+    // device -> host copy of 8 B/point is a quarter of the call at config 1
+    NearChunks ch;
+    ch.n = kappa_host_out ? 4 : 1;
+    bool copies_pending = false;
+    for (int i = 0; i < kMaxNearChunks; ++i) ch.done[i] = hc->done[i];
+    rc = opacity_impl(&dl, n_lines, T, P_atm, nu_min, nu_max, dnu, cutoff, d_kappa, prm, &ch);
+    if (rc == HK_OK && kappa_host_out) {
+      int64_t lo = 0;
+      for (int c = 0; c < ch.n && e == cudaSuccess; ++c) {
+        e = cudaStreamWaitEvent(hc->copy, ch.done[c], 0);
+        if (e == cudaSuccess && ch.hi[c] > lo)
+          e = cudaMemcpyAsync(kappa_host_out + lo, d_kappa + lo, (size_t)(ch.hi[c] - lo) * sizeof(double),
+                              cudaMemcpyDeviceToHost, hc->copy);
+        lo = ch.hi[c];
+      }
+      if (e == cudaSuccess) e = cudaEventRecord(hc->copied, hc->copy);
+      copies_pending = e == cudaSuccess;
+    }
+    if (rc == HK_OK && e == cudaSuccess && k_host_out) rc = hk_kdist(d_kappa, N, dnu, bin_width, n_g, d_k, prm->stream);
     if (rc == HK_OK && e == cudaSuccess && k_host_out)
       e = cudaMemcpyAsync(k_host_out, d_k, (size_t)n_bins * n_g * sizeof(double), cudaMemcpyDeviceToHost, st);
+    if (copies_pending && e == cudaSuccess) e = cudaStreamWaitEvent(st, hc->copied, 0);  // st frees the buffer after them
   }
+  if (e != cudaSuccess || rc != HK_OK) cudaStreamSynchronize(hc->copy);  // error path: nothing may still read the buffer
   pool_free(dev, st);
   const cudaError_t es = cudaStreamSynchronize(st);
   if (rc != HK_OK) return rc;
