@@ -208,8 +208,9 @@ int hk_voigt_K(const double *x, const double *y, int64_t n, double *out, int pre
  * temperature and pressure"): the line list is bound once, scratch is kept between calls.
  * hk_create copies nothing when nu0 is ascending: the hk_lines device arrays must outlive the context; with
  * lines_sorted = 0 and an unordered list the context owns an ordered copy (made once).  A list with a pressure shift
- * (delta != NULL) would have to be re-ordered at every pressure: hk_create returns HK_ERR_UNSUPPORTED for it (use
- * hk_opacity).  self_fraction, abundance and accumulate are taken from prm at hk_create. */
+ * (delta != NULL) has to be re-ordered at every pressure: the context then only binds the arrays, and every
+ * hk_opacity_ctx call works like hk_opacity (shifted copy, order check — synchronises the stream — scratch from the pool).
+ * self_fraction, abundance, cutoff_widths and accumulate are taken from prm at hk_create. */
 typedef struct hk_ctx hk_ctx;
 int hk_create(const hk_lines *lines, int64_t n_lines, const hk_params *prm, hk_ctx **out);
 int hk_opacity_ctx(hk_ctx *ctx, double T, double P_atm, double q_ratio, double nu_min, double nu_max, double dnu,

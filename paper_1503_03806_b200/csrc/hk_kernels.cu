@@ -1393,16 +1393,23 @@ int hk_create(const hk_lines *lines, int64_t n_lines, const hk_params *prm, hk_c
   if (n_lines > 2000000000LL) return HK_ERR_UNSUPPORTED;
   if (!pos_finite(prm->mass_amu)) return HK_ERR_INVALID;
   if (prm->precision != HK_FP64 && prm->precision != HK_FP32) return HK_ERR_INVALID;
-  if (lines->delta) return HK_ERR_UNSUPPORTED;  // the order of shifted centres depends on P: use hk_opacity
   hk_ctx *c = new (std::nothrow) hk_ctx();
   if (!c) return HK_ERR_NOMEM;
+  c->n_lines = n_lines;
+  c->prm = *prm;
+  if (lines->delta) {
+    // eq. 21: the order of the shifted centres depends on P, so nothing can be ordered once: every hk_opacity_ctx call
+    // shifts, checks and (if needed) orders a copy, as the one-shot call does
+    c->lines = *lines;
+    c->sorted_buf = nullptr;
+    *out = c;
+    return HK_OK;
+  }
   int rc = ordered_lines(lines, n_lines, prm, &c->lines, &c->sorted_buf);
   if (rc != HK_OK) {
     delete c;
     return rc;
   }
-  c->n_lines = n_lines;
-  c->prm = *prm;
   c->prm.lines_sorted = 1;
   *out = c;
   return HK_OK;
@@ -1414,6 +1421,8 @@ int hk_opacity_ctx(hk_ctx *ctx, double T, double P_atm, double q_ratio, double n
   if (!ctx) return HK_ERR_INVALID;
   hk_params p = ctx->prm;
   p.q_ratio = q_ratio;
+  if (ctx->lines.delta)
+    return opacity_impl(&ctx->lines, ctx->n_lines, T, P_atm, nu_min, nu_max, dnu, cutoff, kappa_out, &p, nullptr);
   int64_t N = 0;
   int rc = validate(&ctx->lines, ctx->n_lines, T, P_atm, nu_min, nu_max, dnu, cutoff, kappa_out, &p, &N);
   if (rc != HK_OK) return rc;

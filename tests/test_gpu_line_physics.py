@@ -89,12 +89,19 @@ def test_no_cutoff_every_line_on_every_point():
     _check(hk.hk_opacity(lines, T, P, wl.nu_min, wl.nu_max, wl.dnu, big, precision=hk.HK_FP32).cpu().numpy(), ref, BAR32)
 
 
-def test_context_rejects_a_pressure_shift_and_bad_fractions():
+def test_context_with_a_pressure_shift_and_bad_fractions():
+    import torch
     wl = workloads.small(seed=61, n_lines=50, nu_max=50.0, cutoff=25.0)
     ex = _fields(wl, 62)
-    with pytest.raises(hk.HKError) as e:
-        hk.Context(hk.Lines.from_numpy(wl.nu0, wl.S, wl.gamma0, delta=ex["delta"]))
-    assert e.value.code == -5
+    shifted = hk.Lines.from_numpy(wl.nu0, wl.S, wl.gamma0, delta=ex["delta"])
+    ctx = hk.Context(shifted)                                       # re-ordered at every pressure
+    for P in (0.5, 40.0):
+        a = ctx.opacity(1200.0, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff)
+        b = hk.hk_opacity(shifted, 1200.0, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff)
+        assert torch.equal(a, b)
+        _check(a.cpu().numpy(), oracle.opacity_full(wl.nu0, wl.S, wl.gamma0, 1200.0, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff,
+                                                    delta=ex["delta"]), BAR)
+    ctx.close()
     ls = hk.Lines.from_numpy(wl.nu0, wl.S, wl.gamma0, gamma_self=ex["gamma_self"])
     for kw in (dict(self_fraction=1.5), dict(abundance=-1.0)):
         with pytest.raises(hk.HKError) as e:
