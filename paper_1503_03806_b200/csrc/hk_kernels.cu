@@ -755,7 +755,10 @@ __device__ __noinline__ void near_inner(const MetaA *pa, const MetaB *pm, const 
   }
 }
 
-__global__ void __launch_bounds__(kNearWarps * 32, 16 / kNearWarps) voigt_near_kernel(const __grid_constant__ VoigtArgs a)
+#ifndef HK_NEAR_MINB
+#define HK_NEAR_MINB (16 / HK_NEAR_WARPS)
+#endif
+__global__ void __launch_bounds__(kNearWarps * 32, HK_NEAR_MINB) voigt_near_kernel(const __grid_constant__ VoigtArgs a)
 {
   __shared__ NearSmem S;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
