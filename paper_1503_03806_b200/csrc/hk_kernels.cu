@@ -741,14 +741,14 @@ __device__ __noinline__ void near_inner(const MetaA *pa, const MetaB *pm, const 
       const double ks = core_K(fmin(x, 6.7), C);
       if (!__all_sync(kFull, core || !inwin)) {  // some point of the group lies outside the series region
         v = gh6_val(d * d, G6);
-        if (mb.rg > 0.0f) v = fma(kc.Acore, exp(-x * x), v);
+        if (mb.rg > 0.0f) v = fma(kc.Acore, exp_fast(-x * x), v);
       }
       if (core) v = kc.Acore * ks;
     } else {
       v = gh6_val(d * d, G6);
       if (dg < mb.rg) {
         const double x = d * inv_alpha;
-        v = fma(kc.Acore, exp(-x * x), v);
+        v = fma(kc.Acore, exp_fast(-x * x), v);
       }
     }
     sk[32 * k + lane] += inwin ? v : 0.0;

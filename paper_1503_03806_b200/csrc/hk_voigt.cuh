@@ -183,6 +183,47 @@ __device__ __forceinline__ double gh6_val(double q, const Gh6 &g)
   return gh_pair_val(q, g.p0) + gh_pair_val(q, g.p1) + gh_pair_val(q, g.p2);
 }
 
+// exp(x) for -700 < x < 700 (no overflow / underflow / NaN handling: the series calls it on [-300, 10]).  n = rint(x log2 e)
+// by the magic-number add, r = x - n ln2 in two pieces, a degree-11 Taylor polynomial on |r| <= ln2/2 (remainder 6e-15)
+// whose coefficients are operands from the constant bank, 2^n added to the exponent field: 16 FP64 + 3 integer
+// instructions.  The library exp() spends about as many FP64 instructions but twice as many issue slots (its 64-bit
+// immediates arrive by UMOV pairs, and it guards the range): the near kernel is issue-bound, not FP64-bound.
+__constant__ double kExpTaylor[12] = {1.0, 1.0, 0.5, 1.0 / 6, 1.0 / 24, 1.0 / 120, 1.0 / 720, 1.0 / 5040, 1.0 / 40320,
+                                      1.0 / 362880, 1.0 / 3628800, 1.0 / 39916800};
+__device__ __forceinline__ double exp_fast(double x)
+{
+  const double kMagic = 6755399441055744.0;  // 1.5 * 2^52
+  const double t = fma(x, 1.4426950408889634074, kMagic);
+  const int n = __double2loint(t);
+  const double nd = t - kMagic;
+  double r = fma(nd, -6.93147180369123816490e-01, x);  // ln2 high part (its low 21 bits are zero)
+  r = fma(nd, -1.90821492927058770002e-10, r);         // ln2 low part
+  double p = kExpTaylor[11];
+#pragma unroll
+  for (int k = 10; k >= 0; --k) p = fma(p, r, kExpTaylor[k]);
+  return __hiloint2double(__double2hiint(p) + (n << 20), __double2loint(p));
+}
+
+// sin(t)^2 for 0 <= t < 1e4 (the series calls it with t = x y <= 44): k = rint(t/pi) by the magic-number add, r = t - k pi in
+// two pieces (|r| <= pi/2; the sign of sin(t) = (-1)^k sin(r) does not matter for the square), sin(r) = r P(r^2) with the
+// Taylor coefficients to degree 19 (remainder 3e-16) from the constant bank.  Relative accuracy holds for small t (the term
+// sin^2(xy)/y -> x^2 y as y -> 0 needs it).  14 FP64 instructions; the library sinpi costs about twice the issue slots.
+__constant__ double kSinTaylor[10] = {1.0, -1.0 / 6, 1.0 / 120, -1.0 / 5040, 1.0 / 362880, -1.0 / 39916800, 1.0 / 6227020800.0,
+                                      -1.0 / 1307674368000.0, 1.0 / 355687428096000.0, -1.0 / 121645100408832000.0};
+__device__ __forceinline__ double sin_sq_fast(double t)
+{
+  const double kMagic = 6755399441055744.0;  // 1.5 * 2^52
+  const double kd = fma(t, 0.31830988618379067154, kMagic) - kMagic;
+  double r = fma(kd, -3.14159265160560607910e+00, t);  // pi high part (low 26 bits zero: kd * it is exact for kd < 2^26)
+  r = fma(kd, -1.98418714791870343106e-09, r);         // pi middle part
+  r = fma(kd, -1.14423774522196636802e-17, r);         // pi low part
+  const double q = r * r;
+  double p = kSinTaylor[9];
+#pragma unroll
+  for (int k = 8; k >= 0; --k) p = fma(p, q, kSinTaylor[k]);
+  return q * p * p;
+}
+
 // ---- core: Algorithm-916-type series (restated in DESIGN.md §4) ---------------------------
 //   K(x,y) = exp(-x^2) [ erfcx(y) cos(2xy) + (2a/pi) sin^2(xy)/y - (2a/pi) y cos(2xy) S1(y)
 //                        + (a/pi) y sum_{n=1..16} W_n (p^n + p^-n) ],
@@ -228,8 +269,8 @@ __device__ __forceinline__ CoreLine core_setup(double y, double inv_y, double er
 // Lanes of a warp call with the same CoreLine.  0 <= x <= 6.7.
 __device__ __forceinline__ double core_K(double x, const CoreLine &c)
 {
-  const double ex2 = exp(-x * x);
-  const double p = exp(2.0 * kA * x);
+  const double ex2 = exp_fast(-x * x);
+  const double p = exp_fast(2.0 * kA * x);
   const double s2c = p + rcp_nr2(p);  // 2 cosh(2 a x) = C_1
   // C_n = p^n + p^-n in two independent chains (odd and even n) with the step-2 recurrence C_{n+2} = (C_1^2 - 2) C_n - C_{n-2},
   // C_{-1} = C_1, C_0 = 2, C_2 = C_1^2 - 2: the dependent-DFMA path is 8 long instead of 16 (this loop is latency-bound at
@@ -246,8 +287,7 @@ __device__ __forceinline__ double core_K(double x, const CoreLine &c)
     Cem = Ce; Ce = Cen;
   }
   const double sum = so + se;
-  const double s = sinpi(x * c.y * kInvPi);  // x y <= 44; sinpi has no slow range-reduction path
-  const double s2 = s * s;
+  const double s2 = sin_sq_fast(x * c.y);
   const double c2 = fma(-2.0, s2, 1.0);
   const double head = fma(c.erfcx_y, c2, k2AoverPi * (s2 * c.inv_y)) - k2AoverPi * c.y * c2 * c.S1;
   return ex2 * fma(kAoverPi * c.y, sum, head);
