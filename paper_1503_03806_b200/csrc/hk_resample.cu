@@ -14,6 +14,7 @@
 #include <vector>
 
 #include "hk_internal.h"
+#include "hk_voigt.cuh"  // exp_fast
 
 namespace hk {
 
@@ -156,7 +157,7 @@ __global__ void __launch_bounds__(128) transmission_kernel(const __grid_constant
   for (int m = threadIdx.x; m < a.n_m; m += blockDim.x) {
     const double mm = a.mcol[m];
     double acc = 0.0;
-    for (int q = 0; q < a.n_g; ++q) acc = fma(a.w[q], exp(-sk[q] * mm), acc);
+    for (int q = 0; q < a.n_g; ++q) acc = fma(a.w[q], exp_fast(fmax(-sk[q] * mm, -700.0)), acc);  // e^-700: 1e-304
     a.T_out[(int64_t)b * a.n_m + m] = acc;
   }
 }
@@ -181,10 +182,10 @@ __global__ void __launch_bounds__(128) transmission_direct_kernel(const double *
     __syncthreads();
     int j = 0;
     for (; j + 1 < cnt; j += 2) {
-      s0 += exp(sk[j] * mm);
-      s1 += exp(sk[j + 1] * mm);
+      s0 += exp_fast(fmax(sk[j] * mm, -700.0));  // 16 FP64 instructions, no range guards (e^-700 = 1e-304 stands for 0)
+      s1 += exp_fast(fmax(sk[j + 1] * mm, -700.0));
     }
-    if (j < cnt) s0 += exp(sk[j] * mm);
+    if (j < cnt) s0 += exp_fast(fmax(sk[j] * mm, -700.0));
   }
   if (m < n_m) T_out[(int64_t)b * n_m + m] = (s0 + s1) / (double)ppb;
 }
