@@ -319,7 +319,10 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
 // decision, no divergence in the loops.
 // ------------------------------------------------------------------------------------------------------
 constexpr int CH = 128;     // lines per ring stage: 128 lines x 128 B
-constexpr int STAGES = 4;
+#ifndef HK_STAGES
+#define HK_STAGES 4
+#endif
+constexpr int STAGES = HK_STAGES;
 
 struct __align__(16) StageHdr {
   int tile_lo;  // first grid point of the tile this chunk belongs to; < 0: no more work
