@@ -35,15 +35,13 @@ namespace hk {
 // classifies 32 lines at once (lane = line) reads the 16-byte meta records without shared-memory bank conflicts.
 // ------------------------------------------------------------------------------------------------------
 struct __align__(16) MetaA {
-  int jlo, jhi;  // inclusive index window of the line (empty if jhi < jlo)
-  float c;       // line centre in grid units, (nu0-nu_min)/dnu
-  float r3;      // |j-c| >= r3 on a whole group of points  =>  r^2 >= kR3 there (3-point rule valid); conservative
+  int jlo, jhi;    // inclusive index window of the line (empty if jhi < jlo)
+  int j3lo, j3hi;  // "3-ball": the grid points closer to the centre than the 3-point radius (the 6-point rule and the series
+                   // live inside it); INT_MAX, INT_MIN if it holds no grid point
 };
 struct __align__(16) MetaB {
-  float r1;      // likewise kR1 (1-point rule)
-  float r2;      // likewise kR2 (2-point rule)
-  float r6;      // likewise kRc (6-point rule); inside it the series region may begin
-  float rg;      // the 6-point rule adds the Gaussian term on groups closer than this (0 unless y < 1e-8)
+  int j1lo, j1hi;  // likewise the 1-ball (beyond it: 1-point rule with the shifted denominator)
+  int j2lo, j2hi;  // and the 2-ball (beyond it: 2-point rule); ball1 contains ball2 contains ball3
 };
 struct __align__(16) LineBase {
   double nu0, A1, g2, a2;  // centre; amp*gamma/pi; gamma^2; alpha^2
@@ -52,23 +50,29 @@ struct __align__(16) LineGH2 {
   double e2, f2, A1a2, inv_alpha;  // gamma^2 - alpha^2/2; 2 alpha^2 gamma^2; A1 alpha^2; 1/alpha (0 if alpha == 0)
 };
 struct __align__(16) LineCore {
-  double y, erfcx_y, Acore, inv_y;  // gamma/alpha; erfcx(y); amp/(alpha sqrt(pi)); alpha/gamma.  alpha = 0: y = 1e150
+  double y, erfcx_y, Acore, inv_y;  // gamma/alpha (>= 1e-200); erfcx(y); amp/(alpha sqrt(pi)); alpha/gamma.  alpha = 0: y = 1e150
+};
+struct __align__(16) LineNear {
+  int jslo, jshi;  // the grid points that take the series (x^2 <= 44.15 - y^2), inside the 3-ball; INT_MAX, INT_MIN if none
+  int tiny;        // 1: y < 1e-8, the 6-point rule adds the Gaussian term exp(-x^2) (no wing rule carries it)
+  int pad;
 };
 // FP32 variant: what the far kernel needs of LineBase + LineGH2, in float, and the line centre in grid units split into an
 // integer and a fraction so that d = ((j - ci) - cf) dnu carries no cancellation (relative error 2^-24 at any distance)
 // Amplitudes span more than the float range (eq. 18's Boltzmann factor alone reaches e^87 in config 4), so A1 = A1m 2^A1e is
 // kept split: the far kernel scales the 32 lines it sums in float by the largest exponent among them.
 struct __align__(16) LineF32 {
-  int ci;                  // floor of the centre in grid units
-  float cf;                // centre - ci, in [0, 1)
+  int ci;                  // the grid point nearest to the centre
+  float cf;                // centre - ci in grid units, in [-1/2, 1/2]
   float A1m;               // amp*gamma/pi = A1m * 2^A1e, A1m in [0.5, 1] (0 for a line of zero strength)
-  int A1e;
+  int A1e;                 // INT_MIN for a line of zero strength (does not enter the batch maximum)
   float g2, e2, f2, a2;    // as LineBase / LineGH2
 };
 static_assert(sizeof(MetaA) == 16 && sizeof(MetaB) == 16 && sizeof(LineBase) == 32 && sizeof(LineGH2) == 32 &&
-                  sizeof(LineCore) == 32 && sizeof(LineF32) == 32,
+                  sizeof(LineCore) == 32 && sizeof(LineF32) == 32 && sizeof(LineNear) == 16,
               "record size");
-constexpr size_t kBytesPerLine = sizeof(MetaA) + sizeof(MetaB) + sizeof(LineBase) + sizeof(LineGH2) + sizeof(LineCore);
+constexpr size_t kBytesPerLine =
+    sizeof(MetaA) + sizeof(MetaB) + sizeof(LineBase) + sizeof(LineGH2) + sizeof(LineCore) + sizeof(LineNear);
 
 constexpr double kCLight = 2.99792458e10;   // cm/s
 constexpr double kBoltz = 1.380649e-16;     // erg/K
@@ -88,7 +92,6 @@ struct PrepArgs {
   double q_ratio;
   double nu_min, dnu, cutoff;
   int N;
-  double margin;  // grid units added to every regime radius: covers the float rounding of c and of the span ends
   double R2, R3;      // switch radii on r^2 of the 2-, 3-point rule (kR2.. for FP64, kR2f.. for the FP32 variant)
   int f32_ladder;     // the 1-point rule's switch is r1_sq(y, f32_ladder)
   LineF32 *f32;       // FP32 variant only (else NULL)
@@ -97,6 +100,7 @@ struct PrepArgs {
   LineBase *base;
   LineGH2 *gh2;
   LineCore *core;
+  LineNear *near;
   int nb;         // number of plan blocks of kPlanBlock grid points, ceil(N / kPlanBlock)
   int *first_hi;  // [nb+1]  first_hi[b] = first line i with jhi_i >= b*kPlanBlock   (n if none)
   int *first_lo;  // [nb+1]  first_lo[b] = first line i with jlo_i >= b*kPlanBlock   (n if none)
@@ -128,13 +132,24 @@ __device__ __forceinline__ int line_centre_index(double nu0, const PrepArgs &a)
 __device__ __forceinline__ int plan_block_floor(int j) { return j >> 8; }
 static_assert(kPlanBlock == 256, "plan_block_floor shifts by 8");
 
-// grid-unit radius outside which x^2 + y^2 >= R holds: sqrt(R alpha^2 - gamma^2)/dnu, rounded outward
-__device__ __forceinline__ float radius_grid(double R, double a2, double g2, double inv_dnu, double margin)
+// The grid points within rho grid steps of the centre c, as an inclusive index range (INT_MAX, INT_MIN if there is none).
+// Every regime decision of a3 is taken on such ranges, in integers, by both kernels: a rule is used on a point only when
+// the point lies outside the ball the rule is valid beyond.
+__device__ __forceinline__ void ball_range(double c, double rho, int &lo, int &hi)
 {
-  double t = R * a2 - g2;
-  if (!(t > 0.0)) return 0.0f;
-  double r = sqrt(t) * inv_dnu + margin;
-  return r < 3.0e38 ? __double2float_ru(r) : 3.0e38f;
+  lo = INT_MAX;
+  hi = INT_MIN;
+  if (!(rho >= 0.0)) return;
+  const double l = fmax(ceil(c - rho), -2.0e9), h = fmin(floor(c + rho), 2.0e9);
+  if (l > h) return;
+  lo = (int)l;
+  hi = (int)h;
+}
+// ... for the ball x^2 + y^2 < R, i.e. |nu - nu0| < sqrt(R alpha^2 - gamma^2) (a hair outward: 1e-9 relative)
+__device__ __forceinline__ void ball_of(double R, double a2, double g2, double c, double inv_dnu, int &lo, int &hi)
+{
+  const double t = R * a2 - g2;
+  ball_range(c, t > 0.0 ? sqrt(t) * inv_dnu * (1.0 + 1.0e-9) : -1.0, lo, hi);
 }
 
 __global__ void __launch_bounds__(256) line_prep_kernel(PrepArgs a)
@@ -144,7 +159,7 @@ __global__ void __launch_bounds__(256) line_prep_kernel(PrepArgs a)
   if (i == 0) *a.queue = 0;
   const double nu0 = a.nu0[i];
   double alpha = nu0 * a.vth;
-  if (!(alpha > 0.0)) alpha = 0.0;  // nu0 <= 0: Lorentzian (A9)
+  if (!(alpha > 1.0e-290)) alpha = 0.0;  // nu0 <= 0 (or a width whose reciprocal overflows): Lorentzian (A9)
   const double tfac = a.n_T ? pow(kT0 / a.T, a.n_T[i]) : a.tfac_half;
   double gamma;
   if (a.gamma_self) {  // eq. 20: air and self broadening, P0 = 1 atm
@@ -173,12 +188,15 @@ __global__ void __launch_bounds__(256) line_prep_kernel(PrepArgs a)
   g.A1a2 = b.A1 * a2;
   g.inv_alpha = alpha > 0.0 ? 1.0 / alpha : 0.0;
   LineCore k;
-  k.y = alpha > 0.0 ? gamma * g.inv_alpha : 1.0e150;  // series region x^2 < 44 - y^2: none for alpha = 0
-  k.inv_y = alpha > 0.0 ? alpha / gamma : 0.0;
+  // gamma = 0 (gamma0 = 0 and no natural width: the pure Doppler limit K(x,0) = exp(-x^2)) is served by the floor on y: every
+  // wing rule is then 0 (A1 = 0), the series has sin^2(xy)/y -> 0, and the 6-point rule adds the Gaussian term (y < 1e-8)
+  k.y = alpha > 0.0 ? fmax(gamma * g.inv_alpha, 1.0e-200) : 1.0e150;  // series region x^2 < 44 - y^2: none for alpha = 0
+  k.inv_y = alpha > 0.0 ? 1.0 / k.y : 0.0;
   k.erfcx_y = core_xc2(k.y) > 0.0 ? erfcx(k.y) : 0.0;
   k.Acore = amp * g.inv_alpha * kInvSqrtPi;
   MetaA ma;
   MetaB mb;
+  LineNear nr;
   // relative cutoff: the line's own window is narrower than the window of the absolute cutoff; the a2 tables are built from
   // the latter (qlo, qhi: non-decreasing in i, a superset), classify32 masks with the former
   double cut = a.cutoff;
@@ -213,27 +231,54 @@ __global__ void __launch_bounds__(256) line_prep_kernel(PrepArgs a)
       for (int b = max(plan_block_floor(jc) + 1, 0); b <= a.nb; ++b) a.first_c[b] = n;
   }
   const double inv_dnu = 1.0 / a.dnu;
-  double c = (nu0 - a.nu_min) * inv_dnu;
-  c = fmin(fmax(c, -3.0e9), 3.0e9);
-  ma.c = (float)c;
-  mb.r1 = alpha > 0.0 ? radius_grid(r1_sq(k.y, a.f32_ladder != 0), a2, g2, inv_dnu, a.margin) : 0.0f;
-  mb.r2 = radius_grid(a.R2, a2, g2, inv_dnu, a.margin);
-  ma.r3 = radius_grid(a.R3, a2, g2, inv_dnu, a.margin);
-  mb.r6 = radius_grid(kRc, a2, g2, inv_dnu, a.margin);
-  const double xg2 = alpha > 0.0 ? gauss_xg2(k.y) : 0.0;
-  mb.rg = xg2 > 0.0 ? __double2float_ru(sqrt(xg2) * alpha * inv_dnu + a.margin) : 0.0f;
-  // only the 6-point branch adds the Gaussian term of a tiny-y line: no cheaper rule inside rg (never binds for kR3 = 280)
-  ma.r3 = fmaxf(ma.r3, mb.rg);
-  mb.r2 = fmaxf(mb.r2, ma.r3);
-  mb.r1 = fmaxf(mb.r1, mb.r2);
+  const double c = (nu0 - a.nu_min) * inv_dnu;
+  // regime balls in index space, nested: series inside ball3 inside ball2 inside ball1
+  if (alpha > 0.0) {
+    ball_of(r1_sq(k.y, a.f32_ladder != 0), a2, g2, c, inv_dnu, mb.j1lo, mb.j1hi);
+    ball_of(a.R2, a2, g2, c, inv_dnu, mb.j2lo, mb.j2hi);
+    ball_of(a.R3, a2, g2, c, inv_dnu, ma.j3lo, ma.j3hi);
+    const double xs2 = core_xc2(k.y) > 0.0 ? core_xc2(k.y) + kSeriesPad : -1.0;
+    ball_range(c, xs2 > 0.0 ? sqrt(xs2) * alpha * inv_dnu : -1.0, nr.jslo, nr.jshi);
+    // only the 6-point rule adds the Gaussian term of a tiny-y line: no cheaper rule inside that radius
+    const double xg2 = gauss_xg2(k.y);
+    nr.tiny = xg2 > 0.0 ? 1 : 0;
+    if (xg2 > 0.0) {
+      int glo, ghi;
+      ball_range(c, sqrt(xg2) * alpha * inv_dnu * (1.0 + 1.0e-9), glo, ghi);
+      ma.j3lo = min(ma.j3lo, glo);
+      ma.j3hi = max(ma.j3hi, ghi);
+    }
+    if (a.f32 && a2 < 1.0e-9) {
+      // FP32 variant: the float 2-/3-point rules form d^4 and d^6, which leave the float range for a line this narrow
+      // (nu0 of a few cm^-1): inside its 1-ball (a fraction of a grid step wide) everything goes to the FP64 near kernel
+      mb.j2lo = mb.j1lo; mb.j2hi = mb.j1hi;
+      ma.j3lo = mb.j1lo; ma.j3hi = mb.j1hi;
+    }
+    ma.j3lo = min(ma.j3lo, nr.jslo); ma.j3hi = max(ma.j3hi, nr.jshi);
+    mb.j2lo = min(mb.j2lo, ma.j3lo); mb.j2hi = max(mb.j2hi, ma.j3hi);
+    mb.j1lo = min(mb.j1lo, mb.j2lo); mb.j1hi = max(mb.j1hi, mb.j2hi);
+  } else {
+    mb.j1lo = mb.j2lo = ma.j3lo = nr.jslo = INT_MAX;
+    mb.j1hi = mb.j2hi = ma.j3hi = nr.jshi = INT_MIN;
+    nr.tiny = 0;
+  }
+  nr.pad = 0;
   if (a.f32) {
+    // FP32 variant: the far kernel forms the distance of point j0 + 32k as 32k dnu + d0 in float, which cancels within a few
+    // grid steps of the centre (error 1.5e-5 grid steps): the three grid points on either side go to the FP64 near kernel
+    int lo3, hi3;
+    ball_range(c, 3.0, lo3, hi3);
+    ma.j3lo = min(ma.j3lo, lo3); ma.j3hi = max(ma.j3hi, hi3);
+    mb.j2lo = min(mb.j2lo, ma.j3lo); mb.j2hi = max(mb.j2hi, ma.j3hi);
+    mb.j1lo = min(mb.j1lo, mb.j2lo); mb.j1hi = max(mb.j1hi, mb.j2hi);
     LineF32 f;
-    const double cfl = floor(fmin(fmax(c, -2.0e9), 2.0e9));
+    const double cc = fmin(fmax(c, -2.0e9), 2.0e9);
+    const double cfl = rint(cc);  // nearest: |cf| <= 1/2, so (j - ci) - cf keeps float relative accuracy at the centre too
     f.ci = (int)cfl;
-    f.cf = (float)fmin(fmax(c - cfl, 0.0), 1.0);
+    f.cf = (float)(cc - cfl);
     int ex = 0;
     f.A1m = (float)frexp(b.A1, &ex);
-    f.A1e = ex;
+    f.A1e = b.A1 > 0.0 ? ex : INT_MIN;  // a line of zero strength does not raise its batch's scale
     f.g2 = (float)g2; f.e2 = (float)g.e2; f.f2 = (float)g.f2; f.a2 = (float)a2;
     a.f32[i] = f;
   }
@@ -242,6 +287,7 @@ __global__ void __launch_bounds__(256) line_prep_kernel(PrepArgs a)
   a.base[i] = b;
   a.gh2[i] = g;
   a.core[i] = k;
+  a.near[i] = nr;
 }
 
 // ------------------------------------------------------------------------------------------------------
@@ -292,17 +338,18 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
 }
 
 // ------------------------------------------------------------------------------------------------------
-// a3 + a4: Voigt accumulation, in two kernels that split the (line, 256-point span) pairs between them by ONE test,
-// classify32(): does the whole span lie at or beyond the line's 2-point radius?
+// a3 + a4: Voigt accumulation, in two kernels that split the (line, 32-point group) pairs between them by ONE integer
+// test: does the group touch the line's 3-ball (MetaA.j3lo..j3hi)?
 //
-//   voigt_far_kernel   every pair whose span lies wholly in the far wing (r^2 >= 3200: 1- or 2-point Gauss-Hermite rule,
-//                      97 % of all evaluations of config 1), and writes kappa;
-//   voigt_near_kernel  every other pair (3-point, 6-point rule, series), rule chosen per 32-point group, and adds to kappa.
+//   voigt_far_kernel   every group that lies wholly outside the 3-ball: 1-, 2- or 3-point Gauss-Hermite rule, chosen per
+//                      (line, 256-point span) where the whole span is beyond a ball, per group on the spans that touch
+//                      the 3-ball (99.4 % of all evaluations of config 1), and writes kappa;
+//   voigt_near_kernel  every group that touches the 3-ball (6-point rule, series), and adds to kappa.
 //
 // Why two: the far work of a chunk of lines is the same for every warp of a CTA, the near work is not (it falls on the one
 // warp whose span holds the line centres; in a dense list, config 3, on the same warp for hundreds of consecutive chunks),
 // and warps that share a line ring can drift apart by only STAGES-1 chunks.  Kept apart, the far kernel streams lines through
-// a shared ring in lockstep at full rate, and the near work is spread over 4x as many independent 64-point units.
+// a shared ring in lockstep at full rate, and the near kernel works off uniform items (one rule, 32 points) in tight loops.
 // Each grid point has one owner per kernel and a fixed summation order: results are bitwise reproducible.
 //
 // Far kernel.  Persistent CTAs of WARPS warps, all of them consumers.  Work unit = tile of WARPS*32*P consecutive grid
@@ -312,11 +359,10 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
 // lines: four 1-D TMA bulk copies per chunk (the four record spans) completing on the stage's `full` mbarrier; the last
 // warp out of a stage refills it (ticket-ordered).  No CTA-wide barrier exists after start-up, and the ring keeps flowing
 // across tile boundaries (each stage carries a header naming its tile).
-// A warp handles a chunk 32 lines at a time.  First it CLASSIFIES them, lane = line: from the span's distance to the line
-// centre (float, grid units, conservative radii from a1) each lane picks the rule valid on the whole span, and ballots turn
-// that into bit masks.  Then it walks each mask: a branch-free loop over the lines of one rule, parameters broadcast from
-// shared memory, an unrolled P-point body accumulating in registers: ~1 instruction per (line, span) for the regime
-// decision, no divergence in the loops.
+// A warp handles a chunk 32 lines at a time.  First it CLASSIFIES them, lane = line: integer compares of the span against
+// the line's window and balls (from a1) pick the rule valid on the whole span, and ballots turn that into bit masks.  Then
+// it walks each mask: a branch-free loop over the lines of one rule, parameters broadcast from shared memory, an unrolled
+// P-point body accumulating in registers: ~1 instruction per (line, span) for the regime decision, no divergence.
 // ------------------------------------------------------------------------------------------------------
 constexpr int CH = 128;     // lines per ring stage: 128 lines x 128 B
 #ifndef HK_STAGES
@@ -365,6 +411,7 @@ struct VoigtArgs {
   const LineBase *base;
   const LineGH2 *gh2;
   const LineCore *core;
+  const LineNear *near;
   const LineF32 *f32;   // FP32 variant only
   const int *first_hi;  // a2 lookup tables (see PrepArgs)
   const int *first_lo;
@@ -377,29 +424,31 @@ struct VoigtArgs {
   int accumulate;  // 1: add to kappa (species of a mixture after the first), 0: overwrite
   int block0;      // near kernel: first 256-point span of this launch (the near kernel may run as several launches)
   double *kappa;
-  double r2_slope, r2_offset;  // near kernel: no line centred beyond r2_slope*j + r2_offset grid units of point j reaches it inside its 2-point radius
+  double r3_slope, r3_offset;  // near kernel: no line centred beyond r3_slope*j + r3_offset grid units of point j has j in its 3-ball
 };
 
-// lane = line classification of 32 lines against the 256-point span [slo, shi] (both kernels call this, on the same
-// records, with the same float arithmetic: it is what splits the pairs between them).  Bit masks of the lines that
-//   m1, m2 : take the 1- / 2-point rule on the whole span, span inside the line's window             (far kernel)
-//   e1, e2 : likewise, but a cutoff edge of the line falls inside the span: masked to the window      (far kernel)
-//   mn     : touch the span, and the span reaches inside the 2-point radius                           (near kernel)
+// lane = line classification of 32 lines against the 256-point span [slo, shi].  Bit masks of the lines that
+//   m1, m2, m3 : take the 1- / 2- / 3-point rule on the whole span, span inside the line's window
+//   e1, e2     : 1- / 2-point rule, but a cutoff edge of the line falls inside the span: masked to the window
+//   n3         : the rest of the lines that touch the span: 3-point rule on the groups outside the 3-ball, masked to the
+//                window (the groups that touch the 3-ball are the near kernel's)
 struct SpanMasks {
-  unsigned m1, m2, e1, e2, mn;
+  unsigned m1, m2, m3, e1, e2, n3;
 };
 __device__ __forceinline__ SpanMasks classify_regs(const MetaA &A, const MetaB &B, bool live, int slo, int shi)
 {
   const bool act = live && (shi >= slo) && (A.jhi >= slo) && (A.jlo <= shi);
   const bool inside = (A.jlo <= slo) && (A.jhi >= shi);
-  const float dist = fmaxf(fmaxf((float)slo - A.c, A.c - (float)shi), 0.0f);
-  const bool w1 = dist >= B.r1, w2 = dist >= B.r2;
+  const bool b1 = (shi < B.j1lo) || (slo > B.j1hi);  // the span lies beyond the 1-ball ...
+  const bool b2 = (shi < B.j2lo) || (slo > B.j2hi);
+  const bool b3 = (shi < A.j3lo) || (slo > A.j3hi);
   SpanMasks M;
-  M.m1 = __ballot_sync(kFull, act && inside && w1);
-  M.m2 = __ballot_sync(kFull, act && inside && !w1 && w2);
-  M.e1 = __ballot_sync(kFull, act && !inside && w1);
-  M.e2 = __ballot_sync(kFull, act && !inside && !w1 && w2);
-  M.mn = __ballot_sync(kFull, act && !w2);
+  M.m1 = __ballot_sync(kFull, act && inside && b1);
+  M.m2 = __ballot_sync(kFull, act && inside && !b1 && b2);
+  M.m3 = __ballot_sync(kFull, act && inside && !b2 && b3);
+  M.e1 = __ballot_sync(kFull, act && !inside && b1);
+  M.e2 = __ballot_sync(kFull, act && !inside && !b1 && b2);
+  M.n3 = __ballot_sync(kFull, act && !b2 && !(inside && b3));
   return M;
 }
 __device__ __forceinline__ SpanMasks classify32(const MetaA *ma, const MetaB *mb, int l, int cnt, int slo, int shi)
@@ -407,6 +456,8 @@ __device__ __forceinline__ SpanMasks classify32(const MetaA *ma, const MetaB *mb
   const bool live = l < cnt;
   return classify_regs(ma[live ? l : 0], mb[live ? l : 0], live, slo, shi);
 }
+// the far kernel's share of a span that touches a line's 3-ball: the 32-point groups [glo, glo+31] wholly outside it
+__device__ __forceinline__ bool group_is_far(int glo, int j3lo, int j3hi) { return (glo + 31 < j3lo) || (glo > j3hi); }
 
 // lines that can touch the grid points [lo, hi): jhi >= lo and jlo < hi, looked up at plan-block granularity (a superset
 // by at most the lines that end or begin inside the two boundary blocks; classify32 masks them out)
@@ -525,15 +576,17 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) voigt_far_kernel(const __gri
 #pragma unroll 1
       for (int b0 = 0; b0 < h.cnt; b0 += 32) {
         const SpanMasks M = classify32(S.ma[stage] + b0, S.mb[stage] + b0, lane, h.cnt - b0, slo, shi);
-        if ((M.m1 | M.m2 | M.e1 | M.e2) == 0u) continue;
+        if ((M.m1 | M.m2 | M.m3 | M.e1 | M.e2 | M.n3) == 0u) continue;
         const int eb = __reduce_max_sync(kFull, (b0 + lane < h.cnt) ? sf[b0 + lane].A1e : INT_MIN);
+        if (eb == INT_MIN) continue;  // every line of the batch has zero strength
+        const int ebm = eb - 127;     // a line more than 2^-127 below the batch maximum flushes to zero
         float af[P];
 #pragma unroll
         for (int k = 0; k < P; ++k) af[k] = 0.0f;
 #pragma unroll 1
         for (unsigned m = M.m1; m; m &= m - 1) {
           const LineF32 L = sf[b0 + (__ffs(m) - 1)];
-          const float w = L.A1m * __int_as_float(max(L.A1e - eb + 127, 0) << 23);
+          const float w = L.A1m * __int_as_float((max(L.A1e, ebm) - ebm) << 23);
           const float d0 = ((float)(j0 - L.ci) - L.cf) * a.dnu_f;
 #pragma unroll
           for (int k = 0; k < P; k += 2)
@@ -543,7 +596,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) voigt_far_kernel(const __gri
 #pragma unroll 1
         for (unsigned m = M.m2; m; m &= m - 1) {
           const LineF32 L = sf[b0 + (__ffs(m) - 1)];
-          const float w = L.A1m * __int_as_float(max(L.A1e - eb + 127, 0) << 23);
+          const float w = L.A1m * __int_as_float((max(L.A1e, ebm) - ebm) << 23);
           const float d0 = ((float)(j0 - L.ci) - L.cf) * a.dnu_f;
           const float wa2 = w * L.a2;
 #pragma unroll
@@ -558,7 +611,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) voigt_far_kernel(const __gri
           const bool one = (M.e1 >> (i - b0)) & 1u;
           const int jlo = S.ma[stage][i].jlo, jhi = S.ma[stage][i].jhi;
           const LineF32 L = sf[i];
-          const float w = L.A1m * __int_as_float(max(L.A1e - eb + 127, 0) << 23);
+          const float w = L.A1m * __int_as_float((max(L.A1e, ebm) - ebm) << 23);
           const float d0 = ((float)(j0 - L.ci) - L.cf) * a.dnu_f;
           const float wa2 = w * L.a2;
           const unsigned wlen = (unsigned)(jhi - jlo);
@@ -571,6 +624,27 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) voigt_far_kernel(const __gri
             else gh2_acc2f(t0, t1, da, db, w, L.e2, L.f2, wa2);
             af[k] += ((unsigned)(jrel + 32 * k) <= wlen) ? t0 : 0.0f;
             af[k + 1] += ((unsigned)(jrel + 32 * k + 32) <= wlen) ? t1 : 0.0f;
+          }
+        }
+        // 3-point rule (float: from r^2 >= 64), whole span / the groups outside the 3-ball, masked to the window
+#pragma unroll 1
+        for (unsigned m = M.m3 | M.n3; m; m &= m - 1) {
+          const int i = b0 + (__ffs(m) - 1);
+          const bool whole = (M.m3 >> (i - b0)) & 1u;
+          const MetaA A = S.ma[stage][i];
+          const LineF32 L = sf[i];
+          const float w = L.A1m * __int_as_float((max(L.A1e, ebm) - ebm) << 23);
+          const float d0 = ((float)(j0 - L.ci) - L.cf) * a.dnu_f;
+          const float e3 = fmaf(-1.5f, L.a2, L.g2), f3 = 3.0f * L.f2;
+          const float c3 = w * (1.0f / 3.0f), c0 = 2.0f * c3, c3a = w * L.a2;
+          const unsigned wlen = (unsigned)(A.jhi - A.jlo);
+          const int jrel = j0 - A.jlo;
+#pragma unroll
+          for (int k = 0; k < P; ++k) {
+            if (whole || group_is_far(slo + 32 * k, A.j3lo, A.j3hi)) {
+              const float t = gh3_accf(0.0f, (k == 0 ? d0 : fmaf((float)(32 * k), a.dnu_f, d0)), L.g2, e3, f3, c0, c3, c3a);
+              af[k] += ((unsigned)(jrel + 32 * k) <= wlen) ? t : 0.0f;
+            }
           }
         }
         const double sc = ldexp(1.0, eb);
@@ -604,6 +678,17 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) voigt_far_kernel(const __gri
 #pragma unroll
         for (int k = 0; k < P; ++k) acc[k] = gh2_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), A1, e2, f2, A1a2);
       }
+      // ---- 3-point rule, span wholly between the 3-ball and the 2-ball's edge, inside the window ----
+#pragma unroll 1
+      for (unsigned m = M.m3; m; m &= m - 1) {
+        const LineBase lb = sbase[b0 + (__ffs(m) - 1)];
+        const double d0 = x0 - lb.nu0;
+        const double e3 = fma(-1.5, lb.a2, lb.g2), f3 = 6.0 * lb.a2 * lb.g2;
+        const double c3 = lb.A1 * (1.0 / 3.0), c0 = 2.0 * c3, c3a = lb.A1 * lb.a2;
+#pragma unroll
+        for (int k = 0; k < P; ++k)
+          acc[k] = gh3_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), lb.g2, e3, f3, c0, c3, c3a);
+      }
       // ---- the same rules on spans that hold a cutoff edge: masked to the line's window ----
 #pragma unroll 1
       for (unsigned m = M.e1; m; m &= m - 1) {
@@ -632,6 +717,26 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) voigt_far_kernel(const __gri
         for (int k = 0; k < P; ++k) {
           const double t = gh2_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), A1, e2, f2, A1a2);
           acc[k] = ((unsigned)(jrel + 32 * k) <= wlen) ? t : acc[k];
+        }
+      }
+      // ---- spans that touch the 3-ball (or hold a cutoff edge inside the 2-ball): 3-point rule on the groups wholly
+      //      outside the 3-ball (warp-uniform skip), masked to the window; the other groups are the near kernel's ----
+#pragma unroll 1
+      for (unsigned m = M.n3; m; m &= m - 1) {
+        const int i = b0 + (__ffs(m) - 1);
+        const MetaA A = S.ma[stage][i];
+        const LineBase lb = sbase[i];
+        const double d0 = x0 - lb.nu0;
+        const double e3 = fma(-1.5, lb.a2, lb.g2), f3 = 6.0 * lb.a2 * lb.g2;
+        const double c3 = lb.A1 * (1.0 / 3.0), c0 = 2.0 * c3, c3a = lb.A1 * lb.a2;
+        const unsigned wlen = (unsigned)(A.jhi - A.jlo);
+        const int jrel = slo + lane - A.jlo;
+#pragma unroll
+        for (int k = 0; k < P; ++k) {
+          if (group_is_far(slo + 32 * k, A.j3lo, A.j3hi)) {
+            const double t = gh3_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), lb.g2, e3, f3, c0, c3, c3a);
+            acc[k] = ((unsigned)(jrel + 32 * k) <= wlen) ? t : acc[k];
+          }
         }
       }
     }
@@ -673,188 +778,210 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) voigt_far_kernel(const __gri
   }
 }
 
-// Near kernel.  CTA = one 256-point span (a plan block), kNearWarps warps, lane l of every warp on the points
-// plo + l + 32k (k < 8).  The CTA walks the lines centred within the block's bound on the 2-point radius (a2 table
-// first_c) 32 per warp at a time, classifies them against the span exactly as the far kernel does (classify32), and
-// compacts the lines the far kernel left out, in line order, into a shared-memory list with their records.  The list is
-// dealt round-robin to the warps.  A line whose span stays outside the 3-point radius takes the 3-point rule on all 8
-// groups (unrolled, register accumulators, masked to the window); any other line gets its rule per 32-point group, warp-
-// uniformly (3-, 6-point rule, series on the groups that hold core points), accumulated in the warp's shared-memory strip.
-// At the end the warps' sums are added in a fixed order to the kappa the far kernel wrote.
+// Near kernel.  CTA = one warp = one 256-point span (a plan block); lane l on the points plo + l + 32k of group k.
+// The warp walks the lines centred within the span's bound on the 3-ball radius (a2 table first_c) 32 at a time, lane = line:
+// a lane whose line has groups of this span inside its 3-ball (and inside its window) computes everything that depends on
+// the line alone — the constants of the 6-point rule, the 16 series weights W_n and the folded series constants — ONCE, into
+// a shared-memory slot, and writes the line's work as uniform ITEMS into two queues:
+//   6-point items  (line, group k): the group's points that are in the window and outside the series interval;
+//   series items   (line, first point, count <= 32): chunks of the series interval [jslo, jshi] taken from ITS lower end, not
+//                  from the group grid, so that only the last chunk of a line has idle lanes.
+// Then the warp works the queues off, two items per iteration (two independent dependency chains per thread), each item one
+// rule on 32 points with its constants broadcast from shared memory: no divergence, no per-point rule choice, no constants
+// recomputed per group.  Sums are kept in a shared-memory strip that starts as the kappa the far kernel wrote (fetched by
+// cp.async while the lines are being listed) and is stored back at the end; order of summation is fixed.
 constexpr int kNearP = kPlanBlock / 32;
-// One warp per span, 16 CTAs/SM (128 registers), a 64-entry list: no warp waits for a sibling with more inner groups, and
-// the 10 KB of shared memory leave the register file as the only limit.  Measured against 4 warps x 256 entries: 1.5 %
-// faster on config 1, 7 % on config 3; 2 x 128 equal; 1 x 128 and 1 x 256 slower (shared memory cuts the CTAs per SM).
-#ifndef HK_NEAR_WARPS
-#define HK_NEAR_WARPS 1
+constexpr int kNearCap = 32;       // lines per round: one per lane
+constexpr int kWStride = kTerms + 2;  // doubles per row of the W table: rows 16-byte aligned, lanes spread over the banks
+constexpr int kG6Stride = 14;         // likewise for the 12 constants of the 6-point rule
+#ifndef HK_NEAR_MINB
+#define HK_NEAR_MINB 16
 #endif
-#ifndef HK_NEAR_CAP
-#define HK_NEAR_CAP 64
-#endif
-constexpr int kNearWarps = HK_NEAR_WARPS;
-constexpr int kNearCap = HK_NEAR_CAP;  // list entries; a round adds at most 32 per warp
 
 struct __align__(16) NearSmem {
-  MetaA ma[kNearCap];
-  MetaB mb[kNearCap];
-  LineBase base[kNearCap];
-  LineGH2 gh2[kNearCap];
-  LineCore core[kNearCap];
-  double sk[kNearWarps][kPlanBlock];
-  double W[kNearWarps][kTerms];  // series weights of the line a warp is working on
-  int counts[kNearWarps];
+  double sk[kPlanBlock];
+  double W[kNearCap][kWStride];
+  double g6[kNearCap][kG6Stride];  // e, f, cE, c0 of the three +-t pairs
+  double nu0[kNearCap];
+  SeriesLine ser[kNearCap];        // 5 doubles
+  double Acore[kNearCap];
+  int jlo[kNearCap], jhi[kNearCap], jslo[kNearCap], jshi[kNearCap], tiny[kNearCap];
+  unsigned short q6[kNearCap * kNearP];
+  unsigned int qs[kNearCap * (kNearP + 1)];
 };
 
-// distance (grid units, float) of the 32-point group [glo, glo+31] from a line centre; both halves of the near kernel's
-// work on a listed line (3-point rule in registers / inner rules below) split the groups by the SAME test dg >= r3
-__device__ __forceinline__ float group_dist(int glo, float c)
+__device__ __forceinline__ void cp_async8(void *smem_dst, const void *gmem_src)
 {
-  return fmaxf(fmaxf((float)glo - c, c - (float)(glo + 31)), 0.0f);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(smem_dst)), "l"(gmem_src) : "memory");
 }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
-// inner groups of one listed line (those closer to its centre than the 3-point radius): 6-point rule, series on the groups
-// that hold core points, Gaussian term of a tiny-y line; accumulated in the warp's strip sk[32k + lane].  Warp-collective.
-__device__ __noinline__ void near_inner(const MetaA *pa, const MetaB *pm, const LineBase *pb, const LineGH2 *pg,
-                                        const LineCore *pk, int plo, int lane, double x0, double dnu, double En, double *sk,
-                                        double *Wsm, unsigned inner)
+// one 6-point item: group k of the span, line slot e
+__device__ __forceinline__ double near_gh6_item(const NearSmem &S, int e, int k, int plo, int lane, double x0, double dnu, bool &ok)
 {
-  const MetaA ma = *pa;
-  const MetaB mb = *pm;
-  const LineBase b = *pb;
-  const double inv_alpha = pg->inv_alpha;
-  const LineCore kc = *pk;
-  const float dist = fmaxf(fmaxf((float)plo - ma.c, ma.c - (float)(plo + kPlanBlock - 1)), 0.0f);
-  const double d0 = x0 - b.nu0;
-  const Gh6 G6 = gh6_consts(b.A1, b.g2, b.a2);
-  const double xc2 = core_xc2(kc.y);
-  CoreLine C;
-  if (dist < mb.r6) C = core_setup(kc.y, kc.inv_y, kc.erfcx_y, En, Wsm);
-#pragma unroll 1
-  for (unsigned m = inner; m; m &= m - 1) {  // groups inside the 3-point radius that touch the line's window
-    const int k = __ffs(m) - 1;
-    const int glo = plo + 32 * k;
-    const float dg = group_dist(glo, ma.c);
-    const int j = glo + lane;
-    const bool inwin = (j >= ma.jlo) && (j <= ma.jhi);
-    const double d = fma((double)(32 * k), dnu, d0);
-    double v = 0.0;
-    if (dg < mb.r6) {  // the series region reaches into this group
-      const double x = fabs(d) * inv_alpha;
-      const bool core = x * x < xc2;
-      const double ks = core_K(fmin(x, 6.7), C);
-      if (!__all_sync(kFull, core || !inwin)) {  // some point of the group lies outside the series region
-        v = gh6_val(d * d, G6);
-        if (mb.rg > 0.0f) v = fma(kc.Acore, exp_fast(-x * x), v);
-      }
-      if (core) v = kc.Acore * ks;
-    } else {
-      v = gh6_val(d * d, G6);
-      if (dg < mb.rg) {
-        const double x = d * inv_alpha;
-        v = fma(kc.Acore, exp_fast(-x * x), v);
-      }
-    }
-    sk[32 * k + lane] += inwin ? v : 0.0;
+  const double d = fma((double)(32 * k), dnu, x0) - S.nu0[e];
+  const double *c = S.g6[e];
+  const double2 c0 = *reinterpret_cast<const double2 *>(c), c1 = *reinterpret_cast<const double2 *>(c + 2),
+                c2 = *reinterpret_cast<const double2 *>(c + 4), c3 = *reinterpret_cast<const double2 *>(c + 6),
+                c4 = *reinterpret_cast<const double2 *>(c + 8), c5 = *reinterpret_cast<const double2 *>(c + 10);
+  Gh6 G;
+  G.p0.e = c0.x; G.p0.f = c0.y; G.p0.cE = c1.x; G.p0.c0 = c1.y;
+  G.p1.e = c2.x; G.p1.f = c2.y; G.p1.cE = c3.x; G.p1.c0 = c3.y;
+  G.p2.e = c4.x; G.p2.f = c4.y; G.p2.cE = c5.x; G.p2.c0 = c5.y;
+  const double q = d * d;
+  double v = gh6_val(q, G);
+  if (S.tiny[e]) {  // warp-uniform: y < 1e-8, the Gaussian term is still visible beyond the series region
+    const double ia = S.ser[e].inv_alpha;
+    v = fma(S.Acore[e], exp_fast(fmax(-(q * ia) * ia, -700.0)), v);
   }
+  const int j = plo + 32 * k + lane;
+  ok = (j >= S.jlo[e]) && (j <= S.jhi[e]) && !((j >= S.jslo[e]) && (j <= S.jshi[e]));
+  return v;
 }
 
-#ifndef HK_NEAR_MINB
-#define HK_NEAR_MINB (16 / HK_NEAR_WARPS)
-#endif
-__global__ void __launch_bounds__(kNearWarps * 32, HK_NEAR_MINB) voigt_near_kernel(const __grid_constant__ VoigtArgs a)
+__global__ void __launch_bounds__(32, HK_NEAR_MINB) voigt_near_kernel(const __grid_constant__ VoigtArgs a)
 {
   __shared__ NearSmem S;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int lane = threadIdx.x;
   const int b = a.block0 + (int)blockIdx.x;
-  const int plo = b * kPlanBlock, phi = min(plo + kPlanBlock, a.N) - 1;  // the span classify32 sees
-  // lines that can be "near" for this span: centre within R of it, and window touching it
-  const double R = fmax(fma(a.r2_slope, (double)phi, a.r2_offset), 4.0);
+  const int plo = b * kPlanBlock, phi = min(plo + kPlanBlock, a.N) - 1;
+  // lines that can have a point of this span in their 3-ball: centre within R of it, and window touching it
+  const double R = fmax(fma(a.r3_slope, (double)phi, a.r3_offset), 4.0);
   const double clo = (double)plo - R, chi = (double)phi + R;
   int L0 = a.first_hi[b], L1 = a.first_lo[min(b + 1, a.nb)];
   if (clo > 0.0) L0 = max(L0, a.first_c[min((int)(clo * (1.0 / kPlanBlock)), a.nb)]);
   if (chi < (double)a.nb * kPlanBlock - 1.0) L1 = min(L1, a.first_c[min((int)(chi * (1.0 / kPlanBlock)) + 1, a.nb)]);
-  if (L1 <= L0) return;  // uniform over the CTA
+  if (L1 <= L0) return;
 
-  const double En = core_lane_const();
+  // the strip starts as the far kernel's kappa: in flight while the lines are listed
+#pragma unroll
+  for (int k = 0; k < kNearP; ++k) {
+    const int j = plo + 32 * k + lane;
+    if (j <= phi) cp_async8(&S.sk[32 * k + lane], a.kappa + j);
+    else S.sk[32 * k + lane] = 0.0;
+  }
   const double x0 = __dadd_rn(a.nu_min, __dmul_rn((double)(plo + lane), a.dnu));
-  double *sk = S.sk[warp];
-#pragma unroll
-  for (int k = 0; k < kNearP; ++k) sk[32 * k + lane] = 0.0;
-  double acc[kNearP];
-#pragma unroll
-  for (int k = 0; k < kNearP; ++k) acc[k] = 0.0;
-  int list_n = 0;
   bool any = false;
 
-  for (int base0 = L0; base0 < L1; base0 += 32 * kNearWarps) {
-    // ---- classify 32 lines per warp, compact the near ones into the list in line order ----
-    const int b0 = base0 + 32 * warp;
-    const int i = b0 + lane;
+  for (int base0 = L0; base0 < L1; base0 += 32) {
+    // ---- lane = line: which groups of the span are this kernel's, per-line constants, items ----
+    const int i = base0 + lane;
     const bool live = i < L1;
     const MetaA A = a.ma[live ? i : L0];
-    const MetaB B = a.mb[live ? i : L0];
-    const SpanMasks M = classify_regs(A, B, live, plo, phi);
-    if (lane == 0) S.counts[warp] = __popc(M.mn);
-    __syncthreads();
-    int off = list_n, total = 0;
-#pragma unroll
-    for (int w = 0; w < kNearWarps; ++w) {
-      const int c = S.counts[w];
-      if (w < warp) off += c;
-      total += c;
+    int kA = 1, kB = 0;  // groups that touch the 3-ball and the window (each on its own: the far kernel's test is on the ball alone)
+    if (live && A.jhi >= plo && A.jlo <= phi && A.j3hi >= plo && A.j3lo <= phi) {
+      kA = (max(max(A.j3lo, A.jlo), plo) - plo) >> 5;
+      kB = (min(min(A.j3hi, A.jhi), phi) - plo) >> 5;
     }
-    if ((M.mn >> lane) & 1u) {
-      const int slot = off + __popc(M.mn & ((1u << lane) - 1u));
-      S.ma[slot] = A;
-      S.mb[slot] = B;
-      S.base[slot] = a.base[i];
-      S.gh2[slot] = a.gh2[i];
-      S.core[slot] = a.core[i];
-    }
-    list_n += total;
-    __syncthreads();
-    // ---- work the list off when it may not hold another round, and at the end ----
-    if (list_n > kNearCap - 32 * kNearWarps || base0 + 32 * kNearWarps >= L1) {
-      any |= list_n > 0;
-#pragma unroll 1
-      for (int e = warp; e < list_n; e += kNearWarps) {
-        const MetaA ea = S.ma[e];
-        unsigned inner = 0u;  // groups inside the 3-point radius that touch the window (warp-uniform bit mask)
-        {  // 3-point rule, unrolled over the 8 groups in registers, on every group at or beyond the 3-point radius
-          const LineBase lb = S.base[e];
-          const double d0 = x0 - lb.nu0;
-          const double e3 = fma(-1.5, lb.a2, lb.g2), f3 = 6.0 * lb.a2 * lb.g2;
-          const double c3 = lb.A1 * (1.0 / 3.0), c0 = 2.0 * c3, c3a = lb.A1 * lb.a2;
-          const unsigned wlen = (unsigned)(ea.jhi - ea.jlo);
-          const int jrel = plo + lane - ea.jlo;
-#pragma unroll
-          for (int k = 0; k < kNearP; ++k) {
-            const double t = gh3_acc(acc[k], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), lb.g2, e3, f3, c0, c3, c3a);
-            const bool far3 = group_dist(plo + 32 * k, ea.c) >= ea.r3;
-            acc[k] = (far3 && (unsigned)(jrel + 32 * k) <= wlen) ? t : acc[k];
-            const int glo = plo + 32 * k;
-            if (!far3 && glo + 31 >= ea.jlo && glo <= ea.jhi) inner |= 1u << k;
-          }
-        }
-        if (inner)
-          near_inner(S.ma + e, S.mb + e, S.base + e, S.gh2 + e, S.core + e, plo, lane, x0, a.dnu, En, sk, S.W[warp], inner);
+    const bool listed = kA <= kB;
+    const unsigned lm = __ballot_sync(kFull, listed);
+    if (lm == 0u) continue;
+    const int e = __popc(lm & ((1u << lane) - 1u));  // slot
+    unsigned cnt = 0u;                               // 6-point items | series items << 16
+    int kS0 = 8, kS1 = -1, sa = 0, sb = -1;
+    if (listed) {
+      const LineBase lb = a.base[i];
+      const LineCore lc = a.core[i];
+      const LineNear ln = a.near[i];
+      const double inv_alpha = a.gh2[i].inv_alpha;
+      const int sa0 = max(ln.jslo, plo + 32 * kA), sb0 = min(ln.jshi, plo + 32 * kB + 31);  // series points in these groups
+      if (sa0 <= sb0) {
+        kS0 = (sa0 - plo + 31) >> 5;        // groups wholly inside the series interval: no 6-point item
+        kS1 = ((sb0 - plo + 1) >> 5) - 1;
+        sa = max(sa0, A.jlo);
+        sb = min(sb0, A.jhi);
       }
-      list_n = 0;
-      __syncthreads();  // the list is free again
+      const int n6 = (kB - kA + 1) - max(kS1 - kS0 + 1, 0);
+      const int ns = sb >= sa ? ((sb - sa) >> 5) + 1 : 0;
+      cnt = (unsigned)n6 | ((unsigned)ns << 16);
+      S.nu0[e] = lb.nu0;
+      S.Acore[e] = lc.Acore;
+      S.jlo[e] = A.jlo; S.jhi[e] = A.jhi; S.jslo[e] = ln.jslo; S.jshi[e] = ln.jshi; S.tiny[e] = ln.tiny;
+      if (n6 > 0) {
+        const Gh6 G = gh6_consts(lb.A1, lb.g2, lb.a2);
+        double *c = S.g6[e];
+        c[0] = G.p0.e; c[1] = G.p0.f; c[2] = G.p0.cE; c[3] = G.p0.c0;
+        c[4] = G.p1.e; c[5] = G.p1.f; c[6] = G.p1.cE; c[7] = G.p1.c0;
+        c[8] = G.p2.e; c[9] = G.p2.f; c[10] = G.p2.cE; c[11] = G.p2.c0;
+      }
+      if (ns > 0) S.ser[e] = series_line_setup(lc.y, lc.inv_y, lc.erfcx_y, lc.Acore, inv_alpha, S.W[e]);
+      else S.ser[e].inv_alpha = inv_alpha;  // the Gaussian term of a tiny-y line reads it
     }
+    // exclusive scan of the item counts over the lanes, both queues at once
+    unsigned incl = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const unsigned t = __shfl_up_sync(kFull, incl, o);
+      if (lane >= o) incl += t;
+    }
+    const unsigned tot = __shfl_sync(kFull, incl, 31);
+    const int n6tot = (int)(tot & 0xffffu), nstot = (int)(tot >> 16);
+    if (listed) {
+      int o6 = (int)((incl - cnt) & 0xffffu), os = (int)((incl - cnt) >> 16);
+      for (int k = kA; k <= kB; ++k)
+        if (k < kS0 || k > kS1) S.q6[o6++] = (unsigned short)((e << 3) | k);
+      for (int j = sa; j <= sb; j += 32)
+        S.qs[os++] = (unsigned)e | ((unsigned)(j - plo) << 8) | ((unsigned)(min(sb - j, 31)) << 16);
+    }
+    if (!any) cp_async_wait_all();
+    any = true;
+    __syncwarp();
+
+    // ---- 6-point items, two per iteration: group-aligned, so a thread meets only its own strip entries ----
+    {
+      int it = 0;
+#pragma unroll 1
+      for (; it + 1 < n6tot; it += 2) {
+        const unsigned u0 = S.q6[it], u1 = S.q6[it + 1];
+        const int k0 = u0 & 7, k1 = u1 & 7;
+        bool ok0, ok1;
+        const double v0 = near_gh6_item(S, u0 >> 3, k0, plo, lane, x0, a.dnu, ok0);
+        const double v1 = near_gh6_item(S, u1 >> 3, k1, plo, lane, x0, a.dnu, ok1);
+        S.sk[32 * k0 + lane] += ok0 ? v0 : 0.0;
+        S.sk[32 * k1 + lane] += ok1 ? v1 : 0.0;
+      }
+      if (it < n6tot) {
+        const unsigned u0 = S.q6[it];
+        const int k0 = u0 & 7;
+        bool ok0;
+        const double v0 = near_gh6_item(S, u0 >> 3, k0, plo, lane, x0, a.dnu, ok0);
+        S.sk[32 * k0 + lane] += ok0 ? v0 : 0.0;
+      }
+    }
+    __syncwarp();
+    // ---- series items, two per iteration: point-aligned, so the strip entries of two items may belong to different
+    //      lanes: the additions are ordered by __syncwarp ----
+    {
+      int it = 0;
+#pragma unroll 1
+      for (; it + 1 < nstot; it += 2) {
+        const unsigned u0 = S.qs[it], u1 = S.qs[it + 1];
+        const int e0 = u0 & 31, e1 = u1 & 31, off0 = (u0 >> 8) & 255, off1 = (u1 >> 8) & 255;
+        const double d0 = fma((double)off0, a.dnu, x0) - S.nu0[e0], d1 = fma((double)off1, a.dnu, x0) - S.nu0[e1];
+        const SeriesLine Ls0 = S.ser[e0], Ls1 = S.ser[e1];
+        const double v0 = series_val(d0, Ls0, S.W[e0]);
+        const double v1 = series_val(d1, Ls1, S.W[e1]);
+        if (lane <= (int)(u0 >> 16)) S.sk[off0 + lane] += v0;
+        __syncwarp();
+        if (lane <= (int)(u1 >> 16)) S.sk[off1 + lane] += v1;
+        __syncwarp();
+      }
+      if (it < nstot) {
+        const unsigned u0 = S.qs[it];
+        const int e0 = u0 & 31, off0 = (u0 >> 8) & 255;
+        const double d0 = fma((double)off0, a.dnu, x0) - S.nu0[e0];
+        const SeriesLine Ls0 = S.ser[e0];
+        const double v0 = series_val(d0, Ls0, S.W[e0]);
+        if (lane <= (int)(u0 >> 16)) S.sk[off0 + lane] += v0;
+      }
+    }
+    __syncwarp();  // the slots and queues are free again
   }
-  if (!any) return;  // uniform over the CTA
+  if (!any) return;
 #pragma unroll
-  for (int k = 0; k < kNearP; ++k) sk[32 * k + lane] += acc[k];
-  __syncthreads();
-  for (int p = threadIdx.x; p < kPlanBlock; p += kNearWarps * 32) {
-    const int j = plo + p;
-    if (j <= phi) {
-      double sum = S.sk[0][p];
-#pragma unroll
-      for (int w = 1; w < kNearWarps; ++w) sum += S.sk[w][p];
-      a.kappa[j] += sum;
-    }
+  for (int k = 0; k < kNearP; ++k) {
+    const int j = plo + 32 * k + lane;
+    if (j <= phi) a.kappa[j] = S.sk[32 * k + lane];
   }
 }
 
@@ -865,14 +992,18 @@ __global__ void __launch_bounds__(128) voigt_K_kernel(const double *x, const dou
   constexpr double R2 = F32 ? kR2f : kR2, R3 = F32 ? kR3f : kR3;
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const bool live = i < n;
-  const double xi = live ? fabs(x[i]) : 1.0e3, yi = live ? y[i] : 1.0;
-  const int lane = threadIdx.x & 31;
+  const double xi = live ? fabs(x[i]) : 1.0e3, yi = live ? fmax(y[i], 1.0e-200) : 1.0;
   const double A1 = yi * kInvSqrtPi;  // amp*gamma/pi with amp = sqrt(pi)  =>  amp*V = K
   const double g2 = yi * yi, a2 = 1.0, q = xi * xi;
   const double r2 = q + g2;
   double v;
   const bool tiny_gauss = q < gauss_xg2(yi);  // only the 6-point branch adds the Gaussian term (as line_prep arranges)
-  if (r2 >= r1_sq(yi, F32) && !tiny_gauss) {
+  const double xc2 = core_xc2(yi);
+  if (xc2 > 0.0 && q <= xc2 + kSeriesPad) {  // the series interval of a1
+    double W[kTerms];
+    const SeriesLine L = series_line_setup(yi, 1.0 / yi, erfcx(yi), 1.0, 1.0, W);
+    v = series_val(xi, L, W);
+  } else if (r2 >= r1_sq(yi, F32) && !tiny_gauss) {
     if constexpr (F32) {  // the far kernel's float arithmetic; the partner point of the pair is a dummy
       float v0 = 0.0f, v1 = 0.0f;
       gh1_acc2f(v0, v1, (float)xi, 1.0f, (float)A1, fmaf(-1.5f, (float)a2, (float)g2));
@@ -889,23 +1020,17 @@ __global__ void __launch_bounds__(128) voigt_K_kernel(const double *x, const dou
       v = gh2_acc(0.0, xi, A1, g2 - 0.5 * a2, 2.0 * a2 * g2, A1 * a2);
     }
   } else if (r2 >= R3 && !tiny_gauss) {
-    const double c3 = A1 * (1.0 / 3.0);
-    v = gh3_acc(0.0, xi, g2, g2 - 1.5 * a2, 6.0 * a2 * g2, 2.0 * c3, c3, A1 * a2);
+    if constexpr (F32) {
+      const float c3 = (float)A1 * (1.0f / 3.0f), g2f = (float)g2, a2f = (float)a2;
+      v = (double)gh3_accf(0.0f, (float)xi, g2f, fmaf(-1.5f, a2f, g2f), 3.0f * (float)(2.0 * a2 * g2), 2.0f * c3, c3,
+                           (float)A1 * a2f);
+    } else {
+      const double c3 = A1 * (1.0 / 3.0);
+      v = gh3_acc(0.0, xi, g2, g2 - 1.5 * a2, 6.0 * a2 * g2, 2.0 * c3, c3, A1 * a2);
+    }
   } else {
     v = gh6_val(q, gh6_consts(A1, g2, a2));
-    if (tiny_gauss) v += exp(-q);
-  }
-  const bool incore = live && (q < core_xc2(yi));
-  __shared__ double Wsm[4][kTerms];
-  const double En = core_lane_const();
-  unsigned need = __ballot_sync(kFull, incore);
-  while (need) {  // the series is warp-collective with a warp-uniform y: serve one lane at a time
-    const int src = __ffs(need) - 1;
-    need &= need - 1;
-    const double ys = __shfl_sync(kFull, yi, src), xs = __shfl_sync(kFull, xi, src);
-    const CoreLine C = core_setup(ys, 1.0 / ys, erfcx(ys), En, Wsm[threadIdx.x >> 5]);
-    const double kc = core_K(fmin(xs, 6.7), C);
-    if (lane == src) v = kc;
+    if (tiny_gauss) v += exp_fast(fmax(-q, -700.0));
   }
   if (live) out[i] = v;
 }
@@ -1025,18 +1150,19 @@ void pool_free(void *p, cudaStream_t st)
 // on config 1, 10 % on config 3, where a 2048-point tile is 40 % of a line's whole window; 16 x 1 and 8 x 3 are slower.
 // The FP32 variant (78 registers) keeps 8 warps per CTA, 3 CTAs/SM: 4 x 6 measured 4 % slower.
 constexpr int kP = HK_P, kWarps = HK_WARPS, kMinB = HK_MINB;
-constexpr int kWarpsF = 8, kMinBF = 2;
+constexpr int kWarpsF = 8, kMinBF = 3;
 constexpr int kTile = kP * kWarps * 32, kTileF = kP * kWarpsF * 32;
 using VoigtSmemT = VoigtSmem<kP, kWarps, false>;
 using VoigtSmemF = VoigtSmem<kP, kWarpsF, true>;
 
 struct Scratch {
-  MetaA *ma = nullptr;  // one allocation: ma | mb | base | gh2 | core, n_lines records each
+  MetaA *ma = nullptr;  // one allocation: ma | mb | base | gh2 | core | near, n_lines records each
   MetaB *mb = nullptr;
   LineBase *base = nullptr;
   LineGH2 *gh2 = nullptr;
   LineCore *core = nullptr;
-  LineF32 *f32 = nullptr;    // FP32 variant only (same allocation, after core)
+  LineNear *near = nullptr;
+  LineF32 *f32 = nullptr;    // FP32 variant only (same allocation, after near)
   int *first_hi = nullptr;   // one allocation: first_hi[nb+1] | first_lo[nb+1] | first_c[nb+1] | queue
   int *first_lo = nullptr;
   int *first_c = nullptr;
@@ -1054,12 +1180,13 @@ static int scratch_reserve(Scratch &s, int64_t n_lines, int nb, bool f32, cudaSt
     void *p = nullptr;
     int rc = pool_alloc(&p, n * (kBytesPerLine + (f32 ? sizeof(LineF32) : 0)), st);
     if (rc != HK_OK) return rc;
-    if (f32) s.f32 = (LineF32 *)((char *)p + n * 128);
+    if (f32) s.f32 = (LineF32 *)((char *)p + n * kBytesPerLine);
     s.ma = (MetaA *)p;
     s.mb = (MetaB *)((char *)p + n * 16);
     s.base = (LineBase *)((char *)p + n * 32);
     s.gh2 = (LineGH2 *)((char *)p + n * 64);
     s.core = (LineCore *)((char *)p + n * 96);
+    s.near = (LineNear *)((char *)p + n * 128);
     s.cap_lines = n_lines;
   }
   if (nb > s.cap_blocks) {
@@ -1180,30 +1307,31 @@ static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double 
   pa.inv_mg = 1.0 / m_g;
   pa.q_ratio = q_ratio;
   pa.nu_min = nu_min; pa.dnu = dnu; pa.cutoff = cutoff; pa.N = (int)N;
-  pa.margin = 2.0 + 2.4e-7 * (double)N;
   pa.R2 = f32 ? kR2f : kR2; pa.R3 = f32 ? kR3f : kR3; pa.f32_ladder = f32 ? 1 : 0;
   pa.f32 = f32 ? s.f32 : nullptr;
-  pa.ma = s.ma; pa.mb = s.mb; pa.base = s.base; pa.gh2 = s.gh2; pa.core = s.core;
+  pa.ma = s.ma; pa.mb = s.mb; pa.base = s.base; pa.gh2 = s.gh2; pa.core = s.core; pa.near = s.near;
   pa.nb = nb; pa.first_hi = s.first_hi; pa.first_lo = s.first_lo; pa.first_c = s.first_c; pa.queue = s.queue;
   line_prep_kernel<<<(unsigned)((n_lines + 255) / 256), 256, 0, st>>>(pa);
   HK_CUDA(cudaGetLastError());
   if (g_timing) HK_CUDA(cudaEventRecord(ev[1], st));
   VoigtArgs va;
-  va.ma = s.ma; va.mb = s.mb; va.base = s.base; va.gh2 = s.gh2; va.core = s.core; va.f32 = pa.f32;
+  va.ma = s.ma; va.mb = s.mb; va.base = s.base; va.gh2 = s.gh2; va.core = s.core; va.near = s.near; va.f32 = pa.f32;
   va.dnu_f = (float)dnu;
   va.first_hi = s.first_hi; va.first_lo = s.first_lo; va.first_c = s.first_c; va.queue = s.queue;
   va.nb = nb; va.n_tiles = n_tiles;
   va.nu_min = nu_min; va.dnu = dnu; va.N = (int)N; va.kappa = kappa_out; va.accumulate = prm.accumulate ? 1 : 0;
   {
-    // bound on the 2-point radius (grid units) of any line that can be near grid point j: r2 <= s*alpha/dnu + margin with
-    // alpha = vth*nu0 and nu0 <= nu_j + r2*dnu, s = sqrt(kR2)  =>  r2 <= (s*vth*(nu_min/dnu + j) + margin)/(1 - s*vth)
-    const double sv = sqrt(pa.R2) * pa.vth;
+    // bound on the 3-ball radius (grid units) of any line that can have grid point j inside its 3-ball:
+    // r3 <= s*alpha/dnu with alpha = vth*nu0 and nu0 <= nu_j + r3*dnu, s^2 = max(R3, Gaussian-term radius) (a hair more)
+    //   =>  r3 <= s*vth*(nu_min/dnu + j)/(1 - s*vth)
+    const double sv = sqrt(fmax(pa.R3, kXgCapSq) + 1.0) * pa.vth;
     if (sv < 0.5) {
-      va.r2_slope = sv / (1.0 - sv);
-      va.r2_offset = (sv * fmax(nu_min / dnu, 0.0) + pa.margin + 4.0) / (1.0 - sv);
+      va.r3_slope = sv / (1.0 - sv);
+      // (FP32 variant: a line with alpha^2 < 1e-9 sends its whole 1-ball, radius <= 200 alpha < 6.4e-3 cm^-1, to this kernel)
+      va.r3_offset = (sv * fmax(nu_min / dnu, 0.0) + 4.0 + (f32 ? 6.4e-3 / dnu : 0.0)) / (1.0 - sv);
     } else {  // absurdly hot / light: no useful bound, the near kernel scans every line that touches the span
-      va.r2_slope = 0.0;
-      va.r2_offset = 4.0e9;
+      va.r3_slope = 0.0;
+      va.r3_offset = 4.0e9;
     }
   }
   if (f32) voigt_far_kernel<kP, kWarpsF, kMinBF, true><<<grid, kWarpsF * 32, sizeof(VoigtSmemF), st>>>(va);
@@ -1214,7 +1342,7 @@ static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double 
   for (int c = 0; c < nch; ++c) {
     const int b_lo = (int)((int64_t)nb * c / nch), b_hi = (int)((int64_t)nb * (c + 1) / nch);
     va.block0 = b_lo;
-    voigt_near_kernel<<<b_hi - b_lo, kNearWarps * 32, 0, st>>>(va);
+    voigt_near_kernel<<<b_hi - b_lo, 32, 0, st>>>(va);
     HK_CUDA(cudaGetLastError());
     if (chunks) {
       chunks->hi[c] = std::min<int64_t>((int64_t)b_hi * kPlanBlock, N);

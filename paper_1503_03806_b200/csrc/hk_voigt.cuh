@@ -147,6 +147,15 @@ __device__ __forceinline__ void gh2_acc2f(float &a0, float &a1, float d0, float 
   a0 = fmaf(B0 * D1, r, a0);
   a1 = fmaf(B1 * D0, r, a1);
 }
+// 3-point rule in float (FP32 variant: from r^2 >= 64), one reciprocal per point (R D ~ d^6 would leave the float range in
+// a product over two points)
+__device__ __forceinline__ float gh3_accf(float acc, float d, float g2, float e3, float f3, float c0, float c3, float c3a)
+{
+  const float R = fmaf(d, d, g2), E = fmaf(d, d, e3);
+  const float D = fmaf(E, E, f3), B = fmaf(c3, E, c3a);
+  const float num = fmaf(c0, D, B * R);
+  return fmaf(num, rcpf(R * D), acc);
+}
 // per-line constants of one +-t pair of the 6-point rule: E = q + e, value = (cE * E + c0) / (E^2 + f)
 struct GhPair {
   double e, f, cE, c0;
@@ -190,7 +199,8 @@ __device__ __forceinline__ double gh6_val(double q, const Gh6 &g)
 // immediates arrive by UMOV pairs, and it guards the range): the near kernel is issue-bound, not FP64-bound.
 __constant__ double kExpTaylor[12] = {1.0, 1.0, 0.5, 1.0 / 6, 1.0 / 24, 1.0 / 120, 1.0 / 720, 1.0 / 5040, 1.0 / 40320,
                                       1.0 / 362880, 1.0 / 3628800, 1.0 / 39916800};
-__device__ __forceinline__ double exp_fast(double x)
+template <int DEG>
+__device__ __forceinline__ double exp_poly(double x)
 {
   const double kMagic = 6755399441055744.0;  // 1.5 * 2^52
   const double t = fma(x, 1.4426950408889634074, kMagic);
@@ -198,11 +208,14 @@ __device__ __forceinline__ double exp_fast(double x)
   const double nd = t - kMagic;
   double r = fma(nd, -6.93147180369123816490e-01, x);  // ln2 high part (its low 21 bits are zero)
   r = fma(nd, -1.90821492927058770002e-10, r);         // ln2 low part
-  double p = kExpTaylor[11];
+  double p = kExpTaylor[DEG];
 #pragma unroll
-  for (int k = 10; k >= 0; --k) p = fma(p, r, kExpTaylor[k]);
+  for (int k = DEG - 1; k >= 0; --k) p = fma(p, r, kExpTaylor[k]);
   return __hiloint2double(__double2hiint(p) + (n << 20), __double2loint(p));
 }
+__device__ __forceinline__ double exp_fast(double x) { return exp_poly<11>(x); }
+// the series' own exponentials: degree 8 (remainder (ln2/2)^9/9! = 2e-10 relative; the series itself is truncated at 1.1e-8)
+__device__ __forceinline__ double exp_series(double x) { return exp_poly<8>(x); }
 
 // sin(t)^2 for 0 <= t < 1e4 (the series calls it with t = x y <= 44): k = rint(t/pi) by the magic-number add, r = t - k pi in
 // two pieces (|r| <= pi/2; the sign of sin(t) = (-1)^k sin(r) does not matter for the square), sin(r) = r P(r^2) with the
@@ -210,7 +223,8 @@ __device__ __forceinline__ double exp_fast(double x)
 // sin^2(xy)/y -> x^2 y as y -> 0 needs it).  14 FP64 instructions; the library sinpi costs about twice the issue slots.
 __constant__ double kSinTaylor[10] = {1.0, -1.0 / 6, 1.0 / 120, -1.0 / 5040, 1.0 / 362880, -1.0 / 39916800, 1.0 / 6227020800.0,
                                       -1.0 / 1307674368000.0, 1.0 / 355687428096000.0, -1.0 / 121645100408832000.0};
-__device__ __forceinline__ double sin_sq_fast(double t)
+template <int STEPS>
+__device__ __forceinline__ double sin_sq_poly(double t)
 {
   const double kMagic = 6755399441055744.0;  // 1.5 * 2^52
   const double kd = fma(t, 0.31830988618379067154, kMagic) - kMagic;
@@ -218,81 +232,90 @@ __device__ __forceinline__ double sin_sq_fast(double t)
   r = fma(kd, -1.98418714791870343106e-09, r);         // pi middle part
   r = fma(kd, -1.14423774522196636802e-17, r);         // pi low part
   const double q = r * r;
-  double p = kSinTaylor[9];
+  double p = kSinTaylor[STEPS];
 #pragma unroll
-  for (int k = 8; k >= 0; --k) p = fma(p, q, kSinTaylor[k]);
+  for (int k = STEPS - 1; k >= 0; --k) p = fma(p, q, kSinTaylor[k]);
   return q * p * p;
 }
+__device__ __forceinline__ double sin_sq_fast(double t) { return sin_sq_poly<9>(t); }
+// the series' own: sin(r)/r to degree 12 in r (remainder (pi/2)^14/15! = 4e-10 relative)
+__device__ __forceinline__ double sin_sq_series(double t) { return sin_sq_poly<6>(t); }
 
 // ---- core: Algorithm-916-type series (restated in DESIGN.md §4) ---------------------------
 //   K(x,y) = exp(-x^2) [ erfcx(y) cos(2xy) + (2a/pi) sin^2(xy)/y - (2a/pi) y cos(2xy) S1(y)
 //                        + (a/pi) y sum_{n=1..16} W_n (p^n + p^-n) ],
 //   W_n = exp(-a^2 n^2)/(a^2 n^2 + y^2),  S1 = sum_n W_n,  p = exp(2 a x)
-// (exp(-(an-x)^2) + exp(-(an+x)^2) = exp(-x^2) exp(-a^2 n^2) (p^n + p^-n)).  y is a per-line constant: lane n-1 of the
-// warp computes W_n into a 16-entry shared-memory table and the series loop reads it by broadcast (one LDS.128 per two terms); C_n = p^n + p^-n advances by the three-term recurrence
-// C_{n+2} = ((p + 1/p)^2 - 2) C_n - C_{n-2} (forward-stable: the growing solution dominates), so a term is 2 DFMA + 1 SHFL.
-// p^16 <= exp(1.4 * 6.64 * 16) = 4e64: no overflow for x <= sqrt(44).
-struct CoreLine {
-  double y, inv_y, erfcx_y, S1;
-  const double *W;  // the warp's shared-memory table W_1 .. W_16 (read by broadcast in the series loop)
+// (exp(-(an-x)^2) + exp(-(an+x)^2) = exp(-x^2) exp(-a^2 n^2) (p^n + p^-n)).  With cos(2xy) = 1 - 2 sin^2(xy) the bracket is
+//   E0 + sin^2(xy) B2 + (a/pi) y sum,     E0 = erfcx(y) - (2a/pi) y S1,   B2 = (2a/pi)/y - 2 E0.
+// y is a per-line constant: E0, B2 and the 16 weights W_n are computed once per line (SeriesLine + a 16-entry table in
+// shared memory, read by broadcast in the series loop, one LDS.128 per two terms) and carry the line's amplitude.
+// C_n = p^n + p^-n advances by the three-term recurrence C_{n+2} = ((p + 1/p)^2 - 2) C_n - C_{n-2} (forward-stable: the
+// growing solution dominates) in two independent chains (odd and even n), so a term is 2 DFMA.
+// p^16 <= exp(1.4 * 6.7 * 16) = 1e65: no overflow for x <= 6.7.
+__constant__ double kSeriesEn[kTerms] = {  // exp(-a^2 n^2), n = 1..16
+    0.612626394184416069,    0.140858420921044996,    0.0121551783299149372,   0.000393669040655078211,
+    4.78511739212900909e-6,  2.18295779512547921e-8,  3.73757132794426203e-11, 2.40173478162095945e-14,
+    5.79231288539485792e-18, 5.24288566336346394e-22, 1.78106663475709136e-26, 2.27081292202639651e-31,
+    1.08661064074598053e-36, 1.95145238029537775e-42, 1.31532589485746453e-48, 3.32736305418299429e-55};
+
+struct SeriesLine {
+  double inv_alpha;  // x = |d| / alpha
+  double y;          // gamma/alpha (>= 1e-200: line prep floors it)
+  double Aay;        // A (a/pi) y,    A = amp/(alpha sqrt(pi)): the result is amp * V(d)
+  double AE0;        // A E0
+  double AB2;        // A B2
 };
 
-// exp(-a^2 n^2) for n = lane + 1 (0 beyond the 16 terms): a per-lane constant, computed once per kernel
-__device__ __forceinline__ double core_lane_const()
+// Per-line constants of the series, by ONE thread: writes W_1..W_16 to W[0..15] and returns the rest.
+__device__ __forceinline__ SeriesLine series_line_setup(double y, double inv_y, double erfcx_y, double Acore, double inv_alpha,
+                                                        double *W)
 {
-  const int lane = threadIdx.x & 31;
-  const double n = (double)(lane + 1);
-  return lane < kTerms ? exp(-kA * kA * n * n) : 0.0;
-}
-
-// All 32 lanes must call (warp-collective).  En = core_lane_const(); Wsm = kTerms doubles of shared memory owned by the warp.
-__device__ __forceinline__ CoreLine core_setup(double y, double inv_y, double erfcx_y, double En, double *Wsm)
-{
-  CoreLine c;
-  const int lane = threadIdx.x & 31;
-  const double n = (double)(lane + 1);
-  c.y = y;
-  c.inv_y = inv_y;
-  c.erfcx_y = erfcx_y;
-  c.W = Wsm;
-  const double W = En * rcp_nr2(fma(kA * kA * n, n, y * y));
-  __syncwarp();  // readers of the previous line's table are done
-  if (lane < kTerms) Wsm[lane] = W;
-  double t = W;
+  const double y2 = y * y;
+  double S1 = 0.0;
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(kFull, t, o);
-  c.S1 = t;
-  __syncwarp();
-  return c;
+  for (int n = 1; n <= kTerms; ++n) {
+    const double w = kSeriesEn[n - 1] * rcp_nr2(fma(kA * kA * (double)n, (double)n, y2));
+    W[n - 1] = w;
+    S1 += w;
+  }
+  const double E0 = fma(-k2AoverPi * y, S1, erfcx_y);
+  SeriesLine L;
+  L.inv_alpha = inv_alpha;
+  L.y = y;
+  L.Aay = Acore * (kAoverPi * y);
+  L.AE0 = Acore * E0;
+  L.AB2 = Acore * fma(k2AoverPi, inv_y, -2.0 * E0);
+  return L;
 }
 
-// Lanes of a warp call with the same CoreLine.  0 <= x <= 6.7.
-__device__ __forceinline__ double core_K(double x, const CoreLine &c)
+// amp * V(d) by the series, |d| / alpha clamped at 6.7 (callers mask the points beyond the series region).  About 90 FP64
+// instructions: two exponentials (13 each), reciprocal (3), recurrence and sums (35), sin^2 (13), the rest head and tail.
+__device__ __forceinline__ double series_val(double d, const SeriesLine &L, const double *W)
 {
-  const double ex2 = exp_fast(-x * x);
-  const double p = exp_fast(2.0 * kA * x);
-  const double s2c = p + rcp_nr2(p);  // 2 cosh(2 a x) = C_1
-  // C_n = p^n + p^-n in two independent chains (odd and even n) with the step-2 recurrence C_{n+2} = (C_1^2 - 2) C_n - C_{n-2},
-  // C_{-1} = C_1, C_0 = 2, C_2 = C_1^2 - 2: the dependent-DFMA path is 8 long instead of 16 (this loop is latency-bound at
-  // the near kernel's 4 warps per scheduler)
+  const double x = fmin(fabs(d) * L.inv_alpha, 6.7);
+  const double ex2 = exp_series(-x * x);
+  const double p = exp_series((2.0 * kA) * x);
+  const double s2 = sin_sq_series(x * L.y);
+  const double s2c = p + rcp_nr(p);  // 2 cosh(2 a x) = C_1
   const double t2 = fma(s2c, s2c, -2.0);
-  double Com = s2c, Co = s2c, Cem = 2.0, Ce = t2, so = 0.0, se = 0.0;
+  double Com = s2c, Co = s2c, Cem = 2.0, Ce = t2, so = 0.0, se = 0.0;  // C_{-1} = C_1, C_0 = 2, C_2 = C_1^2 - 2
 #pragma unroll
   for (int i = 0; i < kTerms / 2; ++i) {
-    const double wo = c.W[2 * i], we = c.W[2 * i + 1];
-    so = fma(wo, Co, so);
-    se = fma(we, Ce, se);
+    const double2 w = *reinterpret_cast<const double2 *>(W + 2 * i);
+    so = fma(w.x, Co, so);
+    se = fma(w.y, Ce, se);
     const double Con = fma(t2, Co, -Com), Cen = fma(t2, Ce, -Cem);
     Com = Co; Co = Con;
     Cem = Ce; Ce = Cen;
   }
-  const double sum = so + se;
-  const double s2 = sin_sq_fast(x * c.y);
-  const double c2 = fma(-2.0, s2, 1.0);
-  const double head = fma(c.erfcx_y, c2, k2AoverPi * (s2 * c.inv_y)) - k2AoverPi * c.y * c2 * c.S1;
-  return ex2 * fma(kAoverPi * c.y, sum, head);
+  const double head = fma(s2, L.AB2, L.AE0);
+  return ex2 * fma(L.Aay, so + se, head);
 }
 
+// Where the kernels switch between the series and the 6-point rule: the series is valid for every x <= 6.7 and the 6-point
+// rule wherever x^2 + y^2 >= 44, so any switch with 44 - y^2 <= x^2 <= 44.89 is valid; a1 puts it at x^2 = 44.15 - y^2, in
+// index space (the band is wide enough that no rounding of the FP64 index arithmetic can leave it).
+constexpr double kSeriesPad = 0.15;
 // series region of a line of damping y: x^2 < xc2 = 44 - y^2 (none for y >= sqrt(44))
 __device__ __host__ __forceinline__ double core_xc2(double y)
 {
