@@ -658,15 +658,28 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) voigt_far_kernel(const __gri
     for (int b0 = 0; b0 < h.cnt; b0 += 32) {
       const SpanMasks M = classify32(S.ma[stage] + b0, S.mb[stage] + b0, lane, h.cnt - b0, slo, shi);
       // ---- 1-point rule ----
+      // (the next line's record is fetched before the current line's arithmetic: the bit scan and the shared-memory load
+      // would otherwise sit at the head of every iteration's dependency chain)
+      if (M.m1) {
+        unsigned m = M.m1;
+        int li = __ffs(m) - 1;
+        LineBase cur = sbase[b0 + li];
+        m &= m - 1;
 #pragma unroll 1
-      for (unsigned m = M.m1; m; m &= m - 1) {
-        const LineBase *pb = sbase + b0 + (__ffs(m) - 1);
-        const double nu0 = pb->nu0, A1 = pb->A1, g2 = fma(-1.5, pb->a2, pb->g2);  // shifted denominator (kR1a)
-        const double d0 = x0 - nu0;
+        for (;;) {
+          const bool more = m != 0u;
+          li = more ? __ffs(m) - 1 : li;  // branch-free: the last iteration re-reads its own record
+          const LineBase nxt = sbase[b0 + li];
+          m &= m - 1;
+          const double A1 = cur.A1, g2 = fma(-1.5, cur.a2, cur.g2);  // shifted denominator (kR1a)
+          const double d0 = x0 - cur.nu0;
 #pragma unroll
-        for (int k = 0; k < P; k += 2)
-          gh1_acc2(acc[k], acc[k + 1], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), fma((double)(32 * k + 32), a.dnu, d0),
-                   A1, g2);
+          for (int k = 0; k < P; k += 2)
+            gh1_acc2(acc[k], acc[k + 1], (k == 0 ? d0 : fma((double)(32 * k), a.dnu, d0)), fma((double)(32 * k + 32), a.dnu, d0),
+                     A1, g2);
+          if (!more) break;
+          cur = nxt;
+        }
       }
       // ---- 2-point rule ----
 #pragma unroll 1
@@ -782,8 +795,9 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) voigt_far_kernel(const __gri
 // The warp walks the lines centred within the span's bound on the 3-ball radius (a2 table first_c) 32 at a time, lane = line:
 // a lane whose line has groups of this span inside its 3-ball (and inside its window) computes everything that depends on
 // the line alone — the constants of the 6-point rule, the 16 series weights W_n and the folded series constants — ONCE, into
-// a shared-memory slot, and writes the line's work as uniform ITEMS into two queues:
-//   6-point items  (line, group k): the group's points that are in the window and outside the series interval;
+// a shared-memory slot, and writes the line's work as uniform ITEMS into queues:
+//   6-point items  (line), one queue per group k of the span: the group's points that are in the window and outside the
+//                  series interval; a queue is summed in registers and added to the strip once;
 //   series items   (line, first point, count <= 32): chunks of the series interval [jslo, jshi] taken from ITS lower end, not
 //                  from the group grid, so that only the last chunk of a line has idle lanes.
 // Then the warp works the queues off, two items per iteration (two independent dependency chains per thread), each item one
@@ -791,23 +805,22 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) voigt_far_kernel(const __gri
 // recomputed per group.  Sums are kept in a shared-memory strip that starts as the kappa the far kernel wrote (fetched by
 // cp.async while the lines are being listed) and is stored back at the end; order of summation is fixed.
 constexpr int kNearP = kPlanBlock / 32;
-constexpr int kNearCap = 32;       // lines per round: one per lane
-constexpr int kWStride = kTerms + 2;  // doubles per row of the W table: rows 16-byte aligned, lanes spread over the banks
-constexpr int kG6Stride = 14;         // likewise for the 12 constants of the 6-point rule
+constexpr int kNearCap = 32;  // lines per round: one per lane
 #ifndef HK_NEAR_MINB
 #define HK_NEAR_MINB 16
 #endif
 
 struct __align__(16) NearSmem {
   double sk[kPlanBlock];
-  double W[kNearCap][kWStride];
-  double g6[kNearCap][kG6Stride];  // e, f, cE, c0 of the three +-t pairs
+  double W[kNearCap][kTerms];
+  double g6[kNearCap][12];  // e, f, cE, c0 of the three +-t pairs
   double nu0[kNearCap];
-  SeriesLine ser[kNearCap];        // 5 doubles
+  SeriesLine ser[kNearCap];  // 5 doubles
   double Acore[kNearCap];
-  int jlo[kNearCap], jhi[kNearCap], jslo[kNearCap], jshi[kNearCap], tiny[kNearCap];
-  unsigned short q6[kNearCap * kNearP];
+  int4 win[kNearCap];        // jlo, jhi - jlo + 1, jslo, jshi - jslo + 1 (0: no series points): two unsigned range tests
   unsigned int qs[kNearCap * (kNearP + 1)];
+  unsigned char q6[kNearP][kNearCap];  // slot | tiny << 5
+  int n6[kNearP];
 };
 
 __device__ __forceinline__ void cp_async8(void *smem_dst, const void *gmem_src)
@@ -816,10 +829,13 @@ __device__ __forceinline__ void cp_async8(void *smem_dst, const void *gmem_src)
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
-// one 6-point item: group k of the span, line slot e
-__device__ __forceinline__ double near_gh6_item(const NearSmem &S, int e, int k, int plo, int lane, double x0, double dnu, bool &ok)
+// one 6-point item: line slot u & 31 (bit 5: the line adds the Gaussian term) on the group whose point of this lane is j, at
+// nu = xk; 0 outside the window and inside the series interval
+__device__ __forceinline__ double near_gh6_item(const NearSmem &S, unsigned u, int j, double xk)
 {
-  const double d = fma((double)(32 * k), dnu, x0) - S.nu0[e];
+  const int e = u & 31;
+  const double d = xk - S.nu0[e];
+  const int4 w = S.win[e];
   const double *c = S.g6[e];
   const double2 c0 = *reinterpret_cast<const double2 *>(c), c1 = *reinterpret_cast<const double2 *>(c + 2),
                 c2 = *reinterpret_cast<const double2 *>(c + 4), c3 = *reinterpret_cast<const double2 *>(c + 6),
@@ -830,20 +846,21 @@ __device__ __forceinline__ double near_gh6_item(const NearSmem &S, int e, int k,
   G.p2.e = c4.x; G.p2.f = c4.y; G.p2.cE = c5.x; G.p2.c0 = c5.y;
   const double q = d * d;
   double v = gh6_val(q, G);
-  if (S.tiny[e]) {  // warp-uniform: y < 1e-8, the Gaussian term is still visible beyond the series region
+  if (u & 32u) {  // warp-uniform: y < 1e-8, the Gaussian term is still visible beyond the series region
     const double ia = S.ser[e].inv_alpha;
     v = fma(S.Acore[e], exp_fast(fmax(-(q * ia) * ia, -700.0)), v);
   }
-  const int j = plo + 32 * k + lane;
-  ok = (j >= S.jlo[e]) && (j <= S.jhi[e]) && !((j >= S.jslo[e]) && (j <= S.jshi[e]));
-  return v;
+  const bool ok = ((unsigned)(j - w.x) < (unsigned)w.y) & !((unsigned)(j - w.z) < (unsigned)w.w);
+  return ok ? v : 0.0;
 }
 
 __global__ void __launch_bounds__(32, HK_NEAR_MINB) voigt_near_kernel(const __grid_constant__ VoigtArgs a)
 {
   __shared__ NearSmem S;
   const int lane = threadIdx.x;
-  const int b = a.block0 + (int)blockIdx.x;
+  // spans from the top of the launch's range down: lines widen with wavenumber, so the heavier spans start first and the
+  // light ones fill the tail
+  const int b = a.block0 + ((int)gridDim.x - 1 - (int)blockIdx.x);
   const int plo = b * kPlanBlock, phi = min(plo + kPlanBlock, a.N) - 1;
   // lines that can have a point of this span in their 3-ball: centre within R of it, and window touching it
   const double R = fmax(fma(a.r3_slope, (double)phi, a.r3_offset), 4.0);
@@ -876,9 +893,10 @@ __global__ void __launch_bounds__(32, HK_NEAR_MINB) voigt_near_kernel(const __gr
     const bool listed = kA <= kB;
     const unsigned lm = __ballot_sync(kFull, listed);
     if (lm == 0u) continue;
-    const int e = __popc(lm & ((1u << lane) - 1u));  // slot
-    unsigned cnt = 0u;                               // 6-point items | series items << 16
-    int kS0 = 8, kS1 = -1, sa = 0, sb = -1;
+    const unsigned lt = (1u << lane) - 1u;
+    const int e = __popc(lm & lt);  // slot
+    int ns = 0, kS0 = 8, kS1 = -1, sa = 0, sb = -1;
+    unsigned tiny = 0u;
     if (listed) {
       const LineBase lb = a.base[i];
       const LineCore lc = a.core[i];
@@ -886,40 +904,47 @@ __global__ void __launch_bounds__(32, HK_NEAR_MINB) voigt_near_kernel(const __gr
       const double inv_alpha = a.gh2[i].inv_alpha;
       const int sa0 = max(ln.jslo, plo + 32 * kA), sb0 = min(ln.jshi, plo + 32 * kB + 31);  // series points in these groups
       if (sa0 <= sb0) {
-        kS0 = (sa0 - plo + 31) >> 5;        // groups wholly inside the series interval: no 6-point item
+        kS0 = (sa0 - plo + 31) >> 5;  // groups wholly inside the series interval: no 6-point item
         kS1 = ((sb0 - plo + 1) >> 5) - 1;
         sa = max(sa0, A.jlo);
         sb = min(sb0, A.jhi);
       }
-      const int n6 = (kB - kA + 1) - max(kS1 - kS0 + 1, 0);
-      const int ns = sb >= sa ? ((sb - sa) >> 5) + 1 : 0;
-      cnt = (unsigned)n6 | ((unsigned)ns << 16);
+      ns = sb >= sa ? ((sb - sa) >> 5) + 1 : 0;
+      tiny = ln.tiny ? 32u : 0u;
       S.nu0[e] = lb.nu0;
       S.Acore[e] = lc.Acore;
-      S.jlo[e] = A.jlo; S.jhi[e] = A.jhi; S.jslo[e] = ln.jslo; S.jshi[e] = ln.jshi; S.tiny[e] = ln.tiny;
-      if (n6 > 0) {
+      S.win[e] = make_int4(A.jlo, A.jhi - A.jlo + 1, ln.jslo <= ln.jshi ? ln.jslo : 0, ln.jslo <= ln.jshi ? ln.jshi - ln.jslo + 1 : 0);
+      if ((kB - kA + 1) > max(kS1 - kS0 + 1, 0)) {
         const Gh6 G = gh6_consts(lb.A1, lb.g2, lb.a2);
         double *c = S.g6[e];
-        c[0] = G.p0.e; c[1] = G.p0.f; c[2] = G.p0.cE; c[3] = G.p0.c0;
-        c[4] = G.p1.e; c[5] = G.p1.f; c[6] = G.p1.cE; c[7] = G.p1.c0;
-        c[8] = G.p2.e; c[9] = G.p2.f; c[10] = G.p2.cE; c[11] = G.p2.c0;
+        *reinterpret_cast<double2 *>(c) = make_double2(G.p0.e, G.p0.f);
+        *reinterpret_cast<double2 *>(c + 2) = make_double2(G.p0.cE, G.p0.c0);
+        *reinterpret_cast<double2 *>(c + 4) = make_double2(G.p1.e, G.p1.f);
+        *reinterpret_cast<double2 *>(c + 6) = make_double2(G.p1.cE, G.p1.c0);
+        *reinterpret_cast<double2 *>(c + 8) = make_double2(G.p2.e, G.p2.f);
+        *reinterpret_cast<double2 *>(c + 10) = make_double2(G.p2.cE, G.p2.c0);
       }
       if (ns > 0) S.ser[e] = series_line_setup(lc.y, lc.inv_y, lc.erfcx_y, lc.Acore, inv_alpha, S.W[e]);
       else S.ser[e].inv_alpha = inv_alpha;  // the Gaussian term of a tiny-y line reads it
     }
-    // exclusive scan of the item counts over the lanes, both queues at once
-    unsigned incl = cnt;
+    // 6-point queues, one per group: ballot = the lines with an item there, in line order
+#pragma unroll
+    for (int k = 0; k < kNearP; ++k) {
+      const bool has = listed && k >= kA && k <= kB && (k < kS0 || k > kS1);
+      const unsigned bk = __ballot_sync(kFull, has);
+      if (has) S.q6[k][__popc(bk & lt)] = (unsigned char)((unsigned)e | tiny);
+      if (lane == 0) S.n6[k] = __popc(bk);
+    }
+    // series queue: exclusive scan of the chunk counts over the lanes
+    int incl = ns;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
-      const unsigned t = __shfl_up_sync(kFull, incl, o);
+      const int t = __shfl_up_sync(kFull, incl, o);
       if (lane >= o) incl += t;
     }
-    const unsigned tot = __shfl_sync(kFull, incl, 31);
-    const int n6tot = (int)(tot & 0xffffu), nstot = (int)(tot >> 16);
-    if (listed) {
-      int o6 = (int)((incl - cnt) & 0xffffu), os = (int)((incl - cnt) >> 16);
-      for (int k = kA; k <= kB; ++k)
-        if (k < kS0 || k > kS1) S.q6[o6++] = (unsigned short)((e << 3) | k);
+    const int nstot = __shfl_sync(kFull, incl, 31);
+    {
+      int os = incl - ns;
       for (int j = sa; j <= sb; j += 32)
         S.qs[os++] = (unsigned)e | ((unsigned)(j - plo) << 8) | ((unsigned)(min(sb - j, 31)) << 16);
     }
@@ -927,35 +952,37 @@ __global__ void __launch_bounds__(32, HK_NEAR_MINB) voigt_near_kernel(const __gr
     any = true;
     __syncwarp();
 
-    // ---- 6-point items, two per iteration: group-aligned, so a thread meets only its own strip entries ----
-    {
-      int it = 0;
+    // ---- 6-point items, group by group, two per iteration, summed in registers ----
 #pragma unroll 1
-      for (; it + 1 < n6tot; it += 2) {
-        const unsigned u0 = S.q6[it], u1 = S.q6[it + 1];
-        const int k0 = u0 & 7, k1 = u1 & 7;
-        bool ok0, ok1;
-        const double v0 = near_gh6_item(S, u0 >> 3, k0, plo, lane, x0, a.dnu, ok0);
-        const double v1 = near_gh6_item(S, u1 >> 3, k1, plo, lane, x0, a.dnu, ok1);
-        S.sk[32 * k0 + lane] += ok0 ? v0 : 0.0;
-        S.sk[32 * k1 + lane] += ok1 ? v1 : 0.0;
+    for (int k = 0; k < kNearP; ++k) {
+      const int n = S.n6[k];
+      if (n == 0) continue;
+      const double xk = fma((double)(32 * k), a.dnu, x0);
+      const int j = plo + 32 * k + lane;
+      const unsigned char *q = S.q6[k];
+      double s0 = 0.0, s1 = 0.0;
+      int it = 0;
+      unsigned nxt = *reinterpret_cast<const unsigned short *>(q);
+#pragma unroll 1
+      for (; it + 1 < n; it += 2) {
+        const unsigned u = nxt;
+        nxt = *reinterpret_cast<const unsigned short *>(q + ((it + 2) & 31));
+        s0 += near_gh6_item(S, u & 255u, j, xk);
+        s1 += near_gh6_item(S, u >> 8, j, xk);
       }
-      if (it < n6tot) {
-        const unsigned u0 = S.q6[it];
-        const int k0 = u0 & 7;
-        bool ok0;
-        const double v0 = near_gh6_item(S, u0 >> 3, k0, plo, lane, x0, a.dnu, ok0);
-        S.sk[32 * k0 + lane] += ok0 ? v0 : 0.0;
-      }
+      if (it < n) s0 += near_gh6_item(S, nxt & 255u, j, xk);
+      S.sk[32 * k + lane] += s0 + s1;
     }
     __syncwarp();
     // ---- series items, two per iteration: point-aligned, so the strip entries of two items may belong to different
     //      lanes: the additions are ordered by __syncwarp ----
     {
       int it = 0;
+      uint2 nxt = *reinterpret_cast<const uint2 *>(S.qs);
 #pragma unroll 1
       for (; it + 1 < nstot; it += 2) {
-        const unsigned u0 = S.qs[it], u1 = S.qs[it + 1];
+        const unsigned u0 = nxt.x, u1 = nxt.y;
+        nxt = *reinterpret_cast<const uint2 *>(S.qs + it + 2);
         const int e0 = u0 & 31, e1 = u1 & 31, off0 = (u0 >> 8) & 255, off1 = (u1 >> 8) & 255;
         const double d0 = fma((double)off0, a.dnu, x0) - S.nu0[e0], d1 = fma((double)off1, a.dnu, x0) - S.nu0[e1];
         const SeriesLine Ls0 = S.ser[e0], Ls1 = S.ser[e1];
@@ -967,7 +994,7 @@ __global__ void __launch_bounds__(32, HK_NEAR_MINB) voigt_near_kernel(const __gr
         __syncwarp();
       }
       if (it < nstot) {
-        const unsigned u0 = S.qs[it];
+        const unsigned u0 = nxt.x;
         const int e0 = u0 & 31, off0 = (u0 >> 8) & 255;
         const double d0 = fma((double)off0, a.dnu, x0) - S.nu0[e0];
         const SeriesLine Ls0 = S.ser[e0];
