@@ -17,14 +17,20 @@
  * Conventions
  *   - Every pointer marked "device" is a CUDA device pointer (e.g. torch .data_ptr()); "host" is host memory.
  *     All arrays are contiguous float64 unless stated.  Inputs are read-only and caller-owned; outputs are
- *     caller-allocated and are OVERWRITTEN, never accumulated into.
+ *     caller-allocated and are OVERWRITTEN — with one exception, kappa_out under hk_params.accumulate = 1 (a mixture's
+ *     running sum), which is added to.
  *   - Calls enqueue work on `stream` (a cudaStream_t passed as void*; NULL = the legacy default stream) and
  *     return without synchronising, except where stated; the caller synchronises before reading results.
  *     Scratch memory is taken from the library's own stream-ordered CUDA memory pool (one per device, kept for reuse)
  *     and returned to it on the same stream.
  *   - Return value: HK_OK (0) or a negative HK_ERR_* code; hk_strerror() names it; after HK_ERR_CUDA,
- *     hk_last_cuda_error() returns the CUDA runtime's message.  No exceptions, no global mutable state
- *     other than that last-error string.
+ *     hk_last_cuda_error() returns the CUDA runtime's message.  No exceptions.
+ *   - State the library keeps.  Per host thread: the last-error string, the hk_set_timing() switch with its events, and
+ *     the copy stream of hk_opacity_host.  Per device, created on first use under a lock and kept for the life of the
+ *     process: the memory pool (hk_trim() returns its idle memory to the driver), the kernels' shared-memory attributes
+ *     and launch grids, and the Chebyshev projection matrices of hk_kdist_cheb.  Calls may come from several host threads
+ *     and, after cudaSetDevice, for several devices; an hk_ctx belongs to the device and stream it was created on and must
+ *     not be used from two threads at once.
  *   - Units: wavenumbers in cm^-1, T in K, P in atm (1 atm = 1.01325 bar), mass in amu,
  *     S in cm/molecule, kappa in cm^2/g.
  *   - There is no CPU fallback: without a CUDA device every compute entry point returns HK_ERR_CUDA.
@@ -100,7 +106,8 @@ int64_t hk_grid_size(double nu_min, double nu_max, double dnu);
  *
  * K = Re w(x+iy) is evaluated to <= 2.5e-7 relative error: Algorithm-916-type series for x^2+y^2 < 44,
  * 6/3/2-point Gauss-Hermite rules beyond 44 / 280 / 3200, and from max(3600, 4100 y) the 1-point rule with the
- * shifted denominator x^2 + y^2 - 3/2.
+ * shifted denominator x^2 + y^2 - 3/2.  Degenerate lines: nu0 <= 0 (alpha = 0) is a pure
+ * Lorentzian; gamma = 0 (gamma0 = 0 and no natural width) is the pure Doppler profile exp(-x^2)/(alpha sqrt(pi)).
  *
  * Full line physics, active per optional array of hk_lines:
  *   gamma_i = A21_i/(4 pi c) + (296/T)^n_i [ gamma0_i (P - P_self) + gamma_self_i P_self ],  P_self = self_fraction * P   eq. 20
@@ -113,11 +120,12 @@ int64_t hk_grid_size(double nu_min, double nu_max, double dnu);
  * approximation).
  *
  * prm->precision = HK_FP32 (north_star's optional FP32 variant, max relative error <= 1e-4): the same ladder with the
- * switches at 44 / 64 / 300 / max(400, 400 y) (each rule <= 4e-5 from exact K); the 1- and 2-point rules — every (line, 256-point
- * span) pair beyond the 2-point radius, ~99 % of all evaluations — run in FP32 (distances from an integer + fraction
- * split of the line centre in grid units, a float partial sum per 32 lines added to FP64 accumulators); the 3-/6-point
- * rules and the series near the centre stay FP64, as do line prep, the index windows and kappa_out.  Line amplitudes
- * S gamma/(pi m) below 1e-38 flush to zero in this mode.
+ * switches at 44 / 64 / 300 / max(400, 400 y) (each rule <= 4e-5 from exact K); the 1-, 2- and 3-point rules — every 32-point
+ * group outside the line's 3-point radius, ~99.7 % of all evaluations — run in FP32 (distances from an integer + fraction
+ * split of the line centre in grid units, a float partial sum per 32 lines added to FP64 accumulators); the 6-point
+ * rule and the series near the centre stay FP64 (and so do the three grid points on either side of every line centre,
+ * where the float distance would cancel), as do line prep, the index windows and kappa_out.  A line whose amplitude
+ * S gamma/(pi m) is more than 2^-127 below the largest of its batch of 32 flushes to zero in this mode.
  *
  * kappa_out: device, N doubles, overwritten.  Lines outside [nu_min, nu_max) still contribute if within the
  * cutoff.  n_lines == 0 gives kappa == 0.
@@ -235,12 +243,16 @@ int hk_regime_census(const double *nu0_host, const double *gamma0_host, int64_t 
 
 /* Per-stage device time of the last hk_opacity / hk_opacity_ctx call on this thread, in milliseconds, measured
  * with CUDA events on the call's stream: [0] line prep (a1, with the lookup tables of a2), [1] Voigt accumulation, far
- * kernel (1- and 2-point rule, writes kappa), [2] Voigt accumulation, near kernel (3-, 6-point rule and series, adds to
- * kappa); a3 + a4 = [1] + [2].  Enabled by hk_set_timing(1) (off by default).  The timed call stays asynchronous: it only
+ * kernel (1-, 2- and 3-point rule, writes kappa), [2] Voigt accumulation, near kernel (6-point rule and series, adds to
+ * kappa); a3 + a4 = [1] + [2].  Enabled by hk_set_timing(1) (off by default; the switch is per host thread).  The timed call stays asynchronous: it only
  * records the events; hk_last_stage_ms() waits for the last one (synchronous) and must be called before the next timed
  * call. */
 int hk_set_timing(int on);
 int hk_last_stage_ms(float ms_out[3]);
+
+/* Returns the idle memory of the current device's pool to the driver (scratch of a config-4-sized call is otherwise kept
+ * for reuse for the life of the process).  Synchronises the device. */
+int hk_trim(void);
 
 const char *hk_strerror(int code);
 const char *hk_last_cuda_error(void);

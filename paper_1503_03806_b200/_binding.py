@@ -104,6 +104,8 @@ def load_library():
     L.hk_set_timing.argtypes = [C.c_int]
     L.hk_last_stage_ms.restype = C.c_int
     L.hk_last_stage_ms.argtypes = [C.POINTER(C.c_float)]
+    L.hk_trim.restype = C.c_int
+    L.hk_trim.argtypes = []
     L.hk_strerror.restype = C.c_char_p
     L.hk_strerror.argtypes = [C.c_int]
     L.hk_last_cuda_error.restype = C.c_char_p
@@ -339,6 +341,10 @@ def hk_fp32_peak(stream=None) -> float:
     return v.value
 
 
+def hk_trim() -> None:
+    _check(load_library().hk_trim(), "hk_trim")
+
+
 def hk_set_timing(on: bool) -> None:
     _check(load_library().hk_set_timing(int(bool(on))), "hk_set_timing")
 
@@ -350,11 +356,16 @@ def hk_last_stage_ms():
 
 
 class Context:
-    """hk_create / hk_opacity_ctx / hk_destroy: line list bound once, scratch kept across (T,P) calls."""
+    """hk_create / hk_opacity_ctx / hk_destroy: line list bound once, scratch kept across (T,P) calls.
+
+    A Context is bound to ONE stream, the one given (or current) at creation: opacity() launches on it and allocates its
+    result under it, whatever stream is current at the time of the call; a consumer on another stream has to wait for it."""
 
     def __init__(self, lines: Lines, mass_amu=18.0, lines_sorted=True, stream=None, precision=HK_FP64, self_fraction=0.5,
                  abundance=1.0, accumulate=False, cutoff_widths=0.0):
         self._lines = lines      # keep the tensors alive
+        self._stream = stream if stream is not None else _torch().cuda.current_stream()
+        stream = self._stream
         self._h = C.c_void_p()
         cl = lines._c()
         prm = _params(mass_amu, 1.0, precision, lines_sorted, stream, self_fraction, abundance, accumulate, cutoff_widths)
@@ -364,7 +375,8 @@ class Context:
         torch = _torch()
         N = hk_grid_size(nu_min, nu_max, dnu)
         if out is None:
-            out = torch.empty(N, dtype=torch.float64, device=self._lines.nu0.device)
+            with torch.cuda.stream(self._stream):
+                out = torch.empty(N, dtype=torch.float64, device=self._lines.nu0.device)
         _check(load_library().hk_opacity_ctx(self._h, T, P_atm, q_ratio, nu_min, nu_max, dnu, cutoff, _dev_ptr(out, "out")),
                "hk_opacity_ctx")
         return out

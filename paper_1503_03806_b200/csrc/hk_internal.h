@@ -5,7 +5,27 @@
 
 #include "../../include/hk.h"
 
+#include <mutex>
+
 namespace hk {
+
+// A step that must run once per DEVICE (cudaFuncSetAttribute, occupancy queries, memory-pool creation): process-wide
+// `static bool` latches are wrong for a process that drives several GPUs, and unsynchronised ones race between host threads.
+struct PerDeviceOnce {
+  std::mutex mu;
+  uint64_t done = 0;  // bit d: done on device d (devices >= 64: redone on every call)
+  template <class F>
+  int run(F &&f)
+  {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return HK_ERR_CUDA;
+    std::lock_guard<std::mutex> lk(mu);
+    if (dev >= 0 && dev < 64 && ((done >> dev) & 1u)) return HK_OK;
+    const int rc = f(dev);
+    if (rc == HK_OK && dev >= 0 && dev < 64) done |= (uint64_t)1 << dev;
+    return rc;
+  }
+};
 
 // records the CUDA error text for hk_last_cuda_error() and maps it to HK_ERR_NOMEM / HK_ERR_CUDA
 int cuda_fail(cudaError_t e, const char *what);

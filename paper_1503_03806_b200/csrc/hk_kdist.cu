@@ -270,12 +270,12 @@ static int launch_kdist_t(const KdistArgs &a, int64_t n_bins, cudaStream_t st)
 {
   const int T = a.n / E;
   const size_t smem = (size_t)(a.n + 2 * T) * sizeof(double);
-  static bool attr_set = false;
-  if (!attr_set) {
+  static PerDeviceOnce attr;  // one per instantiation; the attribute is a per-device setting
+  const int rca = attr.run([](int) {
     cudaError_t e = cudaFuncSetAttribute(kdist_kernel<E, MAXT, CHEB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (16384 + 2048) * 8);
-    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(kdist_kernel)");
-    attr_set = true;
-  }
+    return e == cudaSuccess ? HK_OK : cuda_fail(e, "cudaFuncSetAttribute(kdist_kernel)");
+  });
+  if (rca != HK_OK) return rca;
   kdist_kernel<E, MAXT, CHEB><<<(unsigned)n_bins, T, smem, st>>>(a);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return cuda_fail(e, "kdist_kernel launch");
@@ -338,13 +338,14 @@ static int kdist_common(const double *kappa, int64_t n_points, double dnu, doubl
   }
   if (rc == HK_OK && coef_out) {
     const size_t cp_bytes = (size_t)(kCpBins + n_c) * (size_t)((ppb < kCpChunk ? ppb : kCpChunk) + 1) * sizeof(double);
-    static bool cp_attr = false;
+    static PerDeviceOnce cp_attr;
     cudaError_t e = cudaSuccess;
-    if (!cp_attr) {
-      e = cudaFuncSetAttribute(cheb_project_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                               (int)((kCpBins + kCpMaxNc) * (kCpChunk + 1) * sizeof(double)));
-      cp_attr = e == cudaSuccess;
-    }
+    if (cp_attr.run([](int) {
+          cudaError_t ea = cudaFuncSetAttribute(cheb_project_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                (int)((kCpBins + kCpMaxNc) * (kCpChunk + 1) * sizeof(double)));
+          return ea == cudaSuccess ? HK_OK : cuda_fail(ea, "cudaFuncSetAttribute(cheb_project_kernel)");
+        }) != HK_OK)
+      e = cudaErrorUnknown;
     if (e == cudaSuccess) {
       cheb_project_kernel<<<(unsigned)((n_bins + kCpBins - 1) / kCpBins), 128, cp_bytes, st>>>(a.ln_out, P, n_bins, ppb, n_c,
                                                                                                 coef_out);

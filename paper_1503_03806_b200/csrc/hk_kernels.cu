@@ -1113,7 +1113,7 @@ static thread_local char g_cuda_err[256] = "";
 static thread_local float g_stage_ms[3] = {0.f, 0.f, 0.f};
 static thread_local cudaEvent_t g_ev[4] = {nullptr, nullptr, nullptr, nullptr};  // stage boundaries of the last timed call
 static thread_local bool g_ev_pending = false;
-static int g_timing = 0;
+static thread_local int g_timing = 0;  // per host thread, like the events it fills
 
 int cuda_fail(cudaError_t e, const char *what)
 {
@@ -1132,21 +1132,24 @@ static bool pos_finite(double v) { return v > 0.0 && isfinite(v); }
 static int lib_pool(cudaMemPool_t *out)
 {
   static cudaMemPool_t pools[64] = {};
+  static PerDeviceOnce once;
   int dev = 0;
   HK_CUDA(cudaGetDevice(&dev));
   if (dev < 0 || dev >= 64) return HK_ERR_UNSUPPORTED;
-  if (!pools[dev]) {
+  const int rc = once.run([](int d) {
     cudaMemPoolProps props = {};
     props.allocType = cudaMemAllocationTypePinned;
     props.handleTypes = cudaMemHandleTypeNone;
     props.location.type = cudaMemLocationTypeDevice;
-    props.location.id = dev;
+    props.location.id = d;
     cudaMemPool_t mp = nullptr;
     HK_CUDA(cudaMemPoolCreate(&mp, &props));
-    uint64_t keep = UINT64_MAX;
+    uint64_t keep = UINT64_MAX;  // scratch freed by one call is reused by the next; hk_trim() hands it back to the driver
     HK_CUDA(cudaMemPoolSetAttribute(mp, cudaMemPoolAttrReleaseThreshold, &keep));
-    pools[dev] = mp;
-  }
+    pools[d] = mp;
+    return (int)HK_OK;
+  });
+  if (rc != HK_OK) return rc;
   *out = pools[dev];
   return HK_OK;
 }
@@ -1241,25 +1244,28 @@ static void scratch_release(Scratch &s, cudaStream_t st)
 // persistent grid of a3: CTAs resident per SM x SMs of the current device (queried once per device)
 static int voigt_grid(bool f32, int *grid_out)
 {
-  static int cached_dev = -1, cached_grid[2] = {0, 0};
+  static int grids[64][2] = {};
+  static PerDeviceOnce once;
   int dev = 0;
   HK_CUDA(cudaGetDevice(&dev));
-  if (dev != cached_dev) {
+  if (dev < 0 || dev >= 64) return HK_ERR_UNSUPPORTED;
+  const int rc = once.run([](int d) {
     int sms = 0, per_sm = 0;
-    HK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    HK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, d));
     HK_CUDA(cudaFuncSetAttribute(voigt_far_kernel<kP, kWarps, kMinB, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  (int)sizeof(VoigtSmemT)));
     HK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, voigt_far_kernel<kP, kWarps, kMinB, false>, kWarps * 32,
                                                           sizeof(VoigtSmemT)));
-    cached_grid[0] = sms * (per_sm < 1 ? 1 : per_sm);
+    grids[d][0] = sms * (per_sm < 1 ? 1 : per_sm);
     HK_CUDA(cudaFuncSetAttribute(voigt_far_kernel<kP, kWarpsF, kMinBF, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  (int)sizeof(VoigtSmemF)));
     HK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, voigt_far_kernel<kP, kWarpsF, kMinBF, true>, kWarpsF * 32,
                                                           sizeof(VoigtSmemF)));
-    cached_grid[1] = sms * (per_sm < 1 ? 1 : per_sm);
-    cached_dev = dev;
-  }
-  *grid_out = cached_grid[f32 ? 1 : 0];
+    grids[d][1] = sms * (per_sm < 1 ? 1 : per_sm);
+    return (int)HK_OK;
+  });
+  if (rc != HK_OK) return rc;
+  *grid_out = grids[dev][f32 ? 1 : 0];
   return HK_OK;
 }
 
@@ -1815,6 +1821,16 @@ int hk_last_stage_ms(float ms_out[3])
     g_ev_pending = false;
   }
   for (int i = 0; i < 3; ++i) ms_out[i] = g_stage_ms[i];
+  return HK_OK;
+}
+
+int hk_trim(void)
+{
+  cudaMemPool_t mp = nullptr;
+  int rc = lib_pool(&mp);
+  if (rc != HK_OK) return rc;
+  HK_CUDA(cudaDeviceSynchronize());
+  HK_CUDA(cudaMemPoolTrimTo(mp, 0));
   return HK_OK;
 }
 

@@ -60,6 +60,50 @@ def test_small_cases_full_grid(n_lines, nu_max, cutoff, T, P):
     _check(_gpu_kappa(wl, T, P, precision=hk.HK_FP32), ref, bar=BAR32)
 
 
+@pytest.mark.parametrize("P", [1e-10, 1e-13])                    # y = gamma/alpha ~ 1e-9 and ~ 1e-12: far below the 1e-8 switch
+@pytest.mark.parametrize("dnu", [0.1, 0.02, 0.0065, 0.001])       # alpha/dnu ~ 0.2, 1, 3, 20 at nu0 = 5000 cm^-1, T = 1500 K
+def test_tiny_damping_on_coarse_and_fine_grids(P, dnu):
+    # with y < 1e-8 the 6-point rule adds the Gaussian term exp(-x^2) out to x^2 ~ 41...50; on a grid coarser
+    # than the line (alpha/dnu < 3) those points reach x^2 > 709, where an unclamped exp_fast wrapped its exponent field
+    rng = np.random.default_rng(7)
+    n = 60
+    nu0 = np.sort(rng.uniform(4990.0, 5010.0, n))
+    S = 10.0 ** rng.uniform(-24.0, -19.0, n)
+    g0 = rng.uniform(0.02, 0.1, n)
+    T, nu_min, nu_max, cutoff = 1500.0, 4980.0, 5020.0, 5.0
+    lines = hk.Lines.from_numpy(nu0, S, g0)
+    ref = oracle.opacity(nu0, S, g0, T, P, nu_min, nu_max, dnu, cutoff)
+    for prec, bar in ((hk.HK_FP64, BAR), (hk.HK_FP32, BAR32)):
+        got = hk.hk_opacity(lines, T, P, nu_min, nu_max, dnu, cutoff, precision=prec).cpu().numpy()
+        assert np.all(got >= 0.0)
+        _check(got, ref, bar=bar)
+
+
+def test_pure_doppler_lines_gamma_zero():
+    # gamma0 = 0 and no natural width gives y = 0, K(x, 0) = exp(-x^2): the profile is finite everywhere
+    # (1/y used to be inf) and matches the oracle; mixed with ordinary lines, on a fine and on a coarse grid
+    rng = np.random.default_rng(11)
+    n = 40
+    nu0 = np.sort(rng.uniform(2990.0, 3010.0, n))
+    S = 10.0 ** rng.uniform(-24.0, -19.0, n)
+    g0 = rng.uniform(0.02, 0.1, n)
+    g0[::2] = 0.0
+    T, P, nu_min, nu_max, cutoff = 1500.0, 1.0, 2980.0, 3020.0, 5.0
+    lines = hk.Lines.from_numpy(nu0, S, g0)
+    for dnu in (0.001, 0.01, 0.05):
+        ref = oracle.opacity(nu0, S, g0, T, P, nu_min, nu_max, dnu, cutoff)
+        for prec, bar in ((hk.HK_FP64, BAR), (hk.HK_FP32, BAR32)):
+            got = hk.hk_opacity(lines, T, P, nu_min, nu_max, dnu, cutoff, precision=prec).cpu().numpy()
+            _check(got, ref, bar=bar)
+    # all lines without damping: kappa is a sum of Gaussians, zero (to underflow) between them
+    only = hk.Lines.from_numpy(nu0, S, np.zeros(n))
+    ref = oracle.opacity(nu0, S, np.zeros(n), T, P, nu_min, nu_max, 0.002, cutoff)
+    got = hk.hk_opacity(only, T, P, nu_min, nu_max, 0.002, cutoff).cpu().numpy()
+    assert np.all(np.isfinite(got)) and np.all(got >= 0.0)
+    mask = ref >= 1e-12 * ref.max()
+    assert np.abs(got[mask] / ref[mask] - 1.0).max() <= BAR
+
+
 def test_lines_far_up_the_spectrum_small_alpha_to_large_alpha():
     # same draw shifted to 20000-20100 cm^-1: alpha ~ 0.08, several regimes per tile
     wl = workloads.small(seed=77, n_lines=500, nu_max=100.0, cutoff=25.0)

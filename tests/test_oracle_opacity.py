@@ -208,3 +208,18 @@ def test_points_entry_equals_range_entry():
     assert np.array_equal(oracle.opacity_points(*args, js), k[js])
     with pytest.raises(ValueError):
         oracle.opacity_points(*args, [8000])
+
+
+def test_pure_doppler_line_gamma_zero_closed_form():
+    """gamma0 = 0: y = 0, K(x, 0) = exp(-x^2), so kappa = (S/m) exp(-((nu-nu0)/alpha)^2)/(alpha sqrt(pi)) exactly (PAPER.md:176-183
+    with a = 0); pins the oracle where the device path has a special case (floor on y)."""
+    nu0 = np.array([50.0]); S = np.array([1e-20]); g0 = np.array([0.0])
+    T, P, dnu = 1500.0, 1.0, 1e-4
+    k = oracle.opacity(nu0, S, g0, T, P, 0.0, 100.0, dnu, 25.0)
+    alpha = 50.0 / 2.99792458e10 * np.sqrt(2 * 1.380649e-16 * T / (18.0 * 1.66053906660e-24))
+    nu = np.arange(k.size) * dnu
+    ref = 1e-20 / (18.0 * 1.66053906660e-24) * np.exp(-((nu - 50.0) / alpha) ** 2) / (alpha * np.sqrt(np.pi))
+    m = ref > 1e-250
+    assert np.isfinite(k).all()
+    assert np.abs(k[m] / ref[m] - 1.0).max() < 1e-12
+    assert k[~m].max() < 1e-240
