@@ -1,13 +1,21 @@
 #!/usr/bin/env python
-"""bench.py — the hot path of HELIOS-K on BASELINE.json config 1.
+"""bench.py — the hot path of HELIOS-K on BASELINE.json's workloads.
 
 One "step" = one whole opacity function plus its k-distribution through the C ABI:
     hk_opacity (a1 line prep, a2 tile plan, a3 Voigt accumulation, a4 kappa store)  +  hk_kdist (a5 per-bin sort, a6 resample)
-on the seeded synthetic 1e5-line workload (workloads.config(1): 3e6 grid points, cutoff 100 cm^-1, 3000 bins x 1000 points,
-20 Gauss-Legendre g-points), FP64.
+The headline (`value`, `e2e`, `roofline`, `cpu_baseline`) is BASELINE.json configs[1] — the configuration the metric "...at
+1e5 lines" is quoted on: 1e5 lines, 3e6 grid points, cutoff 100 cm^-1, 3000 bins x 1000 points, 20 Gauss-Legendre g-points, FP64.
 
     python bench.py [--gpus N] [--steps K] [--warmup W]                  our arm (CUDA, sm_100a)
     python bench.py --impl reference [...]                                the oracle, as it stands, on the host cores
+    python bench.py --config k                                            one line for config k alone (same code as the `configs` key)
+    python bench.py --stage-times                                         per-stage times of configs 1-3, both precisions
+
+At N = 1 the default line also carries `parity` (the oracle's kappa and k-table rows of the cpu_baseline sample compared with
+the GPU's of the same run: the run fails above 1e-6) and `configs`: configs 0, 2, 3, 4 at BASELINE size (config 2 all six
+pressures, config 3 the full 1e8 lines, config 4 all 200 (T,P) pairs through hk.Context), each with CUDA-event times, line-point
+evaluations/s, the regime census, the a3 roofline fraction, parity on seeded 1000-point units and the oracle's time on those
+units extrapolated to the whole config by N_evals (SURVEY.md:386-391).  `--no-configs` leaves them out.
 
 N > 1 (torchrun, one rank per GPU): the path shards with NO collective — rank r computes the opacity function of the r-th
 (T, P) pair of a small T-P table over the same line list ("repeat this calculation for multiple combinations of
@@ -39,18 +47,22 @@ import workloads  # noqa: E402
 METRIC = "voigt_line_point_evals_per_s"
 UNIT = "line-point evals/s"
 WORKLOAD = "BASELINE.json configs[1]: 1e5 lines, 3e6 grid points, cutoff 100 cm^-1, T=1500 K, P=1 atm, 3000 bins x 1000 pts, 20 g-points"
+PARITY_BAR = 1.0e-6          # north_star, FP64 path
+PARITY_BAR32 = 1.0e-4
 
-# FP64-pipe thread-instructions the method needs per line-point evaluation, by regime (counted from
-# the formulas of hk_voigt.cuh with the Newton reciprocal; these are the algorithmic figures, not the executed SASS).
-# gh1 = the 1-point rule with the shifted denominator (from r^2 >= max(3600, 4100 y)), gh2 the shell between 3200 and that.
-FP64_INST_PER_EVAL = {"gh1": 5.0, "gh2": 7.0, "gh3": 11.0, "gh6": 22.0, "series": 150.0}
-# --precision fp32: FP32-pipe thread-instructions per evaluation of the two rules the far kernel runs in float, two points per
-# reciprocal (hk_voigt.cuh gh1_acc2f / gh2_acc2f: 8 and 13 per pair, + 1 MUFU.RCP per pair)
-FP32_INST_PER_EVAL = {"gh1": 4.0, "gh2": 6.5}
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the roofline kernel(s), from the committed `ncu --set full` captures
-# of this command (profiles/r01c_voigt_{far,near,far32}_kernel_ncu_full.txt): far 9.76 MB + near 36.90 MB read, ~0 written
-# (kappa, 24 MB, stays in the 126 MB L2 between the two kernels); FP32 far kernel 6.52 MB.  Not memory-bound: context only.
-NCU_DRAM_BYTES = {"fp64": 9.719e6 + 36.894e6 + 0.020e6, "fp32": 6.518e6}
+# FP64-pipe thread-instructions the method needs per line-point evaluation, by regime.  The wing rules are
+# counted from the formulas of hk_voigt.cuh with the Newton reciprocal; the series is counted from the kernel as built: the
+# SASS of the near kernel's two-item series loop holds 136 DFMA + 16 DMUL + 14 DADD = 166 FP64 instructions for two
+# evaluations.  These are per POINT, for the cheapest valid rule (hk_regime_census), not the rule a whole group happened to get.
+FP64_INST_PER_EVAL = {"gh1": 5.0, "gh2": 7.0, "gh3": 11.0, "gh6": 22.0, "series": 83.0}
+FAR_REGIMES, NEAR_REGIMES = ("gh1", "gh2", "gh3"), ("gh6", "series")
+# --precision fp32: FP32-pipe thread-instructions per evaluation of the rules the far kernel runs in float (hk_voigt.cuh
+# gh1_acc2f / gh2_acc2f: 8 and 13 per pair of points, + 1 MUFU.RCP per pair; gh3_accf: 10 + 1 MUFU.RCP per point)
+FP32_INST_PER_EVAL = {"gh1": 4.0, "gh2": 6.5, "gh3": 10.0}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the roofline kernels, from the committed `ncu --set full` capture
+# named here (not live: ncu cannot run inside a timed bench).  Not memory-bound: context only.
+NCU_DRAM = {"fp64": {"bytes": None, "source": None}, "fp32": {"bytes": None, "source": None}}
+NOMINAL_FP64_LANES = 148 * 64   # DFMA lanes of a B200 (B200_PROFILING.md): nominal peak = lanes x SM clock
 
 
 def tp_table(wl, world):
@@ -112,31 +124,233 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def oracle_sample(wl, T, P, target_s, seed=1):
-    """Times the oracle, as it stands, on whole seeded bins of the workload (kappa of every point of the bin + the bin's
-    k-distribution).  A 4-bin pilot sizes the sample for about `target_s` seconds.  Returns (evals/s, description, cores)."""
+def host_cores():
+    return len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+
+
+def _reach(wl, j_lo, j_hi):
+    """Slice of the (ordered) line list that can reach grid points j_lo..j_hi: a superset; the oracle windows exactly."""
+    lo = np.searchsorted(wl.nu0, wl.nu_min + j_lo * wl.dnu - wl.cutoff - 1.0, "left")
+    hi = np.searchsorted(wl.nu0, wl.nu_min + j_hi * wl.dnu + wl.cutoff + 1.0, "right")
+    return slice(int(lo), int(hi))
+
+
+def oracle_units(wl, T, P, target_s, unit, seed, q_ratio=1.0, with_kdist=False, max_units=None):
+    """Times the oracle, as it stands, on seeded whole units of `unit` consecutive grid points (a k-distribution bin where the
+    config has 1000-point bins): kappa of every point of the unit (+ the unit's k-distribution row when `with_kdist`).  A
+    2-unit pilot sizes the sample for about `target_s` seconds.  Returns a dict with the timing, the sampled indices and the
+    oracle's values (for the parity check of the same run)."""
     import oracle
-    ppb = int(round(wl.bin_width / wl.dnu))
-    n_bins = wl.n_points // ppb
-    rng = np.random.default_rng(seed)
-    order = rng.permutation(n_bins)
+    n_units = wl.n_points // unit
+    order = np.random.default_rng(seed).permutation(n_units)
+    ar = np.arange(unit, dtype=np.int64)
 
-    def run(bins):
-        js = (np.sort(bins)[:, None] * ppb + np.arange(ppb)[None, :]).ravel()
+    def run(units):
+        us = np.sort(units)
         t0 = time.perf_counter()
-        kap = oracle.opacity_points(wl.nu0, wl.S, wl.gamma0, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, js,
-                                    mass_amu=wl.mass_amu)
-        oracle.kdist(kap, ppb, wl.n_g)
+        kap = np.empty(us.size * unit)
+        ne = 0
+        for n, u in enumerate(us):           # unit by unit: each call sees only the lines that can reach its unit
+            js = u * unit + ar
+            sl = _reach(wl, int(js[0]), int(js[-1]))
+            E = None if wl.E_low is None else wl.E_low[sl]
+            kap[n * unit:(n + 1) * unit] = oracle.opacity_points(wl.nu0[sl], wl.S[sl], wl.gamma0[sl], T, P, wl.nu_min, wl.nu_max,
+                                                                 wl.dnu, wl.cutoff, js, mass_amu=wl.mass_amu, E_low=E,
+                                                                 q_ratio=q_ratio)
+        ktab = oracle.kdist(kap, unit, wl.n_g) if with_kdist else None
         dt = time.perf_counter() - t0
-        nu = wl.nu_min + js * wl.dnu
-        ne = int(np.sum(np.searchsorted(wl.nu0, nu + wl.cutoff, "right") - np.searchsorted(wl.nu0, nu - wl.cutoff, "left")))
-        return dt, ne
+        for u in us:
+            nu = wl.nu_min + (u * unit + ar) * wl.dnu
+            ne += int(np.sum(np.searchsorted(wl.nu0, nu + wl.cutoff, "right") - np.searchsorted(wl.nu0, nu - wl.cutoff, "left")))
+        return dt, ne, us, kap, ktab
 
-    dt, ne = run(order[:4])
-    nb = int(min(n_bins, max(4, round(4 * target_s / max(dt, 1e-3)))))
-    dt, ne = run(order[:nb])
-    cores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
-    return ne / dt, dt, ne, f"{nb} seeded whole bins ({nb * ppb} grid points, {ne} line-point evals, {dt:.1f} s) of the {n_bins}-bin workload", cores
+    dt, ne, us, kap, ktab = run(order[:2])
+    nu_ = int(min(n_units, max(2, round(2 * target_s / max(dt, 1e-3)))))
+    if max_units:
+        nu_ = min(nu_, max_units)
+    if nu_ > 2:
+        dt, ne, us, kap, ktab = run(order[:nu_])
+    return {"evals_per_s": ne / dt, "seconds": dt, "evals": ne, "units": us, "unit": unit, "kappa": kap, "ktab": ktab,
+            "cores": host_cores(),
+            "sample": f"{us.size} seeded whole units of {unit} consecutive grid points ({us.size * unit} points, {ne} "
+                      f"line-point evals, {dt:.1f} s) of the {n_units}-unit grid" + (", with their k-distribution rows" if with_kdist else "")}
+
+
+def parity_of(got, ref, bar):
+    """max relative error where the oracle value >= 1e-12 x the largest oracle value of the compared set (A11)."""
+    mask = ref >= 1e-12 * ref.max()
+    if not np.all(np.isfinite(got)):
+        return float("inf")
+    err = float(np.abs(got[mask] / ref[mask] - 1.0).max()) if mask.any() else 0.0
+    if np.any(got[ref == 0.0] != 0.0):
+        return float("inf")
+    return err
+
+
+def unit_indices(units, unit):
+    return (np.asarray(units)[:, None] * unit + np.arange(unit)[None, :]).ravel()
+
+
+def roofline_fp64(census, ms_far, ms_near, fp64_peak, sm_mhz):
+    """a3 = far + near kernel: FMA-equivalent TFLOP/s (1 FP64 instruction = 2 flop) of the algorithmic work against the
+    live-measured DFMA peak, per kernel and as a whole, and against the nominal peak at the sampled SM clock."""
+    far = sum(FP64_INST_PER_EVAL[k] * census[k] for k in FAR_REGIMES)
+    near = sum(FP64_INST_PER_EVAL[k] * census[k] for k in NEAR_REGIMES)
+    peak = 2.0 * fp64_peak / 1e12
+    ach = 2.0 * (far + near) / ((ms_far + ms_near) * 1e-3) / 1e12
+    out = {"achieved": ach, "peak": peak, "frac": ach / peak,
+           "frac_far": 2.0 * far / (ms_far * 1e-3) / 1e12 / peak if ms_far > 0 else None,
+           "frac_near": 2.0 * near / (ms_near * 1e-3) / 1e12 / peak if ms_near > 0 else None,
+           "algorithmic_fp64_instructions": far + near}
+    if sm_mhz:
+        nominal = 2.0 * NOMINAL_FP64_LANES * sm_mhz * 1e6 / 1e12
+        out["nominal_peak"] = nominal
+        out["frac_vs_nominal"] = ach / nominal
+    return out
+
+
+def hbm_peak():
+    try:
+        return float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except (OSError, KeyError, ValueError):
+        return 6650.0, "fallback (6.65 TB/s, B200_PROFILING.md)"
+
+
+# ---------------------------------------------------------------------------------------------------------------------------
+# one config at BASELINE size: device times, census, roofline, parity and oracle time on seeded units
+# ---------------------------------------------------------------------------------------------------------------------------
+def config_leg(hk, k, fp64_peak, flush, oracle_s=6.0, sm_mhz=None, precision=None):
+    import torch
+    prec = hk.HK_FP64 if precision is None else precision
+    bar = PARITY_BAR if prec == hk.HK_FP64 else PARITY_BAR32
+    t_gen = time.perf_counter()
+    wl = workloads.config(k)
+    t_gen = time.perf_counter() - t_gen
+    N = wl.n_points
+    ppb = int(round(wl.bin_width / wl.dnu)) if wl.bin_width else None
+    unit = 1000
+    lines = hk.Lines.from_numpy(wl.nu0, wl.S, wl.gamma0, E_low=wl.E_low)
+    n_evals = hk.hk_count_evals(wl.nu0, wl.nu_min, N, wl.dnu, wl.cutoff)
+    pairs = [(T, P) for T in wl.T for P in wl.P_atm]
+    qr = (lambda T: wl.q_ratio(T)) if wl.q_ratio else (lambda T: 1.0)
+    ctx = hk.Context(lines, precision=prec)
+    kap = torch.empty(N, dtype=torch.float64, device="cuda")
+    ktab = torch.empty((N // ppb, wl.n_g), dtype=torch.float64, device="cuda") if ppb else None
+    stream = torch.cuda.current_stream()
+    big = wl.n_lines >= 10_000_000                 # records >> L2: nothing to flush, and one repetition is 0.3 s
+    reps = 1 if (big or len(pairs) > 6) else 5
+
+    def step(T, P):
+        ctx.opacity(T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, q_ratio=qr(T), out=kap)
+        if ppb:
+            hk.hk_kdist(kap, wl.dnu, wl.bin_width, wl.n_g, out=ktab)
+
+    step(*pairs[0])                                # warm-up: allocates scratch, loads the kernels
+    step(*pairs[-1])
+    torch.cuda.synchronize()
+    # parity sample: seeded pairs of the config's (T,P) list; oracle units on each (sized for ~oracle_s seconds in all)
+    rng = np.random.default_rng(100 + k)
+    if len(pairs) == 1:
+        chk = [0]
+    elif len(pairs) <= 6:
+        chk = list(range(len(pairs)))
+    else:
+        chk = sorted({0, len(pairs) - 1} | set(int(i) for i in rng.choice(len(pairs), 4, replace=False)))
+    hk.hk_set_timing(True)
+    ms_op = ms_kd = 0.0
+    stage = np.zeros(3)
+    per_pair, got_kappa, got_ktab = [], {}, {}
+    for ip, (T, P) in enumerate(pairs):
+        best = None
+        for _ in range(reps):
+            if not big:
+                flush.zero_()
+            e = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+            e[0].record(stream)
+            ctx.opacity(T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, q_ratio=qr(T), out=kap)
+            e[1].record(stream)
+            if ppb:
+                hk.hk_kdist(kap, wl.dnu, wl.bin_width, wl.n_g, out=ktab)
+            e[2].record(stream)
+            st = np.array(hk.hk_last_stage_ms())
+            torch.cuda.synchronize()
+            t = (e[0].elapsed_time(e[1]), e[1].elapsed_time(e[2]), st)
+            if best is None or t[0] + t[1] < best[0] + best[1]:
+                best = t
+        ms_op += best[0]
+        ms_kd += best[1]
+        stage += best[2]
+        per_pair.append({"T_K": T, "P_atm": P, "opacity_ms": best[0], "far_ms": float(best[2][1]), "near_ms": float(best[2][2])})
+        if ip in chk:
+            got_kappa[ip] = kap.cpu().numpy()
+            if ppb:
+                got_ktab[ip] = ktab.cpu().numpy()
+    hk.hk_set_timing(False)
+    ctx.close()
+    # census + roofline on the checked pairs (all pairs when there are at most six)
+    cen_tot = {r: 0 for r in FP64_INST_PER_EVAL}
+    far_ms = near_ms = 0.0
+    for ip in chk:
+        T, P = pairs[ip]
+        c = hk.hk_regime_census(wl.nu0, wl.gamma0, T, P, wl.mass_amu, wl.nu_min, N, wl.dnu, wl.cutoff, precision=prec)
+        for r in cen_tot:
+            cen_tot[r] += c[r]
+        far_ms += per_pair[ip]["far_ms"]
+        near_ms += per_pair[ip]["near_ms"]
+    roof = roofline_fp64(cen_tot, far_ms, near_ms, fp64_peak, sm_mhz) if prec == hk.HK_FP64 else None
+    # oracle on seeded units of the checked pairs: parity of this run's kappa (and k-table rows), and the CPU time
+    worst_k, worst_t, o_ev, o_s, n_pts, samples = 0.0, 0.0, 0, 0.0, 0, []
+    for ip in chk:
+        T, P = pairs[ip]
+        o = oracle_units(wl, T, P, oracle_s / len(chk), unit, seed=1000 * k + ip, q_ratio=qr(T),
+                         with_kdist=(ppb == unit), max_units=64)
+        js = unit_indices(o["units"], unit)
+        worst_k = max(worst_k, parity_of(got_kappa[ip][js], o["kappa"], bar))
+        if ppb == unit:
+            gk, rk = got_ktab[ip][o["units"]].ravel(), o["ktab"].ravel()
+            worst_t = max(worst_t, parity_of(gk, rk, bar))
+        o_ev += o["evals"]
+        o_s += o["seconds"]
+        n_pts += js.size
+        samples.append(o["sample"])
+    n_tot = n_evals * len(pairs)
+    leg = {
+        "workload": f"BASELINE.json configs[{k}] at full size", "n_lines": wl.n_lines, "n_points": N, "pairs": len(pairs),
+        "precision": "fp32" if prec == hk.HK_FP32 else "fp64",
+        "line_point_evals": n_tot, "opacity_ms": ms_op, "kdist_ms": ms_kd if ppb else None,
+        "s_per_opacity_function": ms_op / len(pairs) * 1e-3,
+        "evals_per_s": n_tot / ((ms_op + ms_kd) * 1e-3),
+        "evals_per_s_opacity_only": n_tot / (ms_op * 1e-3),
+        "stage_ms": {"line_prep": float(stage[0]), "voigt_far": float(stage[1]), "voigt_near": float(stage[2])},
+        "timing": f"CUDA events on the launching stream, best of {reps} per (T,P) pair, "
+                  + ("line records (14 GB) >> L2" if big else "L2 flushed before each repetition"),
+        "regime_census": cen_tot, "census_pairs": len(chk),
+        "roofline": roof,
+        "parity": {"kappa_max_rel": worst_k, "ktable_max_rel": worst_t if ppb == unit else None, "points": n_pts,
+                   "pairs_checked": len(chk), "bar": bar},
+        "cpu_baseline": {"value": o_ev / o_s, "unit": UNIT, "cores": host_cores(), "kind": "oracle",
+                         "sample": samples[0] + (f" (+ {len(samples) - 1} more (T,P) pairs, same size)" if len(samples) > 1 else ""),
+                         "seconds_full_config_extrapolated_by_n_evals": n_tot / (o_ev / o_s)},
+        "host_generation_s": t_gen,
+    }
+    if len(pairs) > 1 and len(pairs) <= 6:
+        leg["per_pair"] = per_pair
+    ok = worst_k <= bar and (worst_t <= bar)
+    return leg, ok
+
+
+def run_config(args):
+    import torch
+    import paper_1503_03806_b200 as hk
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --config: no CUDA device — the hot path has no CPU fallback")
+    hk.load_library()
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
+    prec = hk.HK_FP32 if args.precision == "fp32" else hk.HK_FP64
+    leg, ok = config_leg(hk, args.config, hk.hk_fp64_peak(), flush, oracle_s=args.oracle_seconds, sm_mhz=None, precision=prec)
+    print(json.dumps(leg))
+    if not ok:
+        raise SystemExit(f"bench.py --config {args.config}: parity above the bar")
 
 
 def run_reference(args):
@@ -149,12 +363,13 @@ def run_reference(args):
     oracle.build()
     per_step_s = max(2.0, min(20.0, 90.0 / max(1, args.steps + args.warmup)))
     for _ in range(args.warmup):
-        oracle_sample(wl, T, P, per_step_s)
+        oracle_units(wl, T, P, per_step_s, 1000, seed=1, with_kdist=True)
     tot_e, tot_t, desc, cores = 0, 0.0, "", 1
     for _ in range(args.steps):
-        _, dt, ne, desc, cores = oracle_sample(wl, T, P, per_step_s)
-        tot_e += ne
-        tot_t += dt
+        o = oracle_units(wl, T, P, per_step_s, 1000, seed=1, with_kdist=True)
+        tot_e += o["evals"]
+        tot_t += o["seconds"]
+        desc, cores = o["sample"], o["cores"]
     v = tot_e / tot_t
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / max(1, args.steps), "higher_is_better": True,
@@ -200,6 +415,7 @@ def run_ours(args):
     stream = torch.cuda.current_stream()
 
     prec = hk.HK_FP32 if args.precision == "fp32" else hk.HK_FP64
+    bar = PARITY_BAR32 if prec == hk.HK_FP32 else PARITY_BAR
 
     def step():
         hk.hk_opacity(lines, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, mass_amu=wl.mass_amu, out=kappa, precision=prec)
@@ -236,6 +452,8 @@ def run_ours(args):
     ms_kdist = sum(e[1].elapsed_time(e[2]) for e in ev)
     ms_total = ms_opacity + ms_kdist
     stage /= args.steps
+    got_kappa = kappa.cpu().numpy() if rank == 0 else None              # this run's result, for the parity check below
+    got_ktab = ktab.cpu().numpy() if rank == 0 else None
     # ---- e2e: host buffers in, host buffers out, through the public API -----------------------------------------------
     pin = lambda a: torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64)).pin_memory()
     h_nu0, h_S, h_g0 = pin(wl.nu0), pin(wl.S), pin(wl.gamma0)
@@ -256,11 +474,11 @@ def run_ours(args):
     d2h = 8 * N + 8 * (N // ppb) * wl.n_g
 
     # ---- max over ranks ------------------------------------------------------------------------------------------------
-    red = torch.tensor([ms_total, ms_opacity, ms_kdist, e2e_s * 1e3, stage[1] + stage[2], stage[1]], dtype=torch.float64,
+    red = torch.tensor([ms_total, ms_opacity, ms_kdist, e2e_s * 1e3, stage[1] + stage[2], stage[1], stage[2]], dtype=torch.float64,
                        device="cuda")
     if world > 1:
         dist.all_reduce(red, op=dist.ReduceOp.MAX)
-    ms_total, ms_opacity, ms_kdist, e2e_ms, ms_voigt, ms_far = [float(v) for v in red.cpu()]
+    ms_total, ms_opacity, ms_kdist, e2e_ms, ms_voigt, ms_far, ms_near = [float(v) for v in red.cpu()]
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -268,33 +486,34 @@ def run_ours(args):
 
     K = args.steps
     value = world * n_evals * K / (ms_total * 1e-3)
-    # roofline of the dominant kernel (voigt_kernel, a3+a4): ALU-bound on the FP64 pipe
+    sm_mhz = clocks.get("sm_mhz") if clocks else None
+    # roofline of the dominant kernels (a3+a4): ALU-bound on the FP64 pipe
     census = hk.hk_regime_census(wl.nu0, wl.gamma0, T, P, wl.mass_amu, wl.nu_min, N, wl.dnu, wl.cutoff, precision=prec)
     if prec == hk.HK_FP32:
-        # the FP32 variant's dominant kernel is the far kernel alone (1-/2-point rules in float, FP32 pipe)
+        # the FP32 variant's dominant kernel is the far kernel alone (1-/2-/3-point rules in float, FP32 pipe)
         alg_inst = sum(FP32_INST_PER_EVAL[k] * census[k] for k in FP32_INST_PER_EVAL)
         achieved = 2.0 * alg_inst / (ms_far * 1e-3) / 1e12
         peak = 2.0 * fp32_peak / 1e12
-        roof_kernel, roof_ms = "voigt_far_kernel<FP32> (a3 far wings + a4)", ms_far
-        roof_note = ("FP32-pipe thread-instructions x2 of the 1-/2-point rules (regime census x per-eval figure, two points per "
-                     "MUFU.RCP); peak = hk_fp32_peak FFMA microbenchmark measured live in this run; the near kernel "
-                     "(3-/6-point rules, series) stays FP64 and is reported in stage_ms")
+        roof = {"kernel": "voigt_far_kernel<FP32> (a3 far wings + a4)", "bound": "alu", "achieved": achieved, "peak": peak,
+                "unit": "TFLOP/s", "frac": achieved / peak, "ms": ms_far,
+                "note": "FP32-pipe thread-instructions x2 of the 1-/2-/3-point rules (regime census x per-eval figure); peak = "
+                        "hk_fp32_peak FFMA microbenchmark measured live in this run; the near kernel (6-point rule, series) "
+                        "stays FP64 and is reported in stage_ms"}
     else:
-        alg_inst = sum(FP64_INST_PER_EVAL[k] * census[k] for k in FP64_INST_PER_EVAL)
-        achieved = 2.0 * alg_inst / (ms_voigt * 1e-3) / 1e12            # FMA-equivalent TFLOP/s (1 FP64 instruction = 2 flop)
-        peak = 2.0 * fp64_peak / 1e12
-        roof_kernel, roof_ms = "voigt_far_kernel + voigt_near_kernel (a3+a4)", ms_voigt
-        roof_note = ("FP64-pipe thread-instructions x2; algorithmic instructions = regime census x per-eval figure "
-                     "(DESIGN.md); peak = hk_fp64_peak DFMA microbenchmark measured live in this run")
-    cpu_v, cpu_dt, cpu_ne, cpu_desc, cores = oracle_sample(wl, T, P, 15.0) if world == 1 else (None, 0, 0, "", 0)
+        r = roofline_fp64(census, ms_far, ms_near, fp64_peak, sm_mhz)
+        roof = {"kernel": "voigt_far_kernel + voigt_near_kernel (a3+a4)", "bound": "alu", "achieved": r["achieved"],
+                "peak": r["peak"], "unit": "TFLOP/s", "frac": r["frac"], "frac_far": r["frac_far"], "frac_near": r["frac_near"],
+                "frac_vs_nominal": r.get("frac_vs_nominal"), "nominal_peak": r.get("nominal_peak"), "ms": ms_voigt,
+                "note": "FP64-pipe thread-instructions x2; algorithmic instructions = regime census x per-evaluation figure "
+                        "(DESIGN.md §4: 5 / 7 / 11 / 22 for the 1-/2-/3-/6-point rules, 83 for the series, counted from the "
+                        "kernel's SASS); peak = hk_fp64_peak DFMA microbenchmark measured live in this run; nominal_peak = "
+                        "148 SMs x 64 lanes x the SM clock sampled under load x 2"}
+    roof.update({"traffic": NCU_DRAM[args.precision]["bytes"], "traffic_source": NCU_DRAM[args.precision]["source"],
+                 "regime_census": census, "fp64_peak_tflops": 2.0 * fp64_peak / 1e12, "fp32_peak_tflops": 2.0 * fp32_peak / 1e12,
+                 "fp64_inst_per_eval": FP64_INST_PER_EVAL})
 
     # HBM-bound steps: a5+a6 reads kappa once and writes the k-table; a4 is the kappa store inside the far kernel
-    hbm_peak, hbm_src = 6650.0, "of fallback (6.65 TB/s, B200_PROFILING.md)"
-    try:
-        hbm_peak = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"])
-        hbm_src = "of measured (MEASURED_PEAKS.json hbm_gbs)"
-    except (OSError, KeyError, ValueError):
-        pass
+    hbm, hbm_src = hbm_peak()
     kdist_bytes = 8.0 * N + 8.0 * (N // ppb) * wl.n_g
     kdist_gbs = kdist_bytes / (ms_kdist / K * 1e-3) / 1e9
     line = {
@@ -306,29 +525,49 @@ def run_ours(args):
                    "l2": "flushed between steps by a 512 MiB memset outside the per-step CUDA events",
                    "T_K": T, "P_atm": P},
         "s_per_opacity_function": ms_opacity / K * 1e-3, "s_per_kdist": ms_kdist / K * 1e-3,
-        "stage_ms": {"line_prep": stage[0], "voigt_far": stage[1], "voigt_near": stage[2], "voigt_accumulate_store": ms_voigt,
+        "stage_ms": {"line_prep": stage[0], "voigt_far": ms_far, "voigt_near": ms_near, "voigt_accumulate_store": ms_voigt,
                      "kdist": ms_kdist / K},
         "wall_s_timed_region": t_wall,
         "e2e": {"value": world * n_evals * K / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": e2e_ms / K},
         "gpu_launches": 4 * K,   # line_prep, voigt_far, voigt_near, kdist
-        "roofline": {"kernel": roof_kernel, "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                     "frac": achieved / peak, "traffic": NCU_DRAM_BYTES[args.precision],
-                     "traffic_note": "DRAM bytes per launch from the committed ncu --set full capture (profiles/r01c_*), not live",
-                     "note": roof_note, "regime_census": census, "ms": roof_ms,
-                     "fp64_peak_tflops": 2.0 * fp64_peak / 1e12, "fp32_peak_tflops": 2.0 * fp32_peak / 1e12},
-        "kdist_hbm": {"kernel": "kdist_kernel (a5+a6)", "bound": "hbm", "achieved": kdist_gbs, "peak": hbm_peak, "unit": "GB/s",
-                      "frac": kdist_gbs / hbm_peak, "algorithmic_bytes": kdist_bytes, "peak_source": hbm_src,
+        "roofline": roof,
+        "kdist_hbm": {"kernel": "kdist_kernel (a5+a6)", "bound": "hbm", "achieved": kdist_gbs, "peak": hbm, "unit": "GB/s",
+                      "frac": kdist_gbs / hbm, "algorithmic_bytes": kdist_bytes, "peak_source": hbm_src,
                       "note": "8 B/point read + 8 n_g B/bin written; the kernel is bound by the bitonic network's "
-                              "compare-exchange count, not by HBM (profiles/r01b_kdist_kernel_ncu_full.txt)"},
+                              "compare-exchange count, not by HBM (profiles/)"},
         "clocks": clocks,
     }
-    if cpu_v is not None:
-        line["cpu_baseline"] = {"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": cpu_desc}
+    ok = True
+    if world == 1:
+        # the oracle, as it stands, on seeded whole bins: the CPU baseline AND the parity check of this run's kappa / k-table
+        o = oracle_units(wl, T, P, args.oracle_seconds_headline, ppb, seed=1, with_kdist=True)
+        line["cpu_baseline"] = {"value": o["evals_per_s"], "unit": UNIT, "cores": o["cores"], "kind": "oracle", "sample": o["sample"],
+                                "seconds_full_config_extrapolated_by_n_evals": n_evals / o["evals_per_s"]}
+        js = unit_indices(o["units"], ppb)
+        pk = parity_of(got_kappa[js], o["kappa"], bar)
+        pt = parity_of(got_ktab[o["units"]].ravel(), o["ktab"].ravel(), bar)
+        line["parity"] = {"kappa_max_rel": pk, "ktable_max_rel": pt, "points": int(js.size), "bins": int(o["units"].size), "bar": bar,
+                          "note": "GPU kappa and k-table of this run's last timed step against the oracle on the cpu_baseline "
+                                  "sample; mask: oracle value >= 1e-12 x the oracle's max over the compared set"}
+        ok = pk <= bar and pt <= bar
+        if not args.no_configs and prec == hk.HK_FP64:
+            del kappa, ktab, lines
+            torch.cuda.empty_cache()
+            legs = {}
+            for k in (0, 2, 3, 4):
+                leg, lok = config_leg(hk, k, fp64_peak, flush, oracle_s=args.oracle_seconds, sm_mhz=sm_mhz)
+                legs[str(k)] = leg
+                ok = ok and lok
+                hk.hk_trim()
+                torch.cuda.empty_cache()
+            line["configs"] = legs
     line["paper_context"] = "~1 s per opacity function of ~1e5 lines on a Tesla K20 (PAPER.md:9, 267); other hardware, not a target"
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
+    if not ok:
+        raise SystemExit("bench.py: parity against the oracle above the bar (see the `parity` keys of the line)")
 
 
 def run_stage_times(args):
@@ -359,6 +598,38 @@ def run_stage_times(args):
                               "opacity_ms": float(st.sum()), "evals_per_s": ne / (st.sum() * 1e-3)}), flush=True)
 
 
+def run_f_rows(args):
+    """--f-rows: device times of the SURVEY §8(f) rows at config 1's size (3000 bins x 1000 points, 20 Chebyshev coefficients,
+    1000 column masses): CUDA events around `reps` back-to-back calls.  One GPU; not a bench line."""
+    import torch
+    import paper_1503_03806_b200 as hk
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --f-rows: no CUDA device")
+    wl = workloads.config(1)
+    lines = hk.Lines.from_numpy(wl.nu0, wl.S, wl.gamma0)
+    kap = hk.hk_opacity(lines, wl.T[0], wl.P_atm[0], wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff)
+    dm = torch.as_tensor(10 ** np.linspace(-6, 4, 1000)).cuda()
+
+    def timed(fn, reps=20):
+        fn()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            out = fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return out, e0.elapsed_time(e1) / reps
+
+    ktab, ms_k = timed(lambda: hk.hk_kdist(kap, wl.dnu, wl.bin_width, wl.n_g))
+    _, ms_c = timed(lambda: hk.hk_kdist_cheb(kap, wl.dnu, wl.bin_width, 20, n_g=wl.n_g))
+    _, ms_tk = timed(lambda: hk.hk_transmission(ktab, dm))
+    _, ms_td = timed(lambda: hk.hk_transmission_direct(kap, wl.dnu, wl.bin_width, dm))
+    print(json.dumps({"workload": "config 1 size: 3000 bins x 1000 points, n_c = 20, n_g = 20, 1000 column masses",
+                      "kdist_ms": ms_k, "kdist_cheb_with_ktable_ms": ms_c, "transmission_ktable_ms": ms_tk,
+                      "transmission_direct_ms": ms_td, "direct_exp_per_s": 3.0e9 / (ms_td * 1e-3),
+                      "timing": "CUDA events around 20 back-to-back calls (host launch overhead included)"}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -367,13 +638,24 @@ def main():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--precision", choices=["fp64", "fp32"], default="fp64",
                     help="fp64 (BASELINE.json config 1, the default) or the optional FP32 variant (bar 1e-4)")
+    ap.add_argument("--config", type=int, choices=[0, 1, 2, 3, 4], default=None,
+                    help="print the per-config leg of config k alone (BASELINE size) and exit")
+    ap.add_argument("--no-configs", action="store_true", help="default line without the `configs` key (configs 0, 2, 3, 4)")
+    ap.add_argument("--oracle-seconds", type=float, default=6.0, help="CPU seconds of oracle per config leg (parity + cpu_baseline)")
+    ap.add_argument("--oracle-seconds-headline", type=float, default=15.0, help="likewise for the headline config 1")
     ap.add_argument("--stage-times", action="store_true",
                     help="print per-stage device times of configs 1, 2, 3 (1e7 lines) in both precisions and exit")
+    ap.add_argument("--f-rows", action="store_true",
+                    help="print device times of the SURVEY 8(f) rows (Chebyshev resampling, transmission) at config 1's size and exit")
     args = ap.parse_args()
-    if args.stage_times:
+    if args.f_rows:
+        run_f_rows(args)
+    elif args.stage_times:
         run_stage_times(args)
     elif args.impl == "reference":
         run_reference(args)
+    elif args.config is not None:
+        run_config(args)
     else:
         run_ours(args)
 

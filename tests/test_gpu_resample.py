@@ -6,9 +6,6 @@ Tolerances: on IDENTICAL kappa input both sides do the same FP64 arithmetic in a
 absolute, relative to max(1, |C|)), 1e-11 (transmission, relative).  End to end from the line list the inputs differ by the
 Voigt routine's <= 2.5e-7, i.e. <= 2.5e-7 absolute in ln kappa: coefficients within 2e-6, resampled kappa(y) within 1e-6 x
 the sum of |T_n| <= n_c (bar written below)."""
-import json
-import os
-
 import numpy as np
 import pytest
 
@@ -18,24 +15,10 @@ import oracle
 import workloads
 import paper_1503_03806_b200 as hk
 
-ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-
 
 def _dev(a):
     import torch
     return torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64)).cuda()
-
-
-def _note(key, value):
-    try:
-        d = os.path.join(ROOT, "gpurun_out")
-        os.makedirs(d, exist_ok=True)
-        path = os.path.join(d, "resample_timings.json")
-        cur = json.load(open(path)) if os.path.exists(path) else {}
-        cur[key] = value
-        json.dump(cur, open(path, "w"), indent=1)
-    except OSError:
-        pass
 
 
 @pytest.mark.parametrize("ppb,n_c,n_bins", [(1000, 20, 7), (10000, 20, 3), (37, 5, 11), (64, 8, 2), (2048, 1, 2), (1, 1, 5)])
@@ -132,24 +115,12 @@ def test_config1_full_size_1000_column_masses():
     m = 10 ** np.linspace(-6, 4, 1000)
     dm = _dev(m)
 
-    def timed(fn, reps=5):
-        fn()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        for _ in range(reps):
-            out = fn()
-        e1.record()
-        torch.cuda.synchronize()
-        return out, e0.elapsed_time(e1) / reps
-
-    ktab, ms_k = timed(lambda: hk.hk_kdist(kap, wl.dnu, wl.bin_width, wl.n_g))
-    (coef, ktab2), ms_c = timed(lambda: hk.hk_kdist_cheb(kap, wl.dnu, wl.bin_width, 20, n_g=wl.n_g))
-    Tk, ms_tk = timed(lambda: hk.hk_transmission(ktab, dm))
-    Td, ms_td = timed(lambda: hk.hk_transmission_direct(kap, wl.dnu, wl.bin_width, dm))
+    ktab = hk.hk_kdist(kap, wl.dnu, wl.bin_width, wl.n_g)
+    coef, ktab2 = hk.hk_kdist_cheb(kap, wl.dnu, wl.bin_width, 20, n_g=wl.n_g)
+    Tk = hk.hk_transmission(ktab, dm)
+    Td = hk.hk_transmission_direct(kap, wl.dnu, wl.bin_width, dm)
+    torch.cuda.synchronize()
     assert torch.equal(ktab, ktab2)
-    _note("config1", {"kdist_ms": ms_k, "kdist_cheb_with_ktable_ms": ms_c, "transmission_ktable_ms": ms_tk,
-                      "transmission_direct_ms": ms_td, "n_bins": 3000, "ppb": 1000, "n_c": 20, "n_g": wl.n_g, "n_m": 1000,
-                      "direct_exp_per_s": 3.0e9 / (ms_td * 1e-3)})
     kh = kap.cpu().numpy()
     rng = np.random.default_rng(6)
     bins = np.sort(rng.choice(3000, 40, replace=False))
