@@ -364,11 +364,14 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
 // it walks each mask: a branch-free loop over the lines of one rule, parameters broadcast from shared memory, an unrolled
 // P-point body accumulating in registers: ~1 instruction per (line, span) for the regime decision, no divergence.
 // ------------------------------------------------------------------------------------------------------
-constexpr int CH = 128;     // lines per ring stage: 128 lines x 128 B
-#ifndef HK_STAGES
-#define HK_STAGES 4
-#endif
-constexpr int STAGES = HK_STAGES;
+// Shape of a far-kernel instantiation: P points per thread (groups per warp), WARPS warps per CTA sharing one line ring of
+// STAGES stages of CH lines, MINB CTAs per SM; F32 = the FP32 variant.
+template <int P_, int WARPS_, int MINB_, int CH_, int STAGES_, bool F32_>
+struct FarShape {
+  static constexpr int P = P_, WARPS = WARPS_, MINB = MINB_, CH = CH_, STAGES = STAGES_;
+  static constexpr bool F32 = F32_;
+  static constexpr int TILE = WARPS_ * 32 * P_;
+};
 
 struct __align__(16) StageHdr {
   int tile_lo;  // first grid point of the tile this chunk belongs to; < 0: no more work
@@ -379,23 +382,25 @@ struct __align__(16) StageHdr {
   int pad[3];
 };
 
-template <bool F32>
+template <bool F32, int CH, int STAGES>
 struct RingRecs {  // FP64: two 32-byte records per line
   LineBase base[STAGES][CH];
   LineGH2 gh2[STAGES][CH];
   static constexpr uint32_t kBytes = 16u + 16u + 32u + 32u;  // ring bytes per line, with MetaA and MetaB
 };
-template <>
-struct RingRecs<true> {  // FP32 variant: one
+template <int CH, int STAGES>
+struct RingRecs<true, CH, STAGES> {  // FP32 variant: one
   LineF32 f32[STAGES][CH];
   static constexpr uint32_t kBytes = 16u + 16u + 32u;
 };
 
-template <int P, int WARPS, bool F32>
+template <class Sh>
 struct __align__(128) VoigtSmem {
+  static constexpr int CH = Sh::CH, STAGES = Sh::STAGES;
+  using Recs = RingRecs<Sh::F32, Sh::CH, Sh::STAGES>;
   MetaA ma[STAGES][CH];
   MetaB mb[STAGES][CH];
-  RingRecs<F32> r;
+  Recs r;
   StageHdr hdr[STAGES];
   uint64_t full[STAGES];
   int done[STAGES];  // warps that have finished with the stage's current chunk
@@ -472,10 +477,11 @@ __device__ __forceinline__ int2 tile_lines(const VoigtArgs &a, int lo, int hi)
 // holds lines, four bulk copies completing on the stage's `full` mbarrier.  Pulls a new tile from the queue when the current
 // one is exhausted; after the last tile one stop header is posted and nothing more.  Called by one thread at a time, in
 // order of n (ticket S.issued).
-template <int P, int WARPS, bool F32>
-__device__ __forceinline__ void issue_chunk(VoigtSmem<P, WARPS, F32> &S, const VoigtArgs &a, int n)
+template <class Sh>
+__device__ __forceinline__ void issue_chunk(VoigtSmem<Sh> &S, const VoigtArgs &a, int n)
 {
-  constexpr int TILE = WARPS * 32 * P;
+  constexpr int TILE = Sh::TILE, CH = Sh::CH, STAGES = Sh::STAGES, P = Sh::P;
+  constexpr bool F32 = Sh::F32;
   if (S.cur_stop) return;
   const int stage = n % STAGES;
   if (S.cur_c == S.cur_nchunks) {
@@ -509,7 +515,7 @@ __device__ __forceinline__ void issue_chunk(VoigtSmem<P, WARPS, F32> &S, const V
   S.cur_c = c + 1;
   const uint32_t nb = (uint32_t)h.cnt;
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // the stage's previous readers (generic proxy) come first
-  mbar_expect_tx(&S.full[stage], nb * RingRecs<F32>::kBytes);  // release: the header store above is visible to the waiters
+  mbar_expect_tx(&S.full[stage], nb * VoigtSmem<Sh>::Recs::kBytes);  // release: the header store above is visible to the waiters
   if (nb) {
     const int first = S.cur_L0 + c * CH;
     bulk_g2s(&S.ma[stage][0], a.ma + first, nb * 16u, &S.full[stage]);
@@ -523,11 +529,13 @@ __device__ __forceinline__ void issue_chunk(VoigtSmem<P, WARPS, F32> &S, const V
   }
 }
 
-template <int P, int WARPS, int MINB, bool F32>
-__global__ void __launch_bounds__(WARPS * 32, MINB) voigt_far_kernel(const __grid_constant__ VoigtArgs a)
+template <class Sh>
+__global__ void __launch_bounds__(Sh::WARPS * 32, Sh::MINB) voigt_far_kernel(const __grid_constant__ VoigtArgs a)
 {
+  constexpr int P = Sh::P, WARPS = Sh::WARPS, STAGES = Sh::STAGES;
+  constexpr bool F32 = Sh::F32;
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  VoigtSmem<P, WARPS, F32> &S = *reinterpret_cast<VoigtSmem<P, WARPS, F32> *>(smem_raw);
+  VoigtSmem<Sh> &S = *reinterpret_cast<VoigtSmem<Sh> *>(smem_raw);
 
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   if (threadIdx.x == 0) {
@@ -538,12 +546,12 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) voigt_far_kernel(const __gri
     S.cur_tile = 0; S.cur_L0 = 0; S.cur_nl = 0; S.cur_c = 0; S.cur_nchunks = 0; S.cur_stop = 0;
     {
       // heavier tiles first: compare the line counts of the first and the last tile
-      constexpr int TILE = WARPS * 32 * P;
+      constexpr int TILE = Sh::TILE;
       const int2 f = tile_lines(a, 0, min(TILE, a.N)), l = tile_lines(a, (a.n_tiles - 1) * TILE, a.N);
       S.descending = (l.y - l.x) >= (f.y - f.x);
     }
     mbar_fence_init();
-    for (int n = 0; n < STAGES; ++n) issue_chunk<P, WARPS, F32>(S, a, n);  // fill the ring
+    for (int n = 0; n < STAGES; ++n) issue_chunk<Sh>(S, a, n);  // fill the ring
     S.issued = STAGES;
   }
   __syncthreads();  // the only CTA-wide barrier
@@ -779,7 +787,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) voigt_far_kernel(const __gri
 #endif
         }
         __threadfence_block();
-        issue_chunk<P, WARPS, F32>(S, a, n + STAGES);
+        issue_chunk<Sh>(S, a, n + STAGES);
         __threadfence_block();
         *issued = n + STAGES + 1;
       }
@@ -1167,23 +1175,16 @@ void pool_free(void *p, cudaStream_t st)
   if (p) cudaFreeAsync(p, st);
 }
 
-#ifndef HK_P
-#define HK_P 8
-#endif
-#ifndef HK_WARPS
-#define HK_WARPS 4
-#endif
-#ifndef HK_MINB
-#define HK_MINB 4
-#endif
-// FP64: 4 warps x 4 CTAs/SM (tiles of 1024 points): the same 16 warps/SM as 8 x 2 but finer tiles on the queue — 1 % faster
-// on config 1, 10 % on config 3, where a 2048-point tile is 40 % of a line's whole window; 16 x 1 and 8 x 3 are slower.
-// The FP32 variant (78 registers) keeps 8 warps per CTA, 3 CTAs/SM: 4 x 6 measured 4 % slower.
-constexpr int kP = HK_P, kWarps = HK_WARPS, kMinB = HK_MINB;
-constexpr int kWarpsF = 8, kMinBF = 3;
-constexpr int kTile = kP * kWarps * 32, kTileF = kP * kWarpsF * 32;
-using VoigtSmemT = VoigtSmem<kP, kWarps, false>;
-using VoigtSmemF = VoigtSmem<kP, kWarpsF, true>;
+// Far-kernel shapes (measured, profiles/r02_README.md).  4 warps sharing a deep ring (4 x 128 lines) on 1024-point tiles, 4
+// CTAs/SM, serve lists up to config 2's density best.  In a very dense list (config 3: 1e5 consecutive lines centred in the same
+// 256-point span) the 3-point work of those lines falls on one warp of the four for hundreds of chunks while the others wait at
+// the ring: there one warp per CTA with a ring of its own (2 x 64 lines) on 256-point tiles, 16 CTAs/SM, is 9 % faster
+// (config 3 at 1e8 lines: far kernel 284 -> 234 ms); on config 1 it is 3 % slower, on config 2 / 4 1-2 % slower over the
+// pressure sweep.  The FP32 variant (80 registers) runs one warp per CTA, 24 CTAs/SM, everywhere (16 % faster on config 3).
+using ShSparse = FarShape<8, 4, 4, 128, 4, false>;
+using ShDense = FarShape<8, 1, 16, 64, 2, false>;
+using ShF32 = FarShape<8, 1, 24, 64, 2, true>;
+constexpr double kDenseLinesPerSpan = 10000.0;  // lines whose window reaches a 256-point span, on average, from which ShDense serves
 
 struct Scratch {
   MetaA *ma = nullptr;  // one allocation: ma | mb | base | gh2 | core | near, n_lines records each
@@ -1242,30 +1243,33 @@ static void scratch_release(Scratch &s, cudaStream_t st)
 }
 
 // persistent grid of a3: CTAs resident per SM x SMs of the current device (queried once per device)
-static int voigt_grid(bool f32, int *grid_out)
+template <class Sh>
+static int far_grid_of(int dev, int *out)
 {
-  static int grids[64][2] = {};
+  int sms = 0, per_sm = 0;
+  HK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  HK_CUDA(cudaFuncSetAttribute(voigt_far_kernel<Sh>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(VoigtSmem<Sh>)));
+  HK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, voigt_far_kernel<Sh>, Sh::WARPS * 32, sizeof(VoigtSmem<Sh>)));
+  *out = sms * (per_sm < 1 ? 1 : per_sm);
+  return HK_OK;
+}
+// persistent grids of a3: CTAs resident per SM x SMs of the current device, per shape (queried once per device)
+enum { kShapeSparse = 0, kShapeDense = 1, kShapeF32 = 2 };
+static int voigt_grid(int shape, int *grid_out)
+{
+  static int grids[64][3] = {};
   static PerDeviceOnce once;
   int dev = 0;
   HK_CUDA(cudaGetDevice(&dev));
   if (dev < 0 || dev >= 64) return HK_ERR_UNSUPPORTED;
   const int rc = once.run([](int d) {
-    int sms = 0, per_sm = 0;
-    HK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, d));
-    HK_CUDA(cudaFuncSetAttribute(voigt_far_kernel<kP, kWarps, kMinB, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)sizeof(VoigtSmemT)));
-    HK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, voigt_far_kernel<kP, kWarps, kMinB, false>, kWarps * 32,
-                                                          sizeof(VoigtSmemT)));
-    grids[d][0] = sms * (per_sm < 1 ? 1 : per_sm);
-    HK_CUDA(cudaFuncSetAttribute(voigt_far_kernel<kP, kWarpsF, kMinBF, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)sizeof(VoigtSmemF)));
-    HK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, voigt_far_kernel<kP, kWarpsF, kMinBF, true>, kWarpsF * 32,
-                                                          sizeof(VoigtSmemF)));
-    grids[d][1] = sms * (per_sm < 1 ? 1 : per_sm);
-    return (int)HK_OK;
+    int rc2 = far_grid_of<ShSparse>(d, &grids[d][kShapeSparse]);
+    if (rc2 == HK_OK) rc2 = far_grid_of<ShDense>(d, &grids[d][kShapeDense]);
+    if (rc2 == HK_OK) rc2 = far_grid_of<ShF32>(d, &grids[d][kShapeF32]);
+    return rc2;
   });
   if (rc != HK_OK) return rc;
-  *grid_out = grids[dev][f32 ? 1 : 0];
+  *grid_out = grids[dev][shape];
   return HK_OK;
 }
 
@@ -1315,10 +1319,13 @@ static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double 
   const int nb = (int)((N + kPlanBlock - 1) / kPlanBlock);
   int rc = scratch_reserve(s, n_lines, nb, f32, st);
   if (rc != HK_OK) return rc;
+  // lines whose window reaches a 256-point span, on average: picks the far kernel's shape
+  const double per_span = (double)n_lines * fmin(2.0 * cutoff / dnu + (double)kPlanBlock, (double)N) / (double)N;
+  const int shape = f32 ? kShapeF32 : (per_span >= kDenseLinesPerSpan ? kShapeDense : kShapeSparse);
   int grid = 0;
-  rc = voigt_grid(f32, &grid);
+  rc = voigt_grid(shape, &grid);
   if (rc != HK_OK) return rc;
-  const int tile = f32 ? kTileF : kTile;
+  const int tile = shape == kShapeF32 ? ShF32::TILE : (shape == kShapeDense ? ShDense::TILE : ShSparse::TILE);
   const int n_tiles = (int)((N + tile - 1) / tile);
   if (grid > n_tiles) grid = n_tiles;
 
@@ -1367,8 +1374,9 @@ static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double 
       va.r3_offset = 4.0e9;
     }
   }
-  if (f32) voigt_far_kernel<kP, kWarpsF, kMinBF, true><<<grid, kWarpsF * 32, sizeof(VoigtSmemF), st>>>(va);
-  else voigt_far_kernel<kP, kWarps, kMinB, false><<<grid, kWarps * 32, sizeof(VoigtSmemT), st>>>(va);
+  if (shape == kShapeF32) voigt_far_kernel<ShF32><<<grid, ShF32::WARPS * 32, sizeof(VoigtSmem<ShF32>), st>>>(va);
+  else if (shape == kShapeDense) voigt_far_kernel<ShDense><<<grid, ShDense::WARPS * 32, sizeof(VoigtSmem<ShDense>), st>>>(va);
+  else voigt_far_kernel<ShSparse><<<grid, ShSparse::WARPS * 32, sizeof(VoigtSmem<ShSparse>), st>>>(va);
   HK_CUDA(cudaGetLastError());
   if (g_timing) HK_CUDA(cudaEventRecord(ev[2], st));
   const int nch = chunks ? std::max(1, std::min(chunks->n, std::min(kMaxNearChunks, nb))) : 1;
