@@ -591,26 +591,38 @@ __global__ void __launch_bounds__(Sh::WARPS * 32, Sh::MINB) voigt_far_kernel(con
         float af[P];
 #pragma unroll
         for (int k = 0; k < P; ++k) af[k] = 0.0f;
-#pragma unroll 1
-        for (unsigned m = M.m1; m; m &= m - 1) {
-          const LineF32 L = sf[b0 + (__ffs(m) - 1)];
-          const float w = L.A1m * __int_as_float((max(L.A1e, ebm) - ebm) << 23);
-          const float d0 = ((float)(j0 - L.ci) - L.cf) * a.dnu_f;
+        if (M.m1 | M.m2) {
+          // whole-span rules on packed pairs of points (k, k+1): FFMA2 / FMUL2 / FADD2, one reciprocal per four (1-point
+          // rule) or two (2-point rule) evaluations
+          static_assert(P % 4 == 0, "the packed 1-point rule takes four points at a time");
+          f32x2 ap[P / 2];
 #pragma unroll
-          for (int k = 0; k < P; k += 2)
-            gh1_acc2f(af[k], af[k + 1], (k == 0 ? d0 : fmaf((float)(32 * k), a.dnu_f, d0)),
-                      fmaf((float)(32 * k + 32), a.dnu_f, d0), w, fmaf(-1.5f, L.a2, L.g2));
-        }
+          for (int k = 0; k < P / 2; ++k) ap[k] = pk2(0.0f, 0.0f);
 #pragma unroll 1
-        for (unsigned m = M.m2; m; m &= m - 1) {
-          const LineF32 L = sf[b0 + (__ffs(m) - 1)];
-          const float w = L.A1m * __int_as_float((max(L.A1e, ebm) - ebm) << 23);
-          const float d0 = ((float)(j0 - L.ci) - L.cf) * a.dnu_f;
-          const float wa2 = w * L.a2;
+          for (unsigned m = M.m1; m; m &= m - 1) {
+            const LineF32 L = sf[b0 + (__ffs(m) - 1)];
+            const float w = L.A1m * __int_as_float((max(L.A1e, ebm) - ebm) << 23);
+            const float d0 = ((float)(j0 - L.ci) - L.cf) * a.dnu_f;
+            const float g2s = fmaf(-1.5f, L.a2, L.g2);
+            const f32x2 dd = pk2(d0, d0), gg = pk2(g2s, g2s);
 #pragma unroll
-          for (int k = 0; k < P; k += 2)
-            gh2_acc2f(af[k], af[k + 1], (k == 0 ? d0 : fmaf((float)(32 * k), a.dnu_f, d0)),
-                      fmaf((float)(32 * k + 32), a.dnu_f, d0), w, L.e2, L.f2, wa2);
+            for (int k = 0; k < P / 2; k += 2)
+              gh1_acc4f(ap[k], ap[k + 1], add2(dd, pk2((float)(64 * k) * a.dnu_f, (float)(64 * k + 32) * a.dnu_f)),
+                        add2(dd, pk2((float)(64 * k + 64) * a.dnu_f, (float)(64 * k + 96) * a.dnu_f)), w, gg);
+          }
+#pragma unroll 1
+          for (unsigned m = M.m2; m; m &= m - 1) {
+            const LineF32 L = sf[b0 + (__ffs(m) - 1)];
+            const float w = L.A1m * __int_as_float((max(L.A1e, ebm) - ebm) << 23);
+            const float d0 = ((float)(j0 - L.ci) - L.cf) * a.dnu_f;
+            const float wa2 = w * L.a2;
+            const f32x2 dd = pk2(d0, d0), ww = pk2(w, w), ee = pk2(L.e2, L.e2), ff = pk2(L.f2, L.f2), wa = pk2(wa2, wa2);
+#pragma unroll
+            for (int k = 0; k < P / 2; ++k)
+              gh2_acc2p(ap[k], add2(dd, pk2((float)(64 * k) * a.dnu_f, (float)(64 * k + 32) * a.dnu_f)), ww, ee, ff, wa);
+          }
+#pragma unroll
+          for (int k = 0; k < P / 2; ++k) upk2(ap[k], af[2 * k], af[2 * k + 1]);
         }
         // cutoff-edge spans: the same rules, masked to the line's window
 #pragma unroll 1

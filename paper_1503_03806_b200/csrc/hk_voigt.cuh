@@ -147,6 +147,60 @@ __device__ __forceinline__ void gh2_acc2f(float &a0, float &a1, float d0, float 
   a0 = fmaf(B0 * D1, r, a0);
   a1 = fmaf(B1 * D0, r, a1);
 }
+// ---- packed FP32 pairs (sm_100: fma / mul / add .f32x2 -> SASS FFMA2 / FMUL2 / FADD2, two floats per 64-bit register and
+// per issue slot).  The FP32 far kernel is issue-bound, and its points already come in pairs. ----
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk2(float lo, float hi)
+{
+  f32x2 r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void upk2(f32x2 v, float &lo, float &hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c)
+{
+  f32x2 r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+  return r;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b)
+{
+  f32x2 r;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b)
+{
+  f32x2 r;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+// 1-point rule on FOUR points (two packed pairs p, q) with one reciprocal, 1/(D0 D1 D2 D3): with the cross products
+// c = (D0 D2, D1 D3) and u = A1 r (c.hi, c.lo), the four terms A1/D_k are u * (D2, D3) and u * (D0, D1): no operand swaps.
+// 10 issue slots + 1 MUFU.RCP for four evaluations (the scalar pair form: 9 + 1 for two).  D^4 stays inside the float range:
+// D <= cutoff^2 ~ 1e4, and D >= (3 dnu)^2 (the FP64 guard band of a1 keeps the far kernel three grid steps off every centre).
+__device__ __forceinline__ void gh1_acc4f(f32x2 &ap, f32x2 &aq, f32x2 dp, f32x2 dq, float A1, f32x2 g2g2)
+{
+  const f32x2 Dp = fma2(dp, dp, g2g2), Dq = fma2(dq, dq, g2g2);
+  const f32x2 c = mul2(Dp, Dq);
+  float c0, c1;
+  upk2(c, c0, c1);
+  const float t = A1 * rcpf(c0 * c1);
+  const f32x2 u = mul2(pk2(t, t), pk2(c1, c0));
+  ap = fma2(u, Dq, ap);
+  aq = fma2(u, Dp, aq);
+}
+// 2-point rule on a packed pair with one reciprocal: 7 issue slots + 1 MUFU.RCP (scalar form: 13 + 1)
+__device__ __forceinline__ void gh2_acc2p(f32x2 &a, f32x2 d, f32x2 A1A1, f32x2 e2e2, f32x2 f2f2, f32x2 wa2)
+{
+  const f32x2 E = fma2(d, d, e2e2);
+  const f32x2 D = fma2(E, E, f2f2);
+  const f32x2 B = fma2(A1A1, E, wa2);
+  float D0, D1;
+  upk2(D, D0, D1);
+  const float r = rcpf(D0 * D1);
+  a = fma2(mul2(B, pk2(D1, D0)), pk2(r, r), a);
+}
 // 3-point rule in float (FP32 variant: from r^2 >= 64), one reciprocal per point (R D ~ d^6 would leave the float range in
 // a product over two points)
 __device__ __forceinline__ float gh3_accf(float acc, float d, float g2, float e3, float f3, float c0, float c3, float c3a)

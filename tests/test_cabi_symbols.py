@@ -100,3 +100,35 @@ def test_cheb_projection_host_against_the_oracle(ppb, n_c):
     assert np.abs(P @ np.log(kappa) - C).max() < tol * max(1.0, np.abs(C).max())
     with pytest.raises(hk.HKError):
         hk.hk_cheb_projection(10, 20)
+
+
+def test_sass_of_the_hot_kernels():
+    """What the kernels are claimed to be built from shows in the SASS of libhk.so (cuobjdump works without a GPU): the far
+    kernel stages line records by 1-D TMA bulk copies completing on mbarriers (UBLKCP, SYNCS) and takes FP64 reciprocals from
+    MUFU.RCP64H; the FP32 variant's far kernel uses sm_100's packed float arithmetic (FFMA2 / FMUL2 / FADD2)."""
+    import shutil
+    import subprocess
+    from paper_1503_03806_b200.build import build_library
+    cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(cuobjdump):
+        pytest.skip("cuobjdump not available")
+    sass = subprocess.run([cuobjdump, "-sass", build_library()], capture_output=True, text=True, check=True).stdout
+    funcs = {}
+    name = None
+    for line in sass.splitlines():
+        if "Function :" in line:
+            name = line.split("Function :")[1].strip()
+            funcs[name] = []
+        elif name is not None:
+            funcs[name].append(line)
+    far = {n: "\n".join(b) for n, b in funcs.items() if "voigt_far_kernel" in n}
+    assert len(far) == 3, sorted(far)                                 # sparse and dense FP64 shapes, FP32 variant
+    for n, body in far.items():
+        assert "UBLKCP" in body and "SYNCS" in body, n                # TMA bulk copy + mbarrier
+    f32 = [b for n, b in far.items() if n.endswith("Lb1EEEEEvNS_9VoigtArgsE")]
+    f64 = [b for n, b in far.items() if n.endswith("Lb0EEEEEvNS_9VoigtArgsE")]
+    assert len(f32) == 1 and len(f64) == 2
+    assert all(k in f32[0] for k in ("FFMA2", "FMUL2", "FADD2"))
+    assert all("MUFU.RCP64H" in b and "DFMA" in b for b in f64)
+    near = [("\n".join(b)) for n, b in funcs.items() if "voigt_near_kernel" in n]
+    assert len(near) == 1 and "DFMA" in near[0] and "LDGSTS" in near[0]   # cp.async prefetch of the kappa strip
