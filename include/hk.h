@@ -140,8 +140,9 @@ int hk_opacity(const hk_lines *lines, int64_t n_lines, double T, double P_atm, d
 
 /* End-to-end form with HOST buffers (what bench.py's `e2e` times): copies the line arrays host -> device, runs
  * hk_opacity and, when k_host_out != NULL, hk_kdist(bin_width, n_g), copies kappa (when kappa_host_out != NULL) and the
- * k-table device -> host, and waits for the stream.  kappa is copied back range by range on a second (library-owned)
- * stream while the near kernel, launched in four parts, still works on the later ranges.  Every array of lines_host is a HOST pointer (pinned memory makes
+ * k-table device -> host, and waits for the stream.  The Voigt accumulation runs as six (far kernel, near kernel) launch pairs
+ * over ranges of the grid, each on a library-owned stream of its own, and every range of kappa is copied back on a further
+ * stream as soon as it is final, while the later ranges are still being computed.  Every array of lines_host is a HOST pointer (pinned memory makes
  * the copies asynchronous to the host but is not required); kappa_host_out: host [N] or NULL; k_host_out: host
  * [n_bins*n_g] or NULL (then bin_width and n_g are ignored); at least one output is required.  Device memory comes from
  * the library's pool.  With prm->accumulate = 1 kappa_host_out is also an INPUT (the running sum of the mixture, copied

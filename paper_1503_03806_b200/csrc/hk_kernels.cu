@@ -156,7 +156,9 @@ __global__ void __launch_bounds__(256) line_prep_kernel(PrepArgs a)
 {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= a.n) return;
-  if (i == 0) *a.queue = 0;
+  if (i < 16) a.queue[i] = 0;  // one ticket counter per far-kernel launch of this call (at most kMaxChunks)
+  if (a.n < 16 && i == 0)
+    for (int q = (int)a.n; q < 16; ++q) a.queue[q] = 0;
   const double nu0 = a.nu0[i];
   double alpha = nu0 * a.vth;
   if (!(alpha > 1.0e-290)) alpha = 0.0;  // nu0 <= 0 (or a width whose reciprocal overflows): Lorentzian (A9)
@@ -422,7 +424,8 @@ struct VoigtArgs {
   const int *first_lo;
   const int *first_c;
   int *queue;           // tile tickets of the far kernel (reset by a1)
-  int nb, n_tiles;
+  int nb, n_tiles;      // plan blocks of the grid; tiles of THIS far-kernel launch, which start at tile0
+  int tile0;
   double nu_min, dnu;
   float dnu_f;
   int N;
@@ -494,7 +497,7 @@ __device__ __forceinline__ void issue_chunk(VoigtSmem<Sh> &S, const VoigtArgs &a
       mbar_expect_tx(&S.full[stage], 0u);
       return;
     }
-    const int tile = S.descending ? a.n_tiles - 1 - ticket : ticket;
+    const int tile = a.tile0 + (S.descending ? a.n_tiles - 1 - ticket : ticket);
     const int2 pl = tile_lines(a, tile * TILE, min((tile + 1) * TILE, a.N));
     const int nl = pl.y - pl.x;
     S.cur_tile = tile;
@@ -547,7 +550,8 @@ __global__ void __launch_bounds__(Sh::WARPS * 32, Sh::MINB) voigt_far_kernel(con
     {
       // heavier tiles first: compare the line counts of the first and the last tile
       constexpr int TILE = Sh::TILE;
-      const int2 f = tile_lines(a, 0, min(TILE, a.N)), l = tile_lines(a, (a.n_tiles - 1) * TILE, a.N);
+      const int2 f = tile_lines(a, a.tile0 * TILE, min((a.tile0 + 1) * TILE, a.N)),
+                 l = tile_lines(a, (a.tile0 + a.n_tiles - 1) * TILE, min((a.tile0 + a.n_tiles) * TILE, a.N));
       S.descending = (l.y - l.x) >= (f.y - f.x);
     }
     mbar_fence_init();
@@ -1236,7 +1240,7 @@ static int scratch_reserve(Scratch &s, int64_t n_lines, int nb, bool f32, cudaSt
     pool_free(s.first_hi, st);
     s.first_hi = nullptr; s.cap_blocks = 0;
     void *p = nullptr;
-    int rc = pool_alloc(&p, ((size_t)3 * (nb + 1) + 4) * sizeof(int), st);
+    int rc = pool_alloc(&p, ((size_t)3 * (nb + 1) + 16) * sizeof(int), st);
     if (rc != HK_OK) return rc;
     s.first_hi = (int *)p;
     s.first_lo = s.first_hi + (nb + 1);
@@ -1305,24 +1309,33 @@ static int validate(const hk_lines *lines, int64_t n_lines, double T, double P_a
   return HK_OK;
 }
 
-// The near kernel in `n` launches over consecutive ranges of spans, an event after each: kappa[0, hi[i]) is final once
-// done[i] has passed — hk_opacity_host copies kappa back range by range while the later ranges are still being computed.
-constexpr int kMaxNearChunks = 8;
-struct NearChunks {
+// hk_opacity_host: a3 runs as `n` (far, near) launch pairs over consecutive ranges of the grid, from the top down, each pair on
+// a stream of its own (streams[i], forked from the call's stream after a1 and joined before the call returns to it) so that
+// the CTAs of the next range's far kernel fill the SMs as those of the previous one retire; kappa[lo[i], hi[i]) is final
+// once done[i] has passed, and is copied to the host while the later ranges are computed.
+constexpr int kMaxChunks = 8;
+#ifndef HK_HOST_CHUNKS
+#define HK_HOST_CHUNKS 6
+#endif
+constexpr int kHostChunks = HK_HOST_CHUNKS;
+struct GridChunks {
   int n = 1;
-  cudaEvent_t done[kMaxNearChunks] = {};
-  int64_t hi[kMaxNearChunks] = {};  // one past the last grid point of range i
+  cudaStream_t streams[kMaxChunks] = {};
+  cudaEvent_t fork = nullptr;
+  cudaEvent_t done[kMaxChunks] = {};
+  int64_t lo[kMaxChunks] = {}, hi[kMaxChunks] = {};
 };
 
 static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double P_atm, double q_ratio, double mass_amu,
                        double nu_min, double dnu, double cutoff, int64_t N, double *kappa_out, Scratch &s, const hk_params &prm,
-                       cudaStream_t st, NearChunks *chunks = nullptr)
+                       cudaStream_t st, GridChunks *chunks = nullptr)
 {
   const bool f32 = prm.precision == HK_FP32;
   if (n_lines == 0) {
     if (!prm.accumulate) HK_CUDA(cudaMemsetAsync(kappa_out, 0, (size_t)N * sizeof(double), st));
     if (chunks) {
       chunks->n = 1;
+      chunks->lo[0] = 0;
       chunks->hi[0] = N;
       HK_CUDA(cudaEventRecord(chunks->done[0], st));
     }
@@ -1370,7 +1383,7 @@ static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double 
   va.ma = s.ma; va.mb = s.mb; va.base = s.base; va.gh2 = s.gh2; va.core = s.core; va.near = s.near; va.f32 = pa.f32;
   va.dnu_f = (float)dnu;
   va.first_hi = s.first_hi; va.first_lo = s.first_lo; va.first_c = s.first_c; va.queue = s.queue;
-  va.nb = nb; va.n_tiles = n_tiles;
+  va.nb = nb; va.n_tiles = n_tiles; va.tile0 = 0;
   va.nu_min = nu_min; va.dnu = dnu; va.N = (int)N; va.kappa = kappa_out; va.accumulate = prm.accumulate ? 1 : 0;
   {
     // bound on the 3-ball radius (grid units) of any line that can have grid point j inside its 3-ball:
@@ -1386,20 +1399,39 @@ static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double 
       va.r3_offset = 4.0e9;
     }
   }
-  if (shape == kShapeF32) voigt_far_kernel<ShF32><<<grid, ShF32::WARPS * 32, sizeof(VoigtSmem<ShF32>), st>>>(va);
-  else if (shape == kShapeDense) voigt_far_kernel<ShDense><<<grid, ShDense::WARPS * 32, sizeof(VoigtSmem<ShDense>), st>>>(va);
-  else voigt_far_kernel<ShSparse><<<grid, ShSparse::WARPS * 32, sizeof(VoigtSmem<ShSparse>), st>>>(va);
-  HK_CUDA(cudaGetLastError());
-  if (g_timing) HK_CUDA(cudaEventRecord(ev[2], st));
-  const int nch = chunks ? std::max(1, std::min(chunks->n, std::min(kMaxNearChunks, nb))) : 1;
-  for (int c = 0; c < nch; ++c) {
-    const int b_lo = (int)((int64_t)nb * c / nch), b_hi = (int)((int64_t)nb * (c + 1) / nch);
+  // ranges only where every one gets a few tiles (a small grid has nothing to overlap)
+  const int nch = (chunks && n_tiles >= 8 * chunks->n) ? std::max(1, std::min(chunks->n, kMaxChunks)) : 1;
+  const int bpt = tile / kPlanBlock;  // plan blocks per tile
+  if (chunks && nch > 1) HK_CUDA(cudaEventRecord(chunks->fork, st));
+  for (int c = 0; c < nch; ++c) {     // ranges of whole tiles, from the top of the grid down
+    cudaStream_t sc = (chunks && nch > 1) ? chunks->streams[c] : st;
+    if (sc != st) HK_CUDA(cudaStreamWaitEvent(sc, chunks->fork, 0));
+    // tapered ranges (weights nch + 1 ... 2, top of the grid first): the copy of the last range trails the call, so it is the
+    // smallest (measured at config 1: e2e 1.41 ms with the near kernel alone in four parts, 1.22 with six equal (far, near)
+    // ranges, 1.21 tapered)
+    auto cut = [&](int k) {  // tiles below the k ranges processed last
+      const int64_t tot = (int64_t)nch * (nch + 1) / 2 + nch, w = (int64_t)k * (k + 1) / 2 + k;
+      return (int)((int64_t)n_tiles * w / tot);
+    };
+    const int t_lo = cut(nch - 1 - c), t_hi = cut(nch - c);
+    va.tile0 = t_lo;
+    va.n_tiles = t_hi - t_lo;
+    va.queue = s.queue + c;
+    const int g = std::min(grid, va.n_tiles);
+    if (shape == kShapeF32) voigt_far_kernel<ShF32><<<g, ShF32::WARPS * 32, sizeof(VoigtSmem<ShF32>), sc>>>(va);
+    else if (shape == kShapeDense) voigt_far_kernel<ShDense><<<g, ShDense::WARPS * 32, sizeof(VoigtSmem<ShDense>), sc>>>(va);
+    else voigt_far_kernel<ShSparse><<<g, ShSparse::WARPS * 32, sizeof(VoigtSmem<ShSparse>), sc>>>(va);
+    HK_CUDA(cudaGetLastError());
+    if (g_timing && c == nch - 1) HK_CUDA(cudaEventRecord(ev[2], sc));
+    const int b_lo = t_lo * bpt, b_hi = std::min(t_hi * bpt, nb);
     va.block0 = b_lo;
-    voigt_near_kernel<<<b_hi - b_lo, 32, 0, st>>>(va);
+    voigt_near_kernel<<<b_hi - b_lo, 32, 0, sc>>>(va);
     HK_CUDA(cudaGetLastError());
     if (chunks) {
+      chunks->lo[c] = (int64_t)b_lo * kPlanBlock;
       chunks->hi[c] = std::min<int64_t>((int64_t)b_hi * kPlanBlock, N);
-      HK_CUDA(cudaEventRecord(chunks->done[c], st));
+      HK_CUDA(cudaEventRecord(chunks->done[c], sc));
+      if (sc != st) HK_CUDA(cudaStreamWaitEvent(st, chunks->done[c], 0));  // join: the call's stream continues after every range
     }
   }
   if (chunks) chunks->n = nch;
@@ -1446,7 +1478,7 @@ int64_t hk_grid_size(double nu_min, double nu_max, double dnu)
 }
 
 static int opacity_impl(const hk_lines *lines, int64_t n_lines, double T, double P_atm, double nu_min, double nu_max,
-                        double dnu, double cutoff, double *kappa_out, const hk_params *prm, NearChunks *chunks)
+                        double dnu, double cutoff, double *kappa_out, const hk_params *prm, GridChunks *chunks)
 {
   int64_t N = 0;
   int rc = validate(lines, n_lines, T, P_atm, nu_min, nu_max, dnu, cutoff, kappa_out, prm, &N);
@@ -1490,7 +1522,9 @@ int hk_opacity(const hk_lines *lines, int64_t n_lines, double T, double P_atm, d
 struct HostCopy {
   int dev = -1;
   cudaStream_t copy = nullptr;
-  cudaEvent_t done[kMaxNearChunks] = {};
+  cudaStream_t range[kMaxChunks] = {};  // one per grid range, earlier ranges at higher priority
+  cudaEvent_t fork = nullptr;
+  cudaEvent_t done[kMaxChunks] = {};
   cudaEvent_t copied = nullptr;
 };
 static thread_local HostCopy g_hc;
@@ -1502,7 +1536,12 @@ static int host_copy_get(HostCopy **out)
   if (h.dev != dev) {
     h = HostCopy();  // a set made on another device is abandoned (a thread that hops devices is not the case served)
     HK_CUDA(cudaStreamCreateWithFlags(&h.copy, cudaStreamNonBlocking));
-    for (int i = 0; i < kMaxNearChunks; ++i) HK_CUDA(cudaEventCreateWithFlags(&h.done[i], cudaEventDisableTiming));
+    for (int i = 0; i < kMaxChunks; ++i) HK_CUDA(cudaEventCreateWithFlags(&h.done[i], cudaEventDisableTiming));
+    HK_CUDA(cudaEventCreateWithFlags(&h.fork, cudaEventDisableTiming));
+    int prio_lo = 0, prio_hi = 0;  // numerically lower = higher priority
+    HK_CUDA(cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));
+    for (int i = 0; i < kMaxChunks; ++i)
+      HK_CUDA(cudaStreamCreateWithPriority(&h.range[i], cudaStreamNonBlocking, std::min(prio_lo, prio_hi + i)));
     HK_CUDA(cudaEventCreateWithFlags(&h.copied, cudaEventDisableTiming));
     h.dev = dev;
   }
@@ -1556,19 +1595,19 @@ int hk_opacity_host(const hk_lines *lines_host, int64_t n_lines, double T, doubl
     hk_lines dl = {dptr[0], dptr[1], dptr[2], dptr[3], dptr[4], dptr[5], dptr[6], dptr[7]};
     // kappa goes back range by range on a second stream while the near kernel still works on the later ranges: the
     // device -> host copy of 8 B/point is a quarter of the call at config 1
-    NearChunks ch;
-    ch.n = kappa_host_out ? 4 : 1;
+    GridChunks ch;
+    ch.n = kappa_host_out ? kHostChunks : 1;
+    ch.fork = hc->fork;
+    for (int i = 0; i < kMaxChunks; ++i) ch.streams[i] = hc->range[i];
     bool copies_pending = false;
-    for (int i = 0; i < kMaxNearChunks; ++i) ch.done[i] = hc->done[i];
+    for (int i = 0; i < kMaxChunks; ++i) ch.done[i] = hc->done[i];
     rc = opacity_impl(&dl, n_lines, T, P_atm, nu_min, nu_max, dnu, cutoff, d_kappa, prm, &ch);
     if (rc == HK_OK && kappa_host_out) {
-      int64_t lo = 0;
       for (int c = 0; c < ch.n && e == cudaSuccess; ++c) {
         e = cudaStreamWaitEvent(hc->copy, ch.done[c], 0);
-        if (e == cudaSuccess && ch.hi[c] > lo)
-          e = cudaMemcpyAsync(kappa_host_out + lo, d_kappa + lo, (size_t)(ch.hi[c] - lo) * sizeof(double),
+        if (e == cudaSuccess && ch.hi[c] > ch.lo[c])
+          e = cudaMemcpyAsync(kappa_host_out + ch.lo[c], d_kappa + ch.lo[c], (size_t)(ch.hi[c] - ch.lo[c]) * sizeof(double),
                               cudaMemcpyDeviceToHost, hc->copy);
-        lo = ch.hi[c];
       }
       if (e == cudaSuccess) e = cudaEventRecord(hc->copied, hc->copy);
       copies_pending = e == cudaSuccess;
