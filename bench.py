@@ -630,6 +630,40 @@ def run_f_rows(args):
                       "timing": "CUDA events around 20 back-to-back calls (host launch overhead included)"}))
 
 
+def run_shift_sweep(args):
+    """--shift-sweep: config 4's 200 (T,P) pairs through hk.Context with and without a pressure-shift field (eq. 21,
+    PAPER.md:189): what the shifted copy, its order check / re-ordering and the per-call scratch cost per opacity function.
+    delta ~ U[-0.02, 0.02] cm^-1/atm (seeded; HITRAN's air-induced shifts are of this size).  One GPU; not a bench line."""
+    import torch
+    import paper_1503_03806_b200 as hk
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --shift-sweep: no CUDA device")
+    wl = workloads.config(4)
+    delta = np.random.default_rng(44).uniform(-0.02, 0.02, wl.n_lines)
+    N = wl.n_points
+    kap = torch.empty(N, dtype=torch.float64, device="cuda")
+    out = {}
+    for name, d in (("no_shift", None), ("with_shift", delta)):
+        lines = hk.Lines.from_numpy(wl.nu0, wl.S, wl.gamma0, E_low=wl.E_low, delta=d)
+        ctx = hk.Context(lines)
+        ctx.opacity(wl.T[0], wl.P_atm[0], wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, q_ratio=wl.q_ratio(wl.T[0]), out=kap)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0 = time.perf_counter()
+        e0.record()
+        for T in wl.T:
+            for P in wl.P_atm:
+                ctx.opacity(T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, q_ratio=wl.q_ratio(T), out=kap)
+        e1.record()
+        torch.cuda.synchronize()
+        out[name] = {"device_ms_200_pairs": e0.elapsed_time(e1), "wall_ms_200_pairs": 1e3 * (time.perf_counter() - t0)}
+        ctx.close()
+    out["overhead_frac_device"] = out["with_shift"]["device_ms_200_pairs"] / out["no_shift"]["device_ms_200_pairs"] - 1.0
+    out["overhead_frac_wall"] = out["with_shift"]["wall_ms_200_pairs"] / out["no_shift"]["wall_ms_200_pairs"] - 1.0
+    out["workload"] = "config 4 (1e6 lines, 200 (T,P) pairs, opacity functions only), delta ~ U[-0.02, 0.02] cm^-1/atm, seed 44"
+    print(json.dumps(out))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -647,8 +681,12 @@ def main():
                     help="print per-stage device times of configs 1, 2, 3 (1e7 lines) in both precisions and exit")
     ap.add_argument("--f-rows", action="store_true",
                     help="print device times of the SURVEY 8(f) rows (Chebyshev resampling, transmission) at config 1's size and exit")
+    ap.add_argument("--shift-sweep", action="store_true",
+                    help="time config 4's T-P sweep with and without a pressure-shift field (eq. 21) and exit")
     args = ap.parse_args()
-    if args.f_rows:
+    if args.shift_sweep:
+        run_shift_sweep(args)
+    elif args.f_rows:
         run_f_rows(args)
     elif args.stage_times:
         run_stage_times(args)

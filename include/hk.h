@@ -113,8 +113,9 @@ int64_t hk_grid_size(double nu_min, double nu_max, double dnu);
  *   gamma_i = A21_i/(4 pi c) + (296/T)^n_i [ gamma0_i (P - P_self) + gamma_self_i P_self ],  P_self = self_fraction * P   eq. 20
  *   nu0_i  -> nu0_i + delta_i * P_atm                                                                                    eq. 21
  * (P0 = 1 atm).  The shifted centre replaces nu0 everywhere downstream (profile centre, Doppler width, window, eq. 18).
- * Shifted centres are in general no longer ascending: with delta != NULL the library shifts a copy, checks it on the
- * device (synchronises the stream) and orders it when needed, whatever lines_sorted says.
+ * The list is NOT re-ordered for the shift: a1 shifts every centre itself and builds its line-range tables from the unshifted,
+ * ordered centres with a halo of max_i |delta_i| * P_atm; the one-shot call finds that maximum by a small reduction
+ * (synchronises the stream once), a context finds it once at hk_create.  lines_sorted refers to the unshifted nu0.
  * Mixtures: call once per species with prm->abundance = X_s and prm->accumulate = 1 from the second species on; the
  * k-distribution of the sum is then taken by hk_kdist (adding k-distributions instead would be the correlated-k
  * approximation).
@@ -216,9 +217,8 @@ int hk_voigt_K(const double *x, const double *y, int64_t n, double *out, int pre
 /* Persistent-context form for T-P sweeps ("repeat this calculation for multiple combinations of
  * temperature and pressure"): the line list is bound once, scratch is kept between calls.
  * hk_create copies nothing when nu0 is ascending: the hk_lines device arrays must outlive the context; with
- * lines_sorted = 0 and an unordered list the context owns an ordered copy (made once).  A list with a pressure shift
- * (delta != NULL) has to be re-ordered at every pressure: the context then only binds the arrays, and every
- * hk_opacity_ctx call works like hk_opacity (shifted copy, order check — synchronises the stream — scratch from the pool).
+ * lines_sorted = 0 and an unordered list the context owns an ordered copy (made once).  A pressure-shift field (delta !=
+ * NULL) costs nothing extra per call (see hk_opacity); hk_create synchronises the stream once to find max |delta|.
  * self_fraction, abundance, cutoff_widths and accumulate are taken from prm at hk_create. */
 typedef struct hk_ctx hk_ctx;
 int hk_create(const hk_lines *lines, int64_t n_lines, const hk_params *prm, hk_ctx **out);

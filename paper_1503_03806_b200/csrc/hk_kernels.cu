@@ -82,7 +82,10 @@ constexpr double kT0 = 296.0;               // K
 
 struct PrepArgs {
   const double *nu0, *S, *gamma0, *n_T, *E_low;
-  const double *gamma_self, *A21;  // eq. 20 (either may be NULL); the shift of eq. 21 is applied before a1
+  const double *gamma_self, *A21;  // eq. 20 (either may be NULL)
+  const double *delta;             // eq. 21 (may be NULL): the centre used downstream is nu0 + delta P
+  double shift_pad;                // >= max |delta| P, cm^-1: the a2 tables are built from the UNSHIFTED (ordered) centres with
+                                   // the cutoff widened by it, a superset of every shifted line's window
   double self_fraction, abundance;
   double cutoff_widths;  // > 0: line i is truncated at min(cutoff, cutoff_widths * gamma_i)
   int64_t n;
@@ -159,7 +162,10 @@ __global__ void __launch_bounds__(256) line_prep_kernel(PrepArgs a)
   if (i < 16) a.queue[i] = 0;  // one ticket counter per far-kernel launch of this call (at most kMaxChunks)
   if (a.n < 16 && i == 0)
     for (int q = (int)a.n; q < 16; ++q) a.queue[q] = 0;
-  const double nu0 = a.nu0[i];
+  // eq. 21: nu0 -> nu0 + delta P/P0, P0 = 1 atm; the shifted centre replaces nu0 everywhere downstream
+  // (C2).  The list stays in the order of the unshifted centres: nothing below needs the shifted ones ordered.
+  const double nu0u = a.nu0[i];
+  const double nu0 = a.delta ? __dadd_rn(nu0u, __dmul_rn(a.delta[i], a.P_atm)) : nu0u;
   double alpha = nu0 * a.vth;
   if (!(alpha > 1.0e-290)) alpha = 0.0;  // nu0 <= 0 (or a width whose reciprocal overflows): Lorentzian (A9)
   const double tfac = a.n_T ? pow(kT0 / a.T, a.n_T[i]) : a.tfac_half;
@@ -199,23 +205,25 @@ __global__ void __launch_bounds__(256) line_prep_kernel(PrepArgs a)
   MetaA ma;
   MetaB mb;
   LineNear nr;
-  // relative cutoff: the line's own window is narrower than the window of the absolute cutoff; the a2 tables are built from
-  // the latter (qlo, qhi: non-decreasing in i, a superset), classify32 masks with the former
+  // relative cutoff, pressure shift: the line's own window is narrower than, or displaced within, the window of the
+  // unshifted centre with the absolute cutoff widened by the largest shift; the a2 tables are built from the latter (qlo,
+  // qhi: non-decreasing in i, a superset), classify32 masks with the former
   double cut = a.cutoff;
   if (a.cutoff_widths > 0.0) cut = fmin(cut, __dmul_rn(a.cutoff_widths, gamma));
   line_window(nu0, cut, a, ma.jlo, ma.jhi);
+  const double tcut = a.cutoff + a.shift_pad;
   int qlo, qhi;
-  line_window(nu0, a.cutoff, a, qlo, qhi);
+  line_window(nu0u, tcut, a, qlo, qhi);
   {
     // a2, line-parallel half: the list is ordered by nu0, so jlo and jhi are non-decreasing in i and line i is the
     // "first line with jhi >= b*kPlanBlock" exactly for the blocks b with jhi_{i-1} < b*kPlanBlock <= jhi_i (same for jlo).
     // Each entry of first_hi / first_lo has exactly one writer; the last line also fills the blocks beyond its window.
     int plo = INT_MIN, phi = INT_MIN, pc = INT_MIN;
     if (i > 0) {
-      line_window(a.nu0[i - 1], a.cutoff, a, plo, phi);
+      line_window(a.nu0[i - 1], tcut, a, plo, phi);
       pc = line_centre_index(a.nu0[i - 1], a);
     }
-    const int jc = line_centre_index(nu0, a);
+    const int jc = line_centre_index(nu0u, a);
     const int n = (int)a.n;
     int b0 = i > 0 ? max(plan_block_floor(phi) + 1, 0) : 0, b1 = min(plan_block_floor(qhi), a.nb);
     for (int b = b0; b <= b1; ++b) a.first_hi[b] = (int)i;
@@ -1086,12 +1094,14 @@ __global__ void __launch_bounds__(128) voigt_K_kernel(const double *x, const dou
   if (live) out[i] = v;
 }
 
-// eq. 21: nu0 -> nu0 + delta P/P0, P0 = 1 atm
-__global__ void __launch_bounds__(256) shift_centres_kernel(const double *nu0, const double *delta, double P_atm, int64_t n,
-                                                            double *out)
+// largest |delta| of a line list (eq. 21): one atomicMax on the bit pattern of a non-negative double per CTA
+__global__ void __launch_bounds__(256) absmax_kernel(const double *v, int64_t n, unsigned long long *out)
 {
-  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < n) out[i] = __dadd_rn(nu0[i], __dmul_rn(delta[i], P_atm));
+  double m = 0.0;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) m = fmax(m, fabs(v[i]));
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(kFull, m, o));
+  if ((threadIdx.x & 31) == 0 && m > 0.0) atomicMax(out, (unsigned long long)__double_as_longlong(m));
 }
 
 __global__ void __launch_bounds__(256) check_sorted_kernel(const double *nu0, int64_t n, int *flag)
@@ -1328,7 +1338,7 @@ struct GridChunks {
 
 static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double P_atm, double q_ratio, double mass_amu,
                        double nu_min, double dnu, double cutoff, int64_t N, double *kappa_out, Scratch &s, const hk_params &prm,
-                       cudaStream_t st, GridChunks *chunks = nullptr)
+                       cudaStream_t st, double delta_max, GridChunks *chunks = nullptr)
 {
   const bool f32 = prm.precision == HK_FP32;
   if (n_lines == 0) {
@@ -1363,6 +1373,7 @@ static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double 
   PrepArgs pa;
   pa.nu0 = lines->nu0; pa.S = lines->S; pa.gamma0 = lines->gamma0; pa.n_T = lines->n_T; pa.E_low = lines->E_low;
   pa.gamma_self = lines->gamma_self; pa.A21 = lines->A21;
+  pa.delta = lines->delta; pa.shift_pad = lines->delta ? delta_max * P_atm * (1.0 + 1.0e-12) : 0.0;
   pa.self_fraction = prm.self_fraction; pa.abundance = prm.abundance > 0.0 ? prm.abundance : 1.0;
   pa.cutoff_widths = prm.cutoff_widths;
   pa.n = n_lines;
@@ -1393,7 +1404,8 @@ static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double 
     if (sv < 0.5) {
       va.r3_slope = sv / (1.0 - sv);
       // (FP32 variant: a line with alpha^2 < 1e-9 sends its whole 1-ball, radius <= 200 alpha < 6.4e-3 cm^-1, to this kernel)
-      va.r3_offset = (sv * fmax(nu_min / dnu, 0.0) + 4.0 + (f32 ? 6.4e-3 / dnu : 0.0)) / (1.0 - sv);
+      // (eq. 21: the tables know the unshifted centres, up to shift_pad away from the shifted ones)
+      va.r3_offset = (sv * fmax(nu_min / dnu, 0.0) + 4.0 + (f32 ? 6.4e-3 / dnu : 0.0) + pa.shift_pad / dnu) / (1.0 - sv);
     } else {  // absurdly hot / light: no useful bound, the near kernel scans every line that touches the span
       va.r3_slope = 0.0;
       va.r3_offset = 4.0e9;
@@ -1452,7 +1464,31 @@ struct hk_ctx {
   int64_t n_lines;
   hk_params prm;
   Scratch scratch;
+  double delta_max;    // max |delta| of the list (eq. 21), found once at hk_create; 0 without a shift field
 };
+
+// max |delta_i| of a device array, on the host (synchronises the stream): sizes the halo of the a2 tables under eq. 21
+static int delta_absmax(const double *delta, int64_t n, cudaStream_t st, double *out)
+{
+  *out = 0.0;
+  if (!delta || n <= 0) return HK_OK;
+  void *buf = nullptr;
+  int rc = pool_alloc(&buf, sizeof(unsigned long long), st);
+  if (rc != HK_OK) return rc;
+  cudaError_t e = cudaMemsetAsync(buf, 0, sizeof(unsigned long long), st);
+  if (e == cudaSuccess) {
+    absmax_kernel<<<(unsigned)std::min<int64_t>((n + 255) / 256, 1184), 256, 0, st>>>(delta, n, (unsigned long long *)buf);
+    e = cudaGetLastError();
+  }
+  unsigned long long bits = 0;
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&bits, buf, sizeof(bits), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  pool_free(buf, st);
+  if (e != cudaSuccess) return cuda_fail(e, "delta_absmax");
+  memcpy(out, &bits, sizeof(double));
+  if (!isfinite(*out)) return HK_ERR_INVALID;
+  return HK_OK;
+}
 
 // Resolves the line list the kernels will read: the caller's arrays when they are ascending (promised by lines_sorted = 1,
 // or found so by the device check), else an ordered copy (*buf, to be released with pool_free).
@@ -1484,31 +1520,20 @@ static int opacity_impl(const hk_lines *lines, int64_t n_lines, double T, double
   int rc = validate(lines, n_lines, T, P_atm, nu_min, nu_max, dnu, cutoff, kappa_out, prm, &N);
   if (rc != HK_OK) return rc;
   cudaStream_t st = (cudaStream_t)prm->stream;
-  hk_lines eff = *lines;
-  hk_params pe = *prm;
-  void *shift_buf = nullptr;
-  if (lines->delta && n_lines > 0) {  // eq. 21: shifted centres on a copy; their order is re-checked
-    rc = pool_alloc(&shift_buf, (size_t)n_lines * sizeof(double), st);
-    if (rc != HK_OK) return rc;
-    shift_centres_kernel<<<(unsigned)((n_lines + 255) / 256), 256, 0, st>>>(lines->nu0, lines->delta, P_atm, n_lines,
-                                                                            (double *)shift_buf);
-    eff.nu0 = (const double *)shift_buf;
-    pe.lines_sorted = 0;
-  }
-  eff.delta = nullptr;
+  // eq. 21 needs no copy and no re-ordering: a1 shifts every centre itself and builds its tables from the unshifted, ordered
+  // centres with a halo of max |delta| P (found here: one small reduction and a stream synchronisation per one-shot call)
+  double dmax = 0.0;
+  rc = delta_absmax(lines->delta, n_lines, st, &dmax);
+  if (rc != HK_OK) return rc;
   hk_lines use;
   void *sorted_buf = nullptr;
-  rc = ordered_lines(&eff, n_lines, &pe, &use, &sorted_buf);
-  if (rc != HK_OK) {
-    pool_free(shift_buf, st);
-    return rc;
-  }
+  rc = ordered_lines(lines, n_lines, prm, &use, &sorted_buf);
+  if (rc != HK_OK) return rc;
   Scratch s;
-  rc = run_opacity(&use, n_lines, T, P_atm, prm->q_ratio, prm->mass_amu, nu_min, dnu, cutoff, N, kappa_out, s, *prm, st,
+  rc = run_opacity(&use, n_lines, T, P_atm, prm->q_ratio, prm->mass_amu, nu_min, dnu, cutoff, N, kappa_out, s, *prm, st, dmax,
                    chunks);
   scratch_release(s, st);
   pool_free(sorted_buf, st);
-  pool_free(shift_buf, st);
   return rc;
 }
 
@@ -1637,20 +1662,18 @@ int hk_create(const hk_lines *lines, int64_t n_lines, const hk_params *prm, hk_c
   if (!c) return HK_ERR_NOMEM;
   c->n_lines = n_lines;
   c->prm = *prm;
-  if (lines->delta) {
-    // eq. 21: the order of the shifted centres depends on P, so nothing can be ordered once: every hk_opacity_ctx call
-    // shifts, checks and (if needed) orders a copy, as the one-shot call does
-    c->lines = *lines;
-    c->sorted_buf = nullptr;
-    *out = c;
-    return HK_OK;
-  }
   int rc = ordered_lines(lines, n_lines, prm, &c->lines, &c->sorted_buf);
   if (rc != HK_OK) {
     delete c;
     return rc;
   }
   c->prm.lines_sorted = 1;
+  rc = delta_absmax(c->lines.delta, n_lines, (cudaStream_t)prm->stream, &c->delta_max);  // eq. 21: halo of the a2 tables
+  if (rc != HK_OK) {
+    pool_free(c->sorted_buf, (cudaStream_t)prm->stream);
+    delete c;
+    return rc;
+  }
   *out = c;
   return HK_OK;
 }
@@ -1661,13 +1684,11 @@ int hk_opacity_ctx(hk_ctx *ctx, double T, double P_atm, double q_ratio, double n
   if (!ctx) return HK_ERR_INVALID;
   hk_params p = ctx->prm;
   p.q_ratio = q_ratio;
-  if (ctx->lines.delta)
-    return opacity_impl(&ctx->lines, ctx->n_lines, T, P_atm, nu_min, nu_max, dnu, cutoff, kappa_out, &p, nullptr);
   int64_t N = 0;
   int rc = validate(&ctx->lines, ctx->n_lines, T, P_atm, nu_min, nu_max, dnu, cutoff, kappa_out, &p, &N);
   if (rc != HK_OK) return rc;
   return run_opacity(&ctx->lines, ctx->n_lines, T, P_atm, q_ratio, p.mass_amu, nu_min, dnu, cutoff, N, kappa_out,
-                     ctx->scratch, p, (cudaStream_t)p.stream);
+                     ctx->scratch, p, (cudaStream_t)p.stream, ctx->delta_max);
 }
 
 int hk_destroy(hk_ctx *ctx)

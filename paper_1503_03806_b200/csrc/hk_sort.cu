@@ -36,7 +36,7 @@ __global__ void __launch_bounds__(256) gather_fields_kernel(const int *perm, int
 int sort_lines_copy(const hk_lines *in, int64_t n, cudaStream_t st, hk_lines *out, void **buf)
 {
   *buf = nullptr;
-  const int nf = 3 + (in->n_T ? 1 : 0) + (in->E_low ? 1 : 0) + (in->gamma_self ? 1 : 0) + (in->A21 ? 1 : 0);
+  const int nf = 3 + (in->n_T ? 1 : 0) + (in->E_low ? 1 : 0) + (in->gamma_self ? 1 : 0) + (in->A21 ? 1 : 0) + (in->delta ? 1 : 0);
   const size_t fbytes = ((size_t)n * sizeof(double) + 255) & ~(size_t)255;
   const size_t ibytes = ((size_t)n * sizeof(int) + 255) & ~(size_t)255;
   size_t tmp_bytes = 0;
@@ -64,14 +64,15 @@ int sort_lines_copy(const hk_lines *in, int64_t n, cudaStream_t st, hk_lines *ou
     int used = 3 + (in->n_T ? 1 : 0) + (in->E_low ? 1 : 0);
     double *dGs = in->gamma_self ? (double *)((char *)keep + (size_t)(used++) * fbytes) : nullptr;
     double *dA = in->A21 ? (double *)((char *)keep + (size_t)(used++) * fbytes) : nullptr;
+    double *dD = in->delta ? (double *)((char *)keep + (size_t)(used++) * fbytes) : nullptr;
     gather_fields_kernel<<<blocks, 256, 0, st>>>(idx_out, n, in->S, in->gamma0, in->n_T, in->E_low, dS, dG, dN, dE);
-    if (dGs || dA)
-      gather_fields_kernel<<<blocks, 256, 0, st>>>(idx_out, n, in->gamma_self, in->A21, nullptr, nullptr, dGs, dA, nullptr,
+    if (dGs || dA || dD)
+      gather_fields_kernel<<<blocks, 256, 0, st>>>(idx_out, n, in->gamma_self, in->A21, in->delta, nullptr, dGs, dA, dD,
                                                    nullptr);
     e = cudaGetLastError();
     out->gamma_self = dGs;
     out->A21 = dA;
-    out->delta = nullptr;  // eq. 21 is applied to nu0 before the list is ordered
+    out->delta = dD;  // eq. 21 is applied by a1: the list is ordered by the unshifted centres
     out->nu0 = f;
     out->S = dS;
     out->gamma0 = dG;

@@ -89,12 +89,34 @@ def test_no_cutoff_every_line_on_every_point():
     _check(hk.hk_opacity(lines, T, P, wl.nu_min, wl.nu_max, wl.dnu, big, precision=hk.HK_FP32).cpu().numpy(), ref, BAR32)
 
 
+def test_large_pressure_shifts_on_a_dense_unsorted_list():
+    # eq. 21 without re-ordering: a1 shifts the centres itself and builds its line-range tables from the unshifted ones with a
+    # halo of max |delta| P.  Here the shifts (up to 1 cm^-1 = 100 grid steps, several 256-point spans apart at the tile
+    # edges) are far larger than the line spacing (0.01 cm^-1) and the list arrives unsorted as well.
+    import torch
+    wl = workloads.small(seed=71, n_lines=20000, nu_max=200.0, cutoff=10.0, sorted_by_nu0=False)
+    delta = np.random.default_rng(72).uniform(-0.02, 0.02, wl.n_lines)
+    T, P = 1200.0, 50.0
+    assert np.count_nonzero(np.diff(np.sort(wl.nu0) + delta[np.argsort(wl.nu0)] * P) < 0) > 5000
+    ref = oracle.opacity_full(wl.nu0, wl.S, wl.gamma0, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, delta=delta)
+    lines = hk.Lines.from_numpy(wl.nu0, wl.S, wl.gamma0, delta=delta)
+    for prec, bar in ((hk.HK_FP64, BAR), (hk.HK_FP32, BAR32)):
+        got = hk.hk_opacity(lines, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, lines_sorted=False, precision=prec)
+        torch.cuda.synchronize()
+        _check(got.cpu().numpy(), ref, bar)
+    ctx = hk.Context(lines, lines_sorted=False)
+    for Pc in (50.0, 0.01):
+        a = ctx.opacity(T, Pc, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff)
+        assert torch.equal(a, hk.hk_opacity(lines, T, Pc, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, lines_sorted=False))
+    ctx.close()
+
+
 def test_context_with_a_pressure_shift_and_bad_fractions():
     import torch
     wl = workloads.small(seed=61, n_lines=50, nu_max=50.0, cutoff=25.0)
     ex = _fields(wl, 62)
     shifted = hk.Lines.from_numpy(wl.nu0, wl.S, wl.gamma0, delta=ex["delta"])
-    ctx = hk.Context(shifted)                                       # re-ordered at every pressure
+    ctx = hk.Context(shifted)                                       # the shift is applied by a1 at every pressure
     for P in (0.5, 40.0):
         a = ctx.opacity(1200.0, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff)
         b = hk.hk_opacity(shifted, 1200.0, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff)
