@@ -61,7 +61,11 @@ FAR_REGIMES, NEAR_REGIMES = ("gh1", "gh2", "gh3"), ("gh6", "series")
 FP32_INST_PER_EVAL = {"gh1": 4.0, "gh2": 6.5, "gh3": 10.0}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the roofline kernels, from the committed `ncu --set full` capture
 # named here (not live: ncu cannot run inside a timed bench).  Not memory-bound: context only.
-NCU_DRAM = {"fp64": {"bytes": None, "source": None}, "fp32": {"bytes": None, "source": None}}
+NCU_DRAM = {"fp64": {"bytes": 9.725e6 + 36.882e6 + 0.016e6,   # far 9.72 MB read, near 36.88 MB read + 16 KB written
+                     "source": "profiles/r02_voigt_far_kernel_ncu_full.txt + r02_voigt_near_kernel_ncu_full.txt (ncu flushes the "
+                               "caches before each kernel: the near kernel's 36.9 MB are the 24 MB of kappa the far kernel wrote, "
+                               "L2-resident in a real step, plus line records)"},
+            "fp32": {"bytes": 6.517e6 + 0.001e6, "source": "profiles/r02_voigt_far32_kernel_ncu_full.txt"}}
 NOMINAL_FP64_LANES = 148 * 64   # DFMA lanes of a B200 (B200_PROFILING.md): nominal peak = lanes x SM clock
 
 
