@@ -1,14 +1,16 @@
 // hk_kernels.cu — sm_100a kernels and the C ABI of include/hk.h.
 //
 // Steps:
-//   a1 line_prep_kernel   per line: alpha, gamma (eq. 20), S(T) (eq. 18), amplitude, index window (absolute or relative
-//                         cutoff), regime radii, packed records
+//   a1 line_prep_kernel   per line: alpha, gamma (eq. 20), centre shift (eq. 21), S(T) (eq. 18), amplitude, index window
+//                         (absolute or relative cutoff), regime balls in index space, packed records
 //   a2 (same kernel)      per 256-point block: first line ending / beginning / centred there (lookup tables: a tile's line
 //                         range is two reads)
-//   a3 voigt_far_kernel   far wings (1-/2-point rule) of kappa_j = sum_i amp_i V_i(nu_j): grid-point-owned register
-//                         accumulation, persistent CTAs on a tile queue, lines streamed through a shared-memory ring by 1-D
-//                         TMA bulk copies completing on mbarriers; FP64, or the FP32 variant (template parameter)
-//      voigt_near_kernel  line cores and near wings (3-, 6-point rule, series), one CTA per 256-point span, adds to kappa
+//   a3 voigt_far_kernel   every 32-point group outside a line's 3-point radius (1-/2-/3-point rule) of kappa_j = sum_i amp_i
+//                         V_i(nu_j): grid-point-owned register accumulation, persistent CTAs on a tile queue, lines streamed
+//                         through a shared-memory ring by 1-D TMA bulk copies completing on mbarriers; FP64 in two shapes
+//                         (by list density), or the FP32 variant (template parameters)
+//      voigt_near_kernel  every group that touches it (6-point rule, series): one warp per 256-point span works off queues
+//                         of uniform items, per-line constants computed once by lane = line; adds to kappa
 //   a4                    coalesced kappa store from the far kernel ("without additional write-outs")
 //   a5/a6 kdist_kernel    (hk_kdist.cu) per-bin register/shuffle bitonic sort + resampling at Gauss-Legendre nodes
 // eq. 20/21 line physics, mixtures and the relative cutoff live in a1 and the host code below;

@@ -9,7 +9,8 @@
 //   r^2 >= 3200  : 2-point Gauss-Hermite                                       7 FP64 + 1 MUFU
 //   r^2 >= 280   : 3-point Gauss-Hermite ("third-order", Letchworth & Benner) 11 FP64 + 1 MUFU
 //   r^2 >= 44    : 6-point Gauss-Hermite                                      22 FP64 + 3 MUFU
-//   else         : Algorithm-916-type series (Zaghloul & Ali 2012), step a = 0.7, 16 terms
+//   else         : Algorithm-916-type series (Zaghloul & Ali 2012), step a = 0.7, 16 terms   83 FP64 + 1 MUFU
+// (the kernels switch between the last two at x^2 = 44.15 - y^2, inside the band where both are valid: kSeriesPad)
 //
 // n-point Gauss-Hermite in dimensional form (no 1/alpha, safe as alpha -> 0), with nodes +-t_k, normalised
 // weights wn_k (sum 1) and q = d^2:
