@@ -103,6 +103,21 @@ __device__ __forceinline__ void gh1_acc2(double &a0, double &a1, double d0, doub
   a0 = fma(t, D1, a0);
   a1 = fma(t, D0, a1);
 }
+// the same for FOUR points with one reciprocal, 1/(D0 D1 D2 D3), through the cross products c02 = D0 D2, c13 = D1 D3:
+// A1/D0 = (t c13) D2, A1/D1 = (t c02) D3, A1/D2 = (t c13) D0, A1/D3 = (t c02) D1 with t = A1/(c02 c13).  20 FP64 + 1 MUFU
+// per four points: the FP64 count of two pairs, a quarter of the MUFU.RCP64H of four single evaluations.
+__device__ __forceinline__ void gh1_acc4(double &a0, double &a1, double &a2, double &a3, double d0, double d1, double d2,
+                                         double d3, double A1, double g2)
+{
+  const double D0 = fma(d0, d0, g2), D1 = fma(d1, d1, g2), D2 = fma(d2, d2, g2), D3 = fma(d3, d3, g2);
+  const double c02 = D0 * D2, c13 = D1 * D3;
+  const double t = A1 * rcp_nr(c02 * c13);
+  const double u0 = t * c13, u1 = t * c02;
+  a0 = fma(u0, D2, a0);
+  a1 = fma(u1, D3, a1);
+  a2 = fma(u0, D0, a2);
+  a3 = fma(u1, D1, a3);
+}
 // 2-point (t^2 = 1/2, wn = 1/2): A1 (E + alpha^2)/(E^2 + f2), E = d^2 + e2, e2 = g2 - a2/2, f2 = 2 a2 g2
 __device__ __forceinline__ double gh2_acc(double acc, double d, double A1, double e2, double f2, double A1a2)
 {
