@@ -20,7 +20,8 @@ units extrapolated to the whole config by N_evals (SURVEY.md:386-391).  `--no-co
 N > 1 (torchrun, one rank per GPU): the path shards with NO collective — rank r computes the opacity function of the r-th
 (T, P) pair of a small T-P table over the same line list ("repeat this calculation for multiple combinations of
 temperature and pressure"); rank 0 keeps config 1's (1500 K, 1 atm).  Per-GPU work is fixed: weak scaling.  NCCL is used only
-for the barrier and the max-over-ranks of the device time.
+for the barrier and the max-over-ranks of the device time.  `--shard grid` instead splits ONE opacity function of config 3 along
+the wavenumber grid (shard.shard_grid: bin-aligned ranges balanced by line-point evaluations; strong scaling).
 
 Prints ONE JSON line (rank 0).  `value` = line-point Voigt evaluations per second, whole job, inputs resident in HBM, device time
 by CUDA events around each step (L2 flushed between steps, outside the events).  `e2e` = the same metric through
@@ -592,6 +593,74 @@ def run_ours(args):
         raise SystemExit("bench.py: parity against the oracle above the bar (see the `parity` keys of the line)")
 
 
+def run_grid_shard(args):
+    """--shard grid (with --gpus N under torchrun): ONE opacity function + k-distribution of config 3 split along the
+    wavenumber grid by shard.shard_grid — contiguous, bin-aligned ranges balanced by line-point evaluations, each rank with the
+    slice of the line list whose windows reach its range (a read-only halo, no collective on the data path).
+    Strong scaling: the total work is fixed.  NCCL carries the barrier and the max-over-ranks of the device time only."""
+    import torch
+    import torch.distributed as dist
+    import paper_1503_03806_b200 as hk
+    from paper_1503_03806_b200 import shard
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --shard grid: no CUDA device")
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    wl = workloads.config(3, n_lines=args.shard_lines)
+    T, P = wl.T[0], wl.P_atm[0]
+    N = wl.n_points
+    ppb = int(round(wl.bin_width / wl.dnu))
+    sh = shard.shard_grid(wl.nu0, wl.nu_min, N, wl.dnu, wl.cutoff, ppb, world)[rank]
+    sl = slice(sh.line_lo, sh.line_hi)
+    lines = hk.Lines.from_numpy(wl.nu0[sl], wl.S[sl], wl.gamma0[sl])
+    n_own = sh.j_hi - sh.j_lo
+    kap = torch.empty(n_own, dtype=torch.float64, device="cuda")
+    ktab = torch.empty((n_own // ppb, wl.n_g), dtype=torch.float64, device="cuda")
+    ctx = hk.Context(lines)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        ctx.opacity(T, P, sh.nu_min, sh.nu_max, wl.dnu, wl.cutoff, out=kap)
+        hk.hk_kdist(kap, wl.dnu, wl.bin_width, wl.n_g, out=ktab)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for i in range(args.steps):
+        ev[i][0].record(stream)
+        step()
+        ev[i][1].record(stream)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    red = torch.tensor([sum(a.elapsed_time(b) for a, b in ev)], dtype=torch.float64, device="cuda")
+    tot = torch.tensor([float(sh.evals)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(red, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+    ctx.close()
+    if rank == 0:
+        ms = float(red.item())
+        print(json.dumps({
+            "metric": METRIC, "value": float(tot.item()) * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"BASELINE.json configs[3] with {wl.n_lines} lines: one opacity function + k-distribution, grid "
+                                   f"split into {world} bin-aligned ranges balanced by line-point evaluations (shard.shard_grid)",
+                       "parallelism": f"grid-range x{world} (no collective)", "line_point_evals": int(tot.item()),
+                       "l2": "line records (144 B/line) >> L2: no flush"},
+            "gpu_launches": 4 * args.steps}))
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def run_stage_times(args):
     """--stage-times: per-stage device times (hk_set_timing) of hk_opacity on configs 1, 2 (its highest pressure) and 3 cut to
     1e7 lines, in both precisions — the figures profiles/ and DESIGN.md quote beside the bench line.  One GPU; not a bench line."""
@@ -703,6 +772,10 @@ def main():
                     help="print per-stage device times of configs 1, 2, 3 (1e7 lines) in both precisions and exit")
     ap.add_argument("--f-rows", action="store_true",
                     help="print device times of the SURVEY 8(f) rows (Chebyshev resampling, transmission) at config 1's size and exit")
+    ap.add_argument("--shard", choices=["pairs", "grid"], default="pairs",
+                    help="N > 1: 'pairs' (default) gives rank r the r-th (T,P) pair of config 1, weak scaling; 'grid' splits ONE "
+                         "opacity function of config 3 along the grid (shard.shard_grid), strong scaling")
+    ap.add_argument("--shard-lines", type=int, default=100_000_000, help="--shard grid: lines of config 3 (default: all 1e8)")
     ap.add_argument("--shift-sweep", action="store_true",
                     help="time config 4's T-P sweep with and without a pressure-shift field (eq. 21) and exit")
     args = ap.parse_args()
@@ -716,6 +789,8 @@ def main():
         run_reference(args)
     elif args.config is not None:
         run_config(args)
+    elif args.shard == "grid":
+        run_grid_shard(args)
     else:
         run_ours(args)
 
