@@ -31,8 +31,12 @@ def is_stale() -> bool:
 
 
 def build_library(force: bool = False, verbose: bool = False) -> str:
+    """HK_DEBUG_CHECKS=1 in the environment compiles the index checks (HK_CHECK: a trap instead of an out-of-range access) and the
+    ring watchdog in: the build the GPU test suite is run against once per round in place of compute-sanitizer, which is
+    closed on this GPU pool."""
     if force or is_stale():
-        cmd = [nvcc_path()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SRC
+        dbg = ["-DHK_DEBUG_CHECKS", "-DHK_WATCHDOG"] if os.environ.get("HK_DEBUG_CHECKS") == "1" else []
+        cmd = [nvcc_path()] + NVCC_FLAGS + dbg + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SRC
         subprocess.run(cmd, check=True)
     return LIB
 

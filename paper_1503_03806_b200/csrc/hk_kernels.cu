@@ -31,6 +31,14 @@
 
 namespace hk {
 
+// Index checks compiled in by -DHK_DEBUG_CHECKS (a trap instead of a silent out-of-range access): compute-sanitizer is closed on
+// the GPU pool this was developed on, so the GPU test suite is run once per round against such a build (profiles/).
+#ifdef HK_DEBUG_CHECKS
+#define HK_CHECK(cond) do { if (!(cond)) __trap(); } while (0)
+#else
+#define HK_CHECK(cond) do { } while (0)
+#endif
+
 // ------------------------------------------------------------------------------------------------------
 // packed line records (written by a1, streamed by a3): two 16-byte and three 32-byte records per line, structure of
 // arrays, so that a chunk of lines is five contiguous 16-byte-aligned spans (one TMA bulk copy each) and a warp that
@@ -228,6 +236,7 @@ __global__ void __launch_bounds__(256) line_prep_kernel(PrepArgs a)
     const int jc = line_centre_index(nu0u, a);
     const int n = (int)a.n;
     int b0 = i > 0 ? max(plan_block_floor(phi) + 1, 0) : 0, b1 = min(plan_block_floor(qhi), a.nb);
+    HK_CHECK(b0 >= 0 && b1 <= a.nb);
     for (int b = b0; b <= b1; ++b) a.first_hi[b] = (int)i;
     if (i == n - 1)
       for (int b = max(plan_block_floor(qhi) + 1, 0); b <= a.nb; ++b) a.first_hi[b] = n;
@@ -439,6 +448,7 @@ struct VoigtArgs {
   double nu_min, dnu;
   float dnu_f;
   int N;
+  int n_lines;
   int accumulate;  // 1: add to kappa (species of a mixture after the first), 0: overwrite
   int block0;      // near kernel: first 256-point span of this launch (the near kernel may run as several launches)
   double *kappa;
@@ -527,6 +537,7 @@ __device__ __forceinline__ void issue_chunk(VoigtSmem<Sh> &S, const VoigtArgs &a
   S.hdr[stage] = h;
   S.cur_c = c + 1;
   const uint32_t nb = (uint32_t)h.cnt;
+  HK_CHECK(h.cnt >= 0 && h.cnt <= CH && S.cur_L0 >= 0 && S.cur_L0 + c * CH + h.cnt <= a.n_lines && stage >= 0 && stage < STAGES);
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // the stage's previous readers (generic proxy) come first
   mbar_expect_tx(&S.full[stage], nb * VoigtSmem<Sh>::Recs::kBytes);  // release: the header store above is visible to the waiters
   if (nb) {
@@ -793,6 +804,7 @@ __global__ void __launch_bounds__(Sh::WARPS * 32, Sh::MINB) voigt_far_kernel(con
 #pragma unroll
       for (int k = 0; k < P; ++k) {
         const int j = slo + lane + 32 * k;
+        HK_CHECK(j > shi || (j >= 0 && j < a.N));
         if (j <= shi) a.kappa[j] = a.accumulate ? a.kappa[j] + acc[k] : acc[k];
         acc[k] = 0.0;
       }
@@ -930,6 +942,7 @@ __global__ void __launch_bounds__(32, HK_NEAR_MINB) voigt_near_kernel(const __gr
     if (lm == 0u) continue;
     const unsigned lt = (1u << lane) - 1u;
     const int e = __popc(lm & lt);  // slot
+    HK_CHECK(!listed || (e < kNearCap && kA >= 0 && kB < kNearP && i < a.n_lines));
     int ns = 0, kS0 = 8, kS1 = -1, sa = 0, sb = -1;
     unsigned tiny = 0u;
     if (listed) {
@@ -967,6 +980,7 @@ __global__ void __launch_bounds__(32, HK_NEAR_MINB) voigt_near_kernel(const __gr
     for (int k = 0; k < kNearP; ++k) {
       const bool has = listed && k >= kA && k <= kB && (k < kS0 || k > kS1);
       const unsigned bk = __ballot_sync(kFull, has);
+      HK_CHECK(__popc(bk) <= kNearCap);
       if (has) S.q6[k][__popc(bk & lt)] = (unsigned char)((unsigned)e | tiny);
       if (lane == 0) S.n6[k] = __popc(bk);
     }
@@ -980,8 +994,10 @@ __global__ void __launch_bounds__(32, HK_NEAR_MINB) voigt_near_kernel(const __gr
     const int nstot = __shfl_sync(kFull, incl, 31);
     {
       int os = incl - ns;
-      for (int j = sa; j <= sb; j += 32)
+      for (int j = sa; j <= sb; j += 32) {
+        HK_CHECK(os < kNearCap * (kNearP + 1) && j >= plo && j - plo < kPlanBlock && min(sb, j + 31) <= phi);
         S.qs[os++] = (unsigned)e | ((unsigned)(j - plo) << 8) | ((unsigned)(min(sb - j, 31)) << 16);
+      }
     }
     if (!any) cp_async_wait_all();
     any = true;
@@ -1023,6 +1039,7 @@ __global__ void __launch_bounds__(32, HK_NEAR_MINB) voigt_near_kernel(const __gr
         const SeriesLine Ls0 = S.ser[e0], Ls1 = S.ser[e1];
         const double v0 = series_val(d0, Ls0, S.W[e0]);
         const double v1 = series_val(d1, Ls1, S.W[e1]);
+        HK_CHECK(off0 + (int)(u0 >> 16) < kPlanBlock && off1 + (int)(u1 >> 16) < kPlanBlock && (u0 >> 16) < 32u && (u1 >> 16) < 32u);
         if (lane <= (int)(u0 >> 16)) S.sk[off0 + lane] += v0;
         __syncwarp();
         if (lane <= (int)(u1 >> 16)) S.sk[off1 + lane] += v1;
@@ -1398,7 +1415,7 @@ static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double 
   va.dnu_f = (float)dnu;
   va.first_hi = s.first_hi; va.first_lo = s.first_lo; va.first_c = s.first_c; va.queue = s.queue;
   va.nb = nb; va.n_tiles = n_tiles; va.tile0 = 0;
-  va.nu_min = nu_min; va.dnu = dnu; va.N = (int)N; va.kappa = kappa_out; va.accumulate = prm.accumulate ? 1 : 0;
+  va.nu_min = nu_min; va.dnu = dnu; va.N = (int)N; va.n_lines = (int)n_lines; va.kappa = kappa_out; va.accumulate = prm.accumulate ? 1 : 0;
   {
     // bound on the 3-ball radius (grid units) of any line that can have grid point j inside its 3-ball:
     // r3 <= s*alpha/dnu with alpha = vth*nu0 and nu0 <= nu_j + r3*dnu, s^2 = max(R3, Gaussian-term radius) (a hair more)
