@@ -22,7 +22,7 @@
  *   - Calls enqueue work on `stream` (a cudaStream_t passed as void*; NULL = the legacy default stream) and
  *     return without synchronising, except where stated; the caller synchronises before reading results.
  *     Scratch memory is taken from the library's own stream-ordered CUDA memory pool (one per device, kept for reuse)
- *     and returned to it on the same stream.
+ *     and returned to it on the same stream (hk_opacity_noalloc excepted: it allocates nothing, see there).
  *   - Return value: HK_OK (0) or a negative HK_ERR_* code; hk_strerror() names it; after HK_ERR_CUDA,
  *     hk_last_cuda_error() returns the CUDA runtime's message.  No exceptions.
  *   - State the library keeps.  Per host thread: the last-error string, the hk_set_timing() switch with its events, and
@@ -151,6 +151,48 @@ int hk_opacity(const hk_lines *lines, int64_t n_lines, double T, double P_atm, d
 int hk_opacity_host(const hk_lines *lines_host, int64_t n_lines, double T, double P_atm, double nu_min, double nu_max,
                     double dnu, double cutoff, double *kappa_host_out, double bin_width, int n_g, double *k_host_out,
                     const hk_params *prm);
+
+/* hk_opacity for callers that must not allocate device memory.
+ *
+ * Who this is for.  Some programs cannot let a library take memory from the CUDA driver at the moment they call it: a
+ * serving or training process that handed all of the GPU's memory to its own arena at start-up (a cudaMalloc, or the
+ * growth of this library's pool, would then fail or eat into what the arena was promised); a latency-bound loop that
+ * shares the device with other running streams (an allocation may take driver locks or make the device wait); a
+ * deployment whose memory is audited after start-up and where later allocation calls are forbidden outright.
+ * hk_opacity() takes its work space — the packed per-line records of step a1 and the line-range tables of step a2 — from
+ * the library's memory pool, which grows through the driver on demand; this entry point runs the same kernels with that
+ * work space in a fixed array compiled into the library (`static __device__`, 256-byte aligned) instead.
+ *
+ * The price and the limits.  The array is HK_NOALLOC_SCRATCH_BYTES (about 11.2 MiB) and exists on every GPU on which
+ * the process has loaded this library, used or not, until the process exits.  It holds at most HK_NOALLOC_MAX_LINES
+ * lines and a grid of at most HK_NOALLOC_MAX_POINTS points; a larger request returns HK_ERR_UNSUPPORTED and
+ * hk_last_cuda_error() says which limit was passed and by how much.  (A longer list can be fed in ordered pieces of
+ * at most HK_NOALLOC_MAX_LINES lines with prm->accumulate = 1 from the second piece on; a longer grid in ranges.)
+ * Two services of hk_opacity() need an allocation and a host wait and are therefore refused here, also with
+ * HK_ERR_UNSUPPORTED: prm->lines_sorted must be 1 (no order check, no ordered copy: pass nu0 ascending), and
+ * lines->delta must be NULL (no pressure shift, eq. 21).  hk_set_timing() has no effect on this call.
+ *
+ * Arguments, results, units, the remaining error codes and both precisions are those of hk_opacity(); for the same
+ * inputs the output is bit-for-bit the same.  The caller still supplies every input and kappa_out as device memory
+ * of its own.  The call enqueues on prm->stream and returns without waiting.  It makes no cudaMalloc / cudaFree /
+ * pool call and calls no library routine that allocates device memory.
+ *
+ * First call on each device.  The first call a process makes on a given device (with that device current) looks up
+ * the device address of the array, sets the kernels' shared-memory attributes and sizes their grids, and lets the
+ * CUDA runtime load the kernels; later calls on that device only launch.  Make that first call during start-up, before
+ * any stream capture is begun.
+ *
+ * One array, shared.  Every call on a device — from any host thread, on any stream — uses the same array, and the array
+ * keeps what the previous call left in it.  Nothing in it is trusted from call to call: every record and table entry a
+ * call reads is written by that call first, and the tile-ticket counters that must start at zero are cleared by the
+ * call's first kernel.  Because the array is shared, two of these calls must not overlap on the GPU: issue them on one
+ * stream, or order them with events.  Calls that overlap race on the array and give wrong results without any error.
+ * hk_opacity() and the other entry points do not touch the array and may run beside it. */
+#define HK_NOALLOC_MAX_LINES 65536
+#define HK_NOALLOC_MAX_POINTS 4194304
+#define HK_NOALLOC_SCRATCH_BYTES (HK_NOALLOC_MAX_LINES * 176 + 196864)
+int hk_opacity_noalloc(const hk_lines *lines, int64_t n_lines, double T, double P_atm, double nu_min, double nu_max,
+                       double dnu, double cutoff, double *kappa_out, const hk_params *prm);
 
 /* Synchronous check that a device nu0 array is ascending (what lines_sorted = 1 promises).
  * Returns HK_OK, HK_ERR_UNSORTED, or an error.  Blocks until the stream is idle. */

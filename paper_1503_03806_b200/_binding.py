@@ -64,6 +64,8 @@ def load_library():
     L.hk_opacity.restype = C.c_int
     L.hk_opacity.argtypes = [C.POINTER(_hk_lines), _i64, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double,
                              C.c_double, C.c_void_p, C.POINTER(_hk_params)]
+    L.hk_opacity_noalloc.restype = C.c_int
+    L.hk_opacity_noalloc.argtypes = L.hk_opacity.argtypes
     L.hk_opacity_host.restype = C.c_int
     L.hk_opacity_host.argtypes = [C.POINTER(_hk_lines), _i64, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double,
                                   C.c_double, C.c_void_p, C.c_double, C.c_int, C.c_void_p, C.POINTER(_hk_params)]
@@ -235,6 +237,35 @@ def hk_opacity(lines: Lines, T, P_atm, nu_min, nu_max, dnu, cutoff, mass_amu=18.
     prm = _params(mass_amu, q_ratio, precision, lines_sorted, stream, self_fraction, abundance, accumulate, cutoff_widths)
     _check(L.hk_opacity(C.byref(cl), lines.n, T, P_atm, nu_min, nu_max, dnu, cutoff, _dev_ptr(out, "out"), C.byref(prm)),
            "hk_opacity")
+    return out
+
+
+HK_NOALLOC_MAX_LINES, HK_NOALLOC_MAX_POINTS = 65536, 4194304
+
+
+def hk_opacity_noalloc(lines: Lines, T, P_atm, nu_min, nu_max, dnu, cutoff, out, mass_amu=18.0, q_ratio=1.0, stream=None,
+                       precision=HK_FP64, self_fraction=0.5, abundance=1.0, accumulate=False, cutoff_widths=0.0):
+    """hk_opacity for a caller that may not allocate GPU memory when it calls (its process gave the whole device to an arena
+    of its own, or it sits in a latency-bound loop, or allocation after start-up is forbidden to it): hk_opacity_noalloc of
+    include/hk.h.  Same kernels and bit-for-bit the same kappa as hk_opacity, with the library's work space in a fixed
+    ~11 MiB array inside libhk.so instead of its memory pool.  `out` (float64 CUDA tensor, one entry per grid point) is
+    required: this binding allocates nothing either.  At most HK_NOALLOC_MAX_LINES lines, ascending in nu0, no pressure
+    shift (lines.delta), at most HK_NOALLOC_MAX_POINTS grid points; beyond that HKError (unsupported) names the limit.
+    Asynchronous on the current (or given) torch stream.  All calls on a device share the one array: keep them on one
+    stream or order them, overlapping calls corrupt each other.  Make the first call on a device at start-up (it does the
+    one-time set-up), outside any stream capture."""
+    L = load_library()
+    N = hk_grid_size(nu_min, nu_max, dnu)
+    if out is None:
+        raise ValueError("out is required: hk_opacity_noalloc allocates nothing")
+    if N >= 1 and int(out.numel()) != N:
+        raise ValueError(f"out has {int(out.numel())} entries, the grid has {N}")
+    cl = lines._c()
+    prm = _params(mass_amu, q_ratio, precision, True, stream, self_fraction, abundance, accumulate, cutoff_widths)
+    rc = L.hk_opacity_noalloc(C.byref(cl), lines.n, T, P_atm, nu_min, nu_max, dnu, cutoff, _dev_ptr(out, "out"), C.byref(prm))
+    if rc == -5:
+        raise HKError(rc, "hk_opacity_noalloc", L.hk_last_cuda_error().decode())
+    _check(rc, "hk_opacity_noalloc")
     return out
 
 

@@ -1474,6 +1474,59 @@ static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double 
   return HK_OK;
 }
 
+// ------------------------------------------------------------------------------------------------------
+// hk_opacity_noalloc (include/hk.h): the work space of a1/a2 as a fixed array in the library image, for callers that may not
+// allocate.  Layout: the six record arrays of Scratch at a stride of kNoAllocMaxLines records each, then the FP32 variant's
+// records, then (256-byte aligned) first_hi | first_lo | first_c | 16 ticket counters for a grid of kNoAllocMaxBlocks blocks.
+// In host code `g_noalloc_scratch` names a host-side shadow of the symbol, NOT device memory: the kernels are given the
+// address cudaGetSymbolAddress returns for the current device, looked up once per device.
+// ------------------------------------------------------------------------------------------------------
+constexpr int64_t kNoAllocMaxLines = HK_NOALLOC_MAX_LINES;
+constexpr int64_t kNoAllocMaxPoints = HK_NOALLOC_MAX_POINTS;
+constexpr int kNoAllocMaxBlocks = (int)(kNoAllocMaxPoints / kPlanBlock);
+constexpr size_t kNoAllocLineBytes = (size_t)kNoAllocMaxLines * (kBytesPerLine + sizeof(LineF32));
+constexpr size_t kNoAllocTableBytes = ((((size_t)3 * (kNoAllocMaxBlocks + 1) + 16) * sizeof(int)) + 255) & ~(size_t)255;
+constexpr size_t kNoAllocBytes = kNoAllocLineBytes + kNoAllocTableBytes;
+static_assert(kNoAllocBytes == (size_t)HK_NOALLOC_SCRATCH_BYTES, "hk.h states the size of the array");
+static_assert(kNoAllocMaxPoints % kPlanBlock == 0 && kNoAllocLineBytes % 256 == 0, "table part stays 256-byte aligned");
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNoAllocBytes];
+
+// device address of the array on the current device (first use per device: one cudaGetSymbolAddress, checked)
+static int noalloc_scratch(Scratch *out)
+{
+  static unsigned char *base[64] = {};
+  static PerDeviceOnce once;
+  int dev = 0;
+  HK_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) return HK_ERR_UNSUPPORTED;
+  const int rc = once.run([](int d) {
+    void *p = nullptr;
+    HK_CUDA(cudaGetSymbolAddress(&p, g_noalloc_scratch));
+    if (!p || ((uintptr_t)p & 255u)) return (int)HK_ERR_CUDA;
+    base[d] = (unsigned char *)p;
+    return (int)HK_OK;
+  });
+  if (rc != HK_OK) return rc;
+  unsigned char *p = base[dev];
+  const size_t n = (size_t)kNoAllocMaxLines;
+  Scratch s;
+  s.ma = (MetaA *)p;
+  s.mb = (MetaB *)(p + n * 16);
+  s.base = (LineBase *)(p + n * 32);
+  s.gh2 = (LineGH2 *)(p + n * 64);
+  s.core = (LineCore *)(p + n * 96);
+  s.near = (LineNear *)(p + n * 128);
+  s.f32 = (LineF32 *)(p + n * kBytesPerLine);
+  s.first_hi = (int *)(p + kNoAllocLineBytes);
+  s.first_lo = s.first_hi + (kNoAllocMaxBlocks + 1);
+  s.first_c = s.first_lo + (kNoAllocMaxBlocks + 1);
+  s.queue = s.first_c + (kNoAllocMaxBlocks + 1);
+  s.cap_lines = kNoAllocMaxLines;   // scratch_reserve() finds room for every admitted size and allocates nothing
+  s.cap_blocks = kNoAllocMaxBlocks;
+  *out = s;
+  return HK_OK;
+}
+
 }  // namespace hk
 
 using namespace hk;
@@ -1561,6 +1614,46 @@ int hk_opacity(const hk_lines *lines, int64_t n_lines, double T, double P_atm, d
                double cutoff, double *kappa_out, const hk_params *prm)
 {
   return opacity_impl(lines, n_lines, T, P_atm, nu_min, nu_max, dnu, cutoff, kappa_out, prm, nullptr);
+}
+
+// hk_opacity on the fixed work space (see include/hk.h): no allocation, no host wait
+int hk_opacity_noalloc(const hk_lines *lines, int64_t n_lines, double T, double P_atm, double nu_min, double nu_max,
+                       double dnu, double cutoff, double *kappa_out, const hk_params *prm)
+{
+  int64_t N = 0;
+  int rc = validate(lines, n_lines, T, P_atm, nu_min, nu_max, dnu, cutoff, kappa_out, prm, &N);
+  if (rc != HK_OK) return rc;
+  if (n_lines > kNoAllocMaxLines) {
+    snprintf(g_cuda_err, sizeof(g_cuda_err),
+             "hk_opacity_noalloc: %lld lines, the fixed work space holds HK_NOALLOC_MAX_LINES = %lld (feed the list in ordered "
+             "pieces with accumulate = 1, or call hk_opacity)", (long long)n_lines, (long long)kNoAllocMaxLines);
+    return HK_ERR_UNSUPPORTED;
+  }
+  if (N > kNoAllocMaxPoints) {
+    snprintf(g_cuda_err, sizeof(g_cuda_err),
+             "hk_opacity_noalloc: %lld grid points, the fixed work space serves HK_NOALLOC_MAX_POINTS = %lld (split the grid "
+             "into ranges, or call hk_opacity)", (long long)N, (long long)kNoAllocMaxPoints);
+    return HK_ERR_UNSUPPORTED;
+  }
+  if (!prm->lines_sorted) {
+    snprintf(g_cuda_err, sizeof(g_cuda_err),
+             "hk_opacity_noalloc: lines_sorted must be 1 (checking or re-ordering the list needs an allocation and a host wait)");
+    return HK_ERR_UNSUPPORTED;
+  }
+  if (lines->delta) {
+    snprintf(g_cuda_err, sizeof(g_cuda_err),
+             "hk_opacity_noalloc: a pressure-shift field (delta) is not served (its halo needs a reduction and a host wait)");
+    return HK_ERR_UNSUPPORTED;
+  }
+  Scratch s;
+  rc = noalloc_scratch(&s);
+  if (rc != HK_OK) return rc;
+  const int timing = g_timing;  // the stage events of hk_set_timing are created on demand: not on this path
+  g_timing = 0;
+  rc = run_opacity(lines, n_lines, T, P_atm, prm->q_ratio, prm->mass_amu, nu_min, dnu, cutoff, N, kappa_out, s, *prm,
+                   (cudaStream_t)prm->stream, 0.0);
+  g_timing = timing;
+  return rc;  // nothing to release: `s` only points into the array
 }
 
 // copy stream and events of hk_opacity_host, one set per host thread (re-made when the thread changes device)
