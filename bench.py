@@ -583,6 +583,13 @@ def run_ours(args):
                           "note": "GPU kappa and k-table of this run's last timed step against the oracle on the cpu_baseline "
                                   "sample; mask: oracle value >= 1e-12 x the oracle's max over the compared set"}
         ok = ok and pk <= bar and pt <= bar
+        # the host-buffer call's own outputs (last e2e step; the ranged path of hk_opacity_host), against the same oracle sample
+        e_k, e_t = h_kappa.numpy(), h_ktab.numpy()
+        pke = parity_of(e_k[js], o["kappa"], bar)
+        pte = parity_of(e_t[o["units"]].ravel(), o["ktab"].ravel(), bar)
+        same = bool(np.array_equal(e_k, got_kappa) and np.array_equal(e_t, got_ktab))
+        line["e2e"]["parity"] = {"kappa_max_rel": pke, "ktable_max_rel": pte, "bitwise_equal_to_device_form": same, "bar": bar}
+        ok = ok and pke <= bar and pte <= bar and same
         if legs:
             line["configs"] = legs
     line["paper_context"] = "~1 s per opacity function of ~1e5 lines on a Tesla K20 (PAPER.md:9, 267); other hardware, not a target"

@@ -126,7 +126,11 @@ int64_t hk_grid_size(double nu_min, double nu_max, double dnu);
  * split of the line centre in grid units, a float partial sum per 32 lines added to FP64 accumulators); the 6-point
  * rule and the series near the centre stay FP64 (and so do the three grid points on either side of every line centre,
  * where the float distance would cancel), as do line prep, the index windows and kappa_out.  A line whose amplitude
- * S gamma/(pi m) is more than 2^-127 below the largest of its batch of 32 flushes to zero in this mode.
+ * S gamma/(pi m) is more than 2^-127 below the largest of the lines of its batch of 32 that reach the same 256-point span
+ * flushes to zero in this mode.  The float wing rules keep their denominators inside the float range by construction: on
+ * grids finer than 1.3e-5 cm^-1 the FP64 band around every centre widens to 4e-5 cm^-1, and a line whose window reaches
+ * beyond 5e4 cm^-1 from its centre takes the 3-point rule throughout; a cutoff beyond 2e6 cm^-1 is refused in this mode
+ * (HK_ERR_UNSUPPORTED; any cutoff wider than the grid and the list already means "no cutoff").
  *
  * kappa_out: device, N doubles, overwritten.  Lines outside [nu_min, nu_max) still contribute if within the
  * cutoff.  n_lines == 0 gives kappa == 0.

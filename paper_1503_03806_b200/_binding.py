@@ -9,7 +9,9 @@ from dataclasses import dataclass
 import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(HERE, "libhk.so")
+# HK_LIB names another build of the library (tests/test_gpu_debug_build.py points it at the checked build); HK_DEBUG_CHECKS=1
+# selects the in-tree checked build libhk_dbg.so (paper_1503_03806_b200.build)
+LIB_PATH = os.environ.get("HK_LIB") or os.path.join(HERE, "libhk_dbg.so" if os.environ.get("HK_DEBUG_CHECKS") == "1" else "libhk.so")
 HEADER = os.path.join(HERE, "..", "include", "hk.h")
 
 HK_FP64, HK_FP32 = 0, 1

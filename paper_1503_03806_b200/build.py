@@ -23,22 +23,30 @@ def nvcc_path() -> str:
     return p
 
 
-def is_stale() -> bool:
-    if not os.path.exists(LIB):
+LIB_CHECKED = os.path.join(HERE, "libhk_dbg.so")
+DEBUG_FLAGS = ["-DHK_DEBUG_CHECKS", "-DHK_WATCHDOG"]
+
+
+def is_stale(lib: str = LIB) -> bool:
+    if not os.path.exists(lib):
         return True
-    t = os.path.getmtime(LIB)
+    t = os.path.getmtime(lib)
     return any(os.path.getmtime(d) > t for d in DEPS)
 
 
-def build_library(force: bool = False, verbose: bool = False) -> str:
-    """HK_DEBUG_CHECKS=1 in the environment compiles the index checks (HK_CHECK: a trap instead of an out-of-range access) and the
-    ring watchdog in: the build the GPU test suite is run against once per round in place of compute-sanitizer, which is
-    closed on this GPU pool."""
-    if force or is_stale():
-        dbg = ["-DHK_DEBUG_CHECKS", "-DHK_WATCHDOG"] if os.environ.get("HK_DEBUG_CHECKS") == "1" else []
-        cmd = [nvcc_path()] + NVCC_FLAGS + dbg + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SRC
+def build_library(force: bool = False, verbose: bool = False, out: str | None = None, debug: bool | None = None) -> str:
+    """Release build -> libhk.so.  The CHECKED build (debug=True, or HK_DEBUG_CHECKS=1 in the environment) compiles in the index
+    checks (HK_CHECK: a trap instead of an out-of-range access) and the watchdogs of the mbarrier / ring spin loops, and goes
+    to a file of its own — libhk_dbg.so, or `out` — so that it can never stand in for the release library in a bench run;
+    hk_version() of such a library says "checked".  It is what tests/test_gpu_debug_build.py runs a slice of the GPU suite
+    against, in place of compute-sanitizer, which is closed on this GPU pool."""
+    if debug is None:
+        debug = os.environ.get("HK_DEBUG_CHECKS") == "1"
+    lib = out or (LIB_CHECKED if debug else LIB)
+    if force or is_stale(lib):
+        cmd = [nvcc_path()] + NVCC_FLAGS + (DEBUG_FLAGS if debug else []) + (["-Xptxas", "-v"] if verbose else []) + ["-o", lib] + SRC
         subprocess.run(cmd, check=True)
-    return LIB
+    return lib
 
 
 if __name__ == "__main__":

@@ -123,6 +123,9 @@ struct PrepArgs {
 
 constexpr int kPlanBlock = 256;  // granularity of the line-range lookup and of the cost model of a2
 
+// FP32 variant: half-width, in grid points, of the band around every line centre that the FP64 near kernel serves (line_prep)
+__host__ __device__ __forceinline__ double f32_guard_points(double dnu) { return fmax(3.0, ceil(4.0e-5 / dnu)); }
+
 // index window of a line: sub, sub, IEEE divide, ceil/floor — no multiply-add, nothing to contract (A4)
 __device__ __forceinline__ void line_window(double nu0, double cutoff, const PrepArgs &a, int &jlo, int &jhi)
 {
@@ -287,9 +290,18 @@ __global__ void __launch_bounds__(256) line_prep_kernel(PrepArgs a)
   if (a.f32) {
     // FP32 variant: the far kernel forms the distance of point j0 + 32k as 32k dnu + d0 in float, which cancels within a few
     // grid steps of the centre (error 1.5e-5 grid steps): the three grid points on either side go to the FP64 near kernel
+    // The float 1- and 2-point rules invert a product of denominators ~ d^8 (gh1_acc4f, gh2_acc2p), inside the float range
+    // only for 1.8e-5 < |d| < 6.5e4 cm^-1.  Small side: on a grid finer than 1.3e-5 cm^-1 the guard band widens from three grid
+    // points to 4e-5 cm^-1 (f32_guard_points, which the near kernel's line search allows for).  Large side: a line whose
+    // window reaches beyond 5e4 cm^-1 from its centre (a cutoff that wide, on a list that far from the grid) takes the
+    // 3-point rule — one pair of denominators ~ d^6, in range to 2.6e6 cm^-1 — on its whole window; validate() refuses the
+    // FP32 variant with a cutoff beyond 2e6 cm^-1.
     int lo3, hi3;
-    ball_range(c, 3.0, lo3, hi3);
+    ball_range(c, f32_guard_points(a.dnu), lo3, hi3);
     ma.j3lo = min(ma.j3lo, lo3); ma.j3hi = max(ma.j3hi, hi3);
+    if (ma.jhi >= ma.jlo && fmax((double)ma.jhi - c, c - (double)ma.jlo) * a.dnu > 5.0e4) {
+      mb.j2lo = min(mb.j2lo, ma.jlo); mb.j2hi = max(mb.j2hi, ma.jhi);
+    }
     mb.j2lo = min(mb.j2lo, ma.j3lo); mb.j2hi = max(mb.j2hi, ma.j3hi);
     mb.j1lo = min(mb.j1lo, mb.j2lo); mb.j1hi = max(mb.j1hi, mb.j2hi);
     LineF32 f;
@@ -609,8 +621,11 @@ __global__ void __launch_bounds__(Sh::WARPS * 32, Sh::MINB) voigt_far_kernel(con
 #pragma unroll 1
       for (int b0 = 0; b0 < h.cnt; b0 += 32) {
         const SpanMasks M = classify32(S.ma[stage] + b0, S.mb[stage] + b0, lane, h.cnt - b0, slo, shi);
-        if ((M.m1 | M.m2 | M.m3 | M.e1 | M.e2 | M.n3) == 0u) continue;
-        const int eb = __reduce_max_sync(kFull, (b0 + lane < h.cnt) ? sf[b0 + lane].A1e : INT_MIN);
+        const unsigned act = M.m1 | M.m2 | M.m3 | M.e1 | M.e2 | M.n3;
+        if (act == 0u) continue;
+        // (of the lines that contribute to this span only: a strong line of the batch that does not reach it must not flush a
+        // weak one that does)
+        const int eb = __reduce_max_sync(kFull, ((act >> lane) & 1u) ? sf[b0 + lane].A1e : INT_MIN);
         if (eb == INT_MIN) continue;  // every line of the batch has zero strength
         const int ebm = eb - 127;     // a line more than 2^-127 below the batch maximum flushes to zero
         float af[P];
@@ -865,7 +880,7 @@ struct __align__(16) NearSmem {
   SeriesLine ser[kNearCap];  // 5 doubles
   double Acore[kNearCap];
   int4 win[kNearCap];        // jlo, jhi - jlo + 1, jslo, jshi - jslo + 1 (0: no series points): two unsigned range tests
-  unsigned int qs[kNearCap * (kNearP + 1)];
+  unsigned int qs[kNearCap * (kNearP + 1) + 2];  // + 2: the series loop prefetches one pair of entries past the last item
   unsigned char q6[kNearP][kNearCap];  // slot | tiny << 5
   int n6[kNearP];
 };
@@ -1329,6 +1344,7 @@ static int validate(const hk_lines *lines, int64_t n_lines, double T, double P_a
     return HK_ERR_INVALID;
   if (!isfinite(nu_min) || !isfinite(nu_max)) return HK_ERR_INVALID;
   if (prm->precision != HK_FP64 && prm->precision != HK_FP32) return HK_ERR_INVALID;
+  if (prm->precision == HK_FP32 && cutoff > 2.0e6) return HK_ERR_UNSUPPORTED;  // float range of the wing rules (line_prep)
   if (lines->E_low && !pos_finite(prm->q_ratio)) return HK_ERR_INVALID;
   if (!(prm->abundance >= 0.0) || !isfinite(prm->abundance)) return HK_ERR_INVALID;
   if (!(prm->cutoff_widths >= 0.0) || !isfinite(prm->cutoff_widths)) return HK_ERR_INVALID;
@@ -1425,7 +1441,9 @@ static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double 
       va.r3_slope = sv / (1.0 - sv);
       // (FP32 variant: a line with alpha^2 < 1e-9 sends its whole 1-ball, radius <= 200 alpha < 6.4e-3 cm^-1, to this kernel)
       // (eq. 21: the tables know the unshifted centres, up to shift_pad away from the shifted ones)
-      va.r3_offset = (sv * fmax(nu_min / dnu, 0.0) + 4.0 + (f32 ? 6.4e-3 / dnu : 0.0) + pa.shift_pad / dnu) / (1.0 - sv);
+      // (and the guard band of f32_guard_points around every centre: three grid points, more on a grid finer than 1.3e-5 cm^-1)
+      va.r3_offset = (sv * fmax(nu_min / dnu, 0.0) + (f32 ? f32_guard_points(dnu) + 1.0 + 6.4e-3 / dnu : 4.0) + pa.shift_pad / dnu) /
+                     (1.0 - sv);
     } else {  // absurdly hot / light: no useful bound, the near kernel scans every line that touches the span
       va.r3_slope = 0.0;
       va.r3_offset = 4.0e9;
@@ -2041,6 +2059,10 @@ const char *hk_strerror(int code)
 }
 
 const char *hk_last_cuda_error(void) { return g_cuda_err; }
+#ifdef HK_DEBUG_CHECKS
+const char *hk_version(void) { return "hk 0.1 (sm_100a, checked: HK_DEBUG_CHECKS)"; }
+#else
 const char *hk_version(void) { return "hk 0.1 (sm_100a)"; }
+#endif
 
 }  // extern "C"

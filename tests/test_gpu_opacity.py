@@ -290,3 +290,95 @@ def test_host_buffer_form_matches_device_form():
     assert none_kap is None and torch.equal(k2, ktab.cpu())
     with pytest.raises(hk.HKError):
         hk.hk_opacity_host(wl.nu0, wl.S, wl.gamma0, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, want_kappa=False)
+
+
+@pytest.mark.parametrize("precision", [hk.HK_FP64, hk.HK_FP32])
+def test_host_buffer_form_on_a_grid_wide_enough_for_the_ranged_path(precision):
+    # with >= 48 far-kernel tiles hk_opacity_host runs a3 as six tapered (far, near) launch pairs on
+    # streams of their own and copies each range of kappa back as it becomes final; the other host-form tests stay below
+    # that size.  N = 100 003 (prime: ragged last tile, last plan block and last range) is 98 tiles of 1024 points (FP64)
+    # or 391 of 256 (FP32 variant).  The result must be the bits of the device form.
+    import torch
+    wl = workloads.small(seed=33, n_lines=6000, nu_max=1000.03, cutoff=25.0, bin_width=None)
+    assert wl.n_points == 100003
+    T, P = 1100.0, 0.3
+    lines = hk.Lines.from_numpy(wl.nu0, wl.S, wl.gamma0)
+    kap = hk.hk_opacity(lines, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, precision=precision)
+    pin = lambda a: torch.as_tensor(a).pin_memory()
+    h = [pin(wl.nu0), pin(wl.S), pin(wl.gamma0)]
+    for _ in range(3):                                       # the streams and events of the ranges are reused between calls
+        got, none_k = hk.hk_opacity_host(*h, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, precision=precision)
+        assert none_k is None and torch.equal(got, kap.cpu())
+    # a mixture: the running sum goes up with the call, every range adds to its own part and comes back
+    run = torch.full((wl.n_points,), 3.0, dtype=torch.float64).pin_memory()
+    dev = torch.full((wl.n_points,), 3.0, dtype=torch.float64, device="cuda")
+    hk.hk_opacity(lines, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, out=dev, accumulate=True, abundance=0.25,
+                  precision=precision)
+    hk.hk_opacity_host(*h, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, kappa_out=run, accumulate=True, abundance=0.25,
+                       precision=precision)
+    assert torch.equal(run, dev.cpu())
+
+
+@pytest.mark.parametrize("precision", [hk.HK_FP64, hk.HK_FP32])
+def test_host_buffer_form_ranged_path_with_the_k_table(precision):
+    # the same path with the k-distribution behind it (what bench.py's e2e leg times at config 1): kappa and k-table, and
+    # the k-table alone (one range: nothing to copy early)
+    import torch
+    wl = workloads.small(seed=34, n_lines=4000, nu_max=800.0, cutoff=100.0, bin_width=10.0)
+    assert wl.n_points == 80000
+    T, P = 1500.0, 1.0
+    lines = hk.Lines.from_numpy(wl.nu0, wl.S, wl.gamma0)
+    kap = hk.hk_opacity(lines, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, precision=precision)
+    ktab = hk.hk_kdist(kap, wl.dnu, wl.bin_width, wl.n_g)
+    hk_kap, hk_k = hk.hk_opacity_host(wl.nu0, wl.S, wl.gamma0, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff,
+                                      bin_width=wl.bin_width, n_g=wl.n_g, precision=precision)
+    assert torch.equal(hk_kap, kap.cpu()) and torch.equal(hk_k, ktab.cpu())
+    none_kap, k2 = hk.hk_opacity_host(wl.nu0, wl.S, wl.gamma0, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff,
+                                      bin_width=wl.bin_width, n_g=wl.n_g, want_kappa=False, precision=precision)
+    assert none_kap is None and torch.equal(k2, ktab.cpu())
+
+
+def test_fp32_variant_stays_inside_the_float_range():
+    # the float 1-/2-point rules invert ~d^8.  (1) Lines 7e4 - 1.2e5 cm^-1 away from the grid under a
+    # cutoff that admits them (d^8 > 3.4e38: the product overflowed and the wing was dropped without notice); (2) a grid of
+    # 2e-6 cm^-1 with lines narrow enough that the 1-point rule starts three grid points from the centre (d^8 denormal:
+    # NaN); (3) a strong line that does not reach a span must not flush a weak one of its batch that does
+    rng = np.random.default_rng(77)
+    T, P = 1500.0, 1.0
+    far0 = np.sort(rng.uniform(7.0e4, 1.2e5, 30))
+    near0 = np.sort(rng.uniform(0.0, 80.0, 5))
+    nu0 = np.concatenate((near0, far0))
+    S = np.concatenate((np.full(5, 1e-27), 10.0 ** rng.uniform(-20.0, -19.0, 30)))
+    g0 = rng.uniform(0.02, 0.1, 35)
+    lines = hk.Lines.from_numpy(nu0, S, g0)
+    ref = oracle.opacity(nu0, S, g0, T, P, 0.0, 80.0, 0.01, 1.0e6)
+    only_near = oracle.opacity(near0, S[:5], g0[:5], T, P, 0.0, 80.0, 0.01, 1.0e6)
+    assert np.median(ref / np.maximum(only_near, 1e-300)) > 2.0           # the distant lines matter on this grid
+    _check(hk.hk_opacity(lines, T, P, 0.0, 80.0, 0.01, 1.0e6, precision=hk.HK_FP32).cpu().numpy(), ref, bar=BAR32)
+    _check(hk.hk_opacity(lines, T, P, 0.0, 80.0, 0.01, 1.0e6).cpu().numpy(), ref)
+    with pytest.raises(hk.HKError) as e:
+        hk.hk_opacity(lines, T, P, 0.0, 80.0, 0.01, 3.0e6, precision=hk.HK_FP32)
+    assert e.value.code == -5
+    # (2)
+    nu0 = np.sort(rng.uniform(0.008, 0.032, 40))
+    S = 10.0 ** rng.uniform(-24.0, -20.0, 40)
+    g0 = rng.uniform(0.02, 0.1, 40)
+    T, P, dnu = 300.0, 2.0e-4, 2.0e-6
+    lines = hk.Lines.from_numpy(nu0, S, g0)
+    ref = oracle.opacity(nu0, S, g0, T, P, 0.0, 0.04, dnu, 0.01)
+    assert ref.shape == (20000,)
+    got32 = hk.hk_opacity(lines, T, P, 0.0, 0.04, dnu, 0.01, precision=hk.HK_FP32).cpu().numpy()
+    _check(got32, ref, bar=BAR32)
+    _check(hk.hk_opacity(lines, T, P, 0.0, 0.04, dnu, 0.01).cpu().numpy(), ref)
+    # (3) one batch of 32 lines under a relative cutoff of 100 Lorentz widths (windows of +-2.2 cm^-1): the line at 10 cm^-1,
+    # 2^150 stronger, is in the batch of every span up to 35 cm^-1 (the tables know the absolute cutoff) and reaches none
+    # of the spans of the weak lines at 20 - 30 cm^-1
+    nu0 = np.concatenate(([10.0], np.linspace(20.0, 30.0, 31)))
+    S = np.concatenate(([1.0e-10], np.full(31, 1.0e-56)))
+    g0 = np.full(32, 0.05)
+    lines = hk.Lines.from_numpy(nu0, S, g0)
+    ref = oracle.opacity_full(nu0, S, g0, 1500.0, 1.0, 0.0, 100.0, 0.01, 25.0, cutoff_widths=100.0)
+    got32 = hk.hk_opacity(lines, 1500.0, 1.0, 0.0, 100.0, 0.01, 25.0, precision=hk.HK_FP32, cutoff_widths=100.0).cpu().numpy()
+    weak = np.arange(1500, 10000)                                         # beyond the strong line's own window
+    assert ref[weak].max() > 0.0 and ref[:1500].max() > 1e40 * ref[weak].max()
+    _check(got32[weak], ref[weak], bar=BAR32)
