@@ -150,7 +150,7 @@ def _reach(wl, j_lo, j_hi):
     return slice(int(lo), int(hi))
 
 
-def oracle_units(wl, T, P, target_s, unit, seed, q_ratio=1.0, with_kdist=False, max_units=None):
+def oracle_units(wl, T, P, target_s, unit, seed, q_ratio=1.0, with_kdist=False, max_units=None, include=(), min_units=2):
     """Times the oracle, as it stands, on seeded whole units of `unit` consecutive grid points (a k-distribution bin where the
     config has 1000-point bins): kappa of every point of the unit (+ the unit's k-distribution row when `with_kdist`).  A
     2-unit pilot sizes the sample for about `target_s` seconds.  Returns a dict with the timing, the sampled indices and the
@@ -158,6 +158,10 @@ def oracle_units(wl, T, P, target_s, unit, seed, q_ratio=1.0, with_kdist=False, 
     import oracle
     n_units = wl.n_points // unit
     order = np.random.default_rng(seed).permutation(n_units)
+    if len(include):     # units that must be in the sample (e.g. unit 0, the dense end of config 3's ramp), after the pilot pair
+        inc = np.asarray(include, dtype=order.dtype)
+        rest = order[~np.isin(order, inc)]
+        order = np.concatenate((rest[:2], inc, rest[2:]))
     ar = np.arange(unit, dtype=np.int64)
 
     def run(units):
@@ -180,7 +184,7 @@ def oracle_units(wl, T, P, target_s, unit, seed, q_ratio=1.0, with_kdist=False, 
         return dt, ne, us, kap, ktab
 
     dt, ne, us, kap, ktab = run(order[:2])
-    nu_ = int(min(n_units, max(2, round(2 * target_s / max(dt, 1e-3)))))
+    nu_ = int(min(n_units, max(2, min_units, 2 + len(include), round(2 * target_s / max(dt, 1e-3)))))
     if max_units:
         nu_ = min(nu_, max_units)
     if nu_ > 2:
@@ -229,6 +233,124 @@ def hbm_peak():
         return float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
     except (OSError, KeyError, ValueError):
         return 6650.0, "fallback (6.65 TB/s, B200_PROFILING.md)"
+
+
+def line_prep_hbm(n_lines, n_inputs, ms, f32=False):
+    """a1 (line_prep_kernel) against the HBM roofline (an HBM-bound step; "Line"): per line it reads
+    8 B of each input array given and writes the packed records (144 B; + 32 B in the FP32 variant); the line-range tables
+    (12 B per 256 grid points) are left out."""
+    hbm, src = hbm_peak()
+    per_line = 8 * n_inputs + 144 + (32 if f32 else 0)
+    gbs = per_line * n_lines / (ms * 1e-3) / 1e9 if ms > 0 else None
+    return {"kernel": "line_prep_kernel (a1+a2)", "bound": "hbm", "achieved": gbs, "peak": hbm, "unit": "GB/s",
+            "frac": gbs / hbm if gbs else None, "algorithmic_bytes_per_line": per_line, "ms": ms, "peak_source": src}
+
+
+def kdist_hbm(n_points, n_bins, n_g, ms, extra_bytes=0.0, kernel="kdist_kernel (a5+a6)"):
+    """a5+a6 against the HBM roofline: 8 B/point read + 8 n_g B/bin written (+ extra_bytes for the Chebyshev variant)."""
+    hbm, src = hbm_peak()
+    b = 8.0 * n_points + 8.0 * n_bins * n_g + extra_bytes
+    gbs = b / (ms * 1e-3) / 1e9 if ms > 0 else None
+    return {"kernel": kernel, "bound": "hbm", "achieved": gbs, "peak": hbm, "unit": "GB/s", "frac": gbs / hbm if gbs else None,
+            "algorithmic_bytes": b, "ms": ms, "points_per_bin": n_points // n_bins, "peak_source": src}
+
+
+def fp32_variant_leg(hk, wl, lines, T, P, flush, fp32_peak, steps=20):
+    """The optional FP32 variant (north_star; BASELINE.json configs[3] names it) on the headline workload, timed like the
+    headline: CUDA events around each step, L2 flushed between steps, per-stage times from the library's own events."""
+    import torch
+    N = wl.n_points
+    ppb = int(round(wl.bin_width / wl.dnu))
+    kap = torch.empty(N, dtype=torch.float64, device="cuda")
+    ktab = torch.empty((N // ppb, wl.n_g), dtype=torch.float64, device="cuda")
+    stream = torch.cuda.current_stream()
+    for _ in range(3):
+        hk.hk_opacity(lines, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, mass_amu=wl.mass_amu, out=kap, precision=hk.HK_FP32)
+    hk.hk_set_timing(True)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    stage = np.zeros(3)
+    for i in range(steps):
+        flush.zero_()
+        ev[i][0].record(stream)
+        hk.hk_opacity(lines, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, mass_amu=wl.mass_amu, out=kap, precision=hk.HK_FP32)
+        hk.hk_kdist(kap, wl.dnu, wl.bin_width, wl.n_g, out=ktab)
+        ev[i][1].record(stream)
+        stage += np.array(hk.hk_last_stage_ms())
+    torch.cuda.synchronize()
+    hk.hk_set_timing(False)
+    stage /= steps
+    ms = sum(a.elapsed_time(b) for a, b in ev) / steps
+    census = hk.hk_regime_census(wl.nu0, wl.gamma0, T, P, wl.mass_amu, wl.nu_min, N, wl.dnu, wl.cutoff, precision=hk.HK_FP32)
+    alg = sum(FP32_INST_PER_EVAL[k] * census[k] for k in FP32_INST_PER_EVAL)
+    ach = 2.0 * alg / (stage[1] * 1e-3) / 1e12
+    peak = 2.0 * fp32_peak / 1e12
+    leg = {"workload": WORKLOAD + " [optional FP32 variant, bar 1e-4]", "steps": steps, "ms_per_step": ms,
+           "stage_ms": {"line_prep": float(stage[0]), "voigt_far": float(stage[1]), "voigt_near": float(stage[2])},
+           "roofline": {"kernel": "voigt_far_kernel<FP32>", "bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
+                        "frac": ach / peak, "ms": float(stage[1]), "regime_census": census,
+                        "note": "FP32-pipe thread-instructions x2 of the float 1-/2-/3-point rules (4 / 6.5 / 10 per evaluation) "
+                                "against the FFMA microbenchmark of this run; the near kernel stays FP64"},
+           "line_prep_hbm": line_prep_hbm(wl.n_lines, 3, float(stage[0]), f32=True)}
+    return leg, kap.cpu().numpy(), ktab.cpu().numpy()
+
+
+def f_rows_leg(hk, wl, kappa, ktab, fp64_peak, n_c=20, n_m=1000, reps=20):
+    """SURVEY.md 8(f1)/(f2) at the headline size (Fig. 5: "Resampling", "Transmission"): device times by CUDA
+    events around `reps` back-to-back calls, each against its roofline; the outputs are returned for the parity check."""
+    import torch
+    N = wl.n_points
+    ppb = int(round(wl.bin_width / wl.dnu))
+    nb = N // ppb
+    mcol = 10 ** np.linspace(-6, 4, n_m)
+    dm = torch.as_tensor(mcol).cuda()
+
+    def timed(fn):
+        fn()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            out = fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return out, e0.elapsed_time(e1) / reps
+
+    (coef, kt2), ms_c = timed(lambda: hk.hk_kdist_cheb(kappa, wl.dnu, wl.bin_width, n_c, n_g=wl.n_g))
+    t_k, ms_tk = timed(lambda: hk.hk_transmission(ktab, dm))
+    t_d, ms_td = timed(lambda: hk.hk_transmission_direct(kappa, wl.dnu, wl.bin_width, dm))
+    inst = 19.0   # FP64-pipe instructions per exp term: product, clamp, exp_fast (16), accumulate
+    peak = 2.0 * fp64_peak / 1e12
+
+    def alu(terms, ms, kernel):
+        a = 2.0 * inst * terms / (ms * 1e-3) / 1e12
+        return {"kernel": kernel, "bound": "alu", "achieved": a, "peak": peak, "unit": "TFLOP/s", "frac": a / peak, "ms": ms,
+                "exp_per_s": terms / (ms * 1e-3), "fp64_inst_per_term": inst}
+
+    leg = {"workload": f"headline size: {nb} bins x {ppb} points, n_c = {n_c}, n_g = {wl.n_g}, {n_m} column masses",
+           "timing": f"CUDA events around {reps} back-to-back calls",
+           "kdist_cheb_with_ktable": kdist_hbm(N, nb, wl.n_g, ms_c, extra_bytes=8.0 * nb * n_c + 16.0 * N,
+                                               kernel="kdist_kernel<ln> + cheb_project_kernel (f1; ln of the sorted bins "
+                                                      "written and read once: + 16 B/point)"),
+           "transmission_ktable": alu(float(nb) * wl.n_g * n_m, ms_tk, "transmission_kernel (f2, Lebesgue side)"),
+           "transmission_direct": alu(float(N) * n_m, ms_td, "transmission_direct_kernel (f2, Riemann side)")}
+    got = {"coef": coef.cpu().numpy(), "ktab": kt2.cpu().numpy(), "t_k": t_k.cpu().numpy(), "t_d": t_d.cpu().numpy(),
+           "mcol": mcol, "n_c": n_c}
+    return leg, got
+
+
+def f_rows_parity(got, o, ppb):
+    """The f-rows against the oracle on the cpu_baseline sample's bins.  The oracle works from ITS OWN kappa of those bins (no
+    oracle input comes from the CUDA path), so each figure includes the <= 1e-6 relative difference of the two kappa: bars
+    1e-5 on the coefficients of ln kappa(y) (absolute, relative to max(1, |C|)), 1e-6 on the transmission (absolute, T <= 1)."""
+    import oracle
+    us = o["units"]
+    C = oracle.kdist_cheb(o["kappa"], ppb, got["n_c"])
+    ce = float((np.abs(got["coef"][us] - C) / np.maximum(1.0, np.abs(C))).max())
+    tk = float(np.abs(got["t_k"][us] - oracle.transmission_kdist(o["ktab"], got["mcol"])).max())
+    td = float(np.abs(got["t_d"][us] - oracle.transmission_direct(o["kappa"], ppb, got["mcol"])).max())
+    kt = parity_of(got["ktab"][us].ravel(), o["ktab"].ravel(), PARITY_BAR)
+    ok = ce <= 1e-5 and tk <= 1e-6 and td <= 1e-6 and kt <= PARITY_BAR
+    return {"bins": int(us.size), "cheb_coef_max_err": ce, "cheb_ktable_max_rel": kt, "transmission_ktable_max_abs": tk,
+            "transmission_direct_max_abs": td, "bars": {"cheb_coef": 1e-5, "ktable": PARITY_BAR, "transmission": 1e-6}}, ok
 
 
 # ---------------------------------------------------------------------------------------------------------------------------
@@ -318,7 +440,7 @@ def config_leg(hk, k, fp64_peak, flush, oracle_s=6.0, sm_mhz=None, precision=Non
     for ip in chk:
         T, P = pairs[ip]
         o = oracle_units(wl, T, P, oracle_s / len(chk), unit, seed=1000 * k + ip, q_ratio=qr(T),
-                         with_kdist=(ppb == unit), max_units=64)
+                         with_kdist=(ppb == unit), max_units=64, include=(0,) if k == 3 else (), min_units=10 if k == 3 else 2)
         js = unit_indices(o["units"], unit)
         worst_k = max(worst_k, parity_of(got_kappa[ip][js], o["kappa"], bar))
         if ppb == unit:
@@ -347,6 +469,8 @@ def config_leg(hk, k, fp64_peak, flush, oracle_s=6.0, sm_mhz=None, precision=Non
                          "sample": samples[0] + (f" (+ {len(samples) - 1} more (T,P) pairs, same size)" if len(samples) > 1 else ""),
                          "seconds_full_config_extrapolated_by_n_evals": n_tot / (o_ev / o_s)},
         "host_generation_s": t_gen,
+        "line_prep_hbm": line_prep_hbm(wl.n_lines, 3 + (wl.E_low is not None), float(stage[0]) / len(pairs), f32=prec == hk.HK_FP32),
+        "kdist_hbm": kdist_hbm(N, N // ppb, wl.n_g, ms_kd / len(pairs)) if ppb else None,
     }
     if len(pairs) > 1 and len(pairs) <= 6:
         leg["per_pair"] = per_pair
@@ -504,6 +628,10 @@ def run_ours(args):
     run_legs = world == 1 and not args.no_configs and prec == hk.HK_FP64
     ok = True
     legs = {}
+    fp32_leg = frows = None
+    if run_legs:   # the optional FP32 variant and the 8(f) rows on the headline workload (a few tens of ms of GPU time)
+        fp32_leg, got32_kappa, got32_ktab = fp32_variant_leg(hk, wl, lines, T, P, flush, fp32_peak)
+        frows, frows_got = f_rows_leg(hk, wl, kappa, ktab, fp64_peak)
     if run_legs:   # configs 0, 2, 3, 4 at BASELINE size; the clock sampler keeps running (config 4 is 2 s of continuous load)
         del kappa, ktab, lines
         torch.cuda.empty_cache()
@@ -569,6 +697,7 @@ def run_ours(args):
                       "frac": kdist_gbs / hbm, "algorithmic_bytes": kdist_bytes, "peak_source": hbm_src,
                       "note": "8 B/point read + 8 n_g B/bin written; the kernel is bound by the bitonic network's "
                               "compare-exchange count, not by HBM (profiles/)"},
+        "line_prep_hbm": line_prep_hbm(wl.n_lines, 3, float(stage[0]), f32=prec == hk.HK_FP32),
         "clocks": clocks,
     }
     if world == 1:
@@ -590,6 +719,15 @@ def run_ours(args):
         same = bool(np.array_equal(e_k, got_kappa) and np.array_equal(e_t, got_ktab))
         line["e2e"]["parity"] = {"kappa_max_rel": pke, "ktable_max_rel": pte, "bitwise_equal_to_device_form": same, "bar": bar}
         ok = ok and pke <= bar and pte <= bar and same
+        if fp32_leg is not None:
+            p32k = parity_of(got32_kappa[js], o["kappa"], PARITY_BAR32)
+            p32t = parity_of(got32_ktab[o["units"]].ravel(), o["ktab"].ravel(), PARITY_BAR32)
+            fp32_leg["parity"] = {"kappa_max_rel": p32k, "ktable_max_rel": p32t, "points": int(js.size), "bar": PARITY_BAR32}
+            line["fp32_variant"] = fp32_leg
+            fpar, fok = f_rows_parity(frows_got, o, ppb)
+            frows["parity"] = fpar
+            line["f_rows"] = frows
+            ok = ok and p32k <= PARITY_BAR32 and p32t <= PARITY_BAR32 and fok
         if legs:
             line["configs"] = legs
     line["paper_context"] = "~1 s per opacity function of ~1e5 lines on a Tesla K20 (PAPER.md:9, 267); other hardware, not a target"
