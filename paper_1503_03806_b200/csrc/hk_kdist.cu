@@ -29,9 +29,19 @@ struct KdistArgs {
   double g[128];
 };
 
+// a > b for kappa >= 0 or +inf (no NaN, no -0): the order of the values is the order of their bit patterns as integers
+__device__ __forceinline__ bool gt(double a, double b)
+{
+#ifdef HK_KDIST_INTCMP
+  return __double_as_longlong(a) > __double_as_longlong(b);
+#else
+  return a > b;
+#endif
+}
+
 __device__ __forceinline__ void ce(double &a, double &b)  // ascending compare-exchange
 {
-  const bool sw = a > b;
+  const bool sw = gt(a, b);
   const double lo = sw ? b : a, hi = sw ? a : b;
   a = lo;
   b = hi;
@@ -113,7 +123,7 @@ __global__ void __launch_bounds__(MAXT) kdist_kernel(const __grid_constant__ Kdi
         const int i = ((p & ~(k / 2 - 1)) << 1) | (p & (k / 2 - 1));
         const int x = pad<E>(i), y = pad<E>(i ^ (k - 1));
         const double u = s[x], w = s[y];
-        if (u > w) { s[x] = w; s[y] = u; }
+        if (gt(u, w)) { s[x] = w; s[y] = u; }
       }
       __syncthreads();
       for (int jj = m >> 2; jj >= 32; jj >>= 1) {
@@ -123,7 +133,7 @@ __global__ void __launch_bounds__(MAXT) kdist_kernel(const __grid_constant__ Kdi
           const int i = ((p & ~(j - 1)) << 1) | (p & (j - 1));
           const int x = pad<E>(i), y = pad<E>(i | j);
           const double u = s[x], w = s[y];
-          if (u > w) { s[x] = w; s[y] = u; }
+          if (gt(u, w)) { s[x] = w; s[y] = u; }
         }
         __syncthreads();
       }
@@ -140,8 +150,8 @@ __global__ void __launch_bounds__(MAXT) kdist_kernel(const __grid_constant__ Kdi
       for (int r = 0; r < E / 2; ++r) {
         const double oa = __shfl_xor_sync(kFullMask, v[E - 1 - r], m - 1);
         const double ob = __shfl_xor_sync(kFullMask, v[r], m - 1);
-        v[r] = ((v[r] > oa) == keep_min) ? oa : v[r];
-        v[E - 1 - r] = ((v[E - 1 - r] > ob) == keep_min) ? ob : v[E - 1 - r];
+        v[r] = (gt(v[r], oa) == keep_min) ? oa : v[r];
+        v[E - 1 - r] = (gt(v[E - 1 - r], ob) == keep_min) ? ob : v[E - 1 - r];
       }
     }
     // ---- half-cleaners inside the warp ----
@@ -150,7 +160,7 @@ __global__ void __launch_bounds__(MAXT) kdist_kernel(const __grid_constant__ Kdi
 #pragma unroll
       for (int r = 0; r < E; ++r) {
         const double o = __shfl_xor_sync(kFullMask, v[r], jj);
-        const bool take = (v[r] > o) == keep_min;
+        const bool take = gt(v[r], o) == keep_min;
         v[r] = take ? o : v[r];
       }
     }

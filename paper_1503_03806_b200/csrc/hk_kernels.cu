@@ -881,8 +881,9 @@ struct __align__(16) NearSmem {
   double Acore[kNearCap];
   int4 win[kNearCap];        // jlo, jhi - jlo + 1, jslo, jshi - jslo + 1 (0: no series points): two unsigned range tests
   unsigned int qs[kNearCap * (kNearP + 1) + 2];  // + 2: the series loop prefetches one pair of entries past the last item
-  unsigned char q6[kNearP][kNearCap];  // slot | tiny << 5
+  unsigned char q6[kNearP][kNearCap];  // slot | tiny << 5; the items whose group needs no per-point test come first
   int n6[kNearP];
+  int n6i[kNearP];                     // how many of them need no test
 };
 
 __device__ __forceinline__ void cp_async8(void *smem_dst, const void *gmem_src)
@@ -893,11 +894,11 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 
 // one 6-point item: line slot u & 31 (bit 5: the line adds the Gaussian term) on the group whose point of this lane is j, at
 // nu = xk; 0 outside the window and inside the series interval
+template <bool TEST = true>
 __device__ __forceinline__ double near_gh6_item(const NearSmem &S, unsigned u, int j, double xk)
 {
   const int e = u & 31;
   const double d = xk - S.nu0[e];
-  const int4 w = S.win[e];
   const double *c = S.g6[e];
   const double2 c0 = *reinterpret_cast<const double2 *>(c), c1 = *reinterpret_cast<const double2 *>(c + 2),
                 c2 = *reinterpret_cast<const double2 *>(c + 4), c3 = *reinterpret_cast<const double2 *>(c + 6),
@@ -912,8 +913,13 @@ __device__ __forceinline__ double near_gh6_item(const NearSmem &S, unsigned u, i
     const double ia = S.ser[e].inv_alpha;
     v = fma(S.Acore[e], exp_fast(fmax(-(q * ia) * ia, -700.0)), v);
   }
-  const bool ok = ((unsigned)(j - w.x) < (unsigned)w.y) & !((unsigned)(j - w.z) < (unsigned)w.w);
-  return ok ? v : 0.0;
+  if constexpr (TEST) {
+    const int4 w = S.win[e];
+    const bool ok = ((unsigned)(j - w.x) < (unsigned)w.y) & !((unsigned)(j - w.z) < (unsigned)w.w);
+    return ok ? v : 0.0;
+  } else {
+    return v;  // the whole group lies in the window and outside the series interval (decided at listing time)
+  }
 }
 
 __global__ void __launch_bounds__(32, HK_NEAR_MINB) voigt_near_kernel(const __grid_constant__ VoigtArgs a)
@@ -958,14 +964,15 @@ __global__ void __launch_bounds__(32, HK_NEAR_MINB) voigt_near_kernel(const __gr
     const unsigned lt = (1u << lane) - 1u;
     const int e = __popc(lm & lt);  // slot
     HK_CHECK(!listed || (e < kNearCap && kA >= 0 && kB < kNearP && i < a.n_lines));
-    int ns = 0, kS0 = 8, kS1 = -1, sa = 0, sb = -1;
+    int ns = 0, kS0 = 8, kS1 = -1, sa = 0, sb = -1, sa0 = 0, sb0 = -1;
     unsigned tiny = 0u;
     if (listed) {
       const LineBase lb = a.base[i];
       const LineCore lc = a.core[i];
       const LineNear ln = a.near[i];
       const double inv_alpha = a.gh2[i].inv_alpha;
-      const int sa0 = max(ln.jslo, plo + 32 * kA), sb0 = min(ln.jshi, plo + 32 * kB + 31);  // series points in these groups
+      sa0 = max(ln.jslo, plo + 32 * kA);  // series points in these groups
+      sb0 = min(ln.jshi, plo + 32 * kB + 31);
       if (sa0 <= sb0) {
         kS0 = (sa0 - plo + 31) >> 5;  // groups wholly inside the series interval: no 6-point item
         kS1 = ((sb0 - plo + 1) >> 5) - 1;
@@ -994,10 +1001,25 @@ __global__ void __launch_bounds__(32, HK_NEAR_MINB) voigt_near_kernel(const __gr
 #pragma unroll
     for (int k = 0; k < kNearP; ++k) {
       const bool has = listed && k >= kA && k <= kB && (k < kS0 || k > kS1);
+#ifndef HK_NEAR_NOSPLIT
+      // a group wholly inside the line's window that holds no series point needs no per-point test: those items are queued
+      // first and worked off by a loop without the test (most items: a window is +-cutoff wide, the 3-ball a few groups)
+      const int g0 = plo + 32 * k;
+      const bool inner = has && A.jlo <= g0 && A.jhi >= g0 + 31 && (sa0 > sb0 || sb0 < g0 || sa0 > g0 + 31);
+      const unsigned bi = __ballot_sync(kFull, inner), be = __ballot_sync(kFull, has && !inner);
+      const int ni = __popc(bi);
+      HK_CHECK(ni + __popc(be) <= kNearCap);
+      if (has) S.q6[k][inner ? __popc(bi & lt) : ni + __popc(be & lt)] = (unsigned char)((unsigned)e | tiny);
+      if (lane == 0) {
+        S.n6[k] = ni + __popc(be);
+        S.n6i[k] = ni;
+      }
+#else
       const unsigned bk = __ballot_sync(kFull, has);
       HK_CHECK(__popc(bk) <= kNearCap);
       if (has) S.q6[k][__popc(bk & lt)] = (unsigned char)((unsigned)e | tiny);
-      if (lane == 0) S.n6[k] = __popc(bk);
+      if (lane == 0) { S.n6[k] = __popc(bk); S.n6i[k] = 0; }
+#endif
     }
     // series queue: exclusive scan of the chunk counts over the lanes
     int incl = ns;
@@ -1028,7 +1050,15 @@ __global__ void __launch_bounds__(32, HK_NEAR_MINB) voigt_near_kernel(const __gr
       const unsigned char *q = S.q6[k];
       double s0 = 0.0, s1 = 0.0;
       int it = 0;
+      const int ni = S.n6i[k] & ~1;  // pairs of untested items; an odd one out goes through the tested loop (same value)
       unsigned nxt = *reinterpret_cast<const unsigned short *>(q);
+#pragma unroll 1
+      for (; it < ni; it += 2) {
+        const unsigned u = nxt;
+        nxt = *reinterpret_cast<const unsigned short *>(q + ((it + 2) & 31));
+        s0 += near_gh6_item<false>(S, u & 255u, j, xk);
+        s1 += near_gh6_item<false>(S, u >> 8, j, xk);
+      }
 #pragma unroll 1
       for (; it + 1 < n; it += 2) {
         const unsigned u = nxt;
@@ -1243,7 +1273,13 @@ void pool_free(void *p, cudaStream_t st)
 // (config 3 at 1e8 lines: far kernel 284 -> 234 ms); on config 1 it is 3 % slower, on config 2 / 4 1-2 % slower over the
 // pressure sweep.  The FP32 variant (80 registers) runs one warp per CTA, 24 CTAs/SM, everywhere (16 % faster on config 3).
 using ShSparse = FarShape<8, 4, 4, 128, 4, false>;
-using ShDense = FarShape<8, 1, 16, 64, 2, false>;
+#ifndef HK_DENSE_WARPS
+#define HK_DENSE_WARPS 1
+#define HK_DENSE_MINB 16
+#define HK_DENSE_CH 64
+#define HK_DENSE_STAGES 2
+#endif
+using ShDense = FarShape<8, HK_DENSE_WARPS, HK_DENSE_MINB, HK_DENSE_CH, HK_DENSE_STAGES, false>;
 using ShF32 = FarShape<8, 1, 24, 64, 2, true>;
 constexpr double kDenseLinesPerSpan = 10000.0;  // lines whose window reaches a 256-point span, on average, from which ShDense serves
 
