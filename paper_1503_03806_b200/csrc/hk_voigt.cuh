@@ -358,11 +358,14 @@ __device__ __forceinline__ SeriesLine series_line_setup(double y, double inv_y, 
   return L;
 }
 
-// amp * V(d) by the series, |d| / alpha clamped at 6.7 (callers mask the points beyond the series region).  About 90 FP64
-// instructions: two exponentials (13 each), reciprocal (3), recurrence and sums (35), sin^2 (13), the rest head and tail.
+// amp * V(d) by the series, valid for |d| / alpha <= 6.7.  Every term is even in x (exp(-x^2), cosh(2 a n x), sin^2(x y)), so the
+// signed x = d / alpha serves, and x is not clamped: callers discard the lanes beyond the series region (there the result
+// is meaningless, possibly inf or NaN, and never stored) — fabs + fmin cost five issue slots per evaluation in an
+// issue-bound kernel (profiles/r03_near_instruction_mix.txt).  About 83 FP64 instructions: two exponentials (13 each),
+// reciprocal (3), recurrence and sums (35), sin^2 (13), the rest head and tail.
 __device__ __forceinline__ double series_val(double d, const SeriesLine &L, const double *W)
 {
-  const double x = fmin(fabs(d) * L.inv_alpha, 6.7);
+  const double x = d * L.inv_alpha;
   const double ex2 = exp_series(-x * x);
   const double p = exp_series((2.0 * kA) * x);
   const double s2 = sin_sq_series(x * L.y);
