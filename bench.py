@@ -60,13 +60,28 @@ FAR_REGIMES, NEAR_REGIMES = ("gh1", "gh2", "gh3"), ("gh6", "series")
 # --precision fp32: FP32-pipe thread-instructions per evaluation of the rules the far kernel runs in float (hk_voigt.cuh
 # gh1_acc2f / gh2_acc2f: 8 and 13 per pair of points, + 1 MUFU.RCP per pair; gh3_accf: 10 + 1 MUFU.RCP per point)
 FP32_INST_PER_EVAL = {"gh1": 4.0, "gh2": 6.5, "gh3": 10.0}
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the roofline kernels, from the committed `ncu --set full` capture
-# named here (not live: ncu cannot run inside a timed bench).  Not memory-bound: context only.
-NCU_DRAM = {"fp64": {"bytes": 9.725e6 + 36.882e6 + 0.016e6,   # far 9.72 MB read, near 36.88 MB read + 16 KB written
-                     "source": "profiles/r02_voigt_far_kernel_ncu_full.txt + r02_voigt_near_kernel_ncu_full.txt (ncu flushes the "
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the roofline kernels, read from the committed `ncu --set full`
+# summaries named here (not live: ncu cannot run inside a timed bench).  Not memory-bound: context only.
+def _ncu_dram(*files):
+    """Sum of the DRAM bytes (read + written) of one launch of each kernel, from profiles/<file>; None if a file is missing."""
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    total = 0.0
+    for f in files:
+        try:
+            rows = [l.split() for l in open(os.path.join(ROOT, "profiles", f)) if l.startswith(("dram__bytes_read.sum ", "dram__bytes_write.sum "))]
+        except OSError:
+            return None
+        if len(rows) != 2:
+            return None
+        total += sum(float(r[2]) * scale[r[1]] for r in rows)
+    return total
+
+
+NCU_DRAM = {"fp64": {"bytes": _ncu_dram("r03_voigt_far_kernel_ncu_full.txt", "r03_voigt_near_kernel_ncu_full.txt"),
+                     "source": "profiles/r03_voigt_far_kernel_ncu_full.txt + r03_voigt_near_kernel_ncu_full.txt (ncu flushes the "
                                "caches before each kernel: the near kernel's 36.9 MB are the 24 MB of kappa the far kernel wrote, "
                                "L2-resident in a real step, plus line records)"},
-            "fp32": {"bytes": 6.517e6 + 0.001e6, "source": "profiles/r02_voigt_far32_kernel_ncu_full.txt"}}
+            "fp32": {"bytes": _ncu_dram("r03_voigt_far32_kernel_ncu_full.txt"), "source": "profiles/r03_voigt_far32_kernel_ncu_full.txt"}}
 NOMINAL_FP64_LANES = 148 * 64   # DFMA lanes of a B200 (B200_PROFILING.md): nominal peak = lanes x SM clock
 
 
