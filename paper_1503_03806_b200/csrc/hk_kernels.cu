@@ -1401,6 +1401,8 @@ constexpr int kMaxChunks = 8;
 #endif
 constexpr int kHostChunks = HK_HOST_CHUNKS;
 struct GridChunks {
+  int64_t align = 0;     // in: > 0 asks for range boundaries at multiples of this many grid points (the k-distribution bin)
+  bool aligned = false;  // out: every lo[] / hi[] is such a multiple (or N)
   int n = 1;
   cudaStream_t streams[kMaxChunks] = {};
   cudaEvent_t fork = nullptr;
@@ -1488,6 +1490,19 @@ static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double 
   // ranges only where every one gets a few tiles (a small grid has nothing to overlap)
   const int nch = (chunks && n_tiles >= 8 * chunks->n) ? std::max(1, std::min(chunks->n, kMaxChunks)) : 1;
   const int bpt = tile / kPlanBlock;  // plan blocks per tile
+  // hk_opacity_host with a k-table: ranges cut at common multiples of the tile and the bin, so that the bins of a range can be
+  // sorted and copied back as soon as that range is final — where the grid holds at least two such units per range
+  int64_t unit_tiles = 0, n_units = 0;
+  if (chunks && nch > 1 && chunks->align > 0) {
+    int64_t g = tile, r = chunks->align;
+    while (r) { const int64_t t = g % r; g = r; r = t; }
+    const int64_t unit = (int64_t)tile / g * chunks->align;  // lcm, in grid points
+    if (N / unit >= 2 * nch) {
+      unit_tiles = unit / tile;
+      n_units = N / unit;
+    }
+  }
+  if (chunks) chunks->aligned = unit_tiles > 0;
   if (chunks && nch > 1) HK_CUDA(cudaEventRecord(chunks->fork, st));
   for (int c = 0; c < nch; ++c) {     // ranges of whole tiles, from the top of the grid down
     cudaStream_t sc = (chunks && nch > 1) ? chunks->streams[c] : st;
@@ -1497,6 +1512,8 @@ static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double 
     // ranges, 1.21 tapered)
     auto cut = [&](int k) {  // tiles below the k ranges processed last
       const int64_t tot = (int64_t)nch * (nch + 1) / 2 + nch, w = (int64_t)k * (k + 1) / 2 + k;
+      if (k >= nch) return n_tiles;
+      if (unit_tiles > 0) return (int)((int64_t)n_units * w / tot * unit_tiles);  // whole units of lcm(tile, bin)
       return (int)((int64_t)n_tiles * w / tot);
     };
     const int t_lo = cut(nch - 1 - c), t_hi = cut(nch - c);
@@ -1504,15 +1521,19 @@ static int run_opacity(const hk_lines *lines, int64_t n_lines, double T, double 
     va.n_tiles = t_hi - t_lo;
     va.queue = s.queue + c;
     const int g = std::min(grid, va.n_tiles);
-    if (shape == kShapeF32) voigt_far_kernel<ShF32><<<g, ShF32::WARPS * 32, sizeof(VoigtSmem<ShF32>), sc>>>(va);
-    else if (shape == kShapeDense) voigt_far_kernel<ShDense><<<g, ShDense::WARPS * 32, sizeof(VoigtSmem<ShDense>), sc>>>(va);
-    else voigt_far_kernel<ShSparse><<<g, ShSparse::WARPS * 32, sizeof(VoigtSmem<ShSparse>), sc>>>(va);
-    HK_CUDA(cudaGetLastError());
-    if (g_timing && c == nch - 1) HK_CUDA(cudaEventRecord(ev[2], sc));
     const int b_lo = t_lo * bpt, b_hi = std::min(t_hi * bpt, nb);
+    if (g > 0) {  // (a range cut at whole units can be empty)
+      if (shape == kShapeF32) voigt_far_kernel<ShF32><<<g, ShF32::WARPS * 32, sizeof(VoigtSmem<ShF32>), sc>>>(va);
+      else if (shape == kShapeDense) voigt_far_kernel<ShDense><<<g, ShDense::WARPS * 32, sizeof(VoigtSmem<ShDense>), sc>>>(va);
+      else voigt_far_kernel<ShSparse><<<g, ShSparse::WARPS * 32, sizeof(VoigtSmem<ShSparse>), sc>>>(va);
+      HK_CUDA(cudaGetLastError());
+    }
+    if (g_timing && c == nch - 1) HK_CUDA(cudaEventRecord(ev[2], sc));
     va.block0 = b_lo;
-    voigt_near_kernel<<<b_hi - b_lo, 32, 0, sc>>>(va);
-    HK_CUDA(cudaGetLastError());
+    if (b_hi > b_lo) {
+      voigt_near_kernel<<<b_hi - b_lo, 32, 0, sc>>>(va);
+      HK_CUDA(cudaGetLastError());
+    }
     if (chunks) {
       chunks->lo[c] = (int64_t)b_lo * kPlanBlock;
       chunks->hi[c] = std::min<int64_t>((int64_t)b_hi * kPlanBlock, N);
@@ -1717,6 +1738,7 @@ struct HostCopy {
   cudaStream_t range[kMaxChunks] = {};  // one per grid range, earlier ranges at higher priority
   cudaEvent_t fork = nullptr;
   cudaEvent_t done[kMaxChunks] = {};
+  cudaEvent_t sorted[kMaxChunks] = {};  // the k-distribution of a range's bins is done
   cudaEvent_t copied = nullptr;
 };
 static thread_local HostCopy g_hc;
@@ -1729,6 +1751,7 @@ static int host_copy_get(HostCopy **out)
     h = HostCopy();  // a set made on another device is abandoned (a thread that hops devices is not the case served)
     HK_CUDA(cudaStreamCreateWithFlags(&h.copy, cudaStreamNonBlocking));
     for (int i = 0; i < kMaxChunks; ++i) HK_CUDA(cudaEventCreateWithFlags(&h.done[i], cudaEventDisableTiming));
+    for (int i = 0; i < kMaxChunks; ++i) HK_CUDA(cudaEventCreateWithFlags(&h.sorted[i], cudaEventDisableTiming));
     HK_CUDA(cudaEventCreateWithFlags(&h.fork, cudaEventDisableTiming));
     int prio_lo = 0, prio_hi = 0;  // numerically lower = higher priority
     HK_CUDA(cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));
@@ -1789,11 +1812,28 @@ int hk_opacity_host(const hk_lines *lines_host, int64_t n_lines, double T, doubl
     // device -> host copy of 8 B/point is a quarter of the call at config 1
     GridChunks ch;
     ch.n = kappa_host_out ? kHostChunks : 1;
+    // Sorting the bins range by range (ranges cut at common multiples of tile and bin, each range's k-distribution on its own
+    // stream, rows copied behind kappa) is built and tested but OFF: at config 1 it measured 1.25 ms per call against 1.20 ms
+    // with the k-distribution taken once after the last range (profiles/r03_README.md); -DHK_HOST_KDIST_BY_RANGE turns it on.
+#ifdef HK_HOST_KDIST_BY_RANGE
+    ch.align = (kappa_host_out && k_host_out) ? N / n_bins : 0;  // points per bin
+#endif
     ch.fork = hc->fork;
     for (int i = 0; i < kMaxChunks; ++i) ch.streams[i] = hc->range[i];
     bool copies_pending = false;
     for (int i = 0; i < kMaxChunks; ++i) ch.done[i] = hc->done[i];
     rc = opacity_impl(&dl, n_lines, T, P_atm, nu_min, nu_max, dnu, cutoff, d_kappa, prm, &ch);
+    // ranges cut at bin boundaries (ch.aligned): the bins of each range are sorted on the range's own stream right behind its
+    // near kernel, and their k-table rows follow the range's kappa to the host — nothing is left to do after the last range
+    const bool k_by_range = rc == HK_OK && kappa_host_out && k_host_out && ch.aligned && ch.n > 1;
+    if (k_by_range) {
+      const int64_t ppb = N / n_bins;
+      for (int c = 0; c < ch.n && rc == HK_OK && e == cudaSuccess; ++c) {
+        if (ch.hi[c] <= ch.lo[c]) continue;
+        rc = hk_kdist(d_kappa + ch.lo[c], ch.hi[c] - ch.lo[c], dnu, bin_width, n_g, d_k + ch.lo[c] / ppb * n_g, ch.streams[c]);
+        if (rc == HK_OK) e = cudaEventRecord(hc->sorted[c], ch.streams[c]);
+      }
+    }
     if (rc == HK_OK && kappa_host_out) {
       for (int c = 0; c < ch.n && e == cudaSuccess; ++c) {
         e = cudaStreamWaitEvent(hc->copy, ch.done[c], 0);
@@ -1801,15 +1841,29 @@ int hk_opacity_host(const hk_lines *lines_host, int64_t n_lines, double T, doubl
           e = cudaMemcpyAsync(kappa_host_out + ch.lo[c], d_kappa + ch.lo[c], (size_t)(ch.hi[c] - ch.lo[c]) * sizeof(double),
                               cudaMemcpyDeviceToHost, hc->copy);
       }
+      // the k-table rows behind all of kappa (a few hundred KB): a sort that waits for free SMs must not hold up the big copies
+      for (int c = 0; k_by_range && c < ch.n && e == cudaSuccess; ++c) {
+        if (ch.hi[c] <= ch.lo[c]) continue;
+        const int64_t ppb = N / n_bins, b0 = ch.lo[c] / ppb, nb_c = (ch.hi[c] - ch.lo[c]) / ppb;
+        e = cudaStreamWaitEvent(hc->copy, hc->sorted[c], 0);
+        if (e == cudaSuccess)
+          e = cudaMemcpyAsync(k_host_out + b0 * n_g, d_k + b0 * n_g, (size_t)nb_c * n_g * sizeof(double), cudaMemcpyDeviceToHost,
+                              hc->copy);
+      }
       if (e == cudaSuccess) e = cudaEventRecord(hc->copied, hc->copy);
       copies_pending = e == cudaSuccess;
     }
-    if (rc == HK_OK && e == cudaSuccess && k_host_out) rc = hk_kdist(d_kappa, N, dnu, bin_width, n_g, d_k, prm->stream);
-    if (rc == HK_OK && e == cudaSuccess && k_host_out)
-      e = cudaMemcpyAsync(k_host_out, d_k, (size_t)n_bins * n_g * sizeof(double), cudaMemcpyDeviceToHost, st);
+    if (!k_by_range) {
+      if (rc == HK_OK && e == cudaSuccess && k_host_out) rc = hk_kdist(d_kappa, N, dnu, bin_width, n_g, d_k, prm->stream);
+      if (rc == HK_OK && e == cudaSuccess && k_host_out)
+        e = cudaMemcpyAsync(k_host_out, d_k, (size_t)n_bins * n_g * sizeof(double), cudaMemcpyDeviceToHost, st);
+    }
     if (copies_pending && e == cudaSuccess) e = cudaStreamWaitEvent(st, hc->copied, 0);  // st frees the buffer after them
   }
-  if (e != cudaSuccess || rc != HK_OK) cudaStreamSynchronize(hc->copy);  // error path: nothing may still read the buffer
+  if (e != cudaSuccess || rc != HK_OK) {  // error path: nothing may still read the buffer
+    cudaStreamSynchronize(hc->copy);
+    for (int i = 0; i < kMaxChunks; ++i) cudaStreamSynchronize(hc->range[i]);
+  }
   pool_free(dev, st);
   const cudaError_t es = cudaStreamSynchronize(st);
   if (rc != HK_OK) return rc;

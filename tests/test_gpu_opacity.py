@@ -382,3 +382,27 @@ def test_fp32_variant_stays_inside_the_float_range():
     weak = np.arange(1500, 10000)                                         # beyond the strong line's own window
     assert ref[weak].max() > 0.0 and ref[:1500].max() > 1e40 * ref[weak].max()
     _check(got32[weak], ref[weak], bar=BAR32)
+
+
+@pytest.mark.parametrize("precision", [hk.HK_FP64, hk.HK_FP32])
+def test_host_buffer_form_on_a_long_grid_with_the_k_table(precision):
+    # 1.6e6 grid points with 1000-point bins: long enough for the library to cut its six ranges at multiples of lcm(tile, bin)
+    # (128 000 points for the FP64 tile of 1024, 32 000 for the FP32 variant's 256) and sort each range's bins on the range's
+    # own stream — the path a build with -DHK_HOST_KDIST_BY_RANGE takes (off by default: it measured slower); either way the
+    # result is the bits of the device form.  Twice, so that the per-thread streams and events are reused
+    import torch
+    wl = workloads.small(seed=35, n_lines=5000, nu_max=16000.0, cutoff=25.0, bin_width=10.0)
+    assert wl.n_points == 1_600_000
+    T, P = 1500.0, 1.0
+    lines = hk.Lines.from_numpy(wl.nu0, wl.S, wl.gamma0)
+    kap = hk.hk_opacity(lines, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, precision=precision)
+    ktab = hk.hk_kdist(kap, wl.dnu, wl.bin_width, wl.n_g)
+    for _ in range(2):
+        hk_kap, hk_k = hk.hk_opacity_host(wl.nu0, wl.S, wl.gamma0, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff,
+                                          bin_width=wl.bin_width, n_g=wl.n_g, precision=precision)
+        assert torch.equal(hk_kap, kap.cpu()) and torch.equal(hk_k, ktab.cpu())
+    # a bin width that shares no useful multiple with the tile (1250 points: lcm 160 000, ten units)
+    k2 = hk.hk_kdist(kap, wl.dnu, 12.5, wl.n_g)
+    _, hk_k2 = hk.hk_opacity_host(wl.nu0, wl.S, wl.gamma0, T, P, wl.nu_min, wl.nu_max, wl.dnu, wl.cutoff, bin_width=12.5,
+                                  n_g=wl.n_g, precision=precision)
+    assert torch.equal(hk_k2, k2.cpu())
