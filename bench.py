@@ -487,6 +487,16 @@ def config_leg(hk, k, fp64_peak, flush, oracle_s=6.0, sm_mhz=None, precision=Non
         "line_prep_hbm": line_prep_hbm(wl.n_lines, 3 + (wl.E_low is not None), float(stage[0]) / len(pairs), f32=prec == hk.HK_FP32),
         "kdist_hbm": kdist_hbm(N, N // ppb, wl.n_g, ms_kd / len(pairs)) if ppb else None,
     }
+    if k == 3 and roof is not None:
+        # wasted re-reads of the dense far shape (one-warp CTAs, each streaming its own +-cutoff window of records): DRAM bytes of
+        # one far-kernel launch at 1e7 lines from the committed ncu capture against the 96 B/line the ring copies once per line
+        t = _ncu_dram("r02_config3_1e7_voigt_far_kernel_ncu_full.txt")
+        roof["traffic"] = t
+        roof["traffic_algorithmic"] = 96.0e7 + 8.0 * N
+        roof["traffic_ratio"] = t / roof["traffic_algorithmic"] if t else None
+        roof["traffic_source"] = ("profiles/r02_config3_1e7_voigt_far_kernel_ncu_full.txt: one launch at 1e7 lines (the far kernel "
+                                  "is unchanged since); algorithmic = 96 B of ring records per line + the kappa store; 662 GB/s, "
+                                  "10 % of the HBM rate: not the limiter")
     if len(pairs) > 1 and len(pairs) <= 6:
         leg["per_pair"] = per_pair
     ok = worst_k <= bar and (worst_t <= bar)
